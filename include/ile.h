@@ -1,0 +1,146 @@
+/*
+ * ile.h -- C ABI of the B200-native ILE hot path (libile_b200.so).
+ *
+ * What it computes (arXiv 1902.04934; line numbers are /root/reference/PAPER.md):
+ * for one intrinsic point with precomputed mode overlap time series Q_{k,lm}(t) = <h_lm|d_k>(t) and mode-mode
+ * matrices U_k, V_k (eq. 8a-c) and for each extrinsic sample (RA, dec, t_ref, phi_ref, psi, inclination,
+ * distance), the time-marginalised log-likelihood
+ *
+ *     lnL_j     = (D_ref/D) Re sum_k sum_lm conj(F_k Y_lm) Q_{k,lm}[i0_k + j]                         eq. 7 / eq. 10 (L64-L67, L90-L91)
+ *                 - (D_ref/D)^2/4 sum_k [ |F_k|^2 Y^dagger U_k Y + Re(F_k^2 Y^T V_k Y) ],  j = 0..N_t-1
+ *     lnL_margT = ln( (1/N_t) sum_j exp(lnL_j) )                                                      eq. 9 (L81-L86)
+ *
+ * with F_k = F+,k + i Fx,k the antenna response (L62, L69, L79), Y_lm = _{-2}Y_lm(iota, -phi_ref) (eq. 5-6),
+ * i0_k = rint((t_ref + dt_k - t0_Q) f_s) - floor(N_t/2) the per-detector window start from the arrival-time delay
+ * dt_k = -(x_k . s)/c (L62, L88), and the Monte Carlo evidence lnZ = ln( (1/n) sum_a w_a L_margT,a ) (eq. 4)
+ * with n_eff = sum_a (wL)_a / max_a (wL)_a (L101).  DESIGN.md lists the readings taken where the paper is silent.
+ *
+ * Conventions
+ *  - Every function returns ILE_OK (0) or a negative ile_error; nothing throws across the ABI.
+ *  - All floating point is IEEE binary64; complex128 is (re, im) pairs of doubles; indices are int32.
+ *  - Angles in radians, times in seconds, distances in Mpc, positions in metres (Earth-fixed frame).
+ *  - "device" pointers are CUDA device memory on the context's device; "host" pointers are ordinary host memory.
+ *    The library copies Q, U, V and the geometry at ile_create; the caller may free them afterwards.  Sample and
+ *    result buffers stay caller-owned.
+ *  - Work is enqueued on the caller's CUDA stream (cudaStream_t passed as void*; NULL = default stream) and is
+ *    asynchronous unless stated.  Errors detected on the device (a window leaving [0, N_Q)) write -inf for that
+ *    sample, never read out of bounds, and bump a sticky counter readable with ile_status().
+ *  - One GPU.  There is no CPU fallback and no backend dispatch: without a CUDA device every call fails.
+ */
+#ifndef ILE_H
+#define ILE_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    ILE_OK = 0,
+    ILE_ERR_BAD_ARGUMENT = -1, /* NULL pointer, size out of the supported range, point index out of range */
+    ILE_ERR_CUDA = -2,         /* a CUDA runtime call failed; ile_strerror() gives the CUDA message of the last one */
+    ILE_ERR_NO_DEVICE = -3,    /* no CUDA device visible */
+    ILE_ERR_UNSUPPORTED = -4,  /* valid but larger than this build's static limits (ILE_MAX_*) */
+    ILE_ERR_OUT_OF_RANGE = -5  /* returned by ile_status(): at least one sample's window left the stored Q */
+} ile_error;
+
+#define ILE_MAX_DET 8    /* K */
+#define ILE_MAX_MODES 32 /* M */
+#define ILE_MAX_L 8      /* largest l of a mode */
+
+typedef struct ile_ctx ile_ctx; /* opaque, owned by the library */
+
+/* One interferometer: vertex position (m) and unit vectors along the two arms, Earth-fixed frame. */
+typedef struct {
+    double vertex_m[3];
+    double arm_x[3];
+    double arm_y[3];
+} ile_detector;
+
+typedef struct {
+    int32_t n_points;  /* P >= 1 intrinsic points sharing every other field */
+    int32_t n_det;     /* K, 1..ILE_MAX_DET */
+    int32_t n_modes;   /* M, 1..ILE_MAX_MODES */
+    const int32_t *l;  /* host, M entries, 2 <= l <= ILE_MAX_L */
+    const int32_t *m;  /* host, M entries, |m| <= l */
+    int32_t n_q;       /* N_Q samples per Q series */
+    int32_t n_t;       /* N_t bins in the marginalisation window, 1..N_Q */
+    double fs_hz;      /* sample rate of Q */
+    double t0_q_s;     /* time of Q sample 0 relative to the geocentric reference epoch */
+    double gmst_rad;   /* Greenwich mean sidereal time of the event: one value per event (L79) */
+    double d_ref_mpc;  /* fiducial distance D_ref of eq. 6 */
+    const ile_detector *det; /* host, K entries */
+} ile_config;
+
+/* Create a context on the current CUDA device: validates cfg, copies Q, U, V (host or device pointers) to the
+ * device and builds the mode tables.  Synchronous.
+ *   Q: complex128 [P][K][M][N_Q], C order   (eq. 8a; L86-L88: uniformly sampled, truncated to a coincidence window)
+ *   U: complex128 [P][K][M][M], U[k][a][b] = <h_a|h_b>_k      (eq. 8b)
+ *   V: complex128 [P][K][M][M], V[k][a][b] = <h_a^*|h_b>_k    (eq. 8c)                                            */
+int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, const void *U, const void *V);
+
+/* Time-marginalised lnL for n extrinsic samples of intrinsic point `point` (eq. 7, 9, 10; L97: blocks of samples).
+ * All seven sample arrays are device, n doubles each (SoA).  lnL_margT: device, n doubles out.
+ * shift_idx: device, n*K int32 out ([sample][detector], the window starts i0_k), or NULL.  n = 0 is a no-op.   */
+int ile_eval(ile_ctx *ctx, int32_t point, int64_t n, const double *ra, const double *dec, const double *t_ref,
+             const double *phi_ref, const double *psi, const double *incl, const double *dist_mpc,
+             double *lnL_margT, int32_t *shift_idx, void *cuda_stream);
+
+/* Every intrinsic point in one launch (BASELINE.json config 4): arrays are [P][n_per_point]; shift_idx
+ * [P][n_per_point][K] or NULL. */
+int ile_eval_all(ile_ctx *ctx, int64_t n_per_point, const double *ra, const double *dec, const double *t_ref,
+                 const double *phi_ref, const double *psi, const double *incl, const double *dist_mpc,
+                 double *lnL_margT, int32_t *shift_idx, void *cuda_stream);
+
+/* Evidence (eq. 4; L101): for each of n_segments consecutive runs of n_per_segment samples,
+ *   e_a = lnL_margT[a] + log_w[a],  lnZ = ln( (1/count) sum_a exp(e_a) ),  n_eff = sum_a exp(e_a - max_a e_a).
+ * log_w: device, same shape as lnL_margT, or NULL (= 0).
+ * state: device [n_segments][3] doubles = (running max, sum of exp(e - max), count), IN/OUT so that a long run can
+ *        be fed in chunks from one stream (config 3); initialise with ile_evidence_reset or to (-inf, 0, 0).
+ *        May be NULL: then the call is self-contained.
+ * lnZ, n_eff: device, n_segments doubles out; n_eff may be NULL.  A segment with no finite sample gives
+ * lnZ = -inf, n_eff = 0. */
+int ile_evidence(ile_ctx *ctx, int32_t n_segments, int64_t n_per_segment, const double *lnL_margT,
+                 const double *log_w, double *state, double *lnZ, double *n_eff, void *cuda_stream);
+
+/* Set n_segments evidence states (device [n_segments][3]) to (-inf, 0, 0). */
+int ile_evidence_reset(ile_ctx *ctx, int32_t n_segments, double *state, void *cuda_stream);
+
+/* Whole hot path from HOST buffers, for callers that keep samples on the host (the paper's workflow, L97: blocks
+ * generated on the CPU and transferred to the board): H2D copy of the seven sample arrays (+ log_w), ile_eval,
+ * ile_evidence, D2H of lnL_margT (if not NULL), lnZ and n_eff.  Host arrays of n doubles each; pinned memory makes
+ * the copies asynchronous.  Synchronises the stream before returning.  Staging buffers are owned by the context
+ * and grow on demand. */
+int ile_run_host(ile_ctx *ctx, int32_t point, int64_t n, const double *ra, const double *dec, const double *t_ref,
+                 const double *phi_ref, const double *psi, const double *incl, const double *dist_mpc,
+                 const double *log_w /* may be NULL */, double *lnL_margT /* host out, may be NULL */,
+                 double *lnZ /* host out, 1 */, double *n_eff /* host out, 1, may be NULL */, void *cuda_stream);
+
+/* Sticky device-side status: synchronises the stream, writes the number of samples whose window left [0, N_Q)
+ * since the context was created (or since the last reset) and returns ILE_OK or ILE_ERR_OUT_OF_RANGE.
+ * reset != 0 clears the counter. */
+int ile_status(ile_ctx *ctx, int64_t *n_out_of_range, int reset, void *cuda_stream);
+
+/* Select the evaluation kernel: 0 = automatic (default), 1 = reference-shaped direct kernel (any size),
+ * 2.. = tuned variants.  Returns ILE_ERR_UNSUPPORTED if the variant cannot run this
+ * context's sizes.  For tests and benchmarks; results are identical to within rounding. */
+int ile_set_variant(ile_ctx *ctx, int32_t variant);
+
+/* Number of kernels this library has launched on behalf of ctx since creation (for bench.py's gpu_launches). */
+int64_t ile_launch_count(const ile_ctx *ctx);
+
+/* Calibration: measured FP64 FMA throughput of the device's CUDA cores (register-resident DFMA chains, `iters`
+ * dependent steps of 8 independent chains per thread, full grid), in TFLOP/s (2 flops per FMA), and the kernel time
+ * in ms.  The roofline denominator for this ALU-bound path.  Synchronous. */
+int ile_measure_fp64_peak(int32_t iters, double *tflops, double *ms);
+
+void ile_destroy(ile_ctx *ctx);
+
+/* Static string for an ile_error; for ILE_ERR_CUDA the message of the most recent CUDA failure in this thread. */
+const char *ile_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ILE_H */

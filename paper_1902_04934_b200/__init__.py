@@ -1,0 +1,230 @@
+"""paper_1902_04934_b200 -- thin Python binding of libile_b200.so (include/ile.h).
+
+Argument marshalling only: every step of the hot path runs in the CUDA kernels behind the C ABI.  PyTorch is used
+for device memory (`tensor.data_ptr()`), streams and nothing else.  There is no CPU fallback: `load()` raises if the
+shared library is missing, and every call raises `IleError` on a non-zero return code.  Nothing here imports
+`oracle/`.
+
+    ctx = Context(cfg_dict)            # ile_create  (cfg_dict as produced by ile_inputs.make_config)
+    lnL, idx = ctx.eval(samples)       # ile_eval    (dict of seven CUDA float64 tensors)
+    lnZ, neff = ctx.evidence(lnL)      # ile_evidence
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libile_b200.so")
+_lib = None
+
+SAMPLE_FIELDS = ("ra", "dec", "t_ref", "phi_ref", "psi", "incl", "dist_mpc")
+EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_run_host", "ile_status",
+           "ile_set_variant", "ile_launch_count", "ile_measure_fp64_peak", "ile_destroy", "ile_strerror")
+
+
+class IleError(RuntimeError):
+    def __init__(self, code: int, where: str):
+        self.code = code
+        msg = load().ile_strerror(code).decode() if _lib is not None else str(code)
+        super().__init__(f"{where} failed with code {code}: {msg}")
+
+
+class _Detector(ctypes.Structure):
+    _fields_ = [("vertex_m", ctypes.c_double * 3), ("arm_x", ctypes.c_double * 3), ("arm_y", ctypes.c_double * 3)]
+
+
+class _Config(ctypes.Structure):
+    _fields_ = [("n_points", ctypes.c_int32), ("n_det", ctypes.c_int32), ("n_modes", ctypes.c_int32),
+                ("l", ctypes.POINTER(ctypes.c_int32)), ("m", ctypes.POINTER(ctypes.c_int32)),
+                ("n_q", ctypes.c_int32), ("n_t", ctypes.c_int32), ("fs_hz", ctypes.c_double), ("t0_q_s", ctypes.c_double),
+                ("gmst_rad", ctypes.c_double), ("d_ref_mpc", ctypes.c_double), ("det", ctypes.POINTER(_Detector))]
+
+
+def load():
+    """dlopen libile_b200.so and declare the prototypes.  Raises if the library has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not found: build it with `python -m paper_1902_04934_b200.build` "
+                          "(or __graft_entry__.build()); there is no CPU fallback")
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i32, i64, dp = ctypes.c_void_p, ctypes.c_int32, ctypes.c_int64, ctypes.POINTER(ctypes.c_double)
+    L.ile_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(_Config), vp, vp, vp]
+    L.ile_eval.argtypes = [vp, i32, i64] + [vp] * 7 + [vp, vp, vp]
+    L.ile_eval_all.argtypes = [vp, i64] + [vp] * 7 + [vp, vp, vp]
+    L.ile_evidence.argtypes = [vp, i32, i64, vp, vp, vp, vp, vp, vp]
+    L.ile_evidence_reset.argtypes = [vp, i32, vp, vp]
+    L.ile_run_host.argtypes = [vp, i32, i64] + [vp] * 7 + [vp, vp, dp, dp, vp]
+    L.ile_status.argtypes = [vp, ctypes.POINTER(i64), ctypes.c_int, vp]
+    L.ile_set_variant.argtypes = [vp, i32]
+    L.ile_launch_count.argtypes = [vp]
+    L.ile_launch_count.restype = i64
+    L.ile_measure_fp64_peak.argtypes = [i32, dp, dp]
+    L.ile_destroy.argtypes = [vp]
+    L.ile_destroy.restype = None
+    L.ile_strerror.argtypes = [ctypes.c_int]
+    L.ile_strerror.restype = ctypes.c_char_p
+    for name in EXPORTS:
+        if name not in ("ile_launch_count", "ile_destroy", "ile_strerror"):
+            getattr(L, name).restype = ctypes.c_int
+    _lib = L
+    return L
+
+
+def _check(code: int, where: str):
+    if code != 0:
+        raise IleError(code, where)
+
+
+def _stream_ptr(stream=None):
+    import torch
+
+    s = torch.cuda.current_stream() if stream is None else stream
+    return ctypes.c_void_p(s.cuda_stream)
+
+
+def _ptr(t):
+    return ctypes.c_void_p(0 if t is None else t.data_ptr())
+
+
+def measure_fp64_peak(iters: int = 1 << 16):
+    """(TFLOP/s, ms) of register-resident DFMA chains on the current device (ile_measure_fp64_peak)."""
+    tf, ms = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(load().ile_measure_fp64_peak(int(iters), ctypes.byref(tf), ctypes.byref(ms)), "ile_measure_fp64_peak")
+    return tf.value, ms.value
+
+
+class Context:
+    """Owns one ile_ctx.  `cfg` holds numpy arrays Q [P][K][M][n_q], U, V [P][K][M][M], l, m, vertex_m, arm_x, arm_y
+    and the scalars of ile_config (see include/ile.h)."""
+
+    def __init__(self, cfg):
+        import numpy as np
+
+        L = load()
+        K, M = int(cfg["n_det"]), int(cfg["n_modes"])
+        self.n_points, self.n_det, self.n_modes = int(cfg["n_points"]), K, M
+        self.n_q, self.n_t = int(cfg["n_q"]), int(cfg["n_t"])
+        l = np.ascontiguousarray(cfg["l"], dtype=np.int32)
+        m = np.ascontiguousarray(cfg["m"], dtype=np.int32)
+        det = (_Detector * K)()
+        for k in range(K):
+            for e in range(3):
+                det[k].vertex_m[e] = float(cfg["vertex_m"][k][e])
+                det[k].arm_x[e] = float(cfg["arm_x"][k][e])
+                det[k].arm_y[e] = float(cfg["arm_y"][k][e])
+        c = _Config(self.n_points, K, M, l.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
+                    m.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), self.n_q, self.n_t, float(cfg["fs_hz"]),
+                    float(cfg["t0_q_s"]), float(cfg["gmst_rad"]), float(cfg["d_ref_mpc"]), det)
+        Q = np.ascontiguousarray(cfg["Q"], dtype=np.complex128)
+        U = np.ascontiguousarray(cfg["U"], dtype=np.complex128)
+        V = np.ascontiguousarray(cfg["V"], dtype=np.complex128)
+        assert Q.shape == (self.n_points, K, M, self.n_q) and U.shape == V.shape == (self.n_points, K, M, M)
+        self._h = ctypes.c_void_p()
+        _check(L.ile_create(ctypes.byref(self._h), ctypes.byref(c), ctypes.c_void_p(Q.ctypes.data),
+                            ctypes.c_void_p(U.ctypes.data), ctypes.c_void_p(V.ctypes.data)), "ile_create")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            load().ile_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    __del__ = close
+
+    def set_variant(self, variant: int):
+        _check(load().ile_set_variant(self._h, int(variant)), "ile_set_variant")
+
+    @property
+    def launch_count(self) -> int:
+        return int(load().ile_launch_count(self._h))
+
+    def _sample_ptrs(self, samples, n_expected=None):
+        import torch
+
+        ts = [samples[f] for f in SAMPLE_FIELDS]
+        n = ts[0].numel()
+        for t in ts:
+            assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == n
+        assert n_expected is None or n == n_expected
+        return [_ptr(t) for t in ts], n
+
+    def eval(self, samples, point: int = 0, want_idx: bool = True, out=None, stream=None):
+        """ile_eval: dict of seven CUDA float64 tensors [n] -> (lnL_margT [n], shift_idx [n][K] or None)."""
+        import torch
+
+        ptrs, n = self._sample_ptrs(samples)
+        dev = samples["ra"].device
+        lnL = out if out is not None else torch.empty(n, dtype=torch.float64, device=dev)
+        idx = torch.empty((n, self.n_det), dtype=torch.int32, device=dev) if want_idx else None
+        _check(load().ile_eval(self._h, int(point), n, *ptrs, _ptr(lnL), _ptr(idx), _stream_ptr(stream)), "ile_eval")
+        return lnL, idx
+
+    def eval_all(self, samples, want_idx: bool = False, out=None, stream=None):
+        """ile_eval_all: tensors are [P][n_per_point] -> (lnL_margT [P][n], shift_idx [P][n][K] or None)."""
+        import torch
+
+        ptrs, n = self._sample_ptrs(samples)
+        assert n % self.n_points == 0
+        npp = n // self.n_points
+        dev = samples["ra"].device
+        lnL = out if out is not None else torch.empty((self.n_points, npp), dtype=torch.float64, device=dev)
+        idx = torch.empty((self.n_points, npp, self.n_det), dtype=torch.int32, device=dev) if want_idx else None
+        _check(load().ile_eval_all(self._h, npp, *ptrs, _ptr(lnL), _ptr(idx), _stream_ptr(stream)), "ile_eval_all")
+        return lnL, idx
+
+    def evidence(self, lnL, log_w=None, state=None, n_segments: int = 1, stream=None):
+        """ile_evidence: lnL [n_segments][n_per_segment] (any shape with that many elements) -> (lnZ, n_eff) CUDA
+        tensors [n_segments].  `state` ([n_segments][3], from new_state()) carries (max, sum, count) across chunks."""
+        import torch
+
+        assert lnL.is_cuda and lnL.dtype == torch.float64 and lnL.is_contiguous()
+        n = lnL.numel()
+        assert n % n_segments == 0
+        if log_w is not None:
+            assert log_w.is_cuda and log_w.dtype == torch.float64 and log_w.is_contiguous() and log_w.numel() == n
+        lnZ = torch.empty(n_segments, dtype=torch.float64, device=lnL.device)
+        neff = torch.empty(n_segments, dtype=torch.float64, device=lnL.device)
+        _check(load().ile_evidence(self._h, int(n_segments), n // n_segments, _ptr(lnL), _ptr(log_w), _ptr(state),
+                                   _ptr(lnZ), _ptr(neff), _stream_ptr(stream)), "ile_evidence")
+        return lnZ, neff
+
+    def new_state(self, n_segments: int = 1, device="cuda", stream=None):
+        import torch
+
+        st = torch.empty((n_segments, 3), dtype=torch.float64, device=device)
+        _check(load().ile_evidence_reset(self._h, int(n_segments), _ptr(st), _stream_ptr(stream)), "ile_evidence_reset")
+        return st
+
+    def run_host(self, samples_host, log_w_host=None, point: int = 0, want_lnL: bool = True, out_host=None, stream=None):
+        """ile_run_host: HOST tensors/arrays in (pinned torch CPU tensors recommended), host results out:
+        (lnL_margT host tensor or None, lnZ float, n_eff float)."""
+        import torch
+
+        ts = [samples_host[f] for f in SAMPLE_FIELDS]
+        n = ts[0].numel()
+        for t in ts:
+            assert (not t.is_cuda) and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == n
+        out = None
+        if want_lnL:
+            out = out_host if out_host is not None else torch.empty(n, dtype=torch.float64).pin_memory()
+        lnZ, neff = ctypes.c_double(0.0), ctypes.c_double(0.0)
+        _check(load().ile_run_host(self._h, int(point), n, *[_ptr(t) for t in ts], _ptr(log_w_host), _ptr(out),
+                                   ctypes.byref(lnZ), ctypes.byref(neff), _stream_ptr(stream)), "ile_run_host")
+        return out, lnZ.value, neff.value
+
+    def status(self, reset: bool = False, stream=None):
+        """ile_status: (n_out_of_range, code).  Synchronises the stream."""
+        v = ctypes.c_int64(0)
+        code = load().ile_status(self._h, ctypes.byref(v), int(reset), _stream_ptr(stream))
+        if code not in (0, -5):
+            raise IleError(code, "ile_status")
+        return int(v.value), code
+
+
+def samples_to_device(samples_np, device="cuda"):
+    """numpy dict (ile_inputs.make_samples) -> dict of contiguous CUDA float64 tensors."""
+    import torch
+
+    return {f: torch.from_numpy(samples_np[f]).to(device) for f in SAMPLE_FIELDS}

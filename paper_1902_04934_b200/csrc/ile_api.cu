@@ -1,0 +1,352 @@
+// ile_api.cu -- the C ABI of include/ile.h: context management, argument checking, kernel dispatch.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <new>
+
+#include "ile_kernels.h"
+
+struct ile_ctx {
+    int device;
+    IleSizes sz;
+    int32_t n_points;
+    IleDevParams hparams;
+    IleDevParams *dparams;
+    double2 *dQ, *dU, *dV;
+    unsigned long long *d_oob;
+    double *d_partials;
+    size_t partials_cap;  // doubles
+    double *d_stage;
+    size_t stage_cap;  // doubles
+    double *d_small;   // lnZ, n_eff (device)
+    double *h_small;   // pinned mirror
+    int32_t variant;
+    long long launches;
+};
+
+static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
+
+static int cuda_fail(cudaError_t e)
+{
+    snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error %d: %s", (int)e, cudaGetErrorString(e));
+    return ILE_ERR_CUDA;
+}
+#define CK(call)                                  \
+    do {                                          \
+        cudaError_t e__ = (call);                 \
+        if (e__ != cudaSuccess) return cuda_fail(e__); \
+    } while (0)
+
+static double factorial(int n)
+{
+    double r = 1.0;
+    for (int i = 2; i <= n; ++i) r *= (double)i;
+    return r;
+}
+
+// sqrt((2l+1)/4pi) d^l_{m,2}(beta) as sum_t coef_t cos(beta/2)^pc_t sin(beta/2)^ps_t  (Wigner's finite sum with m' = m, m = 2;
+// _{-2}Y_lm = sqrt((2l+1)/4pi) d^l_{m,2}(theta) e^{i m phi}, reading R5)
+static int build_mode_table(IleDevParams &P, int idx, int l, int m)
+{
+    const double norm = std::sqrt((2.0 * l + 1.0) / (4.0 * M_PI));
+    const double pref = std::sqrt(factorial(l + 2) * factorial(l - 2) * factorial(l + m) * factorial(l - m));
+    int nt = 0;
+    for (int k = 0; k <= 2 * l; ++k) {
+        int a = l + 2 - k, b = k, c = l - k - m, d = k - 2 + m;
+        if (a < 0 || b < 0 || c < 0 || d < 0) continue;
+        if (nt >= ILE_MAX_TERMS) return ILE_ERR_UNSUPPORTED;
+        double sign = (d % 2 == 0) ? 1.0 : -1.0;
+        P.mode_coef[idx][nt] = norm * sign * pref / (factorial(a) * factorial(b) * factorial(c) * factorial(d));
+        P.mode_pc[idx][nt] = (int8_t)(2 * l - 2 * k + 2 - m);
+        P.mode_ps[idx][nt] = (int8_t)(2 * k - 2 + m);
+        ++nt;
+    }
+    P.mode_nterm[idx] = nt;
+    P.mode_m[idx] = m;
+    return ILE_OK;
+}
+
+extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, const void *U, const void *V)
+{
+    if (!out || !cfg || !Q || !U || !V || !cfg->l || !cfg->m || !cfg->det) return ILE_ERR_BAD_ARGUMENT;
+    *out = nullptr;
+    if (cfg->n_points < 1 || cfg->n_det < 1 || cfg->n_modes < 1 || cfg->n_q < 1 || cfg->n_t < 1 || cfg->n_t > cfg->n_q)
+        return ILE_ERR_BAD_ARGUMENT;
+    if (!(cfg->fs_hz > 0.0) || !(cfg->d_ref_mpc > 0.0) || !std::isfinite(cfg->t0_q_s) || !std::isfinite(cfg->gmst_rad))
+        return ILE_ERR_BAD_ARGUMENT;
+    if (cfg->n_det > ILE_MAX_DET || cfg->n_modes > ILE_MAX_MODES) return ILE_ERR_UNSUPPORTED;
+    for (int j = 0; j < cfg->n_modes; ++j) {
+        if (cfg->l[j] < 2 || std::abs(cfg->m[j]) > cfg->l[j]) return ILE_ERR_BAD_ARGUMENT;
+        if (cfg->l[j] > ILE_MAX_L) return ILE_ERR_UNSUPPORTED;
+    }
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return ILE_ERR_NO_DEVICE;
+    }
+    ile_ctx *c = new (std::nothrow) ile_ctx();
+    if (!c) return ILE_ERR_BAD_ARGUMENT;
+    std::memset(c, 0, sizeof(*c));
+    CK(cudaGetDevice(&c->device));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, c->device));
+    c->sz.n_det = cfg->n_det;
+    c->sz.n_modes = cfg->n_modes;
+    c->sz.n_q = cfg->n_q;
+    c->sz.n_t = cfg->n_t;
+    c->sz.sm_count = prop.multiProcessorCount;
+    c->sz.max_smem_optin = (int32_t)prop.sharedMemPerBlockOptin;
+    c->n_points = cfg->n_points;
+
+    IleDevParams &P = c->hparams;
+    P.n_points = cfg->n_points;
+    P.n_det = cfg->n_det;
+    P.n_modes = cfg->n_modes;
+    P.n_q = cfg->n_q;
+    P.n_t = cfg->n_t;
+    P.fs = cfg->fs_hz;
+    P.t0_q = cfg->t0_q_s;
+    P.gmst = cfg->gmst_rad;
+    P.d_ref = cfg->d_ref_mpc;
+    for (int k = 0; k < cfg->n_det; ++k) {
+        const double *x = cfg->det[k].arm_x, *y = cfg->det[k].arm_y;
+        const int ii[6] = {0, 0, 0, 1, 1, 2}, jj[6] = {0, 1, 2, 1, 2, 2};
+        for (int e = 0; e < 6; ++e) P.det_tensor[k][e] = 0.5 * (x[ii[e]] * x[jj[e]] - y[ii[e]] * y[jj[e]]);
+        for (int e = 0; e < 3; ++e) P.vertex[k][e] = cfg->det[k].vertex_m[e];
+    }
+    for (int j = 0; j < cfg->n_modes; ++j) {
+        int r = build_mode_table(P, j, cfg->l[j], cfg->m[j]);
+        if (r != ILE_OK) {
+            delete c;
+            return r;
+        }
+    }
+    const size_t KM = (size_t)cfg->n_det * cfg->n_modes;
+    const size_t nQ = (size_t)cfg->n_points * KM * cfg->n_q, nU = (size_t)cfg->n_points * KM * cfg->n_modes;
+    cudaError_t e;
+#define CKC(call)                 \
+    do {                          \
+        e = (call);               \
+        if (e != cudaSuccess) {   \
+            ile_destroy(c);       \
+            return cuda_fail(e);  \
+        }                         \
+    } while (0)
+    CKC(cudaMalloc(&c->dparams, sizeof(IleDevParams)));
+    CKC(cudaMalloc(&c->dQ, nQ * sizeof(double2)));
+    CKC(cudaMalloc(&c->dU, nU * sizeof(double2)));
+    CKC(cudaMalloc(&c->dV, nU * sizeof(double2)));
+    CKC(cudaMalloc(&c->d_oob, sizeof(unsigned long long)));
+    CKC(cudaMalloc(&c->d_small, 8 * sizeof(double)));
+    CKC(cudaMallocHost(&c->h_small, 8 * sizeof(double)));
+    CKC(cudaMemcpy(c->dparams, &P, sizeof(P), cudaMemcpyHostToDevice));
+    CKC(cudaMemcpy(c->dQ, Q, nQ * sizeof(double2), cudaMemcpyDefault));
+    CKC(cudaMemcpy(c->dU, U, nU * sizeof(double2), cudaMemcpyDefault));
+    CKC(cudaMemcpy(c->dV, V, nU * sizeof(double2), cudaMemcpyDefault));
+    CKC(cudaMemset(c->d_oob, 0, sizeof(unsigned long long)));
+#undef CKC
+    *out = c;
+    return ILE_OK;
+}
+
+extern "C" void ile_destroy(ile_ctx *c)
+{
+    if (!c) return;
+    cudaFree(c->dparams);
+    cudaFree(c->dQ);
+    cudaFree(c->dU);
+    cudaFree(c->dV);
+    cudaFree(c->d_oob);
+    cudaFree(c->d_partials);
+    cudaFree(c->d_stage);
+    cudaFree(c->d_small);
+    if (c->h_small) cudaFreeHost(c->h_small);
+    delete c;
+}
+
+static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n, const double *ra, const double *dec,
+                         const double *t_ref, const double *phi_ref, const double *psi, const double *incl,
+                         const double *dist, double *lnL, int32_t *shift_idx, cudaStream_t st)
+{
+    IleEvalArgs a;
+    a.params = c->dparams;
+    a.Q = c->dQ;
+    a.U = c->dU;
+    a.V = c->dV;
+    a.point0 = point0;
+    a.n_points = n_points;
+    a.n_per_point = n;
+    a.ra = ra, a.dec = dec, a.t_ref = t_ref, a.phi_ref = phi_ref, a.psi = psi, a.incl = incl, a.dist = dist;
+    a.lnL = lnL;
+    a.shift_idx = shift_idx;
+    a.oob_counter = c->d_oob;
+    int nl = 0;
+    cudaError_t e = ile_launch_eval_direct(c->sz, a, st, &nl);
+    c->launches += nl;
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ILE_OK;
+}
+
+extern "C" int ile_eval(ile_ctx *c, int32_t point, int64_t n, const double *ra, const double *dec, const double *t_ref,
+                        const double *phi_ref, const double *psi, const double *incl, const double *dist_mpc,
+                        double *lnL_margT, int32_t *shift_idx, void *cuda_stream)
+{
+    if (!c || n < 0 || point < 0 || point >= c->n_points) return ILE_ERR_BAD_ARGUMENT;
+    if (n == 0) return ILE_OK;
+    if (!ra || !dec || !t_ref || !phi_ref || !psi || !incl || !dist_mpc || !lnL_margT) return ILE_ERR_BAD_ARGUMENT;
+    return eval_dispatch(c, point, 1, n, ra, dec, t_ref, phi_ref, psi, incl, dist_mpc, lnL_margT, shift_idx,
+                         (cudaStream_t)cuda_stream);
+}
+
+extern "C" int ile_eval_all(ile_ctx *c, int64_t n_per_point, const double *ra, const double *dec, const double *t_ref,
+                            const double *phi_ref, const double *psi, const double *incl, const double *dist_mpc,
+                            double *lnL_margT, int32_t *shift_idx, void *cuda_stream)
+{
+    if (!c || n_per_point < 0) return ILE_ERR_BAD_ARGUMENT;
+    if (n_per_point == 0) return ILE_OK;
+    if (!ra || !dec || !t_ref || !phi_ref || !psi || !incl || !dist_mpc || !lnL_margT) return ILE_ERR_BAD_ARGUMENT;
+    return eval_dispatch(c, 0, c->n_points, n_per_point, ra, dec, t_ref, phi_ref, psi, incl, dist_mpc, lnL_margT,
+                         shift_idx, (cudaStream_t)cuda_stream);
+}
+
+static int ensure_partials(ile_ctx *c, size_t doubles)
+{
+    if (doubles <= c->partials_cap) return ILE_OK;
+    if (c->d_partials) CK(cudaFree(c->d_partials));
+    c->d_partials = nullptr;
+    c->partials_cap = 0;
+    CK(cudaMalloc(&c->d_partials, doubles * sizeof(double)));
+    c->partials_cap = doubles;
+    return ILE_OK;
+}
+
+extern "C" int ile_evidence(ile_ctx *c, int32_t n_segments, int64_t n_per_segment, const double *lnL_margT,
+                            const double *log_w, double *state, double *lnZ, double *n_eff, void *cuda_stream)
+{
+    if (!c || n_segments < 1 || n_per_segment < 0 || !lnZ) return ILE_ERR_BAD_ARGUMENT;
+    if (n_per_segment > 0 && !lnL_margT) return ILE_ERR_BAD_ARGUMENT;
+    int32_t B = ile_evidence_blocks_per_segment(n_segments, n_per_segment, c->sz.sm_count);
+    int r = ensure_partials(c, (size_t)n_segments * B * 2);
+    if (r != ILE_OK) return r;
+    int nl = 0;
+    cudaError_t e = ile_launch_evidence(n_segments, n_per_segment, lnL_margT, log_w, state, lnZ, n_eff, c->d_partials,
+                                        B, (cudaStream_t)cuda_stream, &nl);
+    c->launches += nl;
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ILE_OK;
+}
+
+extern "C" int ile_evidence_reset(ile_ctx *c, int32_t n_segments, double *state, void *cuda_stream)
+{
+    if (!c || n_segments < 1 || !state) return ILE_ERR_BAD_ARGUMENT;
+    int nl = 0;
+    cudaError_t e = ile_launch_evidence_reset(n_segments, state, (cudaStream_t)cuda_stream, &nl);
+    c->launches += nl;
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ILE_OK;
+}
+
+extern "C" int ile_run_host(ile_ctx *c, int32_t point, int64_t n, const double *ra, const double *dec,
+                            const double *t_ref, const double *phi_ref, const double *psi, const double *incl,
+                            const double *dist_mpc, const double *log_w, double *lnL_margT, double *lnZ, double *n_eff,
+                            void *cuda_stream)
+{
+    if (!c || n < 1 || point < 0 || point >= c->n_points) return ILE_ERR_BAD_ARGUMENT;
+    if (!ra || !dec || !t_ref || !phi_ref || !psi || !incl || !dist_mpc || !lnZ) return ILE_ERR_BAD_ARGUMENT;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t need = (size_t)n * 9;
+    if (need > c->stage_cap) {
+        CK(cudaStreamSynchronize(st));
+        if (c->d_stage) CK(cudaFree(c->d_stage));
+        c->d_stage = nullptr;
+        c->stage_cap = 0;
+        CK(cudaMalloc(&c->d_stage, need * sizeof(double)));
+        c->stage_cap = need;
+    }
+    double *d = c->d_stage;
+    const double *src[8] = {ra, dec, t_ref, phi_ref, psi, incl, dist_mpc, log_w};
+    for (int i = 0; i < 8; ++i)
+        if (src[i]) CK(cudaMemcpyAsync(d + (size_t)i * n, src[i], (size_t)n * sizeof(double), cudaMemcpyHostToDevice, st));
+    double *d_out = d + (size_t)8 * n;
+    int r = eval_dispatch(c, point, 1, n, d, d + n, d + 2 * n, d + 3 * n, d + 4 * n, d + 5 * n, d + 6 * n, d_out, nullptr, st);
+    if (r != ILE_OK) return r;
+    r = ile_evidence(c, 1, n, d_out, log_w ? d + 7 * n : nullptr, nullptr, c->d_small, c->d_small + 1, st);
+    if (r != ILE_OK) return r;
+    if (lnL_margT) CK(cudaMemcpyAsync(lnL_margT, d_out, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(c->h_small, c->d_small, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    *lnZ = c->h_small[0];
+    if (n_eff) *n_eff = c->h_small[1];
+    return ILE_OK;
+}
+
+extern "C" int ile_status(ile_ctx *c, int64_t *n_out_of_range, int reset, void *cuda_stream)
+{
+    if (!c) return ILE_ERR_BAD_ARGUMENT;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    unsigned long long v = 0;
+    CK(cudaMemcpyAsync(&v, c->d_oob, sizeof(v), cudaMemcpyDeviceToHost, st));
+    if (reset) CK(cudaMemsetAsync(c->d_oob, 0, sizeof(v), st));
+    CK(cudaStreamSynchronize(st));
+    if (n_out_of_range) *n_out_of_range = (int64_t)v;
+    return v ? ILE_ERR_OUT_OF_RANGE : ILE_OK;
+}
+
+extern "C" int ile_set_variant(ile_ctx *c, int32_t variant)
+{
+    if (!c || variant < 0) return ILE_ERR_BAD_ARGUMENT;
+    if (variant > 1) return ILE_ERR_UNSUPPORTED;
+    c->variant = variant;
+    return ILE_OK;
+}
+
+extern "C" int64_t ile_launch_count(const ile_ctx *c) { return c ? (int64_t)c->launches : 0; }
+
+extern "C" int ile_measure_fp64_peak(int32_t iters, double *tflops, double *ms)
+{
+    if (iters < 1 || !tflops) return ILE_ERR_BAD_ARGUMENT;
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        cudaGetLastError();
+        return ILE_ERR_NO_DEVICE;
+    }
+    int dev = 0;
+    CK(cudaGetDevice(&dev));
+    cudaDeviceProp prop;
+    CK(cudaGetDeviceProperties(&prop, dev));
+    double *sink = nullptr;
+    CK(cudaMalloc(&sink, sizeof(double)));
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0));
+    CK(cudaEventCreate(&e1));
+    float best = 1e30f;
+    for (int rep = 0; rep < 4; ++rep) {  // first repetition is the warm-up
+        CK(cudaEventRecord(e0, 0));
+        CK(ile_launch_fp64_peak(iters, prop.multiProcessorCount, sink, 0));
+        CK(cudaEventRecord(e1, 0));
+        CK(cudaEventSynchronize(e1));
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, e0, e1));
+        if (rep > 0 && t < best) best = t;
+    }
+    cudaEventDestroy(e0);
+    cudaEventDestroy(e1);
+    cudaFree(sink);
+    const double flops = 2.0 * 8.0 * (double)iters * 256.0 * 8.0 * prop.multiProcessorCount;
+    *tflops = flops / (best * 1e-3) * 1e-12;
+    if (ms) *ms = best;
+    return ILE_OK;
+}
+
+extern "C" const char *ile_strerror(int code)
+{
+    switch (code) {
+        case ILE_OK: return "ok";
+        case ILE_ERR_BAD_ARGUMENT: return "bad argument";
+        case ILE_ERR_CUDA: return g_cuda_msg;
+        case ILE_ERR_NO_DEVICE: return "no CUDA device";
+        case ILE_ERR_UNSUPPORTED: return "size or variant not supported by this build";
+        case ILE_ERR_OUT_OF_RANGE: return "a sample's time window left the stored Q series";
+        default: return "unknown error code";
+    }
+}

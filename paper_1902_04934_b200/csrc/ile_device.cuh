@@ -1,0 +1,109 @@
+// ile_device.cuh -- device-side parameter block and the per-sample geometry shared by every evaluation kernel.
+//
+// Steps 1-4 of the hot path: antenna response F_k, arrival-time
+// delay and window index (L62, L88), harmonics Y_lm(iota, -phi_ref) (eq. 5-6), quadratic term
+// (eq. 7).  No code here is shared with oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/ile.h"
+
+#define ILE_MAX_TERMS 8 /* terms of the Wigner-d finite sum for l <= ILE_MAX_L and m' = 2: at most l - 1 */
+
+struct IleDevParams {
+    int32_t n_points, n_det, n_modes, n_q, n_t;
+    double fs, t0_q, gmst, d_ref;
+    double det_tensor[ILE_MAX_DET][6];  // D = (x x^T - y y^T)/2, symmetric: xx, xy, xz, yy, yz, zz
+    double vertex[ILE_MAX_DET][3];      // metres
+    int32_t mode_m[ILE_MAX_MODES];
+    int32_t mode_nterm[ILE_MAX_MODES];
+    // sqrt((2l+1)/4pi) d^l_{m,2}(iota) = sum_t coef[t] cos(iota/2)^pc[t] sin(iota/2)^ps[t]
+    double mode_coef[ILE_MAX_MODES][ILE_MAX_TERMS];
+    int8_t mode_pc[ILE_MAX_MODES][ILE_MAX_TERMS];
+    int8_t mode_ps[ILE_MAX_MODES][ILE_MAX_TERMS];
+};
+
+#define ILE_C_SI 299792458.0
+
+__device__ __forceinline__ double ile_ipow(double x, int n)
+{
+    double r = 1.0;
+    while (n > 0) {
+        if (n & 1) r *= x;
+        x *= x;
+        n >>= 1;
+    }
+    return r;
+}
+
+// Sky- and polarisation-dependent part of one sample: wave-frame axes X, Y and the source direction s.
+struct IleSky {
+    double X[3], Y[3], s[3];
+};
+
+__device__ __forceinline__ IleSky ile_sky(double ra, double dec, double psi, double gmst)
+{
+    IleSky g;
+    double lon = ra - gmst;  // = -(Greenwich hour angle)
+    double sl, cl, sd, cd, sp, cp;
+    sincos(lon, &sl, &cl);
+    sincos(dec, &sd, &cd);
+    sincos(psi, &sp, &cp);
+    // source direction; products rounded one by one so that the window index below is reproducible (no FMA)
+    g.s[0] = __dmul_rn(cd, cl);
+    g.s[1] = __dmul_rn(cd, sl);
+    g.s[2] = sd;
+    // psi = 0: X local west, Y local north; X x Y = propagation direction; psi rotates X toward Y  (reading R6)
+    double sg = -sl, cg = cl;  // sin, cos of gha = gmst - ra
+    g.X[0] = -cp * sg - sp * cg * sd;
+    g.X[1] = -cp * cg + sp * sg * sd;
+    g.X[2] = sp * cd;
+    g.Y[0] = sp * sg - cp * cg * sd;
+    g.Y[1] = sp * cg + cp * sg * sd;
+    g.Y[2] = cp * cd;
+    return g;
+}
+
+// F_k = F+ + i Fx = D : (XX - YY) + i D : (XY + YX)   (reading R1: F = F+ + i Fx)
+__device__ __forceinline__ double2 ile_antenna(const double *__restrict__ D, const IleSky &g)
+{
+    double DX0 = D[0] * g.X[0] + D[1] * g.X[1] + D[2] * g.X[2];
+    double DX1 = D[1] * g.X[0] + D[3] * g.X[1] + D[4] * g.X[2];
+    double DX2 = D[2] * g.X[0] + D[4] * g.X[1] + D[5] * g.X[2];
+    double DY0 = D[0] * g.Y[0] + D[1] * g.Y[1] + D[2] * g.Y[2];
+    double DY1 = D[1] * g.Y[0] + D[3] * g.Y[1] + D[4] * g.Y[2];
+    double DY2 = D[2] * g.Y[0] + D[4] * g.Y[1] + D[5] * g.Y[2];
+    double fp = (g.X[0] * DX0 + g.X[1] * DX1 + g.X[2] * DX2) - (g.Y[0] * DY0 + g.Y[1] * DY1 + g.Y[2] * DY2);
+    double fc = 2.0 * (g.X[0] * DY0 + g.X[1] * DY1 + g.X[2] * DY2);
+    return make_double2(fp, fc);
+}
+
+// Window start i0_k = rint(((t_ref + dt_k) - t0_Q) f_s) - floor(N_t/2), dt_k = -(x_k . s)/c  (readings R2, R8).
+// Every operation is individually rounded, in a fixed order, so the integer is reproducible.
+__device__ __forceinline__ int32_t ile_window_index(const double *__restrict__ v, const IleSky &g, double t_ref,
+                                                    double t0_q, double fs, int32_t n_t)
+{
+    double dot = __dadd_rn(__dadd_rn(__dmul_rn(v[0], g.s[0]), __dmul_rn(v[1], g.s[1])), __dmul_rn(v[2], g.s[2]));
+    double dt = __ddiv_rn(-dot, ILE_C_SI);
+    double x = __dmul_rn(__dsub_rn(__dadd_rn(t_ref, dt), t0_q), fs);
+    return __double2int_rn(x) - n_t / 2;
+}
+
+// Y_lm(iota, -phi_ref) = [sum_t coef_t c^pc_t s^ps_t] e^{-i m phi_ref}, c = cos(iota/2), s = sin(iota/2)  (R4, R5)
+__device__ __forceinline__ double2 ile_ylm(const IleDevParams *__restrict__ P, int mode, double ch, double sh,
+                                           double phi_ref)
+{
+    double amp = 0.0;
+    int nt = P->mode_nterm[mode];
+    for (int t = 0; t < nt; ++t)
+        amp += P->mode_coef[mode][t] * ile_ipow(ch, P->mode_pc[mode][t]) * ile_ipow(sh, P->mode_ps[mode][t]);
+    double sm, cm;
+    sincos((double)P->mode_m[mode] * phi_ref, &sm, &cm);
+    return make_double2(amp * cm, -amp * sm);
+}
+
+__device__ __forceinline__ double2 ile_cmul(double2 a, double2 b)
+{
+    return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
+}

@@ -1,0 +1,367 @@
+// ile_kernels.cu -- CUDA kernels of the ILE hot path for sm_100a (B200).
+//
+//   ile_eval_direct_kernel   steps 1-6 of SURVEY.md §8(a), general sizes (variant 1)
+//   ile_evidence_*           step 7 (eq. 4; n_eff L101)
+//   ile_fp64_peak_kernel     calibration of the FP64 FMA roofline
+//
+// The tuned evaluation kernels live in ile_eval_tuned.cu.
+#include <math_constants.h>
+
+#include "ile_kernels.h"
+
+// ------------------------------------------------------------------------------------------------------------
+// per-sample setup, one THREAD per sample (no redundant geometry across a warp)
+// ------------------------------------------------------------------------------------------------------------
+// On return: A[k*M + m] = (D_ref/D) F_k Y_m (so that lin_j = Re sum conj(A) Q), i0[k] = window start,
+// returns quad = (a^2/4) sum_k [|F_k|^2 Re(Y^dagger U_k Y) + Re(F_k^2 Y^T V_k Y)]  (eq. 7; do not assume U Hermitian: R15).
+// *bad is set when a window leaves [0, n_q) (reading R9).
+__device__ double ile_setup_sample(const IleDevParams *__restrict__ P, const double2 *__restrict__ U,
+                                   const double2 *__restrict__ V, double ra, double dec, double t_ref, double phi_ref,
+                                   double psi, double incl, double dist, double2 *A, int32_t *i0, int *bad)
+{
+    const int K = P->n_det, M = P->n_modes;
+    IleSky g = ile_sky(ra, dec, psi, P->gmst);
+    double sh, ch;
+    sincos(0.5 * incl, &sh, &ch);
+    const double a = P->d_ref / dist;
+    for (int m = 0; m < M; ++m) A[m] = ile_ylm(P, m, ch, sh, phi_ref);  // Y_m, parked in the k = 0 slots
+
+    double tot = 0.0;
+    int oob = 0;
+    for (int k = 0; k < K; ++k) {
+        double2 F = ile_antenna(P->det_tensor[k], g);
+        double yuy = 0.0;
+        double2 yvy = make_double2(0.0, 0.0);
+        for (int p = 0; p < M; ++p) {
+            double2 tu = make_double2(0.0, 0.0), tv = make_double2(0.0, 0.0);
+            const double2 *Ur = U + ((size_t)k * M + p) * M;
+            const double2 *Vr = V + ((size_t)k * M + p) * M;
+            for (int q = 0; q < M; ++q) {
+                double2 Yq = A[q], u = __ldg(Ur + q), v = __ldg(Vr + q);
+                tu.x += u.x * Yq.x - u.y * Yq.y;
+                tu.y += u.x * Yq.y + u.y * Yq.x;
+                tv.x += v.x * Yq.x - v.y * Yq.y;
+                tv.y += v.x * Yq.y + v.y * Yq.x;
+            }
+            double2 Yp = A[p];
+            yuy += Yp.x * tu.x + Yp.y * tu.y;  // Re(conj(Y_p) (U Y)_p)
+            double2 t = ile_cmul(Yp, tv);
+            yvy.x += t.x;
+            yvy.y += t.y;
+        }
+        double F2 = F.x * F.x + F.y * F.y;
+        double2 FF = ile_cmul(F, F);
+        tot += F2 * yuy + (FF.x * yvy.x - FF.y * yvy.y);
+        int32_t idx = ile_window_index(P->vertex[k], g, t_ref, P->t0_q, P->fs, P->n_t);
+        i0[k] = idx;
+        if (idx < 0 || (long long)idx + P->n_t > P->n_q) oob = 1;
+    }
+    for (int k = K - 1; k >= 0; --k) {  // k = 0 last: it overwrites the parked Y_m in place
+        double2 F = ile_antenna(P->det_tensor[k], g);
+        double2 aF = make_double2(a * F.x, a * F.y);
+        for (int m = 0; m < M; ++m) A[k * M + m] = ile_cmul(aF, A[m]);
+    }
+    *bad = oob;
+    return 0.25 * a * a * tot;
+}
+
+__device__ __forceinline__ double warp_max(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
+    return v;
+}
+__device__ __forceinline__ double warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// variant 1: direct kernel.  A warp takes G samples at a time: lane g sets up sample g (steps 1-4), then the
+// whole warp walks the G samples, lanes over time bins (step 5), lane-local online log-sum-exp + warp shuffle
+// reduction (step 6).  Q is read straight from global memory (L1/L2) with 16-byte loads.
+// ------------------------------------------------------------------------------------------------------------
+#define DIRECT_WARPS 8
+#define DIRECT_RB 4
+
+__global__ void __launch_bounds__(DIRECT_WARPS * 32) ile_eval_direct_kernel(IleEvalArgs a, int G)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const IleDevParams *__restrict__ P = a.params;
+    const int K = P->n_det, M = P->n_modes, KM = K * M, n_q = P->n_q, n_t = P->n_t;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+    // per-warp carve-up
+    const size_t per_warp = (size_t)G * KM * sizeof(double2) + (size_t)G * sizeof(double) + (size_t)G * K * sizeof(int32_t) + (size_t)G * sizeof(int32_t);
+    const size_t per_warp_al = (per_warp + 15) & ~(size_t)15;
+    unsigned char *wbase = smem_raw + warp * per_warp_al;
+    double2 *A = reinterpret_cast<double2 *>(wbase);
+    double *quadS = reinterpret_cast<double *>(A + (size_t)G * KM);
+    int32_t *i0S = reinterpret_cast<int32_t *>(quadS + G);
+    int32_t *badS = i0S + (size_t)G * K;
+
+    const long long groups_per_point = (a.n_per_point + G - 1) / G;
+    const long long n_groups = groups_per_point * a.n_points;
+    const double log_nt = log((double)n_t);
+
+    for (long long grp = (long long)blockIdx.x * DIRECT_WARPS + warp; grp < n_groups; grp += (long long)gridDim.x * DIRECT_WARPS) {
+        const int pt = (int)(grp / groups_per_point);
+        const long long s0 = (grp - (long long)pt * groups_per_point) * G;
+        const int cnt = (int)min((long long)G, a.n_per_point - s0);
+        const long long flat0 = (long long)pt * a.n_per_point + s0;
+        const size_t pglob = (size_t)(a.point0 + pt);
+        const double2 *__restrict__ Qp = a.Q + pglob * (size_t)KM * n_q;
+
+        if (lane < cnt) {
+            const long long s = flat0 + lane;
+            int bad;
+            double q = ile_setup_sample(P, a.U + pglob * (size_t)KM * M, a.V + pglob * (size_t)KM * M, a.ra[s], a.dec[s],
+                                        a.t_ref[s], a.phi_ref[s], a.psi[s], a.incl[s], a.dist[s], A + (size_t)lane * KM,
+                                        i0S + lane * K, &bad);
+            quadS[lane] = q;
+            badS[lane] = bad;
+            if (a.shift_idx)
+                for (int k = 0; k < K; ++k) a.shift_idx[s * K + k] = i0S[lane * K + k];
+            if (bad) atomicAdd(a.oob_counter, 1ULL);
+        }
+        __syncwarp();
+
+        for (int g = 0; g < cnt; ++g) {
+            if (badS[g]) {
+                if (lane == 0) a.lnL[flat0 + g] = -CUDART_INF;
+                continue;
+            }
+            const double2 *Ag = A + (size_t)g * KM;
+            double mx = -CUDART_INF, sm = 0.0;
+            for (int j0 = 0; j0 < n_t; j0 += 32 * DIRECT_RB) {
+                double acc[DIRECT_RB];
+                int jj[DIRECT_RB];
+#pragma unroll
+                for (int r = 0; r < DIRECT_RB; ++r) {
+                    acc[r] = 0.0;
+                    jj[r] = min(j0 + r * 32 + lane, n_t - 1);
+                }
+                for (int k = 0; k < K; ++k) {
+                    const double2 *Qk = Qp + (size_t)k * M * n_q + i0S[g * K + k];
+                    for (int m = 0; m < M; ++m) {
+                        const double2 c = Ag[k * M + m];
+                        const double2 *Qkm = Qk + (size_t)m * n_q;
+#pragma unroll
+                        for (int r = 0; r < DIRECT_RB; ++r) {
+                            double2 q = __ldg(Qkm + jj[r]);
+                            acc[r] = fma(c.x, q.x, fma(c.y, q.y, acc[r]));  // Re(conj(A) Q)
+                        }
+                    }
+                }
+                double cm = -CUDART_INF;
+#pragma unroll
+                for (int r = 0; r < DIRECT_RB; ++r) {
+                    if (j0 + r * 32 + lane >= n_t) acc[r] = -CUDART_INF;
+                    cm = fmax(cm, acc[r]);
+                }
+                double nm = fmax(mx, cm);
+                if (nm > -CUDART_INF) {
+                    double s = sm * exp(mx - nm);
+#pragma unroll
+                    for (int r = 0; r < DIRECT_RB; ++r) s += exp(acc[r] - nm);
+                    sm = s;
+                    mx = nm;
+                }
+            }
+            double Mx = warp_max(mx);
+            double s = (mx > -CUDART_INF) ? sm * exp(mx - Mx) : 0.0;
+            double S = warp_sum(s);
+            if (lane == 0) a.lnL[flat0 + g] = Mx + log(S) - log_nt - quadS[g];
+        }
+        __syncwarp();
+    }
+}
+
+static size_t direct_smem_bytes(const IleSizes &sz, int G)
+{
+    size_t KM = (size_t)sz.n_det * sz.n_modes;
+    size_t per_warp = (size_t)G * KM * sizeof(double2) + (size_t)G * sizeof(double) + (size_t)G * sz.n_det * sizeof(int32_t) + (size_t)G * sizeof(int32_t);
+    per_warp = (per_warp + 15) & ~(size_t)15;
+    return per_warp * DIRECT_WARPS;
+}
+
+cudaError_t ile_launch_eval_direct(const IleSizes &sz, const IleEvalArgs &a, cudaStream_t st, int *n_launches)
+{
+    if (a.n_per_point <= 0 || a.n_points <= 0) return cudaSuccess;
+    int G = 32;
+    while (G > 1 && direct_smem_bytes(sz, G) > 96 * 1024) G >>= 1;
+    size_t smem = direct_smem_bytes(sz, G);
+    if (smem > (size_t)sz.max_smem_optin) return cudaErrorInvalidValue;
+    cudaError_t e = cudaFuncSetAttribute(ile_eval_direct_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    int per_sm = 0;
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ile_eval_direct_kernel, DIRECT_WARPS * 32, smem);
+    if (e != cudaSuccess) return e;
+    if (per_sm < 1) per_sm = 1;
+    long long groups = ((a.n_per_point + G - 1) / G) * a.n_points;
+    long long blocks_needed = (groups + DIRECT_WARPS - 1) / DIRECT_WARPS;
+    long long grid = (long long)sz.sm_count * per_sm;
+    if (blocks_needed < grid) grid = blocks_needed;
+    ile_eval_direct_kernel<<<(unsigned)grid, DIRECT_WARPS * 32, smem, st>>>(a, G);
+    if (n_launches) *n_launches += 1;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// step 7: evidence.  lnZ = ln((1/n) sum_a exp(lnL_a + ln w_a)), max-subtracted; n_eff = sum / max  (eq. 4).
+// Kernel 1: each block reduces one slice of one segment to (max, sum exp(e - max)) with warp shuffles, then a
+// block-level combine.  Kernel 2: one warp per segment folds the partials into the carried state.
+// ------------------------------------------------------------------------------------------------------------
+#define EV_THREADS 256
+
+__global__ void __launch_bounds__(EV_THREADS) ile_evidence_partial_kernel(int64_t n_per_segment, const double *__restrict__ lnL,
+                                                                          const double *__restrict__ log_w,
+                                                                          double *__restrict__ partials)
+{
+    __shared__ double red[EV_THREADS / 32];
+    __shared__ double bmax_s;
+    const int seg = blockIdx.y, B = gridDim.x, b = blockIdx.x;
+    const int64_t len = (n_per_segment + B - 1) / B;
+    const int64_t lo = (int64_t)b * len, hi = min(lo + len, n_per_segment);
+    const double *x = lnL + (int64_t)seg * n_per_segment;
+    const double *w = log_w ? log_w + (int64_t)seg * n_per_segment : nullptr;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+
+    double mx = -CUDART_INF;
+    for (int64_t i = lo + threadIdx.x; i < hi; i += EV_THREADS) {
+        double e = x[i] + (w ? w[i] : 0.0);
+        mx = fmax(mx, e);
+    }
+    mx = warp_max(mx);
+    if (lane == 0) red[warp] = mx;
+    __syncthreads();
+    if (warp == 0) {
+        double v = lane < EV_THREADS / 32 ? red[lane] : -CUDART_INF;
+        v = warp_max(v);
+        if (lane == 0) bmax_s = v;
+    }
+    __syncthreads();
+    const double bmax = bmax_s;
+    double sm = 0.0;
+    if (bmax > -CUDART_INF)
+        for (int64_t i = lo + threadIdx.x; i < hi; i += EV_THREADS) {
+            double e = x[i] + (w ? w[i] : 0.0);
+            sm += exp(e - bmax);
+        }
+    sm = warp_sum(sm);
+    __syncthreads();
+    if (lane == 0) red[warp] = sm;
+    __syncthreads();
+    if (warp == 0) {
+        double v = lane < EV_THREADS / 32 ? red[lane] : 0.0;
+        v = warp_sum(v);
+        if (lane == 0) {
+            partials[((size_t)seg * B + b) * 2 + 0] = bmax;
+            partials[((size_t)seg * B + b) * 2 + 1] = v;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(32) ile_evidence_combine_kernel(int32_t B, int64_t n_per_segment, const double *__restrict__ partials,
+                                                                  double *__restrict__ state, double *__restrict__ lnZ,
+                                                                  double *__restrict__ n_eff)
+{
+    const int seg = blockIdx.x, lane = threadIdx.x;
+    double smax = -CUDART_INF, ssum = 0.0, scount = 0.0;
+    if (state) {
+        smax = state[seg * 3 + 0];
+        ssum = state[seg * 3 + 1];
+        scount = state[seg * 3 + 2];
+    }
+    double mx = -CUDART_INF;
+    for (int b = lane; b < B; b += 32) mx = fmax(mx, partials[((size_t)seg * B + b) * 2]);
+    mx = fmax(warp_max(mx), smax);
+    double sm = 0.0;
+    if (mx > -CUDART_INF) {
+        for (int b = lane; b < B; b += 32) {
+            double bm = partials[((size_t)seg * B + b) * 2], bs = partials[((size_t)seg * B + b) * 2 + 1];
+            if (bm > -CUDART_INF) sm += bs * exp(bm - mx);
+        }
+        sm = warp_sum(sm);
+        if (smax > -CUDART_INF) sm += ssum * exp(smax - mx);
+    }
+    if (lane == 0) {
+        double cnt = scount + (double)n_per_segment;
+        if (state) {
+            state[seg * 3 + 0] = mx;
+            state[seg * 3 + 1] = sm;
+            state[seg * 3 + 2] = cnt;
+        }
+        bool ok = mx > -CUDART_INF;
+        lnZ[seg] = ok ? mx + log(sm) - log(cnt) : -CUDART_INF;
+        if (n_eff) n_eff[seg] = ok ? sm : 0.0;
+    }
+}
+
+__global__ void ile_evidence_reset_kernel(int32_t n_segments, double *state)
+{
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n_segments) {
+        state[i * 3 + 0] = -CUDART_INF;
+        state[i * 3 + 1] = 0.0;
+        state[i * 3 + 2] = 0.0;
+    }
+}
+
+int32_t ile_evidence_blocks_per_segment(int32_t n_segments, int64_t n_per_segment, int32_t sm_count)
+{
+    int64_t want = (n_per_segment + 4095) / 4096;
+    int64_t cap = ((int64_t)sm_count * 8 + n_segments - 1) / n_segments;
+    if (cap < 1) cap = 1;
+    if (want > cap) want = cap;
+    if (want < 1) want = 1;
+    return (int32_t)want;
+}
+
+cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const double *lnL, const double *log_w,
+                                double *state, double *lnZ, double *n_eff, double *partials, int32_t B,
+                                cudaStream_t st, int *n_launches)
+{
+    dim3 grid((unsigned)B, (unsigned)n_segments);
+    ile_evidence_partial_kernel<<<grid, EV_THREADS, 0, st>>>(n_per_segment, lnL, log_w, partials);
+    ile_evidence_combine_kernel<<<(unsigned)n_segments, 32, 0, st>>>(B, n_per_segment, partials, state, lnZ, n_eff);
+    if (n_launches) *n_launches += 2;
+    return cudaGetLastError();
+}
+
+cudaError_t ile_launch_evidence_reset(int32_t n_segments, double *state, cudaStream_t st, int *n_launches)
+{
+    ile_evidence_reset_kernel<<<(n_segments + 127) / 128, 128, 0, st>>>(n_segments, state);
+    if (n_launches) *n_launches += 1;
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// calibration: register-resident DFMA chains (8 independent accumulators per thread)
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) ile_fp64_peak_kernel(int iters, double *sink)
+{
+    double x0 = 1.0 + threadIdx.x * 1e-9, x1 = x0 + 1e-3, x2 = x0 + 2e-3, x3 = x0 + 3e-3, x4 = x0 + 4e-3, x5 = x0 + 5e-3,
+           x6 = x0 + 6e-3, x7 = x0 + 7e-3;
+    const double a = 0.9999999, b = 1e-7;
+    for (int i = 0; i < iters; ++i) {
+        x0 = fma(x0, a, b);
+        x1 = fma(x1, a, b);
+        x2 = fma(x2, a, b);
+        x3 = fma(x3, a, b);
+        x4 = fma(x4, a, b);
+        x5 = fma(x5, a, b);
+        x6 = fma(x6, a, b);
+        x7 = fma(x7, a, b);
+    }
+    double s = ((x0 + x1) + (x2 + x3)) + ((x4 + x5) + (x6 + x7));
+    if (s == 123.456) sink[0] = s;  // never true; keeps the chains alive
+}
+
+cudaError_t ile_launch_fp64_peak(int32_t iters, int32_t sm_count, double *sink, cudaStream_t st)
+{
+    ile_fp64_peak_kernel<<<sm_count * 8, 256, 0, st>>>(iters, sink);
+    return cudaGetLastError();
+}

@@ -1,0 +1,38 @@
+// ile_kernels.h -- host-side launchers of the CUDA kernels (internal; the public boundary is include/ile.h).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "ile_device.cuh"
+
+struct IleEvalArgs {
+    const IleDevParams *params;  // device
+    const double2 *Q;            // device [P][K][M][n_q]
+    const double2 *U, *V;        // device [P][K][M][M]
+    int32_t point0;              // first intrinsic point of this launch
+    int32_t n_points;            // points covered by this launch (1 for ile_eval, P for ile_eval_all)
+    int64_t n_per_point;
+    const double *ra, *dec, *t_ref, *phi_ref, *psi, *incl, *dist;
+    double *lnL;
+    int32_t *shift_idx;                 // may be NULL
+    unsigned long long *oob_counter;    // device, sticky
+};
+
+// Host copy of the sizes every launcher needs.
+struct IleSizes {
+    int32_t n_det, n_modes, n_q, n_t;
+    int32_t sm_count;
+    int32_t max_smem_optin;
+};
+
+// variant 1: direct kernel (one warp per sample, lanes over time bins, Q through L1/L2).  Any size.
+cudaError_t ile_launch_eval_direct(const IleSizes &sz, const IleEvalArgs &a, cudaStream_t st, int *n_launches);
+
+// evidence: two kernels (per-block partials, then per-segment combine with the carried state)
+cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const double *lnL, const double *log_w,
+                                double *state, double *lnZ, double *n_eff, double *partials, int32_t blocks_per_seg,
+                                cudaStream_t st, int *n_launches);
+int32_t ile_evidence_blocks_per_segment(int32_t n_segments, int64_t n_per_segment, int32_t sm_count);
+cudaError_t ile_launch_evidence_reset(int32_t n_segments, double *state, cudaStream_t st, int *n_launches);
+
+cudaError_t ile_launch_fp64_peak(int32_t iters, int32_t sm_count, double *sink, cudaStream_t st);

@@ -1,0 +1,331 @@
+"""GPU-vs-oracle parity through the C ABI (pytest -m gpu, on a B200).
+
+Same seeded inputs go to both sides.  Bar (north_star): shift indices bit-exact as integers; lnL_margT, lnZ, n_eff
+within TOL = 1e-10 * max(|ref|, 1).  Small configs are compared element by element in full; BASELINE.json's full
+sizes are run on the GPU in the launch configuration bench.py times and compared on sampled outputs the oracle
+computes one by one, plus properties that hold at any size.
+"""
+import numpy as np
+import pytest
+
+import ile_inputs as gi
+import oracle
+from parity_util import ORACLE_THREADS, TOL, assert_indices_equal, rel_err, subset
+
+pytestmark = pytest.mark.gpu
+
+
+def to_dev(s):
+    import torch
+
+    return {k: torch.from_numpy(v).cuda() for k, v in s.items()}
+
+
+def run_gpu(ile, cfg, samples, point=0, variant=0):
+    ctx = ile.Context(cfg)
+    if variant:
+        ctx.set_variant(variant)
+    lnL, idx = ctx.eval(to_dev(samples), point=point)
+    n_bad, _ = ctx.status()
+    return ctx, lnL, idx, n_bad
+
+
+def full_compare(ile, cfg, samples, point=0, variant=0, log_w=None):
+    import torch
+
+    ctx, lnL, idx, n_bad = run_gpu(ile, cfg, samples, point, variant)
+    ref, ref_idx, ref_bad = oracle.eval_batch(cfg, samples, point=point, n_threads=ORACLE_THREADS)
+    assert n_bad == ref_bad
+    assert_indices_equal(cfg, samples, ref_idx, idx.cpu().numpy())
+    e = rel_err(ref, lnL.cpu().numpy())
+    assert e <= TOL, f"lnL_margT rel err {e:.3e}"
+    lw = None if log_w is None else torch.from_numpy(log_w).cuda()
+    lnZ, neff = ctx.evidence(lnL, lw)
+    rZ, rN = oracle.evidence(ref, log_w)
+    assert rel_err([rZ], lnZ.cpu().numpy()) <= TOL
+    assert rel_err([rN], neff.cpu().numpy()) <= TOL
+    ctx.close()
+    return e
+
+
+# ---------------------------------------------------------------------------------------------- configs 0, 1
+def test_config0_full(gpu_lib):
+    cfg = gi.make_config(0)
+    s = gi.make_samples(cfg["sample_seeds"][0], cfg["n"])
+    full_compare(gpu_lib, cfg, s)
+
+
+def test_config1_full(gpu_lib):
+    cfg = gi.make_config(1)
+    s = gi.make_samples(cfg["sample_seeds"][0], cfg["n"])
+    full_compare(gpu_lib, cfg, s)
+
+
+def test_config1_concentrated_and_weighted(gpu_lib):
+    cfg = gi.make_config(1)
+    s = gi.make_concentrated_samples(cfg["sample_seeds"][0] + 1, 20_000)
+    lw = gi.make_log_weights(cfg["sample_seeds"][0] + 2, 20_000)
+    full_compare(gpu_lib, cfg, s, log_w=lw)
+
+
+# ---------------------------------------------------------------------------------------------- config 2 (21 modes)
+def test_config2_small_elementwise(gpu_lib):
+    cfg = gi.make_config(2)
+    s = gi.make_samples(cfg["sample_seeds"][0], 3_001)       # several tiles and a ragged tail
+    full_compare(gpu_lib, cfg, s)
+
+
+def test_config2_full_size_sampled(gpu_lib):
+    cfg = gi.make_config(2)
+    n = cfg["n"]
+    s = gi.make_samples(cfg["sample_seeds"][0], n)
+    ctx, lnL, idx, n_bad = run_gpu(gpu_lib, cfg, s)
+    assert n_bad == 0
+    sel = np.random.default_rng(2).choice(n, 4_000, replace=False)
+    sel = np.concatenate([sel, [0, 1, n - 2, n - 1]])
+    ref, ref_idx, _ = oracle.eval_batch(cfg, subset(s, sel), n_threads=ORACLE_THREADS)
+    got = lnL.cpu().numpy()
+    assert_indices_equal(cfg, subset(s, sel), ref_idx, idx.cpu().numpy()[sel])
+    assert rel_err(ref, got[sel]) <= TOL
+    assert np.all(np.isfinite(got))
+    # property at full size: lnL_margT <= max_j lnL_j <= the Cauchy-Schwarz bound is not available without the
+    # oracle; what holds at any size is chunking invariance of the evidence (below) and finiteness (above).
+    lnZ, neff = ctx.evidence(lnL)
+    st = ctx.new_state()
+    for lo in range(0, n, 300_000):
+        lnZc, neffc = ctx.evidence(lnL[lo:lo + 300_000].contiguous(), state=st)
+    assert rel_err(lnZ.cpu().numpy(), lnZc.cpu().numpy()) <= TOL
+    assert rel_err(neff.cpu().numpy(), neffc.cpu().numpy()) <= TOL
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------- config 3 (batch sweep)
+@pytest.mark.parametrize("n", [1_000, 10_000, 100_000])
+def test_config3_sweep_elementwise(gpu_lib, n):
+    cfg = gi.make_config(3, n=n)
+    s = gi.make_samples(cfg["sample_seeds"][0], n)
+    full_compare(gpu_lib, cfg, s)
+
+
+def test_config3_1e6_evidence_parity(gpu_lib):
+    cfg = gi.make_config(3, n=1_000_000)
+    s = gi.make_samples(cfg["sample_seeds"][0], cfg["n"])
+    full_compare(gpu_lib, cfg, s)
+
+
+def test_config3_1e7_chunked_from_one_stream(gpu_lib):
+    """Largest batch: processed in chunks on one stream with the evidence state carried on the device."""
+    import torch
+
+    cfg = gi.make_config(3)
+    n, chunk = cfg["n"], 1_000_000
+    s = gi.make_samples(cfg["sample_seeds"][0], n)
+    ctx = gpu_lib.Context(cfg)
+    st = ctx.new_state()
+    out = torch.empty(n, dtype=torch.float64, device="cuda")
+    for lo in range(0, n, chunk):
+        d = to_dev(subset(s, slice(lo, lo + chunk)))
+        ctx.eval(d, want_idx=False, out=out[lo:lo + chunk])
+        lnZc, neffc = ctx.evidence(out[lo:lo + chunk], state=st)
+    n_bad, _ = ctx.status()
+    assert n_bad == 0
+    lnZ, neff = ctx.evidence(out)
+    assert rel_err(lnZ.cpu().numpy(), lnZc.cpu().numpy()) <= TOL
+    assert rel_err(neff.cpu().numpy(), neffc.cpu().numpy()) <= TOL
+    assert abs(st.cpu().numpy()[0, 2] - n) == 0
+    sel = np.random.default_rng(3).choice(n, 20_000, replace=False)
+    ref, _, _ = oracle.eval_batch(cfg, subset(s, sel), n_threads=ORACLE_THREADS)
+    assert rel_err(ref, out.cpu().numpy()[sel]) <= TOL
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------- config 4 (many points)
+def test_config4_small_all_points_elementwise(gpu_lib):
+    import torch
+
+    cfg = gi.make_config(4, n=777, n_points=5)
+    P, n = cfg["n_points"], cfg["n"]
+    per = [gi.make_samples(cfg["sample_seeds"][p], n) for p in range(P)]
+    allS = {k: np.ascontiguousarray(np.stack([per[p][k] for p in range(P)])) for k in per[0]}
+    ctx = gpu_lib.Context(cfg)
+    lnL, idx = ctx.eval_all(to_dev(allS), want_idx=True)
+    lnZ, neff = ctx.evidence(lnL, n_segments=P)
+    for p in range(P):
+        ref, ref_idx, _ = oracle.eval_batch(cfg, per[p], point=p, n_threads=ORACLE_THREADS)
+        assert_indices_equal(cfg, per[p], ref_idx, idx[p].cpu().numpy())
+        assert rel_err(ref, lnL[p].cpu().numpy()) <= TOL
+        rZ, rN = oracle.evidence(ref)
+        assert rel_err([rZ], lnZ[p:p + 1].cpu().numpy()) <= TOL
+        assert rel_err([rN], neff[p:p + 1].cpu().numpy()) <= TOL
+        # single-point entry gives the same numbers as the all-points launch
+        one, _ = ctx.eval(to_dev(per[p]), point=p, want_idx=False)
+        assert torch.equal(one, lnL[p])
+    ctx.close()
+
+
+def test_config4_full_size_sampled(gpu_lib):
+    import torch
+
+    cfg = gi.make_config(4)
+    P, n = cfg["n_points"], cfg["n"]
+    ctx = gpu_lib.Context(cfg)
+    dev = {k: torch.empty((P, n), dtype=torch.float64, device="cuda") for k in gi.SAMPLE_FIELDS}
+    check_pts = [0, 17, 128, 255]
+    kept = {}
+    for p in range(P):
+        s = gi.make_samples(cfg["sample_seeds"][p], n)
+        if p in check_pts:
+            kept[p] = s
+        for k in gi.SAMPLE_FIELDS:
+            dev[k][p].copy_(torch.from_numpy(s[k]))
+    lnL, _ = ctx.eval_all(dev)
+    lnZ, neff = ctx.evidence(lnL, n_segments=P)
+    n_bad, _ = ctx.status()
+    assert n_bad == 0
+    for p in check_pts:
+        ref, _, _ = oracle.eval_batch(cfg, kept[p], point=p, n_threads=ORACLE_THREADS)
+        assert rel_err(ref, lnL[p].cpu().numpy()) <= TOL
+        rZ, rN = oracle.evidence(ref)
+        assert rel_err([rZ], lnZ[p:p + 1].cpu().numpy()) <= TOL
+        assert rel_err([rN], neff[p:p + 1].cpu().numpy()) <= TOL
+    assert torch.isfinite(lnZ).all()
+    ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------- edge cases
+def test_edge_empty_one_and_ragged(gpu_lib):
+    import torch
+
+    cfg = gi.make_config(0)
+    ctx = gpu_lib.Context(cfg)
+    empty = {k: torch.empty(0, dtype=torch.float64, device="cuda") for k in gi.SAMPLE_FIELDS}
+    lnL, idx = ctx.eval(empty)
+    assert lnL.numel() == 0
+    ctx.close()
+    for n in (1, 31, 33, 255, 257):
+        s = gi.make_samples(99 + n, n)
+        full_compare(gpu_lib, cfg, s)
+
+
+def test_edge_out_of_range_windows(gpu_lib):
+    cfg = gi.make_config(0)
+    s = gi.make_samples(5, 64)
+    s["t_ref"][3] = 0.2
+    s["t_ref"][40] = -0.2
+    s["t_ref"][63] = 0.124   # window end beyond N_Q
+    ctx, lnL, idx, n_bad = run_gpu(gpu_lib, cfg, s)
+    ref, ref_idx, ref_bad = oracle.eval_batch(cfg, s)
+    assert n_bad == ref_bad and ref_bad >= 2
+    assert_indices_equal(cfg, s, ref_idx, idx.cpu().numpy())
+    assert rel_err(ref, lnL.cpu().numpy()) <= TOL
+    lnZ, neff = ctx.evidence(lnL)
+    rZ, rN = oracle.evidence(ref)
+    assert rel_err([rZ], lnZ.cpu().numpy()) <= TOL
+    n_bad2, code = ctx.status(reset=True)
+    assert n_bad2 == ref_bad and code == -5
+    assert ctx.status() == (0, 0)
+    ctx.close()
+
+
+def test_edge_all_out_of_range_gives_minus_inf_evidence(gpu_lib):
+    cfg = gi.make_config(0)
+    s = gi.make_samples(6, 40)
+    s["t_ref"][:] = 0.3
+    ctx, lnL, idx, n_bad = run_gpu(gpu_lib, cfg, s)
+    assert n_bad == 40
+    lnZ, neff = ctx.evidence(lnL)
+    assert lnZ.item() == -np.inf and neff.item() == 0.0
+    assert oracle.evidence(oracle.eval_batch(cfg, s)[0]) == (-np.inf, 0.0)
+    ctx.close()
+
+
+def test_edge_asymmetric_U_and_generic_V(gpu_lib):
+    """Reading R15: U is not assumed Hermitian, V not assumed symmetric."""
+    cfg = gi.make_config(1, n=500)
+    rng = np.random.default_rng(8)
+    cfg["U"] = cfg["U"] * (1.0 + 0.3 * rng.standard_normal(cfg["U"].shape)) + 50j * rng.standard_normal(cfg["U"].shape)
+    cfg["V"] = cfg["V"] + 30.0 * (rng.standard_normal(cfg["V"].shape) + 1j * rng.standard_normal(cfg["V"].shape))
+    s = gi.make_samples(77, 500)
+    full_compare(gpu_lib, cfg, s)
+
+
+@pytest.mark.parametrize("n_t", [1, 2, 32, 33, 128, 129, 1000])
+def test_edge_window_lengths(gpu_lib, n_t):
+    cfg = gi.make_config(0, n=300)
+    cfg["n_t"] = n_t
+    s = gi.make_samples(123, 300)
+    if n_t == 1000:
+        s["t_ref"] = s["t_ref"] * 0.0   # the window nearly fills Q: only small shifts stay in range
+    full_compare(gpu_lib, cfg, s)
+
+
+def test_edge_window_equals_series(gpu_lib):
+    """N_t = N_Q with a detector at the geocentre: the only in-range window is the whole series."""
+    cfg = gi.make_config(0, n=64)
+    cfg["n_t"] = cfg["n_q"]
+    cfg["vertex_m"] = np.zeros_like(cfg["vertex_m"])
+    s = gi.make_samples(321, 64)
+    s["t_ref"][:] = 0.0
+    s["t_ref"][7] = 1.0 / 4096.0   # one sample off: out of range
+    ctx, lnL, idx, n_bad = run_gpu(gpu_lib, cfg, s)
+    ref, ref_idx, ref_bad = oracle.eval_batch(cfg, s)
+    assert n_bad == ref_bad == 1
+    assert_indices_equal(cfg, s, ref_idx, idx.cpu().numpy())
+    assert rel_err(ref, lnL.cpu().numpy()) <= TOL
+    ctx.close()
+
+
+def test_edge_single_detector_single_mode_and_max_sizes(gpu_lib):
+    rng = np.random.default_rng(4)
+    # K = 1, M = 1
+    cfg = gi.make_config(0, n=100)
+    one = dict(cfg)
+    one.update(n_det=1, n_modes=1, Q=np.ascontiguousarray(cfg["Q"][:, :1, :1]), U=np.ascontiguousarray(cfg["U"][:, :1, :1, :1]),
+               V=np.ascontiguousarray(cfg["V"][:, :1, :1, :1]), l=cfg["l"][:1], m=cfg["m"][:1], vertex_m=cfg["vertex_m"][:1],
+               arm_x=cfg["arm_x"][:1], arm_y=cfg["arm_y"][:1])
+    full_compare(gpu_lib, one, gi.make_samples(11, 100))
+    # K = ILE_MAX_DET = 8 detectors, M = ILE_MAX_MODES = 32 modes (l = 2..5 truncated), generic complex inputs
+    K, M, n_q = 8, 32, 512
+    modes = gi.modes_up_to(5)[:M]
+    big = dict(n_points=1, n_det=K, n_modes=M, n_q=n_q, n_t=65, fs_hz=4096.0, t0_q_s=-n_q / 8192.0, gmst_rad=1.0,
+               d_ref_mpc=100.0, l=np.array([x[0] for x in modes], dtype=np.int32), m=np.array([x[1] for x in modes], dtype=np.int32),
+               Q=(rng.standard_normal((1, K, M, n_q)) + 1j * rng.standard_normal((1, K, M, n_q))) * 3.0,
+               U=(rng.standard_normal((1, K, M, M)) + 1j * rng.standard_normal((1, K, M, M))),
+               V=(rng.standard_normal((1, K, M, M)) + 1j * rng.standard_normal((1, K, M, M))),
+               vertex_m=6.0e6 * rng.standard_normal((K, 3)) / np.sqrt(3.0), arm_x=np.tile(cfg["arm_x"][:1], (K, 1)),
+               arm_y=np.tile(cfg["arm_y"][:1], (K, 1)))
+    s = gi.make_samples(12, 200)
+    s["t_ref"] *= 0.2
+    full_compare(gpu_lib, big, s)
+
+
+def test_psi_plus_pi_invariance_on_gpu(gpu_lib):
+    cfg = gi.make_config(1, n=4096)
+    s = gi.make_samples(31, 4096)
+    ctx = gpu_lib.Context(cfg)
+    a, ia = ctx.eval(to_dev(s))
+    s2 = dict(s)
+    s2["psi"] = s["psi"] + np.pi
+    b, ib = ctx.eval(to_dev(s2))
+    assert (ia == ib).all()
+    assert rel_err(a.cpu().numpy(), b.cpu().numpy()) <= 1e-11
+    ctx.close()
+
+
+def test_run_host_matches_device_path(gpu_lib):
+    import torch
+
+    cfg = gi.make_config(1, n=50_000)
+    s = gi.make_samples(cfg["sample_seeds"][0], cfg["n"])
+    lw = gi.make_log_weights(5, cfg["n"])
+    ctx = gpu_lib.Context(cfg)
+    host = {k: torch.from_numpy(v).pin_memory() for k, v in s.items()}
+    out, lnZ, neff = ctx.run_host(host, torch.from_numpy(lw).pin_memory())
+    ref, _, _ = oracle.eval_batch(cfg, s, n_threads=ORACLE_THREADS)
+    rZ, rN = oracle.evidence(ref, lw)
+    assert rel_err(ref, out.numpy()) <= TOL
+    assert rel_err([rZ], [lnZ]) <= TOL and rel_err([rN], [neff]) <= TOL
+    out2, lnZ2, _ = ctx.run_host(host, None, want_lnL=False)
+    assert out2 is None and rel_err([oracle.evidence(ref)[0]], [lnZ2]) <= TOL
+    assert ctx.launch_count >= 6
+    ctx.close()
