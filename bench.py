@@ -1,0 +1,301 @@
+#!/usr/bin/env python
+"""bench.py -- the driver's benchmark contract for the ILE hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config C] [--variant V]
+
+A "step" is one pass of the whole hot path (ile_eval + ile_evidence) over one batch of
+synthetic extrinsic samples.  Default workload: BASELINE.json configs[1] -- 3 detectors (H1, L1, V1), the five l = 2
+modes, Q of 2048 complex128 samples at 4096 Hz per (detector, mode), 100,000 prior-drawn extrinsic samples, 410 time
+bins.  Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+
+N > 1 (torchrun): the paper's own parallelism is independent workers, one GPU each, no communication
+(PAPER.md L134-L141), so each rank evaluates its own seeded intrinsic point and batch; there is no data-path
+collective; `value` = samples of all ranks / max-over-ranks device time ("scaling": "weak").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "time-marginalized ILE lnL samples/sec (3 det, l<=2)"
+UNIT = "samples/s"
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# algorithmic work per sample in DFMA-equivalents
+# ------------------------------------------------------------------------------------------------------------------
+EXP_DFMA = 21.7      # measured on B200: CUDA exp(double) costs 21.7 DFMA issue slots (profiles/r01_microbench.md)
+LSE_MISC = 5.0       # per bin: two detector adds, max, subtract, accumulate
+
+
+def dfma_per_sample(K: int, M: int, n_t: int) -> float:
+    linear = 2.0 * K * M * n_t                      # step 5: Re sum conj(A) Q, 2 DFMA per complex element
+    quad = 2.0 * K * (4.0 * M * M + 4.0 * M)        # step 4: Y^dagger U Y and Y^T V Y per detector
+    lse = n_t * (EXP_DFMA + LSE_MISC)               # step 6
+    geom = 400.0 + 30.0 * M                         # steps 1-3: five sincos, F_k, dt_k, Y_lm, K*M coefficient products
+    return linear + quad + lse + geom
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index: int, period_s: float = 0.005):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period_s
+        self.samples, self.reasons, self.stop_flag = [], set(), False
+        self.max_mhz = None
+        try:
+            import pynvml
+
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    def run(self):
+        if self.nv is None:
+            return
+        nv = self.nv
+        names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown", nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
+                 nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown", nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
+                 nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        while not self.stop_flag:
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, nm in names.items():
+                    if r & bit:
+                        self.reasons.add(nm)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "n_samples": 0}
+        s = sorted(self.samples)
+        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "n_samples": len(s)}
+
+
+def read_traffic_bytes():
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    try:
+        return json.load(open(p)).get("dram_bytes_per_launch")
+    except Exception:
+        return None
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# reference arm: the CPU oracle, as it stands, on the host cores
+# ------------------------------------------------------------------------------------------------------------------
+def run_reference(args, rank: int):
+    if rank != 0:
+        return
+    import ile_inputs as gi
+    import oracle
+
+    cores = os.cpu_count() or 1
+    cfg = gi.make_config(args.config, n_points=1)
+    n_step = min(cfg["n"], args.ref_samples_per_step)
+    s = gi.make_samples(cfg["sample_seeds"][0], n_step)
+    for _ in range(args.warmup):
+        out, _, _ = oracle.eval_batch(cfg, s, n_threads=cores)
+        oracle.evidence(out)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        out, _, _ = oracle.eval_batch(cfg, s, n_threads=cores)
+        oracle.evidence(out)
+    dt = time.perf_counter() - t0
+    val = n_step * args.steps / dt
+    sample = f"{n_step} of the {cfg['n']} samples of the workload per step, {args.steps} steps, OpenMP over samples"
+    line = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": dt / args.steps * 1e3, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": workload_config(cfg, n_step, args, extra={"note": "CPU oracle (oracle/ile_oracle.c) on host cores"}),
+            "cpu_baseline": {"value": val, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def workload_config(cfg, n, args, extra=None):
+    c = {"workload": f"BASELINE.json configs[{cfg['config_id']}]: {cfg['n_det']} detectors ({','.join(cfg['dets'])}), "
+                     f"{cfg['n_modes']} modes (l<= {int(max(cfg['l']))}), Q {cfg['n_q']} complex128 @ {int(cfg['fs_hz'])} Hz, "
+                     f"{n} extrinsic samples/step/GPU, {cfg['n_t']} time bins",
+         "n_det": cfg["n_det"], "n_modes": cfg["n_modes"], "n_q": cfg["n_q"], "n_t": cfg["n_t"], "samples_per_step_per_gpu": n,
+         "parallelism": f"independent intrinsic points, 1 per GPU x{args.gpus}", "l2": "flushed between timed steps (256 MiB write)"}
+    if extra:
+        c.update(extra)
+    return c
+
+
+# ------------------------------------------------------------------------------------------------------------------
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=1)
+    ap.add_argument("--n", type=int, default=None, help="samples per step per GPU (default: the config's)")
+    ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--samples", default="prior", choices=["prior", "concentrated"])
+    ap.add_argument("--ref-samples-per-step", type=int, default=100_000)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        if args.steps > 20:
+            args.steps = 20
+        run_reference(args, rank)
+        return
+
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    import ile_inputs as gi
+    import paper_1902_04934_b200 as ile
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    ile.load()
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    # ---- workload: one intrinsic point and one batch per rank (independent workers)
+    base = gi.make_config(args.config, n_points=1)
+    n = args.n if args.n is not None else base["n"]
+    if rank > 0:  # a different seeded intrinsic point per rank, same recipe
+        c = gi.CONFIGS[args.config]
+        snr = c["snr"] if not isinstance(c["snr"], tuple) else 20.0
+        Q, U, V, meta = gi.make_point(gi.point_seed(args.config, 0) + 7919 * rank, c["dets"], c["modes"], c["n_q"], snr, admix=c["admix"])
+        base["Q"], base["U"], base["V"] = Q[None], U[None], V[None]
+    seed = base["sample_seeds"][0] + 7919 * rank
+    s_np = gi.make_samples(seed, n) if args.samples == "prior" else gi.make_concentrated_samples(seed, n)
+    ctx = ile.Context(base)
+    if args.variant:
+        ctx.set_variant(args.variant)
+    dev = ile.samples_to_device(s_np)
+    host = {k: torch.from_numpy(v).pin_memory() for k, v in s_np.items()}
+    host_out = torch.empty(n, dtype=torch.float64).pin_memory()
+    lnL = torch.empty(n, dtype=torch.float64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def step():
+        ctx.eval(dev, want_idx=False, out=lnL)
+        return ctx.evidence(lnL)
+
+    for _ in range(args.warmup):
+        flush.fill_(1)
+        step()
+        ctx.run_host(host, None, out_host=host_out)
+    torch.cuda.synchronize()
+
+    peak_tflops, _ = ile.measure_fp64_peak(1 << 15)
+
+    # ---- timed region: exactly K steps, device-timed with CUDA events on the launching stream
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+          for _ in range(args.steps)]
+    sampler = ClockSampler(local_rank)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    launches0 = ctx.launch_count
+    sampler.start()
+    wall0 = time.perf_counter()
+    for i in range(args.steps):
+        flush.fill_(i & 1)                      # L2 flush, outside the event pair
+        ev[i][0].record(stream)
+        ctx.eval(dev, want_idx=False, out=lnL)
+        ev[i][1].record(stream)
+        lnZ, neff = ctx.evidence(lnL)
+        ev[i][2].record(stream)
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - wall0
+    sampler.stop_flag = True
+    launches = ctx.launch_count - launches0
+    if world > 1:
+        dist.barrier()
+    step_ms = sum(a.elapsed_time(c) for a, _, c in ev)
+    eval_ms = sum(a.elapsed_time(b) for a, b, _ in ev)
+    n_bad, _ = ctx.status()
+
+    # ---- end to end through the C ABI with HOST buffers (ile_run_host): H2D + kernels + D2H inside the timed region
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    for i in range(args.steps):
+        _, lnZ_h, neff_h = ctx.run_host(host, None, out_host=host_out)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    e2e_ms = e0.elapsed_time(e1)
+    e2e_wall = time.perf_counter() - t0
+    e2e_ms = max(e2e_ms, e2e_wall * 1e3)        # the call synchronises: wall clock and device time agree; take the larger
+
+    t = torch.tensor([step_ms, eval_ms, e2e_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    step_ms, eval_ms, e2e_ms = (float(x) for x in t.cpu())
+
+    if rank == 0:
+        K, M, n_t = base["n_det"], base["n_modes"], base["n_t"]
+        w = dfma_per_sample(K, M, n_t)
+        value = world * n * args.steps / (step_ms * 1e-3)
+        eval_avg_ms = eval_ms / args.steps
+        achieved = 2.0 * w * n / (eval_avg_ms * 1e-3) * 1e-12
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": step_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": workload_config(base, n, args, extra={"variant": args.variant, "samples": args.samples}),
+            "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+                         "traffic": read_traffic_bytes(), "kernel": "ile_eval (steps 1-6)", "kernel_ms": eval_avg_ms,
+                         "dfma_equiv_per_sample": w, "peak_source": "ile_measure_fp64_peak: register-resident DFMA chains, measured in this run "
+                         "(nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2 TFLOP/s)"},
+            "e2e": {"value": world * n * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 7 * 8 * n,
+                    "d2h_bytes_per_step": 8 * n + 16, "ms_per_step": e2e_ms / args.steps, "api": "ile_run_host (pinned host buffers)"},
+            "gpu_launches": int(launches), "clocks": sampler.summary(), "wall_ms_per_step": wall / args.steps * 1e3,
+            "lnZ": float(lnZ.item()), "n_eff": float(neff.item()), "n_out_of_range": int(n_bad),
+        }
+        if not args.no_cpu_baseline:
+            import oracle  # cpu_baseline leg: the one place bench.py's product arm may execute oracle/
+
+            cores = os.cpu_count() or 1
+            n_cpu = min(n, 100_000)
+            sub = {k: v[:n_cpu] for k, v in s_np.items()}
+            passes = 4
+            oracle.eval_batch(base, {k: v[:2000] for k, v in s_np.items()}, n_threads=cores)  # page in / spin up
+            t0 = time.perf_counter()
+            for _ in range(passes):
+                ref, _, _ = oracle.eval_batch(base, sub, n_threads=cores)
+                rZ, _ = oracle.evidence(ref)
+            dt = time.perf_counter() - t0
+            line["cpu_baseline"] = {"value": n_cpu * passes / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                    "sample": f"{passes} passes over the first {n_cpu} samples of the same batch (eval + evidence), OpenMP over samples",
+                                    "lnZ_oracle": rZ if n_cpu == n else None}
+        print(json.dumps(line), flush=True)
+    ctx.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
