@@ -96,6 +96,7 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     c->sz.n_t = cfg->n_t;
     c->sz.sm_count = prop.multiProcessorCount;
     c->sz.max_smem_optin = (int32_t)prop.sharedMemPerBlockOptin;
+    c->sz.smem_per_sm = (int32_t)prop.sharedMemPerMultiprocessor;
     c->n_points = cfg->n_points;
 
     IleDevParams &P = c->hparams;
@@ -181,7 +182,9 @@ static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n
     a.shift_idx = shift_idx;
     a.oob_counter = c->d_oob;
     int nl = 0;
-    cudaError_t e = ile_launch_eval_direct(c->sz, a, st, &nl);
+    IleTiledLayout L;
+    const bool tiled = c->variant == 2 || (c->variant == 0 && ile_tiled_plan(c->sz, (long long)n * n_points, &L));
+    cudaError_t e = tiled ? ile_launch_eval_tiled(c->sz, a, st, &nl) : ile_launch_eval_direct(c->sz, a, st, &nl);
     c->launches += nl;
     if (e != cudaSuccess) return cuda_fail(e);
     return ILE_OK;
@@ -295,7 +298,11 @@ extern "C" int ile_status(ile_ctx *c, int64_t *n_out_of_range, int reset, void *
 extern "C" int ile_set_variant(ile_ctx *c, int32_t variant)
 {
     if (!c || variant < 0) return ILE_ERR_BAD_ARGUMENT;
-    if (variant > 1) return ILE_ERR_UNSUPPORTED;
+    if (variant > 2) return ILE_ERR_UNSUPPORTED;
+    if (variant == 2) {
+        IleTiledLayout L;
+        if (!ile_tiled_plan(c->sz, 1LL << 40, &L)) return ILE_ERR_UNSUPPORTED;
+    }
     c->variant = variant;
     return ILE_OK;
 }

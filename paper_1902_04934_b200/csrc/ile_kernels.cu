@@ -4,79 +4,10 @@
 //   ile_evidence_*           step 7 (eq. 4; n_eff L101)
 //   ile_fp64_peak_kernel     calibration of the FP64 FMA roofline
 //
-// The tuned evaluation kernels live in ile_eval_tuned.cu.
+// The tuned evaluation kernel lives in ile_eval_tiled.cu.
 #include <math_constants.h>
 
 #include "ile_kernels.h"
-
-// ------------------------------------------------------------------------------------------------------------
-// per-sample setup, one THREAD per sample (no redundant geometry across a warp)
-// ------------------------------------------------------------------------------------------------------------
-// On return: A[k*M + m] = (D_ref/D) F_k Y_m (so that lin_j = Re sum conj(A) Q), i0[k] = window start,
-// returns quad = (a^2/4) sum_k [|F_k|^2 Re(Y^dagger U_k Y) + Re(F_k^2 Y^T V_k Y)]  (eq. 7; do not assume U Hermitian: R15).
-// *bad is set when a window leaves [0, n_q) (reading R9).
-__device__ double ile_setup_sample(const IleDevParams *__restrict__ P, const double2 *__restrict__ U,
-                                   const double2 *__restrict__ V, double ra, double dec, double t_ref, double phi_ref,
-                                   double psi, double incl, double dist, double2 *A, int32_t *i0, int *bad)
-{
-    const int K = P->n_det, M = P->n_modes;
-    IleSky g = ile_sky(ra, dec, psi, P->gmst);
-    double sh, ch;
-    sincos(0.5 * incl, &sh, &ch);
-    const double a = P->d_ref / dist;
-    for (int m = 0; m < M; ++m) A[m] = ile_ylm(P, m, ch, sh, phi_ref);  // Y_m, parked in the k = 0 slots
-
-    double tot = 0.0;
-    int oob = 0;
-    for (int k = 0; k < K; ++k) {
-        double2 F = ile_antenna(P->det_tensor[k], g);
-        double yuy = 0.0;
-        double2 yvy = make_double2(0.0, 0.0);
-        for (int p = 0; p < M; ++p) {
-            double2 tu = make_double2(0.0, 0.0), tv = make_double2(0.0, 0.0);
-            const double2 *Ur = U + ((size_t)k * M + p) * M;
-            const double2 *Vr = V + ((size_t)k * M + p) * M;
-            for (int q = 0; q < M; ++q) {
-                double2 Yq = A[q], u = __ldg(Ur + q), v = __ldg(Vr + q);
-                tu.x += u.x * Yq.x - u.y * Yq.y;
-                tu.y += u.x * Yq.y + u.y * Yq.x;
-                tv.x += v.x * Yq.x - v.y * Yq.y;
-                tv.y += v.x * Yq.y + v.y * Yq.x;
-            }
-            double2 Yp = A[p];
-            yuy += Yp.x * tu.x + Yp.y * tu.y;  // Re(conj(Y_p) (U Y)_p)
-            double2 t = ile_cmul(Yp, tv);
-            yvy.x += t.x;
-            yvy.y += t.y;
-        }
-        double F2 = F.x * F.x + F.y * F.y;
-        double2 FF = ile_cmul(F, F);
-        tot += F2 * yuy + (FF.x * yvy.x - FF.y * yvy.y);
-        int32_t idx = ile_window_index(P->vertex[k], g, t_ref, P->t0_q, P->fs, P->n_t);
-        i0[k] = idx;
-        if (idx < 0 || (long long)idx + P->n_t > P->n_q) oob = 1;
-    }
-    for (int k = K - 1; k >= 0; --k) {  // k = 0 last: it overwrites the parked Y_m in place
-        double2 F = ile_antenna(P->det_tensor[k], g);
-        double2 aF = make_double2(a * F.x, a * F.y);
-        for (int m = 0; m < M; ++m) A[k * M + m] = ile_cmul(aF, A[m]);
-    }
-    *bad = oob;
-    return 0.25 * a * a * tot;
-}
-
-__device__ __forceinline__ double warp_max(double v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v = fmax(v, __shfl_xor_sync(0xffffffffu, v, o));
-    return v;
-}
-__device__ __forceinline__ double warp_sum(double v)
-{
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-    return v;
-}
 
 // ------------------------------------------------------------------------------------------------------------
 // variant 1: direct kernel.  A warp takes G samples at a time: lane g sets up sample g (steps 1-4), then the
@@ -118,7 +49,7 @@ __global__ void __launch_bounds__(DIRECT_WARPS * 32) ile_eval_direct_kernel(IleE
             const long long s = flat0 + lane;
             int bad;
             double q = ile_setup_sample(P, a.U + pglob * (size_t)KM * M, a.V + pglob * (size_t)KM * M, a.ra[s], a.dec[s],
-                                        a.t_ref[s], a.phi_ref[s], a.psi[s], a.incl[s], a.dist[s], A + (size_t)lane * KM,
+                                        a.t_ref[s], a.phi_ref[s], a.psi[s], a.incl[s], a.dist[s], A + (size_t)lane * KM, M,
                                         i0S + lane * K, &bad);
             quadS[lane] = q;
             badS[lane] = bad;

@@ -22,11 +22,26 @@ struct IleEvalArgs {
 struct IleSizes {
     int32_t n_det, n_modes, n_q, n_t;
     int32_t sm_count;
-    int32_t max_smem_optin;
+    int32_t max_smem_optin;  // largest dynamic shared memory one block may ask for
+    int32_t smem_per_sm;     // shared memory of one SM
+};
+
+// Shared-memory carve-up of the tiled kernel (byte offsets), computed on the host and passed by value.
+struct IleTiledLayout {
+    int32_t mg;        // modes per group (template parameter of the kernel)
+    int32_t n_groups;  // G = ceil(M / mg)
+    int32_t S;         // samples per tile, <= 32
+    int32_t ldl;       // row stride of lin in doubles
+    uint32_t off_A, off_lin, off_quad, off_i0, off_bad, off_misc;
+    uint32_t bytes;
 };
 
 // variant 1: direct kernel (one warp per sample, lanes over time bins, Q through L1/L2).  Any size.
 cudaError_t ile_launch_eval_direct(const IleSizes &sz, const IleEvalArgs &a, cudaStream_t st, int *n_launches);
+
+// variant 2: tiled, Q-stationary kernel (ile_eval_tiled.cu).  ile_tiled_plan returns false when the sizes do not fit.
+bool ile_tiled_plan(const IleSizes &sz, long long n_total, IleTiledLayout *out);
+cudaError_t ile_launch_eval_tiled(const IleSizes &sz, const IleEvalArgs &a, cudaStream_t st, int *n_launches);
 
 // evidence: two kernels (per-block partials, then per-segment combine with the carried state)
 cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const double *lnL, const double *log_w,
