@@ -184,7 +184,7 @@ static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n
     int nl = 0;
     IleTiledLayout L;
     const bool tiled = c->variant == 2 || (c->variant == 0 && ile_tiled_plan(c->sz, (long long)n * n_points, &L));
-    cudaError_t e = tiled ? ile_launch_eval_tiled(c->sz, a, st, &nl) : ile_launch_eval_direct(c->sz, a, st, &nl);
+    cudaError_t e = tiled ? ile_launch_eval_tiled(c->sz, c->hparams, a, st, &nl) : ile_launch_eval_direct(c->sz, a, st, &nl);
     c->launches += nl;
     if (e != cudaSuccess) return cuda_fail(e);
     return ILE_OK;

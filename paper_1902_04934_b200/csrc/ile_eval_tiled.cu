@@ -11,16 +11,17 @@
 // by exactly one thread per phase.  A last pass does the max-subtracted log-sum-exp over each row (eq. 9),
 // one warp per sample, row in registers, warp-shuffle reductions.
 //
-// Per tile of S <= 32 samples:  setup (warp 0, lane = sample: steps 1-4)  ->  K*G accumulation phases  ->  LSE pass.
+// Per tile of S <= 32 samples:  setup (lane = sample: steps 1-4)  ->  K*G accumulation phases  ->  LSE pass.
+// The setup of tile t+1 runs in a ninth, producer warp while the eight consumer warps work on tile t; its outputs
+// (A, i0, quad, flags, index ranges, chunk counters) are double-buffered and handed over with named barriers.
 #include <limits.h>
 #include <math_constants.h>
 
 #include "ile_kernels.h"
 
-#define TILED_WARPS 8
-#define TILED_THREADS (TILED_WARPS * 32)
+#define TILED_CWARPS 8                         /* consumer warps: accumulation phases and the LSE pass */
+#define TILED_THREADS ((TILED_CWARPS + 1) * 32) /* + one producer warp: per-sample setup of the next tile */
 #define TILED_CHUNK 64
-#define TILED_ROW_REGS 16 /* LSE pass keeps a row of up to 32 * 16 bins in registers */
 
 // exp(x) for x <= 0 (max-subtracted arguments): Cody-Waite reduction x = k ln2 + r, |r| <= ln2/2, degree-11
 // near-minimax polynomial (Chebyshev-node interpolant, relative error 1.7e-17 before rounding), exponent patched in
@@ -49,40 +50,174 @@ __device__ __forceinline__ double ile_exp_nonpos(double x)
     return x < -708.0 ? 0.0 : res;
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// named barriers (PTX bar.sync / bar.arrive): producer warp <-> consumer warps hand-off of the per-tile setup
+// ------------------------------------------------------------------------------------------------------------
+#define BAR_FULL0 1  /* +b: setup buffer b written (producer arrives, consumers wait)   */
+#define BAR_EMPTY0 3 /* +b: setup buffer b no longer read (consumers arrive, producer waits) */
+#define BAR_CONS 5   /* consumer warps only */
+#define FULLMASK 0xffffffffu
+
+__device__ __forceinline__ void bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+__device__ __forceinline__ void bar_arrive(int id, int n) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(n) : "memory"); }
+
+// One chunk of one accumulation phase: this warp holds Q[m][b + lane] (q0) and Q[m][b + 32 + lane] (q1) for the MG
+// modes of the group; m_int / m_edge are the samples whose window covers the chunk completely / partly.
+//   soff_l : (lane = sample) byte offset of lin[sample][b - i0_k(sample)] from the start of lin
+//   rel_l  : (lane = sample) b - i0_k(sample)
+//   Ab     : &A[sample 0][k][g * MG], a_stride = bytes between samples
+//   linl   : (unsigned char*)lin + lane * 8
+template <int MG, bool FIRST>
+__device__ __forceinline__ void tiled_chunk(const double2 (&q0)[MG], const double2 (&q1)[MG], unsigned m_int,
+                                            unsigned m_edge, int soff_l, int rel_l, const unsigned char *__restrict__ Ab,
+                                            int a_stride, unsigned char *__restrict__ linl, int n_t, int lane)
+{
+    // ---- windows that cover all 64 indices: no per-lane predicates, two samples in flight
+    while (m_int) {
+        const int a0 = __ffs(m_int) - 1;
+        m_int &= m_int - 1;
+        if (m_int) {
+            const int a1 = __ffs(m_int) - 1;
+            m_int &= m_int - 1;
+            const int so0 = __shfl_sync(FULLMASK, soff_l, a0), so1 = __shfl_sync(FULLMASK, soff_l, a1);
+            const double2 *__restrict__ A0 = reinterpret_cast<const double2 *>(Ab + a0 * a_stride);
+            const double2 *__restrict__ A1 = reinterpret_cast<const double2 *>(Ab + a1 * a_stride);
+            double *__restrict__ r0 = reinterpret_cast<double *>(linl + so0);
+            double *__restrict__ r1 = reinterpret_cast<double *>(linl + so1);
+            double2 c0[MG], c1[MG];
+#pragma unroll
+            for (int mm = 0; mm < MG; ++mm) {
+                c0[mm] = A0[mm];
+                c1[mm] = A1[mm];
+            }
+            double o00 = 0.0, o01 = 0.0, o10 = 0.0, o11 = 0.0;
+            if (!FIRST) {
+                o00 = r0[0];
+                o01 = r0[32];
+                o10 = r1[0];
+                o11 = r1[32];
+            }
+            double x00 = 0.0, y00 = 0.0, x01 = 0.0, y01 = 0.0, x10 = 0.0, y10 = 0.0, x11 = 0.0, y11 = 0.0;
+#pragma unroll
+            for (int mm = 0; mm < MG; ++mm) {
+                x00 = fma(c0[mm].x, q0[mm].x, x00);
+                y00 = fma(c0[mm].y, q0[mm].y, y00);
+                x01 = fma(c0[mm].x, q1[mm].x, x01);
+                y01 = fma(c0[mm].y, q1[mm].y, y01);
+                x10 = fma(c1[mm].x, q0[mm].x, x10);
+                y10 = fma(c1[mm].y, q0[mm].y, y10);
+                x11 = fma(c1[mm].x, q1[mm].x, x11);
+                y11 = fma(c1[mm].y, q1[mm].y, y11);
+            }
+            if (FIRST) {
+                r0[0] = x00 + y00;
+                r0[32] = x01 + y01;
+                r1[0] = x10 + y10;
+                r1[32] = x11 + y11;
+            } else {
+                r0[0] = o00 + (x00 + y00);
+                r0[32] = o01 + (x01 + y01);
+                r1[0] = o10 + (x10 + y10);
+                r1[32] = o11 + (x11 + y11);
+            }
+        } else {
+            const int so0 = __shfl_sync(FULLMASK, soff_l, a0);
+            const double2 *__restrict__ A0 = reinterpret_cast<const double2 *>(Ab + a0 * a_stride);
+            double *__restrict__ r0 = reinterpret_cast<double *>(linl + so0);
+            double2 c0[MG];
+#pragma unroll
+            for (int mm = 0; mm < MG; ++mm) c0[mm] = A0[mm];
+            double o00 = 0.0, o01 = 0.0;
+            if (!FIRST) {
+                o00 = r0[0];
+                o01 = r0[32];
+            }
+            double x00 = 0.0, y00 = 0.0, x01 = 0.0, y01 = 0.0;
+#pragma unroll
+            for (int mm = 0; mm < MG; ++mm) {
+                x00 = fma(c0[mm].x, q0[mm].x, x00);
+                y00 = fma(c0[mm].y, q0[mm].y, y00);
+                x01 = fma(c0[mm].x, q1[mm].x, x01);
+                y01 = fma(c0[mm].y, q1[mm].y, y01);
+            }
+            if (FIRST) {
+                r0[0] = x00 + y00;
+                r0[32] = x01 + y01;
+            } else {
+                r0[0] = o00 + (x00 + y00);
+                r0[32] = o01 + (x01 + y01);
+            }
+        }
+    }
+    // ---- windows that start or end inside the chunk: 32-index halves skipped when untouched, lanes predicated
+    while (m_edge) {
+        const int a0 = __ffs(m_edge) - 1;
+        m_edge &= m_edge - 1;
+        const int so0 = __shfl_sync(FULLMASK, soff_l, a0), rel = __shfl_sync(FULLMASK, rel_l, a0);
+        const double2 *__restrict__ A0 = reinterpret_cast<const double2 *>(Ab + a0 * a_stride);
+        double *__restrict__ r0 = reinterpret_cast<double *>(linl + so0);
+        double2 c0[MG];
+#pragma unroll
+        for (int mm = 0; mm < MG; ++mm) c0[mm] = A0[mm];
+        if (rel + 31 >= 0 && rel < n_t) {
+            double x = 0.0, y = 0.0;
+#pragma unroll
+            for (int mm = 0; mm < MG; ++mm) {
+                x = fma(c0[mm].x, q0[mm].x, x);
+                y = fma(c0[mm].y, q0[mm].y, y);
+            }
+            if ((unsigned)(rel + lane) < (unsigned)n_t) r0[0] = FIRST ? (x + y) : (r0[0] + (x + y));
+        }
+        if (rel + 63 >= 0 && rel + 32 < n_t) {
+            double x = 0.0, y = 0.0;
+#pragma unroll
+            for (int mm = 0; mm < MG; ++mm) {
+                x = fma(c0[mm].x, q1[mm].x, x);
+                y = fma(c0[mm].y, q1[mm].y, y);
+            }
+            if ((unsigned)(rel + 32 + lane) < (unsigned)n_t) r0[32] = FIRST ? (x + y) : (r0[32] + (x + y));
+        }
+    }
+}
+
 template <int MG>
-__global__ void __launch_bounds__(TILED_THREADS, 2) ile_eval_tiled_kernel(IleEvalArgs a, IleTiledLayout L)
+__global__ void __launch_bounds__(TILED_THREADS, 2)
+    ile_eval_tiled_kernel(const __grid_constant__ IleDevParams P, const __grid_constant__ IleEvalArgs a,
+                          const __grid_constant__ IleTiledLayout L)
 {
     extern __shared__ __align__(16) unsigned char smem[];
     double *__restrict__ lin = reinterpret_cast<double *>(smem + L.off_lin);
-    double2 *__restrict__ A = reinterpret_cast<double2 *>(smem + L.off_A);
-    double *__restrict__ quadS = reinterpret_cast<double *>(smem + L.off_quad);
-    int32_t *__restrict__ i0S = reinterpret_cast<int32_t *>(smem + L.off_i0);
-    int32_t *__restrict__ badS = reinterpret_cast<int32_t *>(smem + L.off_bad);
-    int32_t *__restrict__ rangeS = reinterpret_cast<int32_t *>(smem + L.off_misc);  // lo[K], hi[K]
-    int32_t *__restrict__ ctrS = rangeS + 2 * ILE_MAX_DET;                          // one chunk counter per phase
 
-    const IleDevParams *__restrict__ P = a.params;
-    const int K = P->n_det, M = P->n_modes, n_q = P->n_q, n_t = P->n_t;
+    const int K = P.n_det, M = P.n_modes, n_q = P.n_q, n_t = P.n_t;
     const int G = L.n_groups, ldA = G * MG, S = L.S, ldl = L.ldl, n_phase = K * G;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const long long tiles_per_point = (a.n_per_point + S - 1) / S;
     const long long n_tiles = tiles_per_point * a.n_points;
-    const double log_nt = log((double)n_t);
 
-    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-        const int pt = (int)(tile / tiles_per_point);
-        const long long s0 = (tile - (long long)pt * tiles_per_point) * S;
-        const int cnt = (int)min((long long)S, a.n_per_point - s0);
-        const long long flat0 = (long long)pt * a.n_per_point + s0;
-        const size_t pglob = (size_t)(a.point0 + pt);
-        const double2 *__restrict__ Qp = a.Q + pglob * (size_t)K * M * n_q;
+    if (warp == TILED_CWARPS) {
+        // ================================================================ producer warp: steps 1-4, lane = sample
+        int it = 0;
+        for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+            const int b = it & 1;
+            unsigned char *sb = smem + L.off_sb + (size_t)b * L.sb_bytes;
+            double2 *A = reinterpret_cast<double2 *>(sb);
+            double *quadS = reinterpret_cast<double *>(sb + L.sb_quad);
+            int32_t *i0S = reinterpret_cast<int32_t *>(sb + L.sb_i0);
+            int32_t *badS = reinterpret_cast<int32_t *>(sb + L.sb_bad);
+            int32_t *rangeS = reinterpret_cast<int32_t *>(sb + L.sb_misc);
+            int32_t *ctrS = rangeS + 2 * ILE_MAX_DET;
 
-        // ---------------------------------------------------------------- setup: steps 1-4, lane = sample
-        if (warp == 0) {
+            const int pt = (int)(tile / tiles_per_point);
+            const long long s0 = (tile - (long long)pt * tiles_per_point) * S;
+            const int cnt = (int)min((long long)S, a.n_per_point - s0);
+            const long long flat0 = (long long)pt * a.n_per_point + s0;
+            const size_t pglob = (size_t)(a.point0 + pt);
+
+            if (it >= 2) bar_sync(BAR_EMPTY0 + b, TILED_THREADS);
             int bad = 1;
             if (lane < cnt) {
                 const long long s = flat0 + lane;
-                double q = ile_setup_sample(P, a.U + pglob * (size_t)K * M * M, a.V + pglob * (size_t)K * M * M, a.ra[s],
+                double q = ile_setup_sample(&P, a.U + pglob * (size_t)K * M * M, a.V + pglob * (size_t)K * M * M, a.ra[s],
                                             a.dec[s], a.t_ref[s], a.phi_ref[s], a.psi[s], a.incl[s], a.dist[s],
                                             A + (size_t)lane * K * ldA, ldA, i0S + lane * K, &bad);
                 quadS[lane] = q;
@@ -95,9 +230,9 @@ __global__ void __launch_bounds__(TILED_THREADS, 2) ile_eval_tiled_kernel(IleEva
             }
             badS[lane] = bad;
             for (int k = 0; k < K; ++k) {
-                int v = bad ? INT_MAX : i0S[lane * K + k];
-                int w = bad ? INT_MIN : i0S[lane * K + k];
-                int lo = __reduce_min_sync(0xffffffffu, v), hi = __reduce_max_sync(0xffffffffu, w);
+                const int v = bad ? INT_MAX : i0S[lane * K + k];
+                const int w = bad ? INT_MIN : i0S[lane * K + k];
+                const int lo = __reduce_min_sync(FULLMASK, v), hi = __reduce_max_sync(FULLMASK, w);
                 if (lane == 0) {
                     const bool any = hi != INT_MIN;
                     rangeS[k] = any ? lo : 0;
@@ -105,24 +240,53 @@ __global__ void __launch_bounds__(TILED_THREADS, 2) ile_eval_tiled_kernel(IleEva
                 }
             }
             for (int p = lane; p < n_phase; p += 32) ctrS[p] = 0;
+            __threadfence_block();
+            bar_arrive(BAR_FULL0 + b, TILED_THREADS);
         }
-        __syncthreads();
+        return;
+    }
+
+    // ==================================================================== consumer warps: steps 5-6
+    const double log_nt = log((double)n_t);
+    unsigned char *__restrict__ linl = reinterpret_cast<unsigned char *>(lin) + lane * 8;
+    int it = 0;
+    for (long long tile = blockIdx.x; tile < n_tiles; tile += gridDim.x, ++it) {
+        const int b = it & 1;
+        unsigned char *sb = smem + L.off_sb + (size_t)b * L.sb_bytes;
+        const unsigned char *Abytes = sb;
+        const double *quadS = reinterpret_cast<const double *>(sb + L.sb_quad);
+        const int32_t *i0S = reinterpret_cast<const int32_t *>(sb + L.sb_i0);
+        const int32_t *badS = reinterpret_cast<const int32_t *>(sb + L.sb_bad);
+        const int32_t *rangeS = reinterpret_cast<const int32_t *>(sb + L.sb_misc);
+        int32_t *ctrS = reinterpret_cast<int32_t *>(sb + L.sb_misc) + 2 * ILE_MAX_DET;
+
+        const int pt = (int)(tile / tiles_per_point);
+        const long long s0 = (tile - (long long)pt * tiles_per_point) * S;
+        const int cnt = (int)min((long long)S, a.n_per_point - s0);
+        const long long flat0 = (long long)pt * a.n_per_point + s0;
+        const size_t pglob = (size_t)(a.point0 + pt);
+        const double2 *__restrict__ Qp = a.Q + pglob * (size_t)K * M * n_q;
+        const int a_stride = K * ldA * (int)sizeof(double2);
+
+        bar_sync(BAR_FULL0 + b, TILED_THREADS);
+        const bool good_l = lane < S && !badS[lane];
 
         // ---------------------------------------------------------------- step 5: accumulation phases
         for (int p = 0; p < n_phase; ++p) {
             const int k = p / G, g = p - k * G;
             const int lo = rangeS[k], hi = rangeS[ILE_MAX_DET + k];
-            const bool first = (p == 0);
+            const int i0_l = good_l ? i0S[lane * K + k] : 0;
+            const unsigned char *Ab = Abytes + (size_t)(k * ldA + g * MG) * sizeof(double2);
             for (;;) {
                 int c = 0;
                 if (lane == 0) c = atomicAdd(&ctrS[p], 1);
-                c = __shfl_sync(0xffffffffu, c, 0);
-                const int b = lo + c * TILED_CHUNK;
-                if (b >= hi) break;
+                c = __shfl_sync(FULLMASK, c, 0);
+                const int bidx = lo + c * TILED_CHUNK;
+                if (bidx >= hi) break;
 
                 double2 q0[MG], q1[MG];
                 {
-                    const int ia = min(b + lane, n_q - 1), ib = min(b + 32 + lane, n_q - 1);
+                    const int ia = min(bidx + lane, n_q - 1), ib = min(bidx + 32 + lane, n_q - 1);
 #pragma unroll
                     for (int mm = 0; mm < MG; ++mm) {
                         const int m = g * MG + mm;
@@ -136,77 +300,48 @@ __global__ void __launch_bounds__(TILED_THREADS, 2) ile_eval_tiled_kernel(IleEva
                         }
                     }
                 }
-                int rel_l = 0;
-                bool act = false;
-                if (lane < S && !badS[lane]) {
-                    rel_l = b - i0S[lane * K + k];
-                    act = (rel_l + (TILED_CHUNK - 1) >= 0) && (rel_l < n_t);
-                }
-                unsigned mask = __ballot_sync(0xffffffffu, act);
-                while (mask) {
-                    const int al = __ffs(mask) - 1;
-                    mask &= mask - 1;
-                    const int rel = __shfl_sync(0xffffffffu, rel_l, al);
-                    const double2 *__restrict__ Aa = A + ((size_t)al * K + k) * ldA + g * MG;
-                    double *__restrict__ row = lin + (size_t)al * ldl;
-                    double2 cf[MG];
-#pragma unroll
-                    for (int mm = 0; mm < MG; ++mm) cf[mm] = Aa[mm];
-                    if (rel + 31 >= 0 && rel < n_t) {
-                        double tx = 0.0, ty = 0.0;
-#pragma unroll
-                        for (int mm = 0; mm < MG; ++mm) {
-                            tx = fma(cf[mm].x, q0[mm].x, tx);
-                            ty = fma(cf[mm].y, q0[mm].y, ty);
-                        }
-                        const int j = rel + lane;
-                        if ((unsigned)j < (unsigned)n_t) row[j] = first ? (tx + ty) : (row[j] + (tx + ty));
-                    }
-                    if (rel + 63 >= 0 && rel + 32 < n_t) {
-                        double tx = 0.0, ty = 0.0;
-#pragma unroll
-                        for (int mm = 0; mm < MG; ++mm) {
-                            tx = fma(cf[mm].x, q1[mm].x, tx);
-                            ty = fma(cf[mm].y, q1[mm].y, ty);
-                        }
-                        const int j = rel + 32 + lane;
-                        if ((unsigned)j < (unsigned)n_t) row[j] = first ? (tx + ty) : (row[j] + (tx + ty));
-                    }
-                }
+                const int rel_l = bidx - i0_l;
+                const bool touch = good_l && (rel_l + (TILED_CHUNK - 1) >= 0) && (rel_l < n_t);
+                const bool inter = touch && rel_l >= 0 && rel_l + TILED_CHUNK <= n_t;
+                const unsigned m_int = __ballot_sync(FULLMASK, inter);
+                const unsigned m_edge = __ballot_sync(FULLMASK, touch && !inter);
+                const int soff_l = (lane * ldl + rel_l) * 8;
+                if (p == 0)
+                    tiled_chunk<MG, true>(q0, q1, m_int, m_edge, soff_l, rel_l, Ab, a_stride, linl, n_t, lane);
+                else
+                    tiled_chunk<MG, false>(q0, q1, m_int, m_edge, soff_l, rel_l, Ab, a_stride, linl, n_t, lane);
             }
-            __syncthreads();
+            bar_sync(BAR_CONS, TILED_CWARPS * 32);
         }
 
         // ---------------------------------------------------------------- step 6: log-sum-exp over each row
-        const int nt32 = (n_t + 31) >> 5;
-        for (int al = warp; al < cnt; al += TILED_WARPS) {
+        for (int al = warp; al < cnt; al += TILED_CWARPS) {
             if (badS[al]) continue;
-            const double *__restrict__ row = lin + (size_t)al * ldl;
-            double mx = -CUDART_INF, sm = 0.0;
-            if (nt32 <= TILED_ROW_REGS) {
-                double v[TILED_ROW_REGS];
-#pragma unroll
-                for (int t = 0; t < TILED_ROW_REGS; ++t) {
-                    v[t] = -CUDART_INF;
-                    if (t < nt32) {
-                        const int j = t * 32 + lane;
-                        if (j < n_t) v[t] = row[j];
-                        mx = fmax(mx, v[t]);
-                    }
-                }
-                mx = warp_max(mx);
-#pragma unroll
-                for (int t = 0; t < TILED_ROW_REGS; ++t)
-                    if (t < nt32) sm += ile_exp_nonpos(v[t] - mx);
-            } else {
-                for (int j = lane; j < n_t; j += 32) mx = fmax(mx, row[j]);
-                mx = warp_max(mx);
-                for (int j = lane; j < n_t; j += 32) sm += ile_exp_nonpos(row[j] - mx);
+            const double *__restrict__ row = lin + (size_t)al * ldl + lane;
+            const int nl = n_t - lane;  // this lane owns row[0], row[32], ... below nl
+            double m0 = -CUDART_INF, m1 = -CUDART_INF;
+            int j = 0;
+            for (; j + 32 < nl; j += 64) {
+                m0 = fmax(m0, row[j]);
+                m1 = fmax(m1, row[j + 32]);
             }
-            sm = warp_sum(sm);
+            if (j < nl) m0 = fmax(m0, row[j]);
+            const double mx = warp_max(fmax(m0, m1));
+            double e0 = 0.0, e1 = 0.0, e2 = 0.0, e3 = 0.0;
+            j = 0;
+            for (; j + 96 < nl; j += 128) {
+                const double x0 = row[j] - mx, x1 = row[j + 32] - mx, x2 = row[j + 64] - mx, x3 = row[j + 96] - mx;
+                e0 += ile_exp_nonpos(x0);
+                e1 += ile_exp_nonpos(x1);
+                e2 += ile_exp_nonpos(x2);
+                e3 += ile_exp_nonpos(x3);
+            }
+            for (; j < nl; j += 32) e0 += ile_exp_nonpos(row[j] - mx);
+            const double sm = warp_sum((e0 + e1) + (e2 + e3));
             if (lane == 0) a.lnL[flat0 + al] = mx + log(sm) - log_nt - quadS[al];
         }
-        __syncthreads();
+        if (tile + 2 * (long long)gridDim.x < n_tiles) bar_arrive(BAR_EMPTY0 + b, TILED_THREADS);
+        bar_sync(BAR_CONS, TILED_CWARPS * 32);
     }
 }
 
@@ -233,20 +368,20 @@ static IleTiledLayout tiled_layout(const IleSizes &sz, int MG, int S)
     L.n_groups = (sz.n_modes + MG - 1) / MG;
     L.S = S;
     L.ldl = sz.n_t;
-    uint32_t off = 0;
-    L.off_A = off;
-    off += (uint32_t)(S * sz.n_det * L.n_groups * MG * sizeof(double2));
-    L.off_lin = off;
-    off += (uint32_t)(S * L.ldl * sizeof(double));
-    L.off_quad = off;
-    off += (uint32_t)(32 * sizeof(double));
-    L.off_i0 = off;
-    off += (uint32_t)(32 * sz.n_det * sizeof(int32_t));
-    L.off_bad = off;
-    off += (uint32_t)(32 * sizeof(int32_t));
-    L.off_misc = off;
-    off += (uint32_t)((2 * ILE_MAX_DET + sz.n_det * L.n_groups) * sizeof(int32_t));
-    L.bytes = (off + 15u) & ~15u;
+    // one setup buffer: A[S][K][G*MG] | quad[32] | i0[32][K] | bad[32] | lo[MAX_DET] hi[MAX_DET] ctr[K*G]
+    uint32_t o = (uint32_t)(S * sz.n_det * L.n_groups * MG * sizeof(double2));
+    L.sb_quad = o;
+    o += (uint32_t)(32 * sizeof(double));
+    L.sb_i0 = o;
+    o += (uint32_t)(32 * sz.n_det * sizeof(int32_t));
+    L.sb_bad = o;
+    o += (uint32_t)(32 * sizeof(int32_t));
+    L.sb_misc = o;
+    o += (uint32_t)((2 * ILE_MAX_DET + sz.n_det * L.n_groups) * sizeof(int32_t));
+    L.sb_bytes = (o + 15u) & ~15u;
+    L.off_sb = 0;
+    L.off_lin = 2 * L.sb_bytes;
+    L.bytes = (L.off_lin + (uint32_t)(S * L.ldl * sizeof(double)) + 15u) & ~15u;
     return L;
 }
 
@@ -280,7 +415,8 @@ bool ile_tiled_plan(const IleSizes &sz, long long n_total, IleTiledLayout *out)
 }
 
 template <int MG>
-static cudaError_t tiled_launch_mg(const IleSizes &sz, const IleEvalArgs &a, const IleTiledLayout &L, cudaStream_t st)
+static cudaError_t tiled_launch_mg(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleTiledLayout &L,
+                                   cudaStream_t st)
 {
     cudaError_t e = cudaFuncSetAttribute(ile_eval_tiled_kernel<MG>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)L.bytes);
     if (e != cudaSuccess) return e;
@@ -291,24 +427,25 @@ static cudaError_t tiled_launch_mg(const IleSizes &sz, const IleEvalArgs &a, con
     const long long tiles = ((a.n_per_point + L.S - 1) / L.S) * a.n_points;
     long long grid = (long long)sz.sm_count * per_sm;
     if (tiles < grid) grid = tiles;
-    ile_eval_tiled_kernel<MG><<<(unsigned)grid, TILED_THREADS, L.bytes, st>>>(a, L);
+    ile_eval_tiled_kernel<MG><<<(unsigned)grid, TILED_THREADS, L.bytes, st>>>(hp, a, L);
     return cudaGetLastError();
 }
 
-cudaError_t ile_launch_eval_tiled(const IleSizes &sz, const IleEvalArgs &a, cudaStream_t st, int *n_launches)
+cudaError_t ile_launch_eval_tiled(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, cudaStream_t st,
+                                  int *n_launches)
 {
     if (a.n_per_point <= 0 || a.n_points <= 0) return cudaSuccess;
     IleTiledLayout L;
     if (!ile_tiled_plan(sz, (long long)a.n_per_point * a.n_points, &L)) return cudaErrorInvalidConfiguration;
     cudaError_t e;
     switch (L.mg) {
-        case 2: e = tiled_launch_mg<2>(sz, a, L, st); break;
-        case 3: e = tiled_launch_mg<3>(sz, a, L, st); break;
-        case 4: e = tiled_launch_mg<4>(sz, a, L, st); break;
-        case 5: e = tiled_launch_mg<5>(sz, a, L, st); break;
-        case 6: e = tiled_launch_mg<6>(sz, a, L, st); break;
-        case 7: e = tiled_launch_mg<7>(sz, a, L, st); break;
-        default: e = tiled_launch_mg<8>(sz, a, L, st); break;
+        case 2: e = tiled_launch_mg<2>(sz, hp, a, L, st); break;
+        case 3: e = tiled_launch_mg<3>(sz, hp, a, L, st); break;
+        case 4: e = tiled_launch_mg<4>(sz, hp, a, L, st); break;
+        case 5: e = tiled_launch_mg<5>(sz, hp, a, L, st); break;
+        case 6: e = tiled_launch_mg<6>(sz, hp, a, L, st); break;
+        case 7: e = tiled_launch_mg<7>(sz, hp, a, L, st); break;
+        default: e = tiled_launch_mg<8>(sz, hp, a, L, st); break;
     }
     if (e == cudaSuccess && n_launches) *n_launches += 1;
     return e;

@@ -32,7 +32,9 @@ struct IleTiledLayout {
     int32_t n_groups;  // G = ceil(M / mg)
     int32_t S;         // samples per tile, <= 32
     int32_t ldl;       // row stride of lin in doubles
-    uint32_t off_A, off_lin, off_quad, off_i0, off_bad, off_misc;
+    uint32_t off_sb, sb_bytes;                  // two setup buffers of sb_bytes each, starting at off_sb
+    uint32_t sb_quad, sb_i0, sb_bad, sb_misc;   // offsets inside a setup buffer (A sits at 0)
+    uint32_t off_lin;                           // lin[S][ldl]
     uint32_t bytes;
 };
 
@@ -41,7 +43,8 @@ cudaError_t ile_launch_eval_direct(const IleSizes &sz, const IleEvalArgs &a, cud
 
 // variant 2: tiled, Q-stationary kernel (ile_eval_tiled.cu).  ile_tiled_plan returns false when the sizes do not fit.
 bool ile_tiled_plan(const IleSizes &sz, long long n_total, IleTiledLayout *out);
-cudaError_t ile_launch_eval_tiled(const IleSizes &sz, const IleEvalArgs &a, cudaStream_t st, int *n_launches);
+cudaError_t ile_launch_eval_tiled(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, cudaStream_t st,
+                                  int *n_launches);
 
 // evidence: two kernels (per-block partials, then per-segment combine with the carried state)
 cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const double *lnL, const double *log_w,
