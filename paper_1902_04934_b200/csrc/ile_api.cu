@@ -22,6 +22,14 @@ struct ile_ctx {
     double *h_small;   // pinned mirror
     int32_t variant;
     long long launches;
+    // variant 3 (sorted FP64-MMA path)
+    bool mma_ok;
+    IleMmaPlan mp;
+    double *dQp;
+    int64_t chunk_samples;  // samples per launch group: keeps the record scratch L2-resident
+    IleMmaScratch sc;
+    size_t sc_samples, sc_hist;  // capacities (samples, histogram words)
+    int32_t sc_points;
 };
 
 static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
@@ -145,6 +153,16 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     CKC(cudaMemcpy(c->dU, U, nU * sizeof(double2), cudaMemcpyDefault));
     CKC(cudaMemcpy(c->dV, V, nU * sizeof(double2), cudaMemcpyDefault));
     CKC(cudaMemset(c->d_oob, 0, sizeof(unsigned long long)));
+    c->mma_ok = ile_mma_plan(c->sz, &c->mp);
+    if (c->mma_ok) {
+        const size_t nQp = (size_t)cfg->n_points * cfg->n_det * c->mp.nblk_q * c->mp.ks * 32;
+        CKC(cudaMalloc(&c->dQp, nQp * sizeof(double)));
+        CKC(ile_launch_pack_q(c->sz, c->mp, cfg->n_points, c->dQ, c->dQp, 0));
+        CKC(cudaDeviceSynchronize());
+        int64_t cs = (int64_t)(64u << 20) / ((int64_t)c->mp.recg * 8);
+        cs = cs < 16384 ? 16384 : cs > 262144 ? 262144 : cs;
+        c->chunk_samples = cs;
+    }
 #undef CKC
     *out = c;
     return ILE_OK;
@@ -161,8 +179,66 @@ extern "C" void ile_destroy(ile_ctx *c)
     cudaFree(c->d_partials);
     cudaFree(c->d_stage);
     cudaFree(c->d_small);
+    cudaFree(c->dQp);
+    cudaFree(c->sc.rec);
+    cudaFree(c->sc.quad);
+    cudaFree(c->sc.i0);
+    cudaFree(c->sc.cell);
+    cudaFree(c->sc.perm);
+    cudaFree(c->sc.hist);
+    cudaFree(c->sc.ngood);
     if (c->h_small) cudaFreeHost(c->h_small);
     delete c;
+}
+
+// Scratch of the sorted path, grown on demand (never inside a launch sequence that still uses the old buffers: the
+// stream is synchronised first).
+static int ensure_scratch(ile_ctx *c, size_t samples, size_t hist_words, int32_t points, cudaStream_t st)
+{
+    if (samples > c->sc_samples) {
+        CK(cudaStreamSynchronize(st));
+        cudaFree(c->sc.rec), cudaFree(c->sc.quad), cudaFree(c->sc.i0), cudaFree(c->sc.cell), cudaFree(c->sc.perm);
+        c->sc.rec = nullptr, c->sc.quad = nullptr, c->sc.i0 = nullptr, c->sc.cell = nullptr, c->sc.perm = nullptr;
+        c->sc_samples = 0;
+        CK(cudaMalloc(&c->sc.rec, samples * c->mp.recg * sizeof(double)));
+        CK(cudaMalloc(&c->sc.quad, samples * sizeof(double)));
+        CK(cudaMalloc(&c->sc.i0, samples * c->sz.n_det * sizeof(int32_t)));
+        CK(cudaMalloc(&c->sc.cell, samples * sizeof(int32_t)));
+        CK(cudaMalloc(&c->sc.perm, samples * sizeof(int32_t)));
+        c->sc_samples = samples;
+    }
+    if (hist_words > c->sc_hist) {
+        CK(cudaStreamSynchronize(st));
+        cudaFree(c->sc.hist);
+        c->sc.hist = nullptr;
+        c->sc_hist = 0;
+        CK(cudaMalloc(&c->sc.hist, hist_words * sizeof(uint32_t)));
+        c->sc_hist = hist_words;
+    }
+    if (points > c->sc_points) {
+        CK(cudaStreamSynchronize(st));
+        cudaFree(c->sc.ngood);
+        c->sc.ngood = nullptr;
+        c->sc_points = 0;
+        CK(cudaMalloc(&c->sc.ngood, (size_t)points * sizeof(int32_t)));
+        c->sc_points = points;
+    }
+    return ILE_OK;
+}
+
+// variant 3 for one launch group: setup + sort + contraction on [point0, point0 + n_points) x n samples each
+static int eval_mma_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
+{
+    const IleSortPlan sp = ile_sort_plan(c->sz, c->hparams, a.n_per_point);
+    int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * sp.ncell, a.n_points, st);
+    if (r != ILE_OK) return r;
+    c->sc.Qp = c->dQp;
+    int nl = 0;
+    cudaError_t e = ile_launch_setup_sort(c->sz, c->hparams, a, c->mp, sp, c->sc, st, &nl);
+    if (e == cudaSuccess) e = ile_launch_eval_mma(c->sz, c->hparams, a, c->mp, c->sc, st, &nl);
+    c->launches += nl;
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ILE_OK;
 }
 
 static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n, const double *ra, const double *dec,
@@ -181,6 +257,37 @@ static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n
     a.lnL = lnL;
     a.shift_idx = shift_idx;
     a.oob_counter = c->d_oob;
+    if (c->variant == 3 || (c->variant == 0 && c->mma_ok)) {
+        // launch groups of at most chunk_samples samples: whole points while they fit, else slices of one point
+        const int64_t cs = c->chunk_samples;
+        const int K = c->sz.n_det;
+        auto shifted = [&](int64_t off, int32_t p0, int32_t np, int64_t cnt) {
+            IleEvalArgs g = a;
+            g.point0 = p0;
+            g.n_points = np;
+            g.n_per_point = cnt;
+            g.ra = ra + off, g.dec = dec + off, g.t_ref = t_ref + off, g.phi_ref = phi_ref + off, g.psi = psi + off;
+            g.incl = incl + off, g.dist = dist + off, g.lnL = lnL + off;
+            g.shift_idx = shift_idx ? shift_idx + off * K : nullptr;
+            return g;
+        };
+        if (n <= cs) {
+            const int32_t per = (int32_t)(cs / n);
+            for (int32_t p = 0; p < n_points; p += per) {
+                const int32_t np = n_points - p < per ? n_points - p : per;
+                int r = eval_mma_group(c, shifted((int64_t)p * n, point0 + p, np, n), st);
+                if (r != ILE_OK) return r;
+            }
+        } else {
+            for (int32_t p = 0; p < n_points; ++p)
+                for (int64_t off = 0; off < n; off += cs) {
+                    const int64_t cnt = n - off < cs ? n - off : cs;
+                    int r = eval_mma_group(c, shifted((int64_t)p * n + off, point0 + p, 1, cnt), st);
+                    if (r != ILE_OK) return r;
+                }
+        }
+        return ILE_OK;
+    }
     int nl = 0;
     IleTiledLayout L;
     const bool tiled = c->variant == 2 || (c->variant == 0 && ile_tiled_plan(c->sz, (long long)n * n_points, &L));
@@ -298,7 +405,8 @@ extern "C" int ile_status(ile_ctx *c, int64_t *n_out_of_range, int reset, void *
 extern "C" int ile_set_variant(ile_ctx *c, int32_t variant)
 {
     if (!c || variant < 0) return ILE_ERR_BAD_ARGUMENT;
-    if (variant > 2) return ILE_ERR_UNSUPPORTED;
+    if (variant > 3) return ILE_ERR_UNSUPPORTED;
+    if (variant == 3 && !c->mma_ok) return ILE_ERR_UNSUPPORTED;
     if (variant == 2) {
         IleTiledLayout L;
         if (!ile_tiled_plan(c->sz, 1LL << 40, &L)) return ILE_ERR_UNSUPPORTED;

@@ -42,18 +42,25 @@ struct IleSky {
     double X[3], Y[3], s[3];
 };
 
+// Unit vector Earth -> source from (RA, dec, GMST); also returns the sines and cosines it is built from.  Products are
+// rounded one by one (no FMA) so that the window index derived from it is reproducible wherever it is computed.
+__device__ __forceinline__ void ile_source_dir(double ra, double dec, double gmst, double s[3], double *sl, double *cl,
+                                               double *sd, double *cd)
+{
+    double lon = ra - gmst;  // = -(Greenwich hour angle)
+    sincos(lon, sl, cl);
+    sincos(dec, sd, cd);
+    s[0] = __dmul_rn(*cd, *cl);
+    s[1] = __dmul_rn(*cd, *sl);
+    s[2] = *sd;
+}
+
 __device__ __forceinline__ IleSky ile_sky(double ra, double dec, double psi, double gmst)
 {
     IleSky g;
-    double lon = ra - gmst;  // = -(Greenwich hour angle)
     double sl, cl, sd, cd, sp, cp;
-    sincos(lon, &sl, &cl);
-    sincos(dec, &sd, &cd);
+    ile_source_dir(ra, dec, gmst, g.s, &sl, &cl, &sd, &cd);
     sincos(psi, &sp, &cp);
-    // source direction; products rounded one by one so that the window index below is reproducible (no FMA)
-    g.s[0] = __dmul_rn(cd, cl);
-    g.s[1] = __dmul_rn(cd, sl);
-    g.s[2] = sd;
     // psi = 0: X local west, Y local north; X x Y = propagation direction; psi rotates X toward Y  (reading R6)
     double sg = -sl, cg = cl;  // sin, cos of gha = gmst - ra
     g.X[0] = -cp * sg - sp * cg * sd;
@@ -81,10 +88,10 @@ __device__ __forceinline__ double2 ile_antenna(const double *__restrict__ D, con
 
 // Window start i0_k = rint(((t_ref + dt_k) - t0_Q) f_s) - floor(N_t/2), dt_k = -(x_k . s)/c  (readings R2, R8).
 // Every operation is individually rounded, in a fixed order, so the integer is reproducible.
-__device__ __forceinline__ int32_t ile_window_index(const double *__restrict__ v, const IleSky &g, double t_ref,
-                                                    double t0_q, double fs, int32_t n_t)
+__device__ __forceinline__ int32_t ile_window_index(const double *__restrict__ v, const double *__restrict__ s,
+                                                    double t_ref, double t0_q, double fs, int32_t n_t)
 {
-    double dot = __dadd_rn(__dadd_rn(__dmul_rn(v[0], g.s[0]), __dmul_rn(v[1], g.s[1])), __dmul_rn(v[2], g.s[2]));
+    double dot = __dadd_rn(__dadd_rn(__dmul_rn(v[0], s[0]), __dmul_rn(v[1], s[1])), __dmul_rn(v[2], s[2]));
     double dt = __ddiv_rn(-dot, ILE_C_SI);
     double x = __dmul_rn(__dsub_rn(__dadd_rn(t_ref, dt), t0_q), fs);
     return __double2int_rn(x) - n_t / 2;
@@ -152,7 +159,7 @@ __device__ __forceinline__ double ile_setup_sample(const IleDevParams *__restric
         double F2 = F.x * F.x + F.y * F.y;
         double2 FF = ile_cmul(F, F);
         tot += F2 * yuy + (FF.x * yvy.x - FF.y * yvy.y);
-        int32_t idx = ile_window_index(P->vertex[k], g, t_ref, P->t0_q, P->fs, P->n_t);
+        int32_t idx = ile_window_index(P->vertex[k], g.s, t_ref, P->t0_q, P->fs, P->n_t);
         i0[k] = idx;
         if (idx < 0 || (long long)idx + P->n_t > P->n_q) oob = 1;
     }

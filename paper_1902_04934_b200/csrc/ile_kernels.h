@@ -46,6 +46,53 @@ bool ile_tiled_plan(const IleSizes &sz, long long n_total, IleTiledLayout *out);
 cudaError_t ile_launch_eval_tiled(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, cudaStream_t st,
                                   int *n_launches);
 
+// ---- variant 3: setup + counting sort + FP64-MMA contraction (ile_setup.cu, ile_eval_mma.cu) --------------------
+// Cell grid of the counting sort: window starts binned to width 2^g in (i0_0, i0_1 - i0_0, i0_2 - i0_0).
+struct IleSortPlan {
+    int32_t g;        // log2 of the cell width in samples
+    int32_t nd;       // detectors that take part in the key (<= 3)
+    int32_t n0, n1, n2;
+    int32_t ncell;    // n0*n1*n2 + 1; the last cell collects out-of-range samples
+    int32_t dmax[3];  // bound on |i0_d - i0_0| from the light travel time between the sites
+};
+
+// Sizes and shared-memory carve-up of the MMA kernel, computed on the host and passed by value.
+struct IleMmaPlan {
+    int32_t ks;      // k-steps of 4 real channels: ceil(2M / 4)
+    int32_t cp;      // padded channels per detector = 4 * ks
+    int32_t tbmax;   // 8-index time blocks a warp can hold per chunk (template parameter)
+    int32_t S;       // samples per tile, multiple of 8
+    int32_t recg;    // doubles per sample record in global memory = K * cp
+    int32_t ldrec;   // doubles per sample record in shared memory (recg padded to 4 mod 16)
+    int32_t nb;      // 8-cell blocks per row = ceil(n_t / 8)
+    int32_t nblk_q;  // 8-index blocks per detector in the packed Q (with zero padding at the end)
+    uint32_t sb_bytes, sb_quad, sb_flat, sb_i0, sb_misc;  // one setup buffer: rec | quad | flat | i0 | ranges
+    uint32_t off_mbar, off_part, part_bytes, off_rows, bytes;
+};
+
+// Device scratch of variant 3 (owned by the context).
+struct IleMmaScratch {
+    const double *Qp;  // packed Q [P][K][nblk_q][ks][32]
+    double *rec;       // [n][recg]
+    double *quad;      // [n]
+    int32_t *i0;       // [n][K]
+    int32_t *cell;     // [n]
+    int32_t *perm;     // [n]
+    uint32_t *hist;    // [n_points][ncell]
+    int32_t *ngood;    // [n_points]
+};
+
+bool ile_mma_plan(const IleSizes &sz, IleMmaPlan *out);
+IleSortPlan ile_sort_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point);
+cudaError_t ile_launch_pack_q(const IleSizes &sz, const IleMmaPlan &mp, int32_t n_points, const double2 *Q, double *Qp,
+                              cudaStream_t st);
+// steps 1-4 for every sample + cell keys + counting sort (4 launches)
+cudaError_t ile_launch_setup_sort(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleMmaPlan &mp,
+                                  const IleSortPlan &sp, const IleMmaScratch &sc, cudaStream_t st, int *n_launches);
+// steps 5-6 on the sorted samples
+cudaError_t ile_launch_eval_mma(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleMmaPlan &mp,
+                                const IleMmaScratch &sc, cudaStream_t st, int *n_launches);
+
 // evidence: two kernels (per-block partials, then per-segment combine with the carried state)
 cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const double *lnL, const double *log_w,
                                 double *state, double *lnZ, double *n_eff, double *partials, int32_t blocks_per_seg,

@@ -157,9 +157,11 @@ def test_config4_small_all_points_elementwise(gpu_lib):
         rZ, rN = oracle.evidence(ref)
         assert rel_err([rZ], lnZ[p:p + 1].cpu().numpy()) <= TOL
         assert rel_err([rN], neff[p:p + 1].cpu().numpy()) <= TOL
-        # single-point entry gives the same numbers as the all-points launch
+        # single-point entry gives the same numbers as the all-points launch, up to the summation order of the
+        # log-sum-exp (the sorted kernel splits a window over warps by the tile's time range, and the order of equal
+        # keys in its counting sort is free): a few ulp, far inside TOL
         one, _ = ctx.eval(to_dev(per[p]), point=p, want_idx=False)
-        assert torch.equal(one, lnL[p])
+        assert rel_err(lnL[p].cpu().numpy(), one.cpu().numpy()) <= 1e-13
     ctx.close()
 
 
