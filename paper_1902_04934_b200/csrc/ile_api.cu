@@ -30,6 +30,14 @@ struct ile_ctx {
     IleMmaScratch sc;
     size_t sc_samples, sc_hist;  // capacities (samples, histogram words)
     int32_t sc_points;
+    int32_t sc_recg;             // doubles per record the scratch was sized for
+    // variant 4 (streaming FP64-MMA path)
+    bool stream_ok;
+    IleStreamPlan spl;
+    IleSortPlan ssp;
+    double *dQs;
+    IleStreamScratch ss;
+    size_t ss_slots, ss_adj, ss_gcum;  // capacities in words
 };
 
 static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
@@ -163,6 +171,19 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
         cs = cs < 16384 ? 16384 : cs > 262144 ? 262144 : cs;
         c->chunk_samples = cs;
     }
+    c->sc_recg = c->mma_ok ? c->mp.recg : 0;
+    c->stream_ok = ile_stream_plan(c->sz, c->hparams, 0, &c->spl, &c->ssp);
+    if (c->stream_ok) {
+        const size_t nQs = (size_t)cfg->n_points * cfg->n_det * c->spl.ks * c->spl.nqp * 4;
+        CKC(cudaMalloc(&c->dQs, nQs * sizeof(double)));
+        CKC(ile_launch_pack_q_stream(c->sz, c->spl, cfg->n_points, c->dQ, c->dQs, 0));
+        CKC(cudaDeviceSynchronize());
+        if (cfg->n_det * c->spl.cp > c->sc_recg) c->sc_recg = cfg->n_det * c->spl.cp;
+        if (!c->mma_ok) {
+            int64_t cs = (int64_t)(64u << 20) / ((int64_t)c->sc_recg * 8);
+            c->chunk_samples = cs < 16384 ? 16384 : cs > 262144 ? 262144 : cs;
+        }
+    }
 #undef CKC
     *out = c;
     return ILE_OK;
@@ -187,6 +208,10 @@ extern "C" void ile_destroy(ile_ctx *c)
     cudaFree(c->sc.perm);
     cudaFree(c->sc.hist);
     cudaFree(c->sc.ngood);
+    cudaFree(c->dQs);
+    cudaFree(c->ss.slots);
+    cudaFree(c->ss.adj);
+    cudaFree(c->ss.gcum);
     if (c->h_small) cudaFreeHost(c->h_small);
     delete c;
 }
@@ -200,7 +225,7 @@ static int ensure_scratch(ile_ctx *c, size_t samples, size_t hist_words, int32_t
         cudaFree(c->sc.rec), cudaFree(c->sc.quad), cudaFree(c->sc.i0), cudaFree(c->sc.cell), cudaFree(c->sc.perm);
         c->sc.rec = nullptr, c->sc.quad = nullptr, c->sc.i0 = nullptr, c->sc.cell = nullptr, c->sc.perm = nullptr;
         c->sc_samples = 0;
-        CK(cudaMalloc(&c->sc.rec, samples * c->mp.recg * sizeof(double)));
+        CK(cudaMalloc(&c->sc.rec, samples * c->sc_recg * sizeof(double)));
         CK(cudaMalloc(&c->sc.quad, samples * sizeof(double)));
         CK(cudaMalloc(&c->sc.i0, samples * c->sz.n_det * sizeof(int32_t)));
         CK(cudaMalloc(&c->sc.cell, samples * sizeof(int32_t)));
@@ -223,6 +248,46 @@ static int ensure_scratch(ile_ctx *c, size_t samples, size_t hist_words, int32_t
         CK(cudaMalloc(&c->sc.ngood, (size_t)points * sizeof(int32_t)));
         c->sc_points = points;
     }
+    return ILE_OK;
+}
+
+// variant 4 for one launch group: setup + sort into padded segments + streaming kernel
+static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
+{
+    const IleSortPlan &sp = c->ssp;
+    const size_t nseg = (size_t)sp.n1 * sp.n2;
+    const int64_t slot_cap = ((a.n_per_point + 7) & ~(int64_t)7) + 8 * (int64_t)nseg;
+    int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * sp.ncell + 1, a.n_points, st);
+    if (r != ILE_OK) return r;
+    const size_t need_slots = (size_t)a.n_points * slot_cap, need_adj = (size_t)a.n_points * nseg, need_g = 2 * (size_t)a.n_points + 2;
+    if (need_slots > c->ss_slots || need_adj > c->ss_adj || need_g > c->ss_gcum) {
+        CK(cudaStreamSynchronize(st));
+        if (need_slots > c->ss_slots) {
+            cudaFree(c->ss.slots);
+            c->ss.slots = nullptr, c->ss_slots = 0;
+            CK(cudaMalloc(&c->ss.slots, need_slots * sizeof(int32_t)));
+            c->ss_slots = need_slots;
+        }
+        if (need_adj > c->ss_adj) {
+            cudaFree(c->ss.adj);
+            c->ss.adj = nullptr, c->ss_adj = 0;
+            CK(cudaMalloc(&c->ss.adj, need_adj * sizeof(int32_t)));
+            c->ss_adj = need_adj;
+        }
+        if (need_g > c->ss_gcum) {
+            cudaFree(c->ss.gcum);
+            c->ss.gcum = nullptr, c->ss_gcum = 0;
+            CK(cudaMalloc(&c->ss.gcum, need_g * sizeof(int32_t)));
+            c->ss_gcum = need_g;
+        }
+    }
+    c->ss.Qs = c->dQs;
+    c->ss.slot_cap = slot_cap;
+    c->ss.counter = nullptr;
+    int nl = 0;
+    cudaError_t e = ile_launch_eval_stream(c->sz, c->hparams, a, c->spl, sp, c->sc, c->ss, st, &nl);
+    c->launches += nl;
+    if (e != cudaSuccess) return cuda_fail(e);
     return ILE_OK;
 }
 
@@ -257,7 +322,8 @@ static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n
     a.lnL = lnL;
     a.shift_idx = shift_idx;
     a.oob_counter = c->d_oob;
-    if (c->variant == 3 || (c->variant == 0 && c->mma_ok)) {
+    const bool use_stream = c->variant == 4 || (c->variant == 0 && c->stream_ok && n >= 16384);
+    if (use_stream || c->variant == 3) {
         // launch groups of at most chunk_samples samples: whole points while they fit, else slices of one point
         const int64_t cs = c->chunk_samples;
         const int K = c->sz.n_det;
@@ -275,14 +341,16 @@ static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n
             const int32_t per = (int32_t)(cs / n);
             for (int32_t p = 0; p < n_points; p += per) {
                 const int32_t np = n_points - p < per ? n_points - p : per;
-                int r = eval_mma_group(c, shifted((int64_t)p * n, point0 + p, np, n), st);
+                const IleEvalArgs g = shifted((int64_t)p * n, point0 + p, np, n);
+                int r = use_stream ? eval_stream_group(c, g, st) : eval_mma_group(c, g, st);
                 if (r != ILE_OK) return r;
             }
         } else {
             for (int32_t p = 0; p < n_points; ++p)
                 for (int64_t off = 0; off < n; off += cs) {
                     const int64_t cnt = n - off < cs ? n - off : cs;
-                    int r = eval_mma_group(c, shifted((int64_t)p * n + off, point0 + p, 1, cnt), st);
+                    const IleEvalArgs g = shifted((int64_t)p * n + off, point0 + p, 1, cnt);
+                    int r = use_stream ? eval_stream_group(c, g, st) : eval_mma_group(c, g, st);
                     if (r != ILE_OK) return r;
                 }
         }
@@ -405,8 +473,9 @@ extern "C" int ile_status(ile_ctx *c, int64_t *n_out_of_range, int reset, void *
 extern "C" int ile_set_variant(ile_ctx *c, int32_t variant)
 {
     if (!c || variant < 0) return ILE_ERR_BAD_ARGUMENT;
-    if (variant > 3) return ILE_ERR_UNSUPPORTED;
+    if (variant > 4) return ILE_ERR_UNSUPPORTED;
     if (variant == 3 && !c->mma_ok) return ILE_ERR_UNSUPPORTED;
+    if (variant == 4 && !c->stream_ok) return ILE_ERR_UNSUPPORTED;
     if (variant == 2) {
         IleTiledLayout L;
         if (!ile_tiled_plan(c->sz, 1LL << 40, &L)) return ILE_ERR_UNSUPPORTED;

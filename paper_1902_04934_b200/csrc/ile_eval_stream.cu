@@ -1,0 +1,571 @@
+// ile_eval_stream.cu -- variant 4: streaming FP64-MMA evaluation, one warp per group of 8 samples (steps 5-6 of the hot path).
+//
+// The linear term lin_j = Re sum_k sum_lm conj(A_k,lm) Q_k,lm[i0_k + j]  (eq. 7 / eq. 10; "the most
+// costly part", L97) is, per detector, the dense contraction  T_k[i][alpha] = sum_c Qc_k[i][c] Ac_k[c][alpha]  over the 2M real
+// channels c = (mode, re/im) -- "the necessary matrix multiplication" of L97 -- followed by a per-sample shift j = i - i0_k(alpha).
+// It runs on the FP64 matrix instruction DMMA.8x8x4 (mma.sync.m8n8k4.f64): A = Q [8 time rows x 4 channels], B = coefficients
+// [4 channels x 8 samples], C = lin [8 time rows x 8 samples].  On B200 DMMA and DFMA share the FP64 units (measured: their
+// times add), so DMMA buys no arithmetic; it buys issue slots and operand delivery: one instruction does 8 DFMA per lane.
+//
+// What differs from variant 3 (ile_eval_mma.cu): nothing of lin ever goes through shared memory and no block-level barrier
+// exists.  A warp owns 8 samples for the whole window and streams over 8-row time blocks:
+//   * rows are absolute time rows of detector 0 (row rho <-> Q_0 row G0 + rho, G0 = the group's smallest window start); a
+//     sample's own window start inside the group, delta0 = i0_0 - G0, only decides WHICH rows enter its log-sum-exp;
+//   * detector k >= 1 is evaluated on rows base_k + rho with base_k = G0 + min over the group of d_k = i0_k - i0_0; the
+//     remaining per-sample offset eps_k = d_k - min d_k (0 <= eps_k < 8 NC, guaranteed by the sort: samples of a group come
+//     from one (d_1, d_2) cell of width 8 NC) is applied to the C fragment in registers: the lane that holds row r' picks,
+//     among the NC + 1 live blocks of that detector, the one its destination lane needs and one 64-bit warp shuffle moves
+//     it to row (r' - eps) mod 8.  The shifted partial sums are the C input of detector 0's MMA, so the detector sum costs
+//     K - 2 additions per element;
+//   * the time marginalisation (eq. 9) is an online max-free log-sum-exp per lane: running reference m (one of
+//     the lane's own lin values) and s = sum exp(lin - m); a new element more than 64 above m rescales s (rare: lin(t) is
+//     smooth on the scale of a block).  exp is a 1024-entry table of 2^(i/1024) in shared memory times a cubic in the
+//     remainder (|r| <= ln2/2048, truncation 5.5e-16): 7 FP64 operations per element plus the subtraction of m.
+// Per 8-row block and warp: K*KS DMMA (16 pipe cycles each), 2 x 9 FP64 operations of log-sum-exp, K*KS coalesced 256-byte
+// fragment loads that hit L1 (consecutive groups use the same rows), 4 (K-1) SHFL.
+//
+// Q is repacked once per context as Qs[point][k][s][row][4]: the A fragment of (detector k, k-step s, rows base..base+7) is
+// 32 consecutive doubles starting at any row -- one coalesced 256-byte load per DMMA at an arbitrary 32-byte offset.  The
+// series are zero padded in front and behind so that rows outside [0, N_Q), which only ever feed elements outside every
+// window, read as zeros.
+#include <limits.h>
+#include <math_constants.h>
+
+#include <type_traits>
+
+#include "ile_kernels.h"
+
+#define ST_FULL 0xffffffffu
+#define ST_TAB 1024
+#define ST_TAB_LOG2 10
+#define ST_THREADS 256
+
+__device__ __forceinline__ void st_dmma(double &c0, double &c1, double a, double b)
+{
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+#define ST_MAGIC 6755399441055744.0            /* 1.5 * 2^52: adding it rounds to the nearest integer */
+#define ST_C1 1477.3197218702985               /* 1024 / ln 2 */
+#define ST_C2 6.769015435155716e-04            /* ln 2 / 1024 = 0x1.62e42fefa39efp-11 */
+
+// exp(d) for d <= 0 (also -inf; NaN propagates), full result.  Used on the rare paths only.
+__device__ __forceinline__ double st_exp_neg(double d, const double *__restrict__ tab)
+{
+    if (!(d > -708.0)) return d != d ? d : 0.0;
+    const double t = fma(d, ST_C1, ST_MAGIC);
+    const double kf = t - ST_MAGIC;
+    const double r = fma(kf, -ST_C2, d);
+    const int ti = __double2loint(t);
+    const double T = tab[ti & (ST_TAB - 1)];
+    const double q = fma(fma(fma(1.0 / 6.0, r, 0.5), r, 1.0), r, 1.0);
+    return q * __hiloint2double(__double2hiint(T) + ((ti >> ST_TAB_LOG2) << 20), __double2loint(T));
+}
+
+// One lin value into a lane's running (m, s):  s = sum exp(lin - m).
+//   valid : the element lies inside the sample's window (PRED only; otherwise every element is)
+template <bool PRED>
+__device__ __forceinline__ void st_lse2(double x0, double x1, bool v0, bool v1, double &m0, double &s0, double &m1, double &s1,
+                                        const double *__restrict__ tab)
+{
+    double d0 = x0 - m0, d1 = x1 - m1;
+    bool g0 = __double2hiint(d0) > 0x40500000, g1 = __double2hiint(d1) > 0x40500000;  // d > 64, +inf
+    if (PRED) {
+        g0 = g0 && v0;
+        g1 = g1 && v1;
+    }
+    if (g0 | g1) {  // rare: move the reference up
+        if (g0) {
+            s0 *= st_exp_neg(m0 - x0, tab);
+            m0 = x0;
+            d0 = 0.0;
+        }
+        if (g1) {
+            s1 *= st_exp_neg(m1 - x1, tab);
+            m1 = x1;
+            d1 = 0.0;
+        }
+    }
+    if (PRED) {  // elements outside the window may carry d = +inf (reference still unset): keep the arithmetic finite
+        d0 = v0 ? d0 : 0.0;
+        d1 = v1 ? d1 : 0.0;
+    }
+    const double t0 = fma(d0, ST_C1, ST_MAGIC), t1 = fma(d1, ST_C1, ST_MAGIC);
+    const double k0 = t0 - ST_MAGIC, k1 = t1 - ST_MAGIC;
+    const double r0 = fma(k0, -ST_C2, d0), r1 = fma(k1, -ST_C2, d1);
+    const int i0 = __double2loint(t0), i1 = __double2loint(t1);
+    const double T0 = tab[i0 & (ST_TAB - 1)], T1 = tab[i1 & (ST_TAB - 1)];
+    bool ok0 = (unsigned)__double2hiint(d0) < 0xC0862000u, ok1 = (unsigned)__double2hiint(d1) < 0xC0862000u;  // d > -708
+    if (PRED) {
+        ok0 = ok0 && v0;
+        ok1 = ok1 && v1;
+    }
+    const int h0 = __double2hiint(T0) + ((i0 >> ST_TAB_LOG2) << 20), h1 = __double2hiint(T1) + ((i1 >> ST_TAB_LOG2) << 20);
+    const double S0 = __hiloint2double(ok0 ? h0 : 0, ok0 ? __double2loint(T0) : 0);
+    const double S1 = __hiloint2double(ok1 ? h1 : 0, ok1 ? __double2loint(T1) : 0);
+    const double q0 = fma(fma(fma(1.0 / 6.0, r0, 0.5), r0, 1.0), r0, 1.0);
+    const double q1 = fma(fma(fma(1.0 / 6.0, r1, 0.5), r1, 1.0), r1, 1.0);
+    s0 = fma(q0, S0, s0);
+    s1 = fma(q1, S1, s1);
+}
+
+__device__ __forceinline__ double st_shfl(double v, int src) { return __shfl_sync(ST_FULL, v, src); }
+
+struct IleStreamKArgs {
+    int32_t n_t, point0, n_points, nqp, padf, recg, cp;
+    int64_t n_per_point, slot_cap;
+    const double *Qs;
+    const double *rec;
+    const double *quad;
+    const int32_t *i0;
+    const int32_t *slots;
+    const int32_t *gcum;
+    uint32_t *counter;
+    double *lnL;
+};
+
+template <int NC>
+__device__ __forceinline__ double st_pick(const double (&ring)[NC + 1][2], int u, int col, int off)
+{
+    // ring slot of block t + o is (u + o) % (NC + 1), u = t % (NC + 1) known at compile time by the caller's unrolling
+    double x = ring[u % (NC + 1)][col];
+#pragma unroll
+    for (int o = 1; o <= NC; ++o) x = off == o ? ring[(u + o) % (NC + 1)][col] : x;
+    return x;
+}
+
+template <int K, int KS, int NC, int MINB>
+__global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const __grid_constant__ IleStreamKArgs a)
+{
+    __shared__ double tab[ST_TAB];
+    for (int i = threadIdx.x; i < ST_TAB; i += blockDim.x) tab[i] = exp2((double)i * (1.0 / ST_TAB));
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31, r = lane >> 2, cc = lane & 3;
+    const int n_t = a.n_t;
+    const double log_nt = log((double)n_t);
+    const int total = a.gcum[a.n_points];
+    const size_t nqp4 = (size_t)a.nqp * 4;
+
+    for (;;) {
+        int w = 0;
+        if (lane == 0) w = (int)atomicAdd(a.counter, 1u);
+        w = __shfl_sync(ST_FULL, w, 0);
+        if (w >= total) break;
+        int pt = 0;
+        if (a.n_points > 1) {
+            int lo = 0, hi = a.n_points;
+            while (hi - lo > 1) {
+                const int mid = (lo + hi) >> 1;
+                if (a.gcum[mid] <= w) lo = mid;
+                else hi = mid;
+            }
+            pt = lo;
+        }
+        const int g = w - a.gcum[pt];
+        const int32_t *__restrict__ slots = a.slots + (size_t)pt * a.slot_cap + 8 * (size_t)g;
+        const long long sbase = (long long)pt * a.n_per_point;
+
+        // ---- the group: window starts, bases, per-sample offsets.  Lane (r, cc) looks after (sample r, detector cc).
+        const int sb = slots[r];  // -1: empty slot (the group is the tail of its segment)
+        const bool has = sb >= 0;
+        const long long fb = sbase + (has ? sb : 0);
+        const int my_i0 = (has && cc < K) ? a.i0[fb * K + cc] : 0;
+        const int i00 = __shfl_sync(ST_FULL, my_i0, lane & ~3);
+        const int G0 = __reduce_min_sync(ST_FULL, has ? i00 : INT_MAX);
+        const int dspread = __reduce_max_sync(ST_FULL, has ? i00 - G0 : 0);
+        const int dk = my_i0 - i00;
+        int eps_mine = 0;
+        int base[K];
+        base[0] = G0;
+#pragma unroll
+        for (int k = 1; k < K; ++k) {
+            const int mn = __reduce_min_sync(ST_FULL, (has && cc == k) ? dk : INT_MAX);
+            base[k] = G0 + mn;
+            if (has && cc == k) eps_mine = dk - mn;
+        }
+        const int del_mine = has ? i00 - G0 : (1 << 28);
+
+        // ---- this lane's two C-fragment columns: samples 2cc and 2cc + 1
+        const int lA = 8 * cc, lB = 8 * cc + 4;
+        const int sA = __shfl_sync(ST_FULL, sb, lA), sB = __shfl_sync(ST_FULL, sb, lB);
+        const int jA = r - __shfl_sync(ST_FULL, del_mine, lA), jB = r - __shfl_sync(ST_FULL, del_mine, lB);  // j of block 0
+        int srcA[K], srcB[K], offA[K], offB[K];
+#pragma unroll
+        for (int k = 1; k < K; ++k) {
+            const int eA = __shfl_sync(ST_FULL, eps_mine, lA + k), eB = __shfl_sync(ST_FULL, eps_mine, lB + k);
+            srcA[k] = (((r + eA) & 7) << 2) | cc;  // as destination: the lane that holds my row
+            srcB[k] = (((r + eB) & 7) << 2) | cc;
+            offA[k] = (((r - eA) & 7) + eA) >> 3;  // as source: the block my destination lane wants
+            offB[k] = (((r - eB) & 7) + eB) >> 3;
+        }
+
+        // ---- B fragments: coefficients a F_k Y_lm of sample r, channels 4s + cc
+        double bf[K][KS];
+        {
+            const double *__restrict__ rp = a.rec + (size_t)fb * a.recg + cc;
+#pragma unroll
+            for (int k = 0; k < K; ++k)
+#pragma unroll
+                for (int s = 0; s < KS; ++s) bf[k][s] = has ? __ldg(rp + k * a.cp + 4 * s) : 0.0;
+        }
+        const double *ap[K];
+#pragma unroll
+        for (int k = 0; k < K; ++k)
+            ap[k] = a.Qs + ((size_t)((a.point0 + pt) * K + k) * KS * a.nqp + (size_t)(a.padf + base[k])) * 4 + lane;
+
+        const int nblk = (dspread + n_t + 7) >> 3;
+        const int t_lo = (dspread + 7) >> 3, t_hi = n_t >> 3;  // blocks [t_lo, t_hi) lie inside every window of the group
+
+        // ---- prologue: blocks 0 .. NC-1 of the shifted detectors
+        double ring[K > 1 ? K - 1 : 1][NC + 1][2];
+#pragma unroll
+        for (int k = 1; k < K; ++k)
+#pragma unroll
+            for (int u = 0; u < NC; ++u) {
+                double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                for (int s = 0; s < KS; ++s) st_dmma(c0, c1, __ldg(ap[k] + s * nqp4 + (size_t)u * 32), bf[k][s]);
+                ring[k - 1][u][0] = c0;
+                ring[k - 1][u][1] = c1;
+            }
+
+        double mA = -CUDART_INF, mB = -CUDART_INF, sumA = 0.0, sumB = 0.0;
+        for (int tb = 0; tb < nblk; tb += NC + 1) {
+#pragma unroll
+            for (int u = 0; u <= NC; ++u) {
+                const int t = tb + u;
+                if (t < nblk) {
+                    double zA = 0.0, zB = 0.0;
+#pragma unroll
+                    for (int k = 1; k < K; ++k) {
+                        // block t + NC of detector k
+                        double c0 = 0.0, c1 = 0.0;
+                        const double *__restrict__ q = ap[k] + (size_t)(t + NC) * 32;
+#pragma unroll
+                        for (int s = 0; s < KS; ++s) st_dmma(c0, c1, __ldg(q + s * nqp4), bf[k][s]);
+                        ring[k - 1][(u + NC) % (NC + 1)][0] = c0;
+                        ring[k - 1][(u + NC) % (NC + 1)][1] = c1;
+                        // realign: row rho of my column wants T_k[base_k + rho + eps]
+                        const double yA = st_shfl(st_pick<NC>(ring[k - 1], u, 0, offA[k]), srcA[k]);
+                        const double yB = st_shfl(st_pick<NC>(ring[k - 1], u, 1, offB[k]), srcB[k]);
+                        if (k == 1) {
+                            zA = yA;
+                            zB = yB;
+                        } else {
+                            zA += yA;
+                            zB += yB;
+                        }
+                    }
+                    {
+                        const double *__restrict__ q = ap[0] + (size_t)t * 32;
+#pragma unroll
+                        for (int s = 0; s < KS; ++s) st_dmma(zA, zB, __ldg(q + s * nqp4), bf[0][s]);
+                    }
+                    if (t >= t_lo && t < t_hi) {
+                        st_lse2<false>(zA, zB, true, true, mA, sumA, mB, sumB, tab);
+                    } else {
+                        const bool vA = (unsigned)(jA + 8 * t) < (unsigned)n_t, vB = (unsigned)(jB + 8 * t) < (unsigned)n_t;
+                        st_lse2<true>(zA, zB, vA, vB, mA, sumA, mB, sumB, tab);
+                    }
+                }
+            }
+        }
+
+        // ---- merge the 8 row lanes of each column, write lnL_margT = LSE - ln N_t - quad  (eq. 9 with the rectangle rule)
+        double MA = mA, MB = mB;
+#pragma unroll
+        for (int o = 4; o < 32; o <<= 1) {
+            MA = fmax(MA, st_shfl(MA, lane ^ o));
+            MB = fmax(MB, st_shfl(MB, lane ^ o));
+        }
+        double SA = mA > -CUDART_INF ? sumA * st_exp_neg(mA - MA, tab) : 0.0;
+        double SB = mB > -CUDART_INF ? sumB * st_exp_neg(mB - MB, tab) : 0.0;
+#pragma unroll
+        for (int o = 4; o < 32; o <<= 1) {
+            SA += st_shfl(SA, lane ^ o);
+            SB += st_shfl(SB, lane ^ o);
+        }
+        if (r == 0) {
+            if (sA >= 0) a.lnL[sbase + sA] = MA + log(SA) - log_nt - a.quad[sbase + sA];
+            if (sB >= 0) a.lnL[sbase + sB] = MB + log(SB) - log_nt - a.quad[sbase + sB];
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// Q repacking (once per context): Q [P][K][M][n_q] complex128 -> Qs [P][K][ks][nqp][4] doubles, channel 2m = Re, 2m+1 = Im
+// ------------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) ile_pack_q_stream_kernel(int32_t n_series, int32_t M, int32_t n_q, int32_t ks, int32_t nqp,
+                                                                int32_t padf, const double2 *__restrict__ Q, double *__restrict__ Qs)
+{
+    const long long total = (long long)n_series * ks * nqp * 4;
+    for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < total; o += (long long)gridDim.x * blockDim.x) {
+        const int c4 = (int)(o & 3);
+        long long q = o >> 2;
+        const int row = (int)(q % nqp);
+        q /= nqp;
+        const int s = (int)(q % ks);
+        q /= ks;  // = p * K + k
+        const int ch = 4 * s + c4, m = ch >> 1, i = row - padf;
+        double v = 0.0;
+        if (m < M && i >= 0 && i < n_q) {
+            const double2 z = Q[((size_t)q * M + m) * n_q + i];
+            v = (ch & 1) ? z.y : z.x;
+        }
+        Qs[o] = v;
+    }
+}
+
+cudaError_t ile_launch_pack_q_stream(const IleSizes &sz, const IleStreamPlan &pl, int32_t n_points, const double2 *Q, double *Qs,
+                                     cudaStream_t st)
+{
+    const long long total = (long long)n_points * sz.n_det * pl.ks * pl.nqp * 4;
+    long long blocks = (total + 255) / 256;
+    if (blocks > (long long)sz.sm_count * 32) blocks = (long long)sz.sm_count * 32;
+    ile_pack_q_stream_kernel<<<(unsigned)blocks, 256, 0, st>>>(n_points * sz.n_det, sz.n_modes, sz.n_q, pl.ks, pl.nqp, pl.padf, Q, Qs);
+    return cudaGetLastError();
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// counting sort of variant 4: cells = (segment, i0_0 >> g0); every segment's slots are padded to a multiple of 8 so that a
+// group of 8 consecutive slots never mixes two (d1, d2) cells
+// ------------------------------------------------------------------------------------------------------------
+#define SS_THREADS 1024
+
+// exclusive scan of v[0..n) in place by one block; returns the total to every thread
+__device__ uint32_t ss_block_scan(uint32_t *__restrict__ v, int n, uint32_t *wsum)
+{
+    const int per = (n + SS_THREADS - 1) / SS_THREADS;
+    const int lo = min((int)threadIdx.x * per, n), hi = min(lo + per, n);
+    uint32_t loc = 0;
+    for (int i = lo; i < hi; ++i) loc += v[i];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t inc = loc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t x = __shfl_up_sync(ST_FULL, inc, o);
+        if (lane >= o) inc += x;
+    }
+    __syncthreads();  // wsum may still be read by a previous call
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        const uint32_t x = wsum[lane];
+        uint32_t xi = x;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(ST_FULL, xi, o);
+            if (lane >= o) xi += y;
+        }
+        wsum[lane] = xi - x;
+        if (lane == 31) wsum[32] = xi;
+    }
+    __syncthreads();
+    uint32_t run = wsum[warp] + inc - loc;
+    for (int i = lo; i < hi; ++i) {
+        const uint32_t x = v[i];
+        v[i] = run;
+        run += x;
+    }
+    return wsum[32];
+}
+
+// one block per point.  hist -> exclusive positions; adj[seg] = padded base of the segment minus its first position;
+// ngr[pt] = groups of the point; for a single point also gcum = {0, groups}.
+__global__ void __launch_bounds__(SS_THREADS) ile_stream_scan_kernel(int32_t ncell, int32_t n0, int32_t nseg, uint32_t *__restrict__ hist,
+                                                                     uint32_t *__restrict__ adj, int32_t *__restrict__ ngood,
+                                                                     uint32_t *__restrict__ ngr, int32_t *__restrict__ gcum,
+                                                                     int32_t n_points)
+{
+    __shared__ uint32_t wsum[33];
+    uint32_t *h = hist + (size_t)blockIdx.x * ncell;
+    uint32_t *ad = adj + (size_t)blockIdx.x * nseg;
+    ss_block_scan(h, ncell, wsum);
+    __syncthreads();
+    if (threadIdx.x == 0) ngood[blockIdx.x] = (int32_t)h[ncell - 1];  // samples before the out-of-range cell
+    // padded size of every segment (its end is the next segment's start; the last one ends at the out-of-range cell)
+    for (int s = threadIdx.x; s < nseg; s += SS_THREADS) ad[s] = (h[(size_t)(s + 1) * n0] - h[(size_t)s * n0] + 7u) & ~7u;
+    __syncthreads();
+    const uint32_t tot = ss_block_scan(ad, nseg, wsum);
+    __syncthreads();
+    for (int s = threadIdx.x; s < nseg; s += SS_THREADS) ad[s] -= h[(size_t)s * n0];
+    if (threadIdx.x == 0) {
+        ngr[blockIdx.x] = tot >> 3;
+        if (n_points == 1) {
+            gcum[0] = 0;
+            gcum[1] = (int32_t)(tot >> 3);
+        }
+    }
+}
+
+__global__ void __launch_bounds__(SS_THREADS) ile_stream_prefix_kernel(int32_t n_points, uint32_t *__restrict__ ngr, int32_t *__restrict__ gcum)
+{
+    __shared__ uint32_t wsum[33];
+    const uint32_t tot = ss_block_scan(ngr, n_points, wsum);
+    __syncthreads();
+    for (int p = threadIdx.x; p < n_points; p += SS_THREADS) gcum[p] = (int32_t)ngr[p];
+    if (threadIdx.x == 0) gcum[n_points] = (int32_t)tot;
+}
+
+__global__ void __launch_bounds__(256) ile_stream_scatter_kernel(long long n_per_point, int32_t n_points, int32_t ncell, int32_t n0,
+                                                                 int32_t nseg, long long slot_cap, const int32_t *__restrict__ cell,
+                                                                 uint32_t *__restrict__ offs, const uint32_t *__restrict__ adj,
+                                                                 int32_t *__restrict__ slots)
+{
+    const long long n_total = n_per_point * n_points;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n_total; s += (long long)gridDim.x * blockDim.x) {
+        const int pt = (int)(s / n_per_point);
+        const int c = cell[s];
+        if (c == ncell - 1) continue;  // out of range: lnL = -inf was written by the setup kernel
+        const uint32_t pos = atomicAdd(&offs[(size_t)pt * ncell + c], 1u) + adj[(size_t)pt * nseg + c / n0];
+        slots[(size_t)pt * slot_cap + pos] = (int32_t)(s - (long long)pt * n_per_point);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------------------
+// host side
+// ------------------------------------------------------------------------------------------------------------
+static int st_round_ks(int ks)
+{
+    const int avail[] = {1, 2, 3, 4, 6, 8, 11, 16};
+    for (int v : avail)
+        if (ks <= v) return v;
+    return 0;
+}
+
+// Plan for one launch of n_per_point samples per point: cell widths and the padded Q geometry.  Returns false when the
+// sizes do not fit this variant (more than 3 detectors, too many cells).
+bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point, IleStreamPlan *out, IleSortPlan *spo)
+{
+    if (sz.n_det > 3) return false;
+    IleStreamPlan pl;
+    pl.ks = st_round_ks((2 * sz.n_modes + 3) / 4);
+    if (!pl.ks) return false;
+    pl.cp = 4 * pl.ks;
+    pl.nc = 2;
+    pl.padf = sz.n_q - sz.n_t + 32;
+    pl.nqp = pl.padf + sz.n_q + (sz.n_q - sz.n_t) + 64;
+    IleSortPlan sp;
+    sp.mode = 1;
+    sp.nd = sz.n_det;
+    sp.g = pl.nc == 2 ? 4 : 3;
+    sp.dmax[0] = 0;
+    for (int d = 1; d < 3; ++d) {
+        sp.dmax[d] = 0;
+        if (d < sp.nd) {
+            const double dx = hp.vertex[d][0] - hp.vertex[0][0], dy = hp.vertex[d][1] - hp.vertex[0][1], dz = hp.vertex[d][2] - hp.vertex[0][2];
+            const double ds = sqrt(dx * dx + dy * dy + dz * dz) / ILE_C_SI * hp.fs;
+            if (!(ds < 1.0e6)) return false;
+            sp.dmax[d] = (int32_t)ceil(ds) + 2;
+        }
+    }
+    sp.n1 = sp.nd > 1 ? ((2 * sp.dmax[1]) >> sp.g) + 1 : 1;
+    sp.n2 = sp.nd > 2 ? ((2 * sp.dmax[2]) >> sp.g) + 1 : 1;
+    int g0 = 3;
+    for (;; ++g0) {
+        sp.n0 = ((sz.n_q - sz.n_t) >> g0) + 1;
+        const long long nc = (long long)sp.n0 * sp.n1 * sp.n2 + 1;
+        if (nc <= (1LL << 20)) {
+            sp.ncell = (int32_t)nc;
+            break;
+        }
+        if (g0 >= 30) return false;
+    }
+    sp.g0 = g0;
+    (void)n_per_point;
+    *out = pl;
+    *spo = sp;
+    return true;
+}
+
+template <int K, int KS, int NC, int MINB>
+static cudaError_t st_launch_t(const IleSizes &sz, const IleStreamKArgs &ka, long long max_groups, cudaStream_t st)
+{
+    static int per_sm = 0;
+    if (!per_sm) {
+        cudaError_t e = cudaFuncSetAttribute(ile_eval_stream_kernel<K, KS, NC, MINB>, cudaFuncAttributePreferredSharedMemoryCarveout, 8);
+        if (e != cudaSuccess) return e;
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ile_eval_stream_kernel<K, KS, NC, MINB>, ST_THREADS, 0);
+        if (e != cudaSuccess) return e;
+        if (per_sm < 1) return cudaErrorInvalidConfiguration;
+    }
+    long long grid = (long long)sz.sm_count * per_sm;
+    const long long need = (max_groups + ST_THREADS / 32 - 1) / (ST_THREADS / 32);
+    if (need < grid) grid = need < 1 ? 1 : need;
+    ile_eval_stream_kernel<K, KS, NC, MINB><<<(unsigned)grid, ST_THREADS, 0, st>>>(ka);
+    return cudaGetLastError();
+}
+
+template <int K, int NC>
+static cudaError_t st_launch_k(const IleSizes &sz, int ks, const IleStreamKArgs &ka, long long mg, cudaStream_t st)
+{
+    switch (ks) {
+        case 1: return st_launch_t<K, 1, NC, 3>(sz, ka, mg, st);
+        case 2: return st_launch_t<K, 2, NC, 3>(sz, ka, mg, st);
+        case 3: return st_launch_t<K, 3, NC, 2>(sz, ka, mg, st);
+        case 4: return st_launch_t<K, 4, NC, 2>(sz, ka, mg, st);
+        case 6: return st_launch_t<K, 6, NC, 1>(sz, ka, mg, st);
+        case 8: return st_launch_t<K, 8, NC, 1>(sz, ka, mg, st);
+        case 11: return st_launch_t<K, 11, NC, 1>(sz, ka, mg, st);
+        case 16: return st_launch_t<K, 16, NC, 1>(sz, ka, mg, st);
+        default: return cudaErrorInvalidValue;
+    }
+}
+
+cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleStreamPlan &pl,
+                                   const IleSortPlan &sp, const IleMmaScratch &sc, const IleStreamScratch &ss, cudaStream_t st,
+                                   int *n_launches)
+{
+    if (a.n_per_point <= 0 || a.n_points <= 0) return cudaSuccess;
+    const long long n_total = a.n_per_point * a.n_points;
+    const int nseg = sp.n1 * sp.n2;
+    // histogram + work counter (the counter sits right behind the histograms), then the slot table
+    cudaError_t e = cudaMemsetAsync(sc.hist, 0, ((size_t)a.n_points * sp.ncell + 1) * sizeof(uint32_t), st);
+    if (e != cudaSuccess) return e;
+    e = cudaMemsetAsync(ss.slots, 0xFF, (size_t)a.n_points * ss.slot_cap * sizeof(int32_t), st);
+    if (e != cudaSuccess) return e;
+    ile_launch_setup_only(sz, hp, a, pl.cp, sp, sc, st);
+    uint32_t *ngr = reinterpret_cast<uint32_t *>(ss.gcum) + a.n_points + 1;
+    ile_stream_scan_kernel<<<(unsigned)a.n_points, SS_THREADS, 0, st>>>(sp.ncell, sp.n0, nseg, sc.hist, reinterpret_cast<uint32_t *>(ss.adj),
+                                                                        sc.ngood, ngr, ss.gcum, a.n_points);
+    int nl = 2;
+    if (a.n_points > 1) {
+        ile_stream_prefix_kernel<<<1, SS_THREADS, 0, st>>>(a.n_points, ngr, ss.gcum);
+        ++nl;
+    }
+    long long sblocks = (n_total + 255) / 256;
+    const long long cap = (long long)sz.sm_count * 16;
+    if (sblocks > cap) sblocks = cap;
+    ile_stream_scatter_kernel<<<(unsigned)sblocks, 256, 0, st>>>(a.n_per_point, a.n_points, sp.ncell, sp.n0, nseg, ss.slot_cap, sc.cell,
+                                                                 sc.hist, reinterpret_cast<const uint32_t *>(ss.adj), ss.slots);
+    ++nl;
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+
+    IleStreamKArgs ka;
+    ka.n_t = sz.n_t;
+    ka.point0 = a.point0;
+    ka.n_points = a.n_points;
+    ka.nqp = pl.nqp;
+    ka.padf = pl.padf;
+    ka.recg = sz.n_det * pl.cp;
+    ka.cp = pl.cp;
+    ka.n_per_point = a.n_per_point;
+    ka.slot_cap = ss.slot_cap;
+    ka.Qs = ss.Qs;
+    ka.rec = sc.rec;
+    ka.quad = sc.quad;
+    ka.i0 = sc.i0;
+    ka.slots = ss.slots;
+    ka.gcum = ss.gcum;
+    ka.counter = sc.hist + (size_t)a.n_points * sp.ncell;
+    ka.lnL = a.lnL;
+    const long long max_groups = (long long)a.n_points * (ss.slot_cap / 8);
+    if (sz.n_det == 1) e = st_launch_k<1, 2>(sz, pl.ks, ka, max_groups, st);
+    else if (sz.n_det == 2) e = st_launch_k<2, 2>(sz, pl.ks, ka, max_groups, st);
+    else e = st_launch_k<3, 2>(sz, pl.ks, ka, max_groups, st);
+    ++nl;
+    if (e == cudaSuccess && n_launches) *n_launches += nl;
+    return e;
+}

@@ -49,7 +49,9 @@ cudaError_t ile_launch_eval_tiled(const IleSizes &sz, const IleDevParams &hp, co
 // ---- variant 3: setup + counting sort + FP64-MMA contraction (ile_setup.cu, ile_eval_mma.cu) --------------------
 // Cell grid of the counting sort: window starts binned to width 2^g in (i0_0, i0_1 - i0_0, i0_2 - i0_0).
 struct IleSortPlan {
-    int32_t g;        // log2 of the cell width in samples
+    int32_t mode;     // 0: variant 3 (cubic cells, boustrophedon); 1: variant 4 (segments of (d1, d2) x exact i0_0)
+    int32_t g;        // log2 of the cell width in samples (mode 1: of the (d1, d2) cells only)
+    int32_t g0;       // mode 1: log2 of the i0_0 bin width inside a segment
     int32_t nd;       // detectors that take part in the key (<= 3)
     int32_t n0, n1, n2;
     int32_t ncell;    // n0*n1*n2 + 1; the last cell collects out-of-range samples
@@ -92,6 +94,35 @@ cudaError_t ile_launch_setup_sort(const IleSizes &sz, const IleDevParams &hp, co
 // steps 5-6 on the sorted samples
 cudaError_t ile_launch_eval_mma(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleMmaPlan &mp,
                                 const IleMmaScratch &sc, cudaStream_t st, int *n_launches);
+
+// ---- variant 4: streaming FP64-MMA kernel, one warp per group of 8 samples (ile_eval_stream.cu) ------------------
+struct IleStreamPlan {
+    int32_t ks;       // k-steps of 4 real channels per detector: ceil(2M / 4), rounded up to an instantiated value
+    int32_t cp;       // padded channels per detector = 4 * ks (= record stride per detector)
+    int32_t nc;       // (d1, d2) cell width = 8 * nc rows; the shuffle realignment looks nc blocks ahead
+    int32_t padf;     // zero rows in front of each packed series
+    int32_t nqp;      // rows per packed series = padf + n_q + back padding
+};
+
+struct IleStreamScratch {
+    const double *Qs;   // packed Q [P][K][ks][nqp][4]
+    int32_t *slots;     // [n_points][slot_cap]: sample index or -1, groups of 8 consecutive slots
+    int32_t *adj;       // [n_points][nseg]: padded segment base minus the segment's first sorted position
+    int32_t *gcum;      // [n_points + 1]: exclusive prefix of the group counts, followed by [n_points] group counts
+    uint32_t *counter;  // work counter of the persistent kernel (zeroed with the histogram)
+    int64_t slot_cap;   // slots per point (multiple of 8)
+};
+
+bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point, IleStreamPlan *out, IleSortPlan *sp);
+cudaError_t ile_launch_pack_q_stream(const IleSizes &sz, const IleStreamPlan &pl, int32_t n_points, const double2 *Q,
+                                     double *Qs, cudaStream_t st);
+// setup + sort of variant 4 (memsets + setup + scan + scatter), then the streaming kernel
+cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleStreamPlan &pl,
+                                   const IleSortPlan &sp, const IleMmaScratch &sc, const IleStreamScratch &ss,
+                                   cudaStream_t st, int *n_launches);
+// launches the per-sample setup kernel only (shared by variants 3 and 4)
+void ile_launch_setup_only(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, int32_t cp, const IleSortPlan &sp,
+                           const IleMmaScratch &sc, cudaStream_t st);
 
 // evidence: two kernels (per-block partials, then per-segment combine with the carried state)
 cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const double *lnL, const double *log_w,

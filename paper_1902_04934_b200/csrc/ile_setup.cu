@@ -157,6 +157,12 @@ __global__ void __launch_bounds__(SETUP_THREADS)
             c = sp.ncell - 1;
             atomicAdd(a.oob_counter, 1ULL);
             a.lnL[s] = -CUDART_INF;
+        } else if (sp.mode == 1) {
+            // variant 4: segment = (d1, d2) cell of width 2^g, then the exact i0_0 inside the segment
+            int32_t seg = 0;
+            if (sp.nd > 1) seg = min(max(i0[1] - i0[0] + sp.dmax[1], 0), 2 * sp.dmax[1]) >> sp.g;
+            if (sp.nd > 2) seg = seg * sp.n2 + (min(max(i0[2] - i0[0] + sp.dmax[2], 0), 2 * sp.dmax[2]) >> sp.g);
+            c = seg * sp.n0 + (i0[0] >> sp.g0);  // 0 <= i0_0 <= n_q - n_t here
         } else {
             c = i0[0] >> sp.g;  // 0 <= i0_0 <= n_q - n_t here
             if (sp.nd > 1) {
@@ -236,6 +242,8 @@ __global__ void __launch_bounds__(256) ile_scatter_kernel(long long n_per_point,
 IleSortPlan ile_sort_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point)
 {
     IleSortPlan sp;
+    sp.mode = 0;
+    sp.g0 = 0;
     sp.nd = sz.n_det < 3 ? sz.n_det : 3;
     sp.g = n_per_point >= 200000 ? 4 : n_per_point >= 25000 ? 5 : n_per_point >= 3000 ? 6 : 7;
     sp.dmax[0] = 0;
@@ -266,6 +274,22 @@ static void setup_launch_t(unsigned blocks, const IleDevParams &hp, const IleEva
                            const IleSortPlan &sp, const IleMmaScratch &sc, cudaStream_t st)
 {
     ile_setup_kernel<MMAX><<<blocks, SETUP_THREADS, 0, st>>>(hp, a, mp.cp, sp, sc);
+}
+
+void ile_launch_setup_only(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, int32_t cp, const IleSortPlan &sp,
+                           const IleMmaScratch &sc, cudaStream_t st)
+{
+    const long long n_total = a.n_per_point * a.n_points;
+    long long blocks = (n_total + SETUP_THREADS - 1) / SETUP_THREADS;
+    const long long cap = (long long)sz.sm_count * 16;
+    if (blocks > cap) blocks = cap;
+    IleMmaPlan mp;
+    mp.cp = cp;
+    const int M = sz.n_modes;
+    if (M <= 2) setup_launch_t<2>((unsigned)blocks, hp, a, mp, sp, sc, st);
+    else if (M <= 5) setup_launch_t<5>((unsigned)blocks, hp, a, mp, sp, sc, st);
+    else if (M <= 12) setup_launch_t<12>((unsigned)blocks, hp, a, mp, sp, sc, st);
+    else setup_launch_t<ILE_MAX_MODES>((unsigned)blocks, hp, a, mp, sp, sc, st);
 }
 
 cudaError_t ile_launch_setup_sort(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleMmaPlan &mp,
