@@ -42,39 +42,49 @@
 
 __device__ __forceinline__ void st_dmma(double &c0, double &c1, double a, double b)
 {
-    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
 #define ST_MAGIC 6755399441055744.0            /* 1.5 * 2^52: adding it rounds to the nearest integer */
 #define ST_C1 1477.3197218702985               /* 1024 / ln 2 */
 #define ST_C2 6.769015435155716e-04            /* ln 2 / 1024 = 0x1.62e42fefa39efp-11 */
 
+// entry i of the table 2^(i/1024) in shared memory (tab = 32-bit shared address of entry 0)
+__device__ __forceinline__ double st_tab(uint32_t tab, int i)
+{
+    double v;
+    asm("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(tab + ((uint32_t)(i & (ST_TAB - 1)) << 3)));
+    return v;
+}
+
 // exp(d) for d <= 0 (also -inf; NaN propagates), full result.  Used on the rare paths only.
-__device__ __forceinline__ double st_exp_neg(double d, const double *__restrict__ tab)
+__device__ __forceinline__ double st_exp_neg(double d, uint32_t tab)
 {
     if (!(d > -708.0)) return d != d ? d : 0.0;
     const double t = fma(d, ST_C1, ST_MAGIC);
     const double kf = t - ST_MAGIC;
     const double r = fma(kf, -ST_C2, d);
     const int ti = __double2loint(t);
-    const double T = tab[ti & (ST_TAB - 1)];
+    const double T = st_tab(tab, ti);
     const double q = fma(fma(fma(1.0 / 6.0, r, 0.5), r, 1.0), r, 1.0);
     return q * __hiloint2double(__double2hiint(T) + ((ti >> ST_TAB_LOG2) << 20), __double2loint(T));
 }
 
-// One lin value into a lane's running (m, s):  s = sum exp(lin - m).
-//   valid : the element lies inside the sample's window (PRED only; otherwise every element is)
+// Log-sum-exp of one block, first half: d = lin - m for the lane's two columns; a valid element more than 64 above the
+// reference moves the reference up (rare: the only branch of the block).
+//   v0, v1 : the element lies inside the sample's window (PRED only; otherwise every element does)
 template <bool PRED>
-__device__ __forceinline__ void st_lse2(double x0, double x1, bool v0, bool v1, double &m0, double &s0, double &m1, double &s1,
-                                        const double *__restrict__ tab)
+__device__ __forceinline__ void st_lse_pre(double x0, double x1, bool v0, bool v1, double &m0, double &s0, double &m1, double &s1,
+                                           double &d0, double &d1, uint32_t tab)
 {
-    double d0 = x0 - m0, d1 = x1 - m1;
+    d0 = x0 - m0;
+    d1 = x1 - m1;
     bool g0 = __double2hiint(d0) > 0x40500000, g1 = __double2hiint(d1) > 0x40500000;  // d > 64, +inf
     if (PRED) {
         g0 = g0 && v0;
         g1 = g1 && v1;
     }
-    if (g0 | g1) {  // rare: move the reference up
+    if (g0 | g1) {
         if (g0) {
             s0 *= st_exp_neg(m0 - x0, tab);
             m0 = x0;
@@ -90,11 +100,17 @@ __device__ __forceinline__ void st_lse2(double x0, double x1, bool v0, bool v1, 
         d0 = v0 ? d0 : 0.0;
         d1 = v1 ? d1 : 0.0;
     }
+}
+
+// second half, branch free: s += exp(d) = 2^k * tab[i] * cubic(r) with d = (1024 k + i) ln2/1024 + r
+template <bool PRED>
+__device__ __forceinline__ void st_lse_main(double d0, double d1, bool v0, bool v1, double &s0, double &s1, uint32_t tab)
+{
     const double t0 = fma(d0, ST_C1, ST_MAGIC), t1 = fma(d1, ST_C1, ST_MAGIC);
     const double k0 = t0 - ST_MAGIC, k1 = t1 - ST_MAGIC;
     const double r0 = fma(k0, -ST_C2, d0), r1 = fma(k1, -ST_C2, d1);
     const int i0 = __double2loint(t0), i1 = __double2loint(t1);
-    const double T0 = tab[i0 & (ST_TAB - 1)], T1 = tab[i1 & (ST_TAB - 1)];
+    const double T0 = st_tab(tab, i0), T1 = st_tab(tab, i1);
     bool ok0 = (unsigned)__double2hiint(d0) < 0xC0862000u, ok1 = (unsigned)__double2hiint(d1) < 0xC0862000u;  // d > -708
     if (PRED) {
         ok0 = ok0 && v0;
@@ -111,6 +127,13 @@ __device__ __forceinline__ void st_lse2(double x0, double x1, bool v0, bool v1, 
 
 __device__ __forceinline__ double st_shfl(double v, int src) { return __shfl_sync(ST_FULL, v, src); }
 
+// m ? b : a for an all-ones / all-zeros mask m: two LOP3, no predicate
+__device__ __forceinline__ double st_bsel(double a, double b, int m)
+{
+    const int al = __double2loint(a), ah = __double2hiint(a), bl = __double2loint(b), bh = __double2hiint(b);
+    return __hiloint2double(ah ^ ((ah ^ bh) & m), al ^ ((al ^ bl) & m));
+}
+
 struct IleStreamKArgs {
     int32_t n_t, point0, n_points, nqp, padf, recg, cp;
     int64_t n_per_point, slot_cap;
@@ -124,15 +147,7 @@ struct IleStreamKArgs {
     double *lnL;
 };
 
-template <int NC>
-__device__ __forceinline__ double st_pick(const double (&ring)[NC + 1][2], int u, int col, int off)
-{
-    // ring slot of block t + o is (u + o) % (NC + 1), u = t % (NC + 1) known at compile time by the caller's unrolling
-    double x = ring[u % (NC + 1)][col];
-#pragma unroll
-    for (int o = 1; o <= NC; ++o) x = off == o ? ring[(u + o) % (NC + 1)][col] : x;
-    return x;
-}
+#define ST_PFD 2 /* blocks the L1 prefetch runs ahead of the fragment loads */
 
 template <int K, int KS, int NC, int MINB>
 __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const __grid_constant__ IleStreamKArgs a)
@@ -140,6 +155,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
     __shared__ double tab[ST_TAB];
     for (int i = threadIdx.x; i < ST_TAB; i += blockDim.x) tab[i] = exp2((double)i * (1.0 / ST_TAB));
     __syncthreads();
+    const uint32_t tab_addr = (uint32_t)__cvta_generic_to_shared(tab);
 
     const int lane = threadIdx.x & 31, r = lane >> 2, cc = lane & 3;
     const int n_t = a.n_t;
@@ -190,14 +206,18 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
         const int lA = 8 * cc, lB = 8 * cc + 4;
         const int sA = __shfl_sync(ST_FULL, sb, lA), sB = __shfl_sync(ST_FULL, sb, lB);
         const int jA = r - __shfl_sync(ST_FULL, del_mine, lA), jB = r - __shfl_sync(ST_FULL, del_mine, lB);  // j of block 0
-        int srcA[K], srcB[K], offA[K], offB[K];
+        int srcA[K], srcB[K], mskA[K][NC], mskB[K][NC];
 #pragma unroll
         for (int k = 1; k < K; ++k) {
             const int eA = __shfl_sync(ST_FULL, eps_mine, lA + k), eB = __shfl_sync(ST_FULL, eps_mine, lB + k);
             srcA[k] = (((r + eA) & 7) << 2) | cc;  // as destination: the lane that holds my row
             srcB[k] = (((r + eB) & 7) << 2) | cc;
-            offA[k] = (((r - eA) & 7) + eA) >> 3;  // as source: the block my destination lane wants
-            offB[k] = (((r - eB) & 7) + eB) >> 3;
+            const int oA = (((r - eA) & 7) + eA) >> 3, oB = (((r - eB) & 7) + eB) >> 3;  // as source: the block my destination wants
+#pragma unroll
+            for (int o = 0; o < NC; ++o) {
+                mskA[k][o] = oA == o + 1 ? -1 : 0;
+                mskB[k][o] = oB == o + 1 ? -1 : 0;
+            }
         }
 
         // ---- B fragments: coefficients a F_k Y_lm of sample r, channels 4s + cc
@@ -209,10 +229,22 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
 #pragma unroll
                 for (int s = 0; s < KS; ++s) bf[k][s] = has ? __ldg(rp + k * a.cp + 4 * s) : 0.0;
         }
-        const double *ap[K];
+        // ---- A fragment pointers: pk[k] = this lane's element of the next block to load of detector k
+        const double *pk[K];
 #pragma unroll
         for (int k = 0; k < K; ++k)
-            ap[k] = a.Qs + ((size_t)((a.point0 + pt) * K + k) * KS * a.nqp + (size_t)(a.padf + base[k])) * 4 + lane;
+            pk[k] = a.Qs + ((size_t)((a.point0 + pt) * K + k) * KS * a.nqp + (size_t)(a.padf + base[k])) * 4 + lane;
+        // L1 prefetch: lane l looks after 128-byte line (l % 3) of fragment (l / 3) = (detector, k-step), ST_PFD blocks ahead
+        const double *pf = nullptr;
+        {
+            const int f = lane / 3, fk = f / KS, fs = f - fk * KS;
+            if (f < K * KS) {
+                const int bk = fk == 0 ? base[0] - 8 * NC : fk == 1 ? base[K > 1 ? 1 : 0] : base[K > 2 ? 2 : 0];
+                const int j = lane - 3 * f;
+                pf = a.Qs + ((size_t)((a.point0 + pt) * K + fk) * KS * a.nqp + (size_t)fs * a.nqp + (size_t)(a.padf + bk)) * 4 +
+                     (size_t)(NC + ST_PFD) * 32 + (j == 2 ? 31 : 16 * j);
+            }
+        }
 
         const int nblk = (dspread + n_t + 7) >> 3;
         const int t_lo = (dspread + 7) >> 3, t_hi = n_t >> 3;  // blocks [t_lo, t_hi) lie inside every window of the group
@@ -220,56 +252,96 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
         // ---- prologue: blocks 0 .. NC-1 of the shifted detectors
         double ring[K > 1 ? K - 1 : 1][NC + 1][2];
 #pragma unroll
-        for (int k = 1; k < K; ++k)
+        for (int k = 1; k < K; ++k) {
 #pragma unroll
             for (int u = 0; u < NC; ++u) {
                 double c0 = 0.0, c1 = 0.0;
 #pragma unroll
-                for (int s = 0; s < KS; ++s) st_dmma(c0, c1, __ldg(ap[k] + s * nqp4 + (size_t)u * 32), bf[k][s]);
+                for (int s = 0; s < KS; ++s) st_dmma(c0, c1, __ldg(pk[k] + s * nqp4 + (size_t)u * 32), bf[k][s]);
                 ring[k - 1][u][0] = c0;
                 ring[k - 1][u][1] = c1;
             }
+            pk[k] += NC * 32;
+        }
 
-        double mA = -CUDART_INF, mB = -CUDART_INF, sumA = 0.0, sumB = 0.0;
-        for (int tb = 0; tb < nblk; tb += NC + 1) {
+        // ---- the stream.  One step = log-sum-exp of block t-1 (its lin values are in linA, linB) + lin of block t; the two
+        // halves are independent, so the DFMA chain of the first fills the dependency gaps of the DMMA chains of the second.
+        double mA = -CUDART_INF, mB = -CUDART_INF, sumA = 0.0, sumB = 0.0, linA = 0.0, linB = 0.0;
+        auto step = [&](auto UC, auto PC, const int t) {
+            constexpr int u = decltype(UC)::value;
+            constexpr bool PRED = decltype(PC)::value;
+            bool vA = true, vB = true;
+            if (PRED) {
+                vA = (unsigned)(jA + 8 * (t - 1)) < (unsigned)n_t;
+                vB = (unsigned)(jB + 8 * (t - 1)) < (unsigned)n_t;
+            }
+            double dA, dB;
+            st_lse_pre<PRED>(linA, linB, vA, vB, mA, sumA, mB, sumB, dA, dB, tab_addr);
+            // fragments of this step: block t + NC of the shifted detectors, block t of detector 0
+            double af[K][KS];
 #pragma unroll
-            for (int u = 0; u <= NC; ++u) {
-                const int t = tb + u;
-                if (t < nblk) {
-                    double zA = 0.0, zB = 0.0;
+            for (int k = 0; k < K; ++k) {
 #pragma unroll
-                    for (int k = 1; k < K; ++k) {
-                        // block t + NC of detector k
-                        double c0 = 0.0, c1 = 0.0;
-                        const double *__restrict__ q = ap[k] + (size_t)(t + NC) * 32;
+                for (int s = 0; s < KS; ++s) af[k][s] = __ldg(pk[(k + 1) % K] + s * nqp4);
+            }
 #pragma unroll
-                        for (int s = 0; s < KS; ++s) st_dmma(c0, c1, __ldg(q + s * nqp4), bf[k][s]);
-                        ring[k - 1][(u + NC) % (NC + 1)][0] = c0;
-                        ring[k - 1][(u + NC) % (NC + 1)][1] = c1;
-                        // realign: row rho of my column wants T_k[base_k + rho + eps]
-                        const double yA = st_shfl(st_pick<NC>(ring[k - 1], u, 0, offA[k]), srcA[k]);
-                        const double yB = st_shfl(st_pick<NC>(ring[k - 1], u, 1, offB[k]), srcB[k]);
-                        if (k == 1) {
-                            zA = yA;
-                            zB = yB;
-                        } else {
-                            zA += yA;
-                            zB += yB;
-                        }
-                    }
-                    {
-                        const double *__restrict__ q = ap[0] + (size_t)t * 32;
+            for (int k = 0; k < K; ++k) pk[k] += 32;
+            if (pf) {
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(pf));
+                pf += 32;
+            }
+            st_lse_main<PRED>(dA, dB, vA, vB, sumA, sumB, tab_addr);
+            double zA = 0.0, zB = 0.0;
 #pragma unroll
-                        for (int s = 0; s < KS; ++s) st_dmma(zA, zB, __ldg(q + s * nqp4), bf[0][s]);
-                    }
-                    if (t >= t_lo && t < t_hi) {
-                        st_lse2<false>(zA, zB, true, true, mA, sumA, mB, sumB, tab);
-                    } else {
-                        const bool vA = (unsigned)(jA + 8 * t) < (unsigned)n_t, vB = (unsigned)(jB + 8 * t) < (unsigned)n_t;
-                        st_lse2<true>(zA, zB, vA, vB, mA, sumA, mB, sumB, tab);
-                    }
+            for (int k = 1; k < K; ++k) {
+                double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                for (int s = 0; s < KS; ++s) st_dmma(c0, c1, af[k - 1][s], bf[k][s]);
+                ring[k - 1][(u + NC) % (NC + 1)][0] = c0;
+                ring[k - 1][(u + NC) % (NC + 1)][1] = c1;
+            }
+#pragma unroll
+            for (int k = 1; k < K; ++k) {
+                // realign: row rho of my column wants T_k[base_k + rho + eps]; I hold it for the lane (rho - eps) mod 8
+                double xA = ring[k - 1][u % (NC + 1)][0], xB = ring[k - 1][u % (NC + 1)][1];
+#pragma unroll
+                for (int o = 1; o <= NC; ++o) {
+                    xA = st_bsel(xA, ring[k - 1][(u + o) % (NC + 1)][0], mskA[k][o - 1]);
+                    xB = st_bsel(xB, ring[k - 1][(u + o) % (NC + 1)][1], mskB[k][o - 1]);
+                }
+                const double yA = st_shfl(xA, srcA[k]), yB = st_shfl(xB, srcB[k]);
+                if (k == 1) {
+                    zA = yA;
+                    zB = yB;
+                } else {
+                    zA += yA;
+                    zB += yB;
                 }
             }
+#pragma unroll
+            for (int s = 0; s < KS; ++s) st_dmma(zA, zB, af[K - 1][s], bf[0][s]);
+            linA = zA;
+            linB = zB;
+        };
+#define ST_STEP(U)                                                                                        \
+    if constexpr (NC >= (U)) {                                                                            \
+        const int t = tb + (U);                                                                           \
+        if (t < nblk) {                                                                                   \
+            if (t > t_lo && t <= t_hi) step(std::integral_constant<int, (U)>(), std::false_type(), t);   \
+            else step(std::integral_constant<int, (U)>(), std::true_type(), t);                          \
+        }                                                                                                 \
+    }
+        for (int tb = 0; tb < nblk; tb += NC + 1) {
+            ST_STEP(0)
+            ST_STEP(1)
+            ST_STEP(2)
+        }
+#undef ST_STEP
+        {  // the last block's log-sum-exp
+            const bool vA = (unsigned)(jA + 8 * (nblk - 1)) < (unsigned)n_t, vB = (unsigned)(jB + 8 * (nblk - 1)) < (unsigned)n_t;
+            double dA, dB;
+            st_lse_pre<true>(linA, linB, vA, vB, mA, sumA, mB, sumB, dA, dB, tab_addr);
+            st_lse_main<true>(dA, dB, vA, vB, sumA, sumB, tab_addr);
         }
 
         // ---- merge the 8 row lanes of each column, write lnL_margT = LSE - ln N_t - quad  (eq. 9 with the rectangle rule)
@@ -279,8 +351,8 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
             MA = fmax(MA, st_shfl(MA, lane ^ o));
             MB = fmax(MB, st_shfl(MB, lane ^ o));
         }
-        double SA = mA > -CUDART_INF ? sumA * st_exp_neg(mA - MA, tab) : 0.0;
-        double SB = mB > -CUDART_INF ? sumB * st_exp_neg(mB - MB, tab) : 0.0;
+        double SA = mA > -CUDART_INF ? sumA * st_exp_neg(mA - MA, tab_addr) : 0.0;
+        double SB = mB > -CUDART_INF ? sumB * st_exp_neg(mB - MB, tab_addr) : 0.0;
 #pragma unroll
         for (int o = 4; o < 32; o <<= 1) {
             SA += st_shfl(SA, lane ^ o);
