@@ -38,7 +38,7 @@
 #define ST_FULL 0xffffffffu
 #define ST_TAB 1024
 #define ST_TAB_LOG2 10
-#define ST_THREADS 256
+#define ST_THREADS 128
 
 __device__ __forceinline__ void st_dmma(double &c0, double &c1, double a, double b)
 {
@@ -125,6 +125,71 @@ __device__ __forceinline__ void st_lse_main(double d0, double d1, bool v0, bool 
     s1 = fma(q1, S1, s1);
 }
 
+// Pair version (two blocks b = 0, 1 of the lane's two columns c = 0, 1; x[b][c], column c carries (m[c], s[c])): one branch
+// for the four elements.  The elements of a column are taken in block order, so the rare path redoes the second one
+// against the reference the first one may have moved.
+template <bool PRED>
+__device__ __forceinline__ void st_lse_pre2(const double (&x)[2][2], const bool (&v)[2][2], double (&m)[2], double (&s)[2],
+                                            double (&d)[2][2], uint32_t tab)
+{
+    bool any = false;
+#pragma unroll
+    for (int b = 0; b < 2; ++b)
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            d[b][c] = x[b][c] - m[c];
+            bool g = __double2hiint(d[b][c]) > 0x40500000;  // d > 64, +inf
+            if (PRED) g = g && v[b][c];
+            any = any || g;
+        }
+    if (any) {
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+#pragma unroll
+            for (int b = 0; b < 2; ++b) {
+                bool g = __double2hiint(x[b][c] - m[c]) > 0x40500000;
+                if (PRED) g = g && v[b][c];
+                if (g) {
+                    s[c] *= st_exp_neg(m[c] - x[b][c], tab);
+                    m[c] = x[b][c];
+                }
+            }
+            // every element of the column against the final reference (none of them has been added to s yet)
+            d[0][c] = x[0][c] - m[c];
+            d[1][c] = x[1][c] - m[c];
+        }
+    }
+    if (PRED) {  // elements outside the window may carry d = +inf (reference still unset): keep the arithmetic finite
+#pragma unroll
+        for (int b = 0; b < 2; ++b)
+#pragma unroll
+            for (int c = 0; c < 2; ++c) d[b][c] = v[b][c] ? d[b][c] : 0.0;
+    }
+}
+
+template <bool PRED>
+__device__ __forceinline__ void st_lse_main2(const double (&d)[2][2], const bool (&v)[2][2], double (&s)[2], uint32_t tab)
+{
+    double e[2][2], S[2][2];
+#pragma unroll
+    for (int b = 0; b < 2; ++b)
+#pragma unroll
+        for (int c = 0; c < 2; ++c) {
+            const double t = fma(d[b][c], ST_C1, ST_MAGIC);
+            const double kf = t - ST_MAGIC;
+            const double r = fma(kf, -ST_C2, d[b][c]);
+            const int ti = __double2loint(t);
+            const double T = st_tab(tab, ti);
+            bool ok = (unsigned)__double2hiint(d[b][c]) < 0xC0862000u;  // d > -708
+            if (PRED) ok = ok && v[b][c];
+            const int h = __double2hiint(T) + ((ti >> ST_TAB_LOG2) << 20);
+            S[b][c] = __hiloint2double(ok ? h : 0, ok ? __double2loint(T) : 0);
+            e[b][c] = fma(fma(fma(1.0 / 6.0, r, 0.5), r, 1.0), r, 1.0);
+        }
+#pragma unroll
+    for (int c = 0; c < 2; ++c) s[c] = fma(e[1][c], S[1][c], fma(e[0][c], S[0][c], s[c]));
+}
+
 __device__ __forceinline__ double st_shfl(double v, int src) { return __shfl_sync(ST_FULL, v, src); }
 
 // m ? b : a for an all-ones / all-zeros mask m: two LOP3, no predicate
@@ -147,7 +212,7 @@ struct IleStreamKArgs {
     double *lnL;
 };
 
-#define ST_PFD 2 /* blocks the L1 prefetch runs ahead of the fragment loads */
+#define ST_PFS 1 /* steps (pairs of blocks) the L1 prefetch runs ahead of the fragment loads */
 
 template <int K, int KS, int NC, int MINB>
 __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const __grid_constant__ IleStreamKArgs a)
@@ -206,19 +271,21 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
         const int lA = 8 * cc, lB = 8 * cc + 4;
         const int sA = __shfl_sync(ST_FULL, sb, lA), sB = __shfl_sync(ST_FULL, sb, lB);
         const int jA = r - __shfl_sync(ST_FULL, del_mine, lA), jB = r - __shfl_sync(ST_FULL, del_mine, lB);  // j of block 0
-        int srcA[K], srcB[K], mskA[K][NC], mskB[K][NC];
+        // per shifted detector k and column c: src = the lane that holds my row; off = as a source, the block (relative to
+        // the destination's) my destination lane wants
+        int src[K][2], msk[K][2][NC];
 #pragma unroll
         for (int k = 1; k < K; ++k) {
-            const int eA = __shfl_sync(ST_FULL, eps_mine, lA + k), eB = __shfl_sync(ST_FULL, eps_mine, lB + k);
-            srcA[k] = (((r + eA) & 7) << 2) | cc;  // as destination: the lane that holds my row
-            srcB[k] = (((r + eB) & 7) << 2) | cc;
-            const int oA = (((r - eA) & 7) + eA) >> 3, oB = (((r - eB) & 7) + eB) >> 3;  // as source: the block my destination wants
 #pragma unroll
-            for (int o = 0; o < NC; ++o) {
-                mskA[k][o] = oA == o + 1 ? -1 : 0;
-                mskB[k][o] = oB == o + 1 ? -1 : 0;
+            for (int c = 0; c < 2; ++c) {
+                const int e = __shfl_sync(ST_FULL, eps_mine, 8 * cc + 4 * c + k);
+                src[k][c] = (((r + e) & 7) << 2) | cc;
+                const int off = (((r - e) & 7) + e) >> 3;
+#pragma unroll
+                for (int o = 0; o < NC; ++o) msk[k][c][o] = off == o + 1 ? -1 : 0;
             }
         }
+        const int jc[2] = {jA, jB};
 
         // ---- B fragments: coefficients a F_k Y_lm of sample r, channels 4s + cc
         double bf[K][KS];
@@ -234,7 +301,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
 #pragma unroll
         for (int k = 0; k < K; ++k)
             pk[k] = a.Qs + ((size_t)((a.point0 + pt) * K + k) * KS * a.nqp + (size_t)(a.padf + base[k])) * 4 + lane;
-        // L1 prefetch: lane l looks after 128-byte line (l % 3) of fragment (l / 3) = (detector, k-step), ST_PFD blocks ahead
+        // L1 prefetch: lane l looks after 128-byte line (l % 3) of fragment (l / 3) = (detector, k-step) of a block
         const double *pf = nullptr;
         {
             const int f = lane / 3, fk = f / KS, fs = f - fk * KS;
@@ -242,15 +309,15 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
                 const int bk = fk == 0 ? base[0] - 8 * NC : fk == 1 ? base[K > 1 ? 1 : 0] : base[K > 2 ? 2 : 0];
                 const int j = lane - 3 * f;
                 pf = a.Qs + ((size_t)((a.point0 + pt) * K + fk) * KS * a.nqp + (size_t)fs * a.nqp + (size_t)(a.padf + bk)) * 4 +
-                     (size_t)(NC + ST_PFD) * 32 + (j == 2 ? 31 : 16 * j);
+                     (size_t)(NC + 2 + 2 * ST_PFS) * 32 + (j == 2 ? 31 : 16 * j);
             }
         }
 
-        const int nblk = (dspread + n_t + 7) >> 3;
+        const int nblk = ((dspread + n_t + 7) >> 3) + 1 & ~1;  // even: the stream advances two blocks per step
         const int t_lo = (dspread + 7) >> 3, t_hi = n_t >> 3;  // blocks [t_lo, t_hi) lie inside every window of the group
 
-        // ---- prologue: blocks 0 .. NC-1 of the shifted detectors
-        double ring[K > 1 ? K - 1 : 1][NC + 1][2];
+        // ---- prologue: blocks 0 .. NC-1 of the shifted detectors into the ring (slot of block b = b % 4); first fragments
+        double ring[K > 1 ? K - 1 : 1][4][2];
 #pragma unroll
         for (int k = 1; k < K; ++k) {
 #pragma unroll
@@ -263,86 +330,123 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
             }
             pk[k] += NC * 32;
         }
-
-        // ---- the stream.  One step = log-sum-exp of block t-1 (its lin values are in linA, linB) + lin of block t; the two
-        // halves are independent, so the DFMA chain of the first fills the dependency gaps of the DMMA chains of the second.
-        double mA = -CUDART_INF, mB = -CUDART_INF, sumA = 0.0, sumB = 0.0, linA = 0.0, linB = 0.0;
-        auto step = [&](auto UC, auto PC, const int t) {
-            constexpr int u = decltype(UC)::value;
-            constexpr bool PRED = decltype(PC)::value;
-            bool vA = true, vB = true;
-            if (PRED) {
-                vA = (unsigned)(jA + 8 * (t - 1)) < (unsigned)n_t;
-                vB = (unsigned)(jB + 8 * (t - 1)) < (unsigned)n_t;
-            }
-            double dA, dB;
-            st_lse_pre<PRED>(linA, linB, vA, vB, mA, sumA, mB, sumB, dA, dB, tab_addr);
-            // fragments of this step: block t + NC of the shifted detectors, block t of detector 0
-            double af[K][KS];
+        // fragments in registers one step ahead while they fit (PIPE); otherwise loaded where they are used
+        constexpr bool PIPE = KS <= 4;
+        double af[K][2][PIPE ? KS : 1];  // [k][block of the pair][k-step]; k = 0 is detector 0
+        if (PIPE) {
 #pragma unroll
             for (int k = 0; k < K; ++k) {
 #pragma unroll
-                for (int s = 0; s < KS; ++s) af[k][s] = __ldg(pk[(k + 1) % K] + s * nqp4);
+                for (int bb = 0; bb < 2; ++bb)
+#pragma unroll
+                    for (int s = 0; s < KS; ++s) af[k][bb][PIPE ? s : 0] = __ldg(pk[k] + s * nqp4 + bb * 32);
+                pk[k] += 64;
+            }
+        }
+
+        // ---- the stream.  One step = two blocks (t0, t0 + 1): the shifted detectors' MMAs of blocks t0 + NC, t0 + NC + 1
+        // (2 (K-1) independent chains), the log-sum-exp of the PREVIOUS pair (independent of everything else in the step),
+        // the realignment, detector 0's MMAs (2 chains).  Fragments are loaded one step ahead into the registers the
+        // chains have just released.
+        double m[2] = {-CUDART_INF, -CUDART_INF}, sm[2] = {0.0, 0.0}, lin[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+        auto step = [&](auto PC, auto PREDC, const int t0) {
+            constexpr int P = decltype(PC)::value;  // t0 % 4 == 2 P
+            constexpr bool PRED = decltype(PREDC)::value;
+            bool v[2][2] = {{true, true}, {true, true}};
+            if (PRED) {
+#pragma unroll
+                for (int bb = 0; bb < 2; ++bb)
+#pragma unroll
+                    for (int c = 0; c < 2; ++c) v[bb][c] = (unsigned)(jc[c] + 8 * (t0 - 2 + bb)) < (unsigned)n_t;
+            }
+            double d[2][2];
+            st_lse_pre2<PRED>(lin, v, m, sm, d, tab_addr);
+            // shifted detectors: blocks t0 + NC + bb into ring slots (2 P + NC + bb) % 4
+#pragma unroll
+            for (int k = 1; k < K; ++k) {
+#pragma unroll
+                for (int bb = 0; bb < 2; ++bb) {
+                    double c0 = 0.0, c1 = 0.0;
+#pragma unroll
+                    for (int s = 0; s < KS; ++s)
+                        st_dmma(c0, c1, PIPE ? af[k][bb][PIPE ? s : 0] : __ldg(pk[k] + s * nqp4 + bb * 32), bf[k][s]);
+                    ring[k - 1][(2 * P + NC + bb) % 4][0] = c0;
+                    ring[k - 1][(2 * P + NC + bb) % 4][1] = c1;
+                }
             }
 #pragma unroll
-            for (int k = 0; k < K; ++k) pk[k] += 32;
+            for (int k = 1; k < K; ++k) {
+                pk[k] += PIPE ? 0 : 64;
+                if (PIPE) {
+#pragma unroll
+                    for (int bb = 0; bb < 2; ++bb)
+#pragma unroll
+                        for (int s = 0; s < KS; ++s) af[k][bb][PIPE ? s : 0] = __ldg(pk[k] + s * nqp4 + bb * 32);
+                    pk[k] += 64;
+                }
+            }
             if (pf) {
                 asm volatile("prefetch.global.L1 [%0];" ::"l"(pf));
-                pf += 32;
+                asm volatile("prefetch.global.L1 [%0];" ::"l"(pf + 32));
+                pf += 64;
             }
-            st_lse_main<PRED>(dA, dB, vA, vB, sumA, sumB, tab_addr);
-            double zA = 0.0, zB = 0.0;
+            st_lse_main2<PRED>(d, v, sm, tab_addr);
+            // realign: row rho of my column wants T_k[base_k + rho + eps]; I hold it for the lane (rho - eps) mod 8
+            double z[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
             for (int k = 1; k < K; ++k) {
-                double c0 = 0.0, c1 = 0.0;
 #pragma unroll
-                for (int s = 0; s < KS; ++s) st_dmma(c0, c1, af[k - 1][s], bf[k][s]);
-                ring[k - 1][(u + NC) % (NC + 1)][0] = c0;
-                ring[k - 1][(u + NC) % (NC + 1)][1] = c1;
+                for (int bb = 0; bb < 2; ++bb)
+#pragma unroll
+                    for (int c = 0; c < 2; ++c) {
+                        double x = ring[k - 1][(2 * P + bb) % 4][c];
+#pragma unroll
+                        for (int o = 1; o <= NC; ++o) x = st_bsel(x, ring[k - 1][(2 * P + bb + o) % 4][c], msk[k][c][o - 1]);
+                        const double y = st_shfl(x, src[k][c]);
+                        z[bb][c] = k == 1 ? y : z[bb][c] + y;
+                    }
             }
 #pragma unroll
-            for (int k = 1; k < K; ++k) {
-                // realign: row rho of my column wants T_k[base_k + rho + eps]; I hold it for the lane (rho - eps) mod 8
-                double xA = ring[k - 1][u % (NC + 1)][0], xB = ring[k - 1][u % (NC + 1)][1];
+            for (int bb = 0; bb < 2; ++bb) {
 #pragma unroll
-                for (int o = 1; o <= NC; ++o) {
-                    xA = st_bsel(xA, ring[k - 1][(u + o) % (NC + 1)][0], mskA[k][o - 1]);
-                    xB = st_bsel(xB, ring[k - 1][(u + o) % (NC + 1)][1], mskB[k][o - 1]);
-                }
-                const double yA = st_shfl(xA, srcA[k]), yB = st_shfl(xB, srcB[k]);
-                if (k == 1) {
-                    zA = yA;
-                    zB = yB;
-                } else {
-                    zA += yA;
-                    zB += yB;
-                }
+                for (int s = 0; s < KS; ++s)
+                    st_dmma(z[bb][0], z[bb][1], PIPE ? af[0][bb][PIPE ? s : 0] : __ldg(pk[0] + s * nqp4 + bb * 32), bf[0][s]);
+                lin[bb][0] = z[bb][0];
+                lin[bb][1] = z[bb][1];
             }
+            pk[0] += PIPE ? 0 : 64;
+            if (PIPE) {
 #pragma unroll
-            for (int s = 0; s < KS; ++s) st_dmma(zA, zB, af[K - 1][s], bf[0][s]);
-            linA = zA;
-            linB = zB;
+                for (int bb = 0; bb < 2; ++bb)
+#pragma unroll
+                    for (int s = 0; s < KS; ++s) af[0][bb][PIPE ? s : 0] = __ldg(pk[0] + s * nqp4 + bb * 32);
+                pk[0] += 64;
+            }
         };
-#define ST_STEP(U)                                                                                        \
-    if constexpr (NC >= (U)) {                                                                            \
-        const int t = tb + (U);                                                                           \
-        if (t < nblk) {                                                                                   \
-            if (t > t_lo && t <= t_hi) step(std::integral_constant<int, (U)>(), std::false_type(), t);   \
-            else step(std::integral_constant<int, (U)>(), std::true_type(), t);                          \
-        }                                                                                                 \
+#define ST_STEP(PP)                                                                                         \
+    {                                                                                                       \
+        const int t0 = tb + 2 * (PP);                                                                       \
+        if (t0 < nblk) {                                                                                    \
+            if (t0 - 2 >= t_lo && t0 <= t_hi) step(std::integral_constant<int, (PP)>(), std::false_type(), t0); \
+            else step(std::integral_constant<int, (PP)>(), std::true_type(), t0);                          \
+        }                                                                                                   \
     }
-        for (int tb = 0; tb < nblk; tb += NC + 1) {
+        for (int tb = 0; tb < nblk; tb += 4) {
             ST_STEP(0)
             ST_STEP(1)
-            ST_STEP(2)
         }
 #undef ST_STEP
-        {  // the last block's log-sum-exp
-            const bool vA = (unsigned)(jA + 8 * (nblk - 1)) < (unsigned)n_t, vB = (unsigned)(jB + 8 * (nblk - 1)) < (unsigned)n_t;
-            double dA, dB;
-            st_lse_pre<true>(linA, linB, vA, vB, mA, sumA, mB, sumB, dA, dB, tab_addr);
-            st_lse_main<true>(dA, dB, vA, vB, sumA, sumB, tab_addr);
+        {  // the last pair's log-sum-exp
+            bool v[2][2];
+#pragma unroll
+            for (int bb = 0; bb < 2; ++bb)
+#pragma unroll
+                for (int c = 0; c < 2; ++c) v[bb][c] = (unsigned)(jc[c] + 8 * (nblk - 2 + bb)) < (unsigned)n_t;
+            double d[2][2];
+            st_lse_pre2<true>(lin, v, m, sm, d, tab_addr);
+            st_lse_main2<true>(d, v, sm, tab_addr);
         }
+        const double mA = m[0], mB = m[1], sumA = sm[0], sumB = sm[1];
 
         // ---- merge the 8 row lanes of each column, write lnL_margT = LSE - ln N_t - quad  (eq. 9 with the rectangle rule)
         double MA = mA, MB = mB;
@@ -573,14 +677,14 @@ template <int K, int NC>
 static cudaError_t st_launch_k(const IleSizes &sz, int ks, const IleStreamKArgs &ka, long long mg, cudaStream_t st)
 {
     switch (ks) {
-        case 1: return st_launch_t<K, 1, NC, 3>(sz, ka, mg, st);
-        case 2: return st_launch_t<K, 2, NC, 3>(sz, ka, mg, st);
-        case 3: return st_launch_t<K, 3, NC, 2>(sz, ka, mg, st);
-        case 4: return st_launch_t<K, 4, NC, 2>(sz, ka, mg, st);
-        case 6: return st_launch_t<K, 6, NC, 1>(sz, ka, mg, st);
-        case 8: return st_launch_t<K, 8, NC, 1>(sz, ka, mg, st);
-        case 11: return st_launch_t<K, 11, NC, 1>(sz, ka, mg, st);
-        case 16: return st_launch_t<K, 16, NC, 1>(sz, ka, mg, st);
+        case 1: return st_launch_t<K, 1, NC, 4>(sz, ka, mg, st);
+        case 2: return st_launch_t<K, 2, NC, 4>(sz, ka, mg, st);
+        case 3: return st_launch_t<K, 3, NC, 3>(sz, ka, mg, st);
+        case 4: return st_launch_t<K, 4, NC, 3>(sz, ka, mg, st);
+        case 6: return st_launch_t<K, 6, NC, 2>(sz, ka, mg, st);
+        case 8: return st_launch_t<K, 8, NC, 2>(sz, ka, mg, st);
+        case 11: return st_launch_t<K, 11, NC, 2>(sz, ka, mg, st);
+        case 16: return st_launch_t<K, 16, NC, 2>(sz, ka, mg, st);
         default: return cudaErrorInvalidValue;
     }
 }
