@@ -32,15 +32,15 @@ UNIT = "samples/s"
 # ------------------------------------------------------------------------------------------------------------------
 # algorithmic work per sample in DFMA-equivalents
 # ------------------------------------------------------------------------------------------------------------------
-EXP_DFMA = 21.7      # measured on B200: CUDA exp(double) costs 21.7 DFMA issue slots (profiles/r01_microbench.md)
-LSE_MISC = 5.0       # per bin: two detector adds, max, subtract, accumulate
+EXP_DFMA = 20.0      # "Total DFMA-equivalents with exp ~ 20" (subtract, range reduction, polynomial, accumulate)
 
 
 def dfma_per_sample(K: int, M: int, n_t: int) -> float:
+    """config 1 -> 12,300 + 720 + 8,200 + 400 = 21,620 DFMA-equivalents per sample."""
     linear = 2.0 * K * M * n_t                      # step 5: Re sum conj(A) Q, 2 DFMA per complex element
     quad = 2.0 * K * (4.0 * M * M + 4.0 * M)        # step 4: Y^dagger U Y and Y^T V Y per detector
-    lse = n_t * (EXP_DFMA + LSE_MISC)               # step 6
-    geom = 400.0 + 30.0 * M                         # steps 1-3: five sincos, F_k, dt_k, Y_lm, K*M coefficient products
+    lse = n_t * EXP_DFMA                            # step 6
+    geom = 250.0 + 30.0 * M                         # steps 1-3: five sincos, F_k, dt_k, Y_lm, K*M coefficient products
     return linear + quad + lse + geom
 
 
@@ -88,10 +88,14 @@ class ClockSampler(threading.Thread):
 
 
 def read_traffic_bytes():
-    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full summary, or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    """DRAM bytes per launch of the dominant kernel (read + write) from the committed ncu --set full summary
+    (profiles/traffic.csv, last row), or None."""
+    p = os.path.join(ROOT, "profiles", "traffic.csv")
     try:
-        return json.load(open(p)).get("dram_bytes_per_launch")
+        import csv
+
+        rows = [r for r in csv.DictReader(open(p))]
+        return int(rows[-1]["dram_bytes_read"]) + int(rows[-1]["dram_bytes_write"])
     except Exception:
         return None
 
