@@ -37,7 +37,7 @@ struct ile_ctx {
     IleSortPlan ssp;
     double *dQs;
     IleStreamScratch ss;
-    size_t ss_slots, ss_adj, ss_gcum;  // capacities in words
+    size_t ss_slots, ss_adj, ss_gcum, ss_gorder;  // capacities in words
 };
 
 static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
@@ -174,6 +174,9 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     c->sc_recg = c->mma_ok ? c->mp.recg : 0;
     c->stream_ok = ile_stream_plan(c->sz, c->hparams, 0, &c->spl, &c->ssp);
     if (c->stream_ok) {
+        CKC(cudaStreamCreateWithFlags(&c->ss.aux, cudaStreamNonBlocking));
+        CKC(cudaEventCreateWithFlags(&c->ss.ev_fork, cudaEventDisableTiming));
+        CKC(cudaEventCreateWithFlags(&c->ss.ev_join, cudaEventDisableTiming));
         const size_t nQs = (size_t)cfg->n_points * cfg->n_det * c->spl.ks * c->spl.nqp * 4;
         CKC(cudaMalloc(&c->dQs, nQs * sizeof(double)));
         CKC(ile_launch_pack_q_stream(c->sz, c->spl, cfg->n_points, c->dQ, c->dQs, 0));
@@ -212,6 +215,10 @@ extern "C" void ile_destroy(ile_ctx *c)
     cudaFree(c->ss.slots);
     cudaFree(c->ss.adj);
     cudaFree(c->ss.gcum);
+    cudaFree(c->ss.gorder);
+    if (c->ss.aux) cudaStreamDestroy(c->ss.aux);
+    if (c->ss.ev_fork) cudaEventDestroy(c->ss.ev_fork);
+    if (c->ss.ev_join) cudaEventDestroy(c->ss.ev_join);
     if (c->h_small) cudaFreeHost(c->h_small);
     delete c;
 }
@@ -257,10 +264,11 @@ static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
     const IleSortPlan &sp = c->ssp;
     const size_t nseg = (size_t)sp.n1 * sp.n2;
     const int64_t slot_cap = ((a.n_per_point + 7) & ~(int64_t)7) + 8 * (int64_t)nseg;
-    int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * sp.ncell + 1, a.n_points, st);
+    int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES, a.n_points, st);
     if (r != ILE_OK) return r;
     const size_t need_slots = (size_t)a.n_points * slot_cap, need_adj = (size_t)a.n_points * nseg, need_g = 2 * (size_t)a.n_points + 2;
-    if (need_slots > c->ss_slots || need_adj > c->ss_adj || need_g > c->ss_gcum) {
+    const size_t need_go = need_slots / 8;
+    if (need_slots > c->ss_slots || need_adj > c->ss_adj || need_g > c->ss_gcum || need_go > c->ss_gorder) {
         CK(cudaStreamSynchronize(st));
         if (need_slots > c->ss_slots) {
             cudaFree(c->ss.slots);
@@ -274,6 +282,12 @@ static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
             CK(cudaMalloc(&c->ss.adj, need_adj * sizeof(int32_t)));
             c->ss_adj = need_adj;
         }
+        if (need_go > c->ss_gorder) {
+            cudaFree(c->ss.gorder);
+            c->ss.gorder = nullptr, c->ss_gorder = 0;
+            CK(cudaMalloc(&c->ss.gorder, need_go * sizeof(int32_t)));
+            c->ss_gorder = need_go;
+        }
         if (need_g > c->ss_gcum) {
             cudaFree(c->ss.gcum);
             c->ss.gcum = nullptr, c->ss_gcum = 0;
@@ -283,7 +297,6 @@ static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
     }
     c->ss.Qs = c->dQs;
     c->ss.slot_cap = slot_cap;
-    c->ss.counter = nullptr;
     int nl = 0;
     cudaError_t e = ile_launch_eval_stream(c->sz, c->hparams, a, c->spl, sp, c->sc, c->ss, st, &nl);
     c->launches += nl;

@@ -38,7 +38,15 @@
 #define ST_FULL 0xffffffffu
 #define ST_TAB 1024
 #define ST_TAB_LOG2 10
+#ifndef ST_THREADS
 #define ST_THREADS 128
+#endif
+#ifndef ST_MINB3
+#define ST_MINB3 3
+#endif
+#ifndef ST_PIPE_MAXKS
+#define ST_PIPE_MAXKS 4
+#endif
 
 __device__ __forceinline__ void st_dmma(double &c0, double &c1, double a, double b)
 {
@@ -208,11 +216,17 @@ struct IleStreamKArgs {
     const int32_t *i0;
     const int32_t *slots;
     const int32_t *gcum;
-    uint32_t *counter;
+    const int32_t *gorder;  // [n_points][gcap]: the groups of a point in the order of their detector-0 window start
+    uint32_t *rcnt;         // [n_ranges] claim counters, zeroed per launch
+    int32_t n_ranges;
+    int64_t gcap;
     double *lnL;
 };
 
 #define ST_PFS 1 /* steps (pairs of blocks) the L1 prefetch runs ahead of the fragment loads */
+#ifndef ST_PREFETCH
+#define ST_PREFETCH 0 /* prefetch.global.L1 always goes to L2 (2.1 GB per 100,000 samples): off */
+#endif
 
 template <int K, int KS, int NC, int MINB>
 __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const __grid_constant__ IleStreamKArgs a)
@@ -228,11 +242,40 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
     const int total = a.gcum[a.n_points];
     const size_t nqp4 = (size_t)a.nqp * 4;
 
+    // Work distribution: the group list (all points, each in window-start order) is cut into n_ranges contiguous ranges and
+    // an SM works through the range of its own id, so that the warps of one SM stream the same few hundred rows of Q and the
+    // fragments stay in its L1.  A warp whose range is used up moves on to the next range for good (ranges only shrink).
+    unsigned smid;
+    asm("mov.u32 %0, %%smid;" : "=r"(smid));
+    int rg = (int)(smid % (unsigned)a.n_ranges);
+    const int nr = a.n_ranges;
     for (;;) {
-        int w = 0;
-        if (lane == 0) w = (int)atomicAdd(a.counter, 1u);
-        w = __shfl_sync(ST_FULL, w, 0);
-        if (w >= total) break;
+        int w = -1;
+        for (;;) {
+            const long long lo = (long long)total * rg / nr, hi = (long long)total * (rg + 1) / nr;
+            unsigned t = 0;
+            if (lane == 0) t = atomicAdd(a.rcnt + rg, 1u);
+            t = __shfl_sync(ST_FULL, t, 0);
+            if (lo + (long long)t < hi) {
+                w = (int)(lo + t);
+                break;
+            }
+            // own range used up: the lanes look at 32 other ranges at a time for one with groups left
+            int found = -1;
+            for (int base = 1; base < nr && found < 0; base += 32) {
+                const int off = base + lane, cand = (rg + off) % nr;
+                bool left = false;
+                if (off < nr) {
+                    const long long clo = (long long)total * cand / nr, chi = (long long)total * (cand + 1) / nr;
+                    left = clo + (long long)*((volatile uint32_t *)a.rcnt + cand) < chi;
+                }
+                const unsigned mk = __ballot_sync(ST_FULL, left);
+                if (mk) found = (rg + base + __ffs(mk) - 1) % nr;
+            }
+            if (found < 0) break;
+            rg = found;
+        }
+        if (w < 0) break;
         int pt = 0;
         if (a.n_points > 1) {
             int lo = 0, hi = a.n_points;
@@ -243,7 +286,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
             }
             pt = lo;
         }
-        const int g = w - a.gcum[pt];
+        const int g = a.gorder[(size_t)pt * a.gcap + (w - a.gcum[pt])];
         const int32_t *__restrict__ slots = a.slots + (size_t)pt * a.slot_cap + 8 * (size_t)g;
         const long long sbase = (long long)pt * a.n_per_point;
 
@@ -305,7 +348,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
         const double *pf = nullptr;
         {
             const int f = lane / 3, fk = f / KS, fs = f - fk * KS;
-            if (f < K * KS) {
+            if (ST_PREFETCH && f < K * KS) {
                 const int bk = fk == 0 ? base[0] - 8 * NC : fk == 1 ? base[K > 1 ? 1 : 0] : base[K > 2 ? 2 : 0];
                 const int j = lane - 3 * f;
                 pf = a.Qs + ((size_t)((a.point0 + pt) * K + fk) * KS * a.nqp + (size_t)fs * a.nqp + (size_t)(a.padf + bk)) * 4 +
@@ -331,7 +374,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
             pk[k] += NC * 32;
         }
         // fragments in registers one step ahead while they fit (PIPE); otherwise loaded where they are used
-        constexpr bool PIPE = KS <= 4;
+        constexpr bool PIPE = KS <= ST_PIPE_MAXKS;
         double af[K][2][PIPE ? KS : 1];  // [k][block of the pair][k-step]; k = 0 is detector 0
         if (PIPE) {
 #pragma unroll
@@ -507,12 +550,17 @@ cudaError_t ile_launch_pack_q_stream(const IleSizes &sz, const IleStreamPlan &pl
 // counting sort of variant 4: cells = (segment, i0_0 >> g0); every segment's slots are padded to a multiple of 8 so that a
 // group of 8 consecutive slots never mixes two (d1, d2) cells
 // ------------------------------------------------------------------------------------------------------------
-#define SS_THREADS 1024
+#define SS_THREADS 1024 /* scan kernel of multi-point launches */
+#ifndef IX_THREADS
+#define IX_THREADS 1024
+#endif
+/* index kernel; its last block does the scan of a single-point launch */
 
-// exclusive scan of v[0..n) in place by one block; returns the total to every thread
+// exclusive scan of v[0..n) in place by the NT threads of a block (v in shared or global memory); returns the total
+template <int NT>
 __device__ uint32_t ss_block_scan(uint32_t *__restrict__ v, int n, uint32_t *wsum)
 {
-    const int per = (n + SS_THREADS - 1) / SS_THREADS;
+    const int per = ((n + NT - 1) / NT) | 1;  // odd: conflict-free when v is in shared memory
     const int lo = min((int)threadIdx.x * per, n), hi = min(lo + per, n);
     uint32_t loc = 0;
     for (int i = lo; i < hi; ++i) loc += v[i];
@@ -527,7 +575,7 @@ __device__ uint32_t ss_block_scan(uint32_t *__restrict__ v, int n, uint32_t *wsu
     if (lane == 31) wsum[warp] = inc;
     __syncthreads();
     if (warp == 0) {
-        const uint32_t x = wsum[lane];
+        const uint32_t x = lane < NT / 32 ? wsum[lane] : 0u;
         uint32_t xi = x;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -547,44 +595,176 @@ __device__ uint32_t ss_block_scan(uint32_t *__restrict__ v, int n, uint32_t *wsu
     return wsum[32];
 }
 
-// one block per point.  hist -> exclusive positions; adj[seg] = padded base of the segment minus its first position;
-// ngr[pt] = groups of the point; for a single point also gcum = {0, groups}.
-__global__ void __launch_bounds__(SS_THREADS) ile_stream_scan_kernel(int32_t ncell, int32_t n0, int32_t nseg, uint32_t *__restrict__ hist,
-                                                                     uint32_t *__restrict__ adj, int32_t *__restrict__ ngood,
-                                                                     uint32_t *__restrict__ ngr, int32_t *__restrict__ gcum,
-                                                                     int32_t n_points)
+struct IleScanArgs {
+    int32_t ncell, n0, nseg, n_points;
+    uint32_t *hist;   // [n_points][ncell] counts in, exclusive positions out
+    uint32_t *adj;    // [n_points][nseg]
+    int32_t *ngood;   // [n_points]
+    uint32_t *ngr;    // [n_points]
+    int32_t *gcum;    // [n_points + 1]
+    int32_t *gorder;  // [n_points][gcap]
+    long long gcap;
+};
+
+// Scan of one point by one block of NT threads; the point's histogram lives in shared memory (h: ncell + 1 + nseg words).
+//   hist  -> exclusive positions (written back for the scatter kernel)
+//   adj[seg] = padded base of the segment minus its first position;  ngr[pt] = groups of the point (a single point also
+//   gets gcum = {0, groups})
+//   gorder[pt][.] = the point's groups listed by i0_0 bin first, segment second: group ids are positions / 8 in the padded
+//   slot table; a group belongs to the (segment, bin) cell its first slot falls in.
+template <int NT>
+__device__ void ss_scan_point(const IleScanArgs &A, int pt, uint32_t *__restrict__ h, uint32_t *wsum)
 {
-    __shared__ uint32_t wsum[33];
-    uint32_t *h = hist + (size_t)blockIdx.x * ncell;
-    uint32_t *ad = adj + (size_t)blockIdx.x * nseg;
-    ss_block_scan(h, ncell, wsum);
+    const int ncell = A.ncell, n0 = A.n0, nseg = A.nseg;
+    uint32_t *hg = A.hist + (size_t)pt * ncell;
+    uint32_t *adg = A.adj + (size_t)pt * nseg;
+    uint32_t *ad = h + ncell + 1;
+    int32_t *go = A.gorder + (size_t)pt * A.gcap;
+    for (int i = threadIdx.x; i < ncell; i += NT) h[i] = __ldcg(hg + i);
     __syncthreads();
-    if (threadIdx.x == 0) ngood[blockIdx.x] = (int32_t)h[ncell - 1];  // samples before the out-of-range cell
-    // padded size of every segment (its end is the next segment's start; the last one ends at the out-of-range cell)
-    for (int s = threadIdx.x; s < nseg; s += SS_THREADS) ad[s] = (h[(size_t)(s + 1) * n0] - h[(size_t)s * n0] + 7u) & ~7u;
+    const uint32_t n_all = ss_block_scan<NT>(h, ncell, wsum);
     __syncthreads();
-    const uint32_t tot = ss_block_scan(ad, nseg, wsum);
-    __syncthreads();
-    for (int s = threadIdx.x; s < nseg; s += SS_THREADS) ad[s] -= h[(size_t)s * n0];
     if (threadIdx.x == 0) {
-        ngr[blockIdx.x] = tot >> 3;
-        if (n_points == 1) {
-            gcum[0] = 0;
-            gcum[1] = (int32_t)(tot >> 3);
+        h[ncell] = n_all;
+        A.ngood[pt] = (int32_t)h[ncell - 1];  // samples before the out-of-range cell
+    }
+    for (int i = threadIdx.x; i < ncell; i += NT) hg[i] = h[i];
+    // padded size of every segment (its end is the next segment's start; the last one ends at the out-of-range cell)
+    for (int s = threadIdx.x; s < nseg; s += NT) ad[s] = (h[(size_t)(s + 1) * n0] - h[(size_t)s * n0] + 7u) & ~7u;
+    __syncthreads();
+    const uint32_t tot = ss_block_scan<NT>(ad, nseg, wsum);
+    __syncthreads();
+    for (int s = threadIdx.x; s < nseg; s += NT) {
+        ad[s] -= h[(size_t)s * n0];
+        adg[s] = ad[s];
+    }
+    if (threadIdx.x == 0) {
+        A.ngr[pt] = tot >> 3;
+        if (A.n_points == 1) {
+            A.gcum[0] = 0;
+            A.gcum[1] = (int32_t)(tot >> 3);
+        }
+    }
+    __syncthreads();
+    // traversal q = bin * nseg + seg: groups that start in cell (seg, bin) = multiples of 8 in [p0, p1)
+    const int nq = n0 * nseg;
+    const int per = (nq + NT - 1) / NT;
+    const int qlo = min((int)threadIdx.x * per, nq), qhi = min(qlo + per, nq);
+    uint32_t loc = 0;
+    {
+        int b = qlo / nseg, sgm = qlo - b * nseg;
+        for (int q = qlo; q < qhi; ++q) {
+            const int c = sgm * n0 + b;
+            const uint32_t p0 = h[c] + ad[sgm], p1 = h[c + 1] + ad[sgm];
+            loc += ((p1 + 7u) >> 3) - ((p0 + 7u) >> 3);
+            if (++sgm == nseg) sgm = 0, ++b;
+        }
+    }
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t inc = loc;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t x = __shfl_up_sync(ST_FULL, inc, o);
+        if (lane >= o) inc += x;
+    }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    if (warp == 0) {
+        const uint32_t x = lane < NT / 32 ? wsum[lane] : 0u;
+        uint32_t xi = x;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t y = __shfl_up_sync(ST_FULL, xi, o);
+            if (lane >= o) xi += y;
+        }
+        wsum[lane] = xi - x;
+    }
+    __syncthreads();
+    uint32_t run = wsum[warp] + inc - loc;
+    {
+        int b = qlo / nseg, sgm = qlo - b * nseg;
+        for (int q = qlo; q < qhi; ++q) {
+            const int c = sgm * n0 + b;
+            const uint32_t p0 = h[c] + ad[sgm], p1 = h[c + 1] + ad[sgm];
+            const uint32_t g0 = (p0 + 7u) >> 3, g1 = (p1 + 7u) >> 3;
+            for (uint32_t g = g0; g < g1; ++g) go[run++] = (int32_t)g;
+            if (++sgm == nseg) sgm = 0, ++b;
         }
     }
 }
 
+__global__ void __launch_bounds__(SS_THREADS) ile_stream_scan_kernel(const __grid_constant__ IleScanArgs A)
+{
+    extern __shared__ uint32_t ss_h[];
+    __shared__ uint32_t wsum[33];
+    ss_scan_point<SS_THREADS>(A, blockIdx.x, ss_h, wsum);
+}
+
+// Index pre-pass: step 2 of the hot path for every sample -- window starts i0_k (readings R2, R8, R9),
+// the cell key and the histogram of the counting sort.  For a single-point launch (FUSED) the block that finishes last
+// goes on to scan the histogram, which saves a launch and a trip through the block scheduler.
+template <bool FUSED>
+__global__ void __launch_bounds__(IX_THREADS)
+    ile_stream_index_kernel(const __grid_constant__ IleDevParams P, const __grid_constant__ IleEvalArgs a,
+                            const __grid_constant__ IleSortPlan sp, int32_t *__restrict__ i0_out, int32_t *__restrict__ cell,
+                            const __grid_constant__ IleScanArgs A, uint32_t *__restrict__ ticket)
+{
+    const long long n_total = a.n_per_point * a.n_points;
+    const int K = P.n_det;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n_total; s += (long long)gridDim.x * blockDim.x) {
+        const int pt = (int)(s / a.n_per_point);
+        double dir[3], sl, cl, sd, cd;
+        ile_source_dir(a.ra[s], a.dec[s], P.gmst, dir, &sl, &cl, &sd, &cd);
+        const double t_ref = a.t_ref[s];
+        int bad = 0;
+        int32_t i0[3] = {0, 0, 0};
+        for (int k = 0; k < K; ++k) {
+            const int32_t idx = ile_window_index(P.vertex[k], dir, t_ref, P.t0_q, P.fs, P.n_t);
+            if (k < 3) i0[k] = idx;
+            if (idx < 0 || (long long)idx + P.n_t > P.n_q) bad = 1;
+            i0_out[s * K + k] = idx;
+            if (a.shift_idx) a.shift_idx[s * K + k] = idx;
+        }
+        int32_t c;
+        if (bad) {  // reading R9: -inf for the sample, sticky counter, never a wrapped or clamped window
+            c = sp.ncell - 1;
+            atomicAdd(a.oob_counter, 1ULL);
+            a.lnL[s] = -CUDART_INF;
+        } else {
+            // segment = (d1, d2) cell of width 2^g, then the i0_0 bin inside the segment
+            int32_t seg = 0;
+            if (sp.nd > 1) seg = min(max(i0[1] - i0[0] + sp.dmax[1], 0), 2 * sp.dmax[1]) >> sp.g;
+            if (sp.nd > 2) seg = seg * sp.n2 + (min(max(i0[2] - i0[0] + sp.dmax[2], 0), 2 * sp.dmax[2]) >> sp.g);
+            c = seg * sp.n0 + (i0[0] >> sp.g0);  // 0 <= i0_0 <= n_q - n_t here
+        }
+        cell[s] = c;
+        atomicAdd(&A.hist[(size_t)pt * sp.ncell + c], 1u);
+    }
+    if (FUSED) {
+        extern __shared__ uint32_t ss_h[];
+        __shared__ uint32_t wsum[33];
+        __shared__ uint32_t last;
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+        __syncthreads();
+        if (!last) return;
+        __threadfence();
+        ss_scan_point<IX_THREADS>(A, 0, ss_h, wsum);
+    }
+}
+
+// exclusive prefix of the points' group counts (multi-point launches)
 __global__ void __launch_bounds__(SS_THREADS) ile_stream_prefix_kernel(int32_t n_points, uint32_t *__restrict__ ngr, int32_t *__restrict__ gcum)
 {
     __shared__ uint32_t wsum[33];
-    const uint32_t tot = ss_block_scan(ngr, n_points, wsum);
+    const uint32_t tot = ss_block_scan<SS_THREADS>(ngr, n_points, wsum);
     __syncthreads();
     for (int p = threadIdx.x; p < n_points; p += SS_THREADS) gcum[p] = (int32_t)ngr[p];
     if (threadIdx.x == 0) gcum[n_points] = (int32_t)tot;
 }
 
-__global__ void __launch_bounds__(256) ile_stream_scatter_kernel(long long n_per_point, int32_t n_points, int32_t ncell, int32_t n0,
+__global__ void __launch_bounds__(IX_THREADS) ile_stream_scatter_kernel(long long n_per_point, int32_t n_points, int32_t ncell, int32_t n0,
                                                                  int32_t nseg, long long slot_cap, const int32_t *__restrict__ cell,
                                                                  uint32_t *__restrict__ offs, const uint32_t *__restrict__ adj,
                                                                  int32_t *__restrict__ slots)
@@ -642,7 +822,7 @@ bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per
     for (;; ++g0) {
         sp.n0 = ((sz.n_q - sz.n_t) >> g0) + 1;
         const long long nc = (long long)sp.n0 * sp.n1 * sp.n2 + 1;
-        if (nc <= (1LL << 20)) {
+        if ((nc + 1 + (long long)sp.n1 * sp.n2) * 4 <= (long long)sz.max_smem_optin - 2048) {  // the scan kernel keeps a point's histogram in shared memory
             sp.ncell = (int32_t)nc;
             break;
         }
@@ -679,7 +859,7 @@ static cudaError_t st_launch_k(const IleSizes &sz, int ks, const IleStreamKArgs 
     switch (ks) {
         case 1: return st_launch_t<K, 1, NC, 4>(sz, ka, mg, st);
         case 2: return st_launch_t<K, 2, NC, 4>(sz, ka, mg, st);
-        case 3: return st_launch_t<K, 3, NC, 3>(sz, ka, mg, st);
+        case 3: return st_launch_t<K, 3, NC, ST_MINB3>(sz, ka, mg, st);
         case 4: return st_launch_t<K, 4, NC, 3>(sz, ka, mg, st);
         case 6: return st_launch_t<K, 6, NC, 2>(sz, ka, mg, st);
         case 8: return st_launch_t<K, 8, NC, 2>(sz, ka, mg, st);
@@ -696,27 +876,65 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     if (a.n_per_point <= 0 || a.n_points <= 0) return cudaSuccess;
     const long long n_total = a.n_per_point * a.n_points;
     const int nseg = sp.n1 * sp.n2;
-    // histogram + work counter (the counter sits right behind the histograms), then the slot table
-    cudaError_t e = cudaMemsetAsync(sc.hist, 0, ((size_t)a.n_points * sp.ncell + 1) * sizeof(uint32_t), st);
+    // histogram + claim counters of the streaming kernel (right behind the histograms), then the slot table
+    cudaError_t e = cudaMemsetAsync(sc.hist, 0, ((size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES) * sizeof(uint32_t), st);
     if (e != cudaSuccess) return e;
     e = cudaMemsetAsync(ss.slots, 0xFF, (size_t)a.n_points * ss.slot_cap * sizeof(int32_t), st);
     if (e != cudaSuccess) return e;
-    ile_launch_setup_only(sz, hp, a, pl.cp, sp, sc, st);
-    uint32_t *ngr = reinterpret_cast<uint32_t *>(ss.gcum) + a.n_points + 1;
-    ile_stream_scan_kernel<<<(unsigned)a.n_points, SS_THREADS, 0, st>>>(sp.ncell, sp.n0, nseg, sc.hist, reinterpret_cast<uint32_t *>(ss.adj),
-                                                                        sc.ngood, ngr, ss.gcum, a.n_points);
-    int nl = 2;
-    if (a.n_points > 1) {
-        ile_stream_prefix_kernel<<<1, SS_THREADS, 0, st>>>(a.n_points, ngr, ss.gcum);
-        ++nl;
+    // window starts + histogram on the caller's stream; a single point's scan runs in the index kernel's last block
+    IleScanArgs sa;
+    sa.ncell = sp.ncell, sa.n0 = sp.n0, sa.nseg = nseg, sa.n_points = a.n_points;
+    sa.hist = sc.hist;
+    sa.adj = reinterpret_cast<uint32_t *>(ss.adj);
+    sa.ngood = sc.ngood;
+    sa.ngr = reinterpret_cast<uint32_t *>(ss.gcum) + a.n_points + 1;
+    sa.gcum = ss.gcum;
+    sa.gorder = ss.gorder;
+    sa.gcap = ss.slot_cap / 8;
+    const size_t scan_smem = ((size_t)sp.ncell + 1 + nseg) * sizeof(uint32_t);
+    static bool scan_attr = false;
+    if (!scan_attr) {
+        e = cudaFuncSetAttribute(ile_stream_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 1024);
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(ile_stream_index_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 1024);
+        if (e != cudaSuccess) return e;
+        scan_attr = true;
     }
-    long long sblocks = (n_total + 255) / 256;
-    const long long cap = (long long)sz.sm_count * 16;
-    if (sblocks > cap) sblocks = cap;
-    ile_stream_scatter_kernel<<<(unsigned)sblocks, 256, 0, st>>>(a.n_per_point, a.n_points, sp.ncell, sp.n0, nseg, ss.slot_cap, sc.cell,
-                                                                 sc.hist, reinterpret_cast<const uint32_t *>(ss.adj), ss.slots);
+    uint32_t *ticket = sc.hist + (size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES - 1;
+    long long iblocks = (n_total + IX_THREADS - 1) / IX_THREADS;
+    const long long cap = (long long)sz.sm_count * 32;
+    if (iblocks > cap) iblocks = cap;
+    // fork: the side stream may start as soon as the caller's stream gets here; the index kernel is enqueued first so that
+    // the short sorting kernels are not starved of SM resources by the coefficient kernel (steps 1, 3, 4)
+    e = cudaEventRecord(ss.ev_fork, st);
+    if (e != cudaSuccess) return e;
+    int nl = 0;
+    if (a.n_points == 1) {
+        ile_stream_index_kernel<true><<<(unsigned)iblocks, IX_THREADS, scan_smem, st>>>(hp, a, sp, sc.i0, sc.cell, sa, ticket);
+        ++nl;
+    } else {
+        ile_stream_index_kernel<false><<<(unsigned)iblocks, IX_THREADS, 0, st>>>(hp, a, sp, sc.i0, sc.cell, sa, ticket);
+    }
+    e = cudaStreamWaitEvent(ss.aux, ss.ev_fork, 0);
+    if (e != cudaSuccess) return e;
+#ifndef DBG_SKIP_SETUP
+    ile_launch_setup_coef(sz, hp, a, pl.cp, sp, sc, ss.aux);
+#endif
+    ++nl;
+    e = cudaEventRecord(ss.ev_join, ss.aux);
+    if (e != cudaSuccess) return e;
+    if (a.n_points > 1) {
+        ile_stream_scan_kernel<<<(unsigned)a.n_points, SS_THREADS, scan_smem, st>>>(sa);
+        ile_stream_prefix_kernel<<<1, SS_THREADS, 0, st>>>(a.n_points, sa.ngr, ss.gcum);
+        nl += 3;
+    }
+    ile_stream_scatter_kernel<<<(unsigned)iblocks, IX_THREADS, 0, st>>>(a.n_per_point, a.n_points, sp.ncell, sp.n0, nseg, ss.slot_cap, sc.cell,
+                                                                        sc.hist, reinterpret_cast<const uint32_t *>(ss.adj), ss.slots);
     ++nl;
     e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+
+    e = cudaStreamWaitEvent(st, ss.ev_join, 0);  // join
     if (e != cudaSuccess) return e;
 
     IleStreamKArgs ka;
@@ -735,9 +953,15 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     ka.i0 = sc.i0;
     ka.slots = ss.slots;
     ka.gcum = ss.gcum;
-    ka.counter = sc.hist + (size_t)a.n_points * sp.ncell;
+    ka.gorder = ss.gorder;
+    ka.rcnt = sc.hist + (size_t)a.n_points * sp.ncell;
+    ka.n_ranges = sz.sm_count < ILE_STREAM_MAX_RANGES ? sz.sm_count : ILE_STREAM_MAX_RANGES;
+    ka.gcap = ss.slot_cap / 8;
     ka.lnL = a.lnL;
     const long long max_groups = (long long)a.n_points * (ss.slot_cap / 8);
+#ifdef DBG_SKIP_STREAM
+    return cudaSuccess;
+#endif
     if (sz.n_det == 1) e = st_launch_k<1, 2>(sz, pl.ks, ka, max_groups, st);
     else if (sz.n_det == 2) e = st_launch_k<2, 2>(sz, pl.ks, ka, max_groups, st);
     else e = st_launch_k<3, 2>(sz, pl.ks, ka, max_groups, st);

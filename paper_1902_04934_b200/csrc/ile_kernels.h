@@ -104,13 +104,17 @@ struct IleStreamPlan {
     int32_t nqp;      // rows per packed series = padf + n_q + back padding
 };
 
+#define ILE_STREAM_MAX_RANGES 256 /* claim counters of the streaming kernel, kept right behind the histograms */
+
 struct IleStreamScratch {
     const double *Qs;   // packed Q [P][K][ks][nqp][4]
     int32_t *slots;     // [n_points][slot_cap]: sample index or -1, groups of 8 consecutive slots
     int32_t *adj;       // [n_points][nseg]: padded segment base minus the segment's first sorted position
     int32_t *gcum;      // [n_points + 1]: exclusive prefix of the group counts, followed by [n_points] group counts
-    uint32_t *counter;  // work counter of the persistent kernel (zeroed with the histogram)
+    int32_t *gorder;    // [n_points][slot_cap / 8]: group ids in the order of their detector-0 window start
     int64_t slot_cap;   // slots per point (multiple of 8)
+    cudaStream_t aux;   // side stream: the coefficient kernel runs there while the caller's stream sorts
+    cudaEvent_t ev_fork, ev_join;
 };
 
 bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point, IleStreamPlan *out, IleSortPlan *sp);
@@ -120,8 +124,8 @@ cudaError_t ile_launch_pack_q_stream(const IleSizes &sz, const IleStreamPlan &pl
 cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleStreamPlan &pl,
                                    const IleSortPlan &sp, const IleMmaScratch &sc, const IleStreamScratch &ss,
                                    cudaStream_t st, int *n_launches);
-// launches the per-sample setup kernel only (shared by variants 3 and 4)
-void ile_launch_setup_only(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, int32_t cp, const IleSortPlan &sp,
+// variant 4: coefficients a F_k Y_lm and quadratic term of every sample (steps 1, 3, 4), no sorting work
+void ile_launch_setup_coef(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, int32_t cp, const IleSortPlan &sp,
                            const IleMmaScratch &sc, cudaStream_t st);
 
 // evidence: two kernels (per-block partials, then per-segment combine with the carried state)

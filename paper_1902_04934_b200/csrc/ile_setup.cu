@@ -57,9 +57,14 @@ cudaError_t ile_launch_pack_q(const IleSizes &sz, const IleMmaPlan &mp, int32_t 
 // per-sample setup + cell key + histogram
 // ------------------------------------------------------------------------------------------------------------
 #define SETUP_THREADS 128
+#ifndef SETUP_MINB
+#define SETUP_MINB 6 /* <= 85 registers: 768 threads per SM, a 100,000-sample batch is one wave */
+#endif
 
-template <int MMAX>
-__global__ void __launch_bounds__(SETUP_THREADS)
+// SORT = false (variant 4): coefficients and quadratic term only -- window starts, cell keys and the histogram come
+// from ile_index_kernel, which runs concurrently on the caller's stream.
+template <int MMAX, bool SORT>
+__global__ void __launch_bounds__(SETUP_THREADS, SETUP_MINB)
     ile_setup_kernel(const __grid_constant__ IleDevParams P, const __grid_constant__ IleEvalArgs a, const int32_t cp,
                      const __grid_constant__ IleSortPlan sp, const __grid_constant__ IleMmaScratch sc)
 {
@@ -136,11 +141,13 @@ __global__ void __launch_bounds__(SETUP_THREADS)
             const double2 FF = ile_cmul(F, F);
             tot += F2 * yuy + (FF.x * yvy.x - FF.y * yvy.y);
 
-            const int32_t idx = ile_window_index(P.vertex[k], g.s, t_ref, P.t0_q, P.fs, P.n_t);
-            if (k < 3) i0[k] = idx;
-            if (idx < 0 || (long long)idx + P.n_t > P.n_q) bad = 1;
-            sc.i0[s * K + k] = idx;
-            if (a.shift_idx) a.shift_idx[s * K + k] = idx;
+            if (SORT) {
+                const int32_t idx = ile_window_index(P.vertex[k], g.s, t_ref, P.t0_q, P.fs, P.n_t);
+                if (k < 3) i0[k] = idx;
+                if (idx < 0 || (long long)idx + P.n_t > P.n_q) bad = 1;
+                sc.i0[s * K + k] = idx;
+                if (a.shift_idx) a.shift_idx[s * K + k] = idx;
+            }
 
             const double2 aF = make_double2(amp_a * F.x, amp_a * F.y);
             double2 *__restrict__ rk = reinterpret_cast<double2 *>(rec + (size_t)k * cp);
@@ -150,6 +157,7 @@ __global__ void __launch_bounds__(SETUP_THREADS)
             for (int m = M; m < cp / 2; ++m) rk[m] = make_double2(0.0, 0.0);
         }
         sc.quad[s] = 0.25 * amp_a * amp_a * tot;
+        if (!SORT) continue;
 
         // ---- cell of the counting sort (boustrophedon enumeration: consecutive cells are neighbours)
         int32_t c;
@@ -269,14 +277,14 @@ IleSortPlan ile_sort_plan(const IleSizes &sz, const IleDevParams &hp, long long 
     return sp;
 }
 
-template <int MMAX>
+template <int MMAX, bool SORT = true>
 static void setup_launch_t(unsigned blocks, const IleDevParams &hp, const IleEvalArgs &a, const IleMmaPlan &mp,
                            const IleSortPlan &sp, const IleMmaScratch &sc, cudaStream_t st)
 {
-    ile_setup_kernel<MMAX><<<blocks, SETUP_THREADS, 0, st>>>(hp, a, mp.cp, sp, sc);
+    ile_setup_kernel<MMAX, SORT><<<blocks, SETUP_THREADS, 0, st>>>(hp, a, mp.cp, sp, sc);
 }
 
-void ile_launch_setup_only(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, int32_t cp, const IleSortPlan &sp,
+void ile_launch_setup_coef(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, int32_t cp, const IleSortPlan &sp,
                            const IleMmaScratch &sc, cudaStream_t st)
 {
     const long long n_total = a.n_per_point * a.n_points;
@@ -286,10 +294,10 @@ void ile_launch_setup_only(const IleSizes &sz, const IleDevParams &hp, const Ile
     IleMmaPlan mp;
     mp.cp = cp;
     const int M = sz.n_modes;
-    if (M <= 2) setup_launch_t<2>((unsigned)blocks, hp, a, mp, sp, sc, st);
-    else if (M <= 5) setup_launch_t<5>((unsigned)blocks, hp, a, mp, sp, sc, st);
-    else if (M <= 12) setup_launch_t<12>((unsigned)blocks, hp, a, mp, sp, sc, st);
-    else setup_launch_t<ILE_MAX_MODES>((unsigned)blocks, hp, a, mp, sp, sc, st);
+    if (M <= 2) setup_launch_t<2, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
+    else if (M <= 5) setup_launch_t<5, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
+    else if (M <= 12) setup_launch_t<12, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
+    else setup_launch_t<ILE_MAX_MODES, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
 }
 
 cudaError_t ile_launch_setup_sort(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleMmaPlan &mp,
