@@ -28,6 +28,7 @@
 // 32 consecutive doubles starting at any row -- one coalesced 256-byte load per DMMA at an arbitrary 32-byte offset.  The
 // series are zero padded in front and behind so that rows outside [0, N_Q), which only ever feed elements outside every
 // window, read as zeros.
+#include <cstdio>
 #include <limits.h>
 #include <math_constants.h>
 
@@ -198,6 +199,11 @@ __device__ __forceinline__ void st_lse_main2(const double (&d)[2][2], const bool
     for (int c = 0; c < 2; ++c) s[c] = fma(e[1][c], S[1][c], fma(e[0][c], S[0][c], s[c]));
 }
 
+// loads of per-sample data that is used once: keep them from evicting the Q rows the SM's warps share in L1
+#ifndef ST_STREAM_LD
+#define ST_STREAM_LD(p) __ldcs(p)
+#endif
+
 __device__ __forceinline__ double st_shfl(double v, int src) { return __shfl_sync(ST_FULL, v, src); }
 
 // m ? b : a for an all-ones / all-zeros mask m: two LOP3, no predicate
@@ -291,10 +297,10 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
         const long long sbase = (long long)pt * a.n_per_point;
 
         // ---- the group: window starts, bases, per-sample offsets.  Lane (r, cc) looks after (sample r, detector cc).
-        const int sb = slots[r];  // -1: empty slot (the group is the tail of its segment)
+        const int sb = ST_STREAM_LD(slots + r);  // -1: empty slot (the group is the tail of its segment)
         const bool has = sb >= 0;
         const long long fb = sbase + (has ? sb : 0);
-        const int my_i0 = (has && cc < K) ? a.i0[fb * K + cc] : 0;
+        const int my_i0 = (has && cc < K) ? ST_STREAM_LD(a.i0 + fb * K + cc) : 0;
         const int i00 = __shfl_sync(ST_FULL, my_i0, lane & ~3);
         const int G0 = __reduce_min_sync(ST_FULL, has ? i00 : INT_MAX);
         const int dspread = __reduce_max_sync(ST_FULL, has ? i00 - G0 : 0);
@@ -337,7 +343,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
 #pragma unroll
             for (int k = 0; k < K; ++k)
 #pragma unroll
-                for (int s = 0; s < KS; ++s) bf[k][s] = has ? __ldg(rp + k * a.cp + 4 * s) : 0.0;
+                for (int s = 0; s < KS; ++s) bf[k][s] = has ? ST_STREAM_LD(rp + k * a.cp + 4 * s) : 0.0;
         }
         // ---- A fragment pointers: pk[k] = this lane's element of the next block to load of detector k
         const double *pk[K];
@@ -403,7 +409,11 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
                     for (int c = 0; c < 2; ++c) v[bb][c] = (unsigned)(jc[c] + 8 * (t0 - 2 + bb)) < (unsigned)n_t;
             }
             double d[2][2];
+#ifndef DBG_NO_LSE
             st_lse_pre2<PRED>(lin, v, m, sm, d, tab_addr);
+#else
+            sm[0] += lin[0][0] + lin[1][0]; sm[1] += lin[0][1] + lin[1][1]; m[0] = 0; m[1] = 0;
+#endif
             // shifted detectors: blocks t0 + NC + bb into ring slots (2 P + NC + bb) % 4
 #pragma unroll
             for (int k = 1; k < K; ++k) {
@@ -433,7 +443,9 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
                 asm volatile("prefetch.global.L1 [%0];" ::"l"(pf + 32));
                 pf += 64;
             }
+#ifndef DBG_NO_LSE
             st_lse_main2<PRED>(d, v, sm, tab_addr);
+#endif
             // realign: row rho of my column wants T_k[base_k + rho + eps]; I hold it for the lane (rho - eps) mod 8
             double z[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
@@ -444,8 +456,12 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
                     for (int c = 0; c < 2; ++c) {
                         double x = ring[k - 1][(2 * P + bb) % 4][c];
 #pragma unroll
+#ifndef DBG_NO_REALIGN
                         for (int o = 1; o <= NC; ++o) x = st_bsel(x, ring[k - 1][(2 * P + bb + o) % 4][c], msk[k][c][o - 1]);
                         const double y = st_shfl(x, src[k][c]);
+#else
+                        const double y = x;
+#endif
                         z[bb][c] = k == 1 ? y : z[bb][c] + y;
                     }
             }
@@ -604,9 +620,35 @@ struct IleScanArgs {
     int32_t *gcum;    // [n_points + 1]
     int32_t *gorder;  // [n_points][gcap]
     long long gcap;
+    int32_t stage;    // words of shared memory behind the histogram for assembling the group list (0: none)
 };
 
 // Scan of one point by one block of NT threads; the point's histogram lives in shared memory (h: ncell + 1 + nseg words).
+//   hist  -> exclusive positions (written back for the scatter kernel)
+//   adj[seg] = padded base of the segment minus its first position;  ngr[pt] = groups of the point (a single point also
+//   gets gcum = {0, groups})
+//   gorder[pt][.] = the point's groups listed by i0_0 bin first, segment second: group ids are positions / 8 in the padded
+//   slot table; a group belongs to the (segment, bin) cell its first slot falls in.
+__device__ __forceinline__ uint32_t ss_warp_incl(uint32_t x, int lane)
+{
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t y = __shfl_up_sync(ST_FULL, x, o);
+        if (lane >= o) x += y;
+    }
+    return x;
+}
+
+// Scan of one point by one block of NT threads; the point's histogram lives in shared memory (h: ncell + 1 + nseg words).
+//   hist  -> exclusive positions (written back for the scatter kernel)
+//   adj[seg] = padded base of the segment minus its first position;  ngr[pt] = groups of the point (a single point also
+//   gets gcum = {0, groups})
+//   gorder[pt][.] = the point's groups listed by i0_0 bin first, segment second: group ids are positions / 8 in the padded
+//   slot table; a group belongs to the (segment, bin) cell its first slot falls in.
+// Every pass gives warp w a contiguous range and walks it 32 consecutive elements at a time (conflict-free shared-memory
+// access, coalesced global writes); the warps' totals are combined through wsum.
+// Scan of one point by one block of NT threads; the point's histogram lives in shared memory (h: ncell + 1 + nseg words,
+// followed by `stage` words in which the group list is assembled when it fits; stage = 0: written straight to global).
 //   hist  -> exclusive positions (written back for the scatter kernel)
 //   adj[seg] = padded base of the segment minus its first position;  ngr[pt] = groups of the point (a single point also
 //   gets gcum = {0, groups})
@@ -620,6 +662,7 @@ __device__ void ss_scan_point(const IleScanArgs &A, int pt, uint32_t *__restrict
     uint32_t *adg = A.adj + (size_t)pt * nseg;
     uint32_t *ad = h + ncell + 1;
     int32_t *go = A.gorder + (size_t)pt * A.gcap;
+#pragma unroll 8
     for (int i = threadIdx.x; i < ncell; i += NT) h[i] = __ldcg(hg + i);
     __syncthreads();
     const uint32_t n_all = ss_block_scan<NT>(h, ncell, wsum);
@@ -680,6 +723,9 @@ __device__ void ss_scan_point(const IleScanArgs &A, int pt, uint32_t *__restrict
         wsum[lane] = xi - x;
     }
     __syncthreads();
+    // the list is assembled in shared memory when it fits (scattered 4-byte global stores cost a cycle each), then copied out
+    const bool staged = (tot >> 3) <= (uint32_t)A.stage;
+    int32_t *__restrict__ dst = staged ? reinterpret_cast<int32_t *>(ad + nseg) : go;
     uint32_t run = wsum[warp] + inc - loc;
     {
         int b = qlo / nseg, sgm = qlo - b * nseg;
@@ -687,9 +733,13 @@ __device__ void ss_scan_point(const IleScanArgs &A, int pt, uint32_t *__restrict
             const int c = sgm * n0 + b;
             const uint32_t p0 = h[c] + ad[sgm], p1 = h[c + 1] + ad[sgm];
             const uint32_t g0 = (p0 + 7u) >> 3, g1 = (p1 + 7u) >> 3;
-            for (uint32_t g = g0; g < g1; ++g) go[run++] = (int32_t)g;
+            for (uint32_t g = g0; g < g1; ++g) dst[run++] = (int32_t)g;
             if (++sgm == nseg) sgm = 0, ++b;
         }
+    }
+    if (staged) {
+        __syncthreads();
+        for (uint32_t i = threadIdx.x; i < (tot >> 3); i += NT) go[i] = dst[i];
     }
 }
 
@@ -799,7 +849,10 @@ bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per
     pl.ks = st_round_ks((2 * sz.n_modes + 3) / 4);
     if (!pl.ks) return false;
     pl.cp = 4 * pl.ks;
-    pl.nc = 2;
+#ifndef ST_NC
+#define ST_NC 2
+#endif
+    pl.nc = ST_NC;
     pl.padf = sz.n_q - sz.n_t + 32;
     pl.nqp = pl.padf + sz.n_q + (sz.n_q - sz.n_t) + 64;
     IleSortPlan sp;
@@ -891,7 +944,12 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     sa.gcum = ss.gcum;
     sa.gorder = ss.gorder;
     sa.gcap = ss.slot_cap / 8;
-    const size_t scan_smem = ((size_t)sp.ncell + 1 + nseg) * sizeof(uint32_t);
+    size_t scan_smem = ((size_t)sp.ncell + 1 + nseg) * sizeof(uint32_t);
+    {
+        const size_t room = (size_t)(sz.max_smem_optin - 1024) - scan_smem, want = (size_t)sa.gcap * sizeof(int32_t);
+        sa.stage = want <= room ? (int32_t)sa.gcap : 0;
+        if (sa.stage) scan_smem += want;
+    }
     static bool scan_attr = false;
     if (!scan_attr) {
         e = cudaFuncSetAttribute(ile_stream_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 1024);
@@ -962,9 +1020,9 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
 #ifdef DBG_SKIP_STREAM
     return cudaSuccess;
 #endif
-    if (sz.n_det == 1) e = st_launch_k<1, 2>(sz, pl.ks, ka, max_groups, st);
-    else if (sz.n_det == 2) e = st_launch_k<2, 2>(sz, pl.ks, ka, max_groups, st);
-    else e = st_launch_k<3, 2>(sz, pl.ks, ka, max_groups, st);
+    if (sz.n_det == 1) e = st_launch_k<1, ST_NC>(sz, pl.ks, ka, max_groups, st);
+    else if (sz.n_det == 2) e = st_launch_k<2, ST_NC>(sz, pl.ks, ka, max_groups, st);
+    else e = st_launch_k<3, ST_NC>(sz, pl.ks, ka, max_groups, st);
     ++nl;
     if (e == cudaSuccess && n_launches) *n_launches += nl;
     return e;
