@@ -16,6 +16,7 @@ struct ile_ctx {
     unsigned long long *d_oob;
     double *d_partials;
     size_t partials_cap;  // doubles
+    size_t ev_tickets_at;  // offset (doubles) of the zeroed ticket words of the last evidence call's layout; 0 = none
     double *d_stage;
     size_t stage_cap;  // doubles
     double *d_small;   // lnZ, n_eff (device)
@@ -417,8 +418,14 @@ extern "C" int ile_evidence(ile_ctx *c, int32_t n_segments, int64_t n_per_segmen
     if (!c || n_segments < 1 || n_per_segment < 0 || !lnZ) return ILE_ERR_BAD_ARGUMENT;
     if (n_per_segment > 0 && !lnL_margT) return ILE_ERR_BAD_ARGUMENT;
     int32_t B = ile_evidence_blocks_per_segment(n_segments, n_per_segment, c->sz.sm_count);
-    int r = ensure_partials(c, (size_t)n_segments * B * 2);
+    const size_t at = (size_t)n_segments * B * 2, need = at + ((size_t)n_segments + 1) / 2;
+    if (need > c->partials_cap) c->ev_tickets_at = 0;
+    int r = ensure_partials(c, need);
     if (r != ILE_OK) return r;
+    if (c->ev_tickets_at != at) {  // new layout: the ticket words behind the partials start at zero (each call leaves them so)
+        CK(cudaMemsetAsync(c->d_partials + at, 0, (((size_t)n_segments + 1) / 2) * sizeof(double), (cudaStream_t)cuda_stream));
+        c->ev_tickets_at = at;
+    }
     int nl = 0;
     cudaError_t e = ile_launch_evidence(n_segments, n_per_segment, lnL_margT, log_w, state, lnZ, n_eff, c->d_partials,
                                         B, (cudaStream_t)cuda_stream, &nl);

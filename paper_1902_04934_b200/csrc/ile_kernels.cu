@@ -142,17 +142,28 @@ cudaError_t ile_launch_eval_direct(const IleSizes &sz, const IleEvalArgs &a, cud
 
 // ------------------------------------------------------------------------------------------------------------
 // step 7: evidence.  lnZ = ln((1/n) sum_a exp(lnL_a + ln w_a)), max-subtracted; n_eff = sum / max  (eq. 4).
-// Kernel 1: each block reduces one slice of one segment to (max, sum exp(e - max)) with warp shuffles, then a
-// block-level combine.  Kernel 2: one warp per segment folds the partials into the carried state.
+// One kernel.  A thread keeps a running (max, sum exp(e - max)) over its elements (one pass over the data), a block
+// merges its threads' pairs with warp shuffles and a block-level combine, and the block of a segment that finishes last
+// (ticket counter behind the partials, reset by that block) folds the segment's partials into the carried state.
 // ------------------------------------------------------------------------------------------------------------
 #define EV_THREADS 256
+#define EV_PER 4
 
-__global__ void __launch_bounds__(EV_THREADS) ile_evidence_partial_kernel(int64_t n_per_segment, const double *__restrict__ lnL,
-                                                                          const double *__restrict__ log_w,
-                                                                          double *__restrict__ partials)
+// (m, s) <- merge of (m, s) and (m2, s2), each meaning s * exp(m); (-inf, 0) is the neutral element
+__device__ __forceinline__ void ev_merge(double &m, double &s, double m2, double s2)
 {
-    __shared__ double red[EV_THREADS / 32];
-    __shared__ double bmax_s;
+    const double mx = fmax(m, m2);
+    if (mx > -CUDART_INF) s = s * exp(m - mx) + s2 * exp(m2 - mx);
+    m = mx;
+}
+
+__global__ void __launch_bounds__(EV_THREADS) ile_evidence_kernel(int64_t n_per_segment, const double *__restrict__ lnL,
+                                                                  const double *__restrict__ log_w, double *__restrict__ partials,
+                                                                  unsigned int *__restrict__ tickets, double *__restrict__ state,
+                                                                  double *__restrict__ lnZ, double *__restrict__ n_eff)
+{
+    __shared__ double red_m[EV_THREADS / 32], red_s[EV_THREADS / 32];
+    __shared__ bool last_s;
     const int seg = blockIdx.y, B = gridDim.x, b = blockIdx.x;
     const int64_t len = (n_per_segment + B - 1) / B;
     const int64_t lo = (int64_t)b * len, hi = min(lo + len, n_per_segment);
@@ -160,46 +171,53 @@ __global__ void __launch_bounds__(EV_THREADS) ile_evidence_partial_kernel(int64_
     const double *w = log_w ? log_w + (int64_t)seg * n_per_segment : nullptr;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
-    double mx = -CUDART_INF;
-    for (int64_t i = lo + threadIdx.x; i < hi; i += EV_THREADS) {
-        double e = x[i] + (w ? w[i] : 0.0);
-        mx = fmax(mx, e);
-    }
-    mx = warp_max(mx);
-    if (lane == 0) red[warp] = mx;
-    __syncthreads();
-    if (warp == 0) {
-        double v = lane < EV_THREADS / 32 ? red[lane] : -CUDART_INF;
-        v = warp_max(v);
-        if (lane == 0) bmax_s = v;
-    }
-    __syncthreads();
-    const double bmax = bmax_s;
-    double sm = 0.0;
-    if (bmax > -CUDART_INF)
-        for (int64_t i = lo + threadIdx.x; i < hi; i += EV_THREADS) {
-            double e = x[i] + (w ? w[i] : 0.0);
-            sm += exp(e - bmax);
+    // a tile = EV_PER elements per thread held in registers: block max first, then one exp per element against it
+    __shared__ double bmax_s;
+    double m = -CUDART_INF, sm = 0.0;  // the block's running pair over its tiles (thread 0's copy is the one written)
+    for (int64_t t0 = lo; t0 < hi; t0 += (int64_t)EV_THREADS * EV_PER) {
+        double e[EV_PER];
+        double mx = -CUDART_INF;
+#pragma unroll
+        for (int u = 0; u < EV_PER; ++u) {
+            const int64_t i = t0 + (int64_t)u * EV_THREADS + threadIdx.x;
+            e[u] = i < hi ? x[i] + (w ? w[i] : 0.0) : -CUDART_INF;
+            mx = fmax(mx, e[u]);
         }
-    sm = warp_sum(sm);
-    __syncthreads();
-    if (lane == 0) red[warp] = sm;
-    __syncthreads();
-    if (warp == 0) {
-        double v = lane < EV_THREADS / 32 ? red[lane] : 0.0;
-        v = warp_sum(v);
-        if (lane == 0) {
-            partials[((size_t)seg * B + b) * 2 + 0] = bmax;
-            partials[((size_t)seg * B + b) * 2 + 1] = v;
+        mx = warp_max(mx);
+        __syncthreads();  // red_m / bmax_s of the previous tile have been read
+        if (lane == 0) red_m[warp] = mx;
+        __syncthreads();
+        if (warp == 0) {
+            double v = lane < EV_THREADS / 32 ? red_m[lane] : -CUDART_INF;
+            v = warp_max(v);
+            if (lane == 0) bmax_s = v;
+        }
+        __syncthreads();
+        const double bmax = bmax_s;
+        double ts = 0.0;
+        if (bmax > -CUDART_INF) {
+#pragma unroll
+            for (int u = 0; u < EV_PER; ++u) ts += exp(e[u] - bmax);  // exp(-inf) = 0 for the padding
+        }
+        ts = warp_sum(ts);
+        if (lane == 0) red_s[warp] = ts;
+        __syncthreads();
+        if (warp == 0) {
+            double v = lane < EV_THREADS / 32 ? red_s[lane] : 0.0;
+            v = warp_sum(v);
+            ev_merge(m, sm, bmax, v);
         }
     }
-}
-
-__global__ void __launch_bounds__(32) ile_evidence_combine_kernel(int32_t B, int64_t n_per_segment, const double *__restrict__ partials,
-                                                                  double *__restrict__ state, double *__restrict__ lnZ,
-                                                                  double *__restrict__ n_eff)
-{
-    const int seg = blockIdx.x, lane = threadIdx.x;
+    if (warp == 0 && lane == 0) {
+        __stcg(&partials[((size_t)seg * B + b) * 2 + 0], m);
+        __stcg(&partials[((size_t)seg * B + b) * 2 + 1], sm);
+        __threadfence();
+        last_s = atomicAdd(&tickets[seg], 1u) == (unsigned)B - 1;
+    }
+    __syncthreads();
+    if (!last_s || warp != 0) return;
+    __threadfence();
+    // ---- the segment's last block: partials + carried state -> state, lnZ, n_eff
     double smax = -CUDART_INF, ssum = 0.0, scount = 0.0;
     if (state) {
         smax = state[seg * 3 + 0];
@@ -207,27 +225,28 @@ __global__ void __launch_bounds__(32) ile_evidence_combine_kernel(int32_t B, int
         scount = state[seg * 3 + 2];
     }
     double mx = -CUDART_INF;
-    for (int b = lane; b < B; b += 32) mx = fmax(mx, partials[((size_t)seg * B + b) * 2]);
+    for (int q = lane; q < B; q += 32) mx = fmax(mx, __ldcg(&partials[((size_t)seg * B + q) * 2]));
     mx = fmax(warp_max(mx), smax);
-    double sm = 0.0;
+    double tot = 0.0;
     if (mx > -CUDART_INF) {
-        for (int b = lane; b < B; b += 32) {
-            double bm = partials[((size_t)seg * B + b) * 2], bs = partials[((size_t)seg * B + b) * 2 + 1];
-            if (bm > -CUDART_INF) sm += bs * exp(bm - mx);
+        for (int q = lane; q < B; q += 32) {
+            const double bm = __ldcg(&partials[((size_t)seg * B + q) * 2]), bs = __ldcg(&partials[((size_t)seg * B + q) * 2 + 1]);
+            if (bm > -CUDART_INF) tot += bs * exp(bm - mx);
         }
-        sm = warp_sum(sm);
-        if (smax > -CUDART_INF) sm += ssum * exp(smax - mx);
+        tot = warp_sum(tot);
+        if (smax > -CUDART_INF) tot += ssum * exp(smax - mx);
     }
     if (lane == 0) {
-        double cnt = scount + (double)n_per_segment;
+        tickets[seg] = 0;  // ready for the next call on this stream
+        const double cnt = scount + (double)n_per_segment;
         if (state) {
             state[seg * 3 + 0] = mx;
-            state[seg * 3 + 1] = sm;
+            state[seg * 3 + 1] = tot;
             state[seg * 3 + 2] = cnt;
         }
-        bool ok = mx > -CUDART_INF;
-        lnZ[seg] = ok ? mx + log(sm) - log(cnt) : -CUDART_INF;
-        if (n_eff) n_eff[seg] = ok ? sm : 0.0;
+        const bool ok = mx > -CUDART_INF;
+        lnZ[seg] = ok ? mx + log(tot) - log(cnt) : -CUDART_INF;
+        if (n_eff) n_eff[seg] = ok ? tot : 0.0;
     }
 }
 
@@ -243,7 +262,7 @@ __global__ void ile_evidence_reset_kernel(int32_t n_segments, double *state)
 
 int32_t ile_evidence_blocks_per_segment(int32_t n_segments, int64_t n_per_segment, int32_t sm_count)
 {
-    int64_t want = (n_per_segment + 4095) / 4096;
+    int64_t want = (n_per_segment + EV_PER * EV_THREADS - 1) / (EV_PER * EV_THREADS);  // one tile per block while the grid allows
     int64_t cap = ((int64_t)sm_count * 8 + n_segments - 1) / n_segments;
     if (cap < 1) cap = 1;
     if (want > cap) want = cap;
@@ -251,14 +270,15 @@ int32_t ile_evidence_blocks_per_segment(int32_t n_segments, int64_t n_per_segmen
     return (int32_t)want;
 }
 
+// partials: n_segments * B * 2 doubles followed by n_segments ticket words (zero before the first call)
 cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const double *lnL, const double *log_w,
                                 double *state, double *lnZ, double *n_eff, double *partials, int32_t B,
                                 cudaStream_t st, int *n_launches)
 {
     dim3 grid((unsigned)B, (unsigned)n_segments);
-    ile_evidence_partial_kernel<<<grid, EV_THREADS, 0, st>>>(n_per_segment, lnL, log_w, partials);
-    ile_evidence_combine_kernel<<<(unsigned)n_segments, 32, 0, st>>>(B, n_per_segment, partials, state, lnZ, n_eff);
-    if (n_launches) *n_launches += 2;
+    unsigned int *tickets = reinterpret_cast<unsigned int *>(partials + (size_t)n_segments * B * 2);
+    ile_evidence_kernel<<<grid, EV_THREADS, 0, st>>>(n_per_segment, lnL, log_w, partials, tickets, state, lnZ, n_eff);
+    if (n_launches) *n_launches += 1;
     return cudaGetLastError();
 }
 
