@@ -44,6 +44,27 @@ def dfma_per_sample(K: int, M: int, n_t: int) -> float:
     return linear + quad + lse + geom
 
 
+def rank_sample_seed(base_seed: int, rank: int) -> int:
+    """Seed of rank `rank`'s batch of extrinsic samples: every rank is an independent worker."""
+    return int(base_seed) + 7919 * int(rank)
+
+
+def rank_point_seed(base_seed: int, rank: int) -> int:
+    """Seed of rank `rank`'s intrinsic point (rank 0 keeps the configuration's own point)."""
+    return int(base_seed) + 7919 * int(rank)
+
+
+def max_over_ranks(values, device):
+    """Timing rule of the bench contract: every device-timed figure is the MAX over ranks."""
+    import torch
+    import torch.distributed as dist
+
+    t = torch.tensor(list(values), dtype=torch.float64, device=device)
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size() > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return [float(x) for x in t.cpu()]
+
+
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
@@ -188,9 +209,9 @@ def main():
     if rank > 0:  # a different seeded intrinsic point per rank, same recipe
         c = gi.CONFIGS[args.config]
         snr = c["snr"] if not isinstance(c["snr"], tuple) else 20.0
-        Q, U, V, meta = gi.make_point(gi.point_seed(args.config, 0) + 7919 * rank, c["dets"], c["modes"], c["n_q"], snr, admix=c["admix"])
+        Q, U, V, meta = gi.make_point(rank_point_seed(gi.point_seed(args.config, 0), rank), c["dets"], c["modes"], c["n_q"], snr, admix=c["admix"])
         base["Q"], base["U"], base["V"] = Q[None], U[None], V[None]
-    seed = base["sample_seeds"][0] + 7919 * rank
+    seed = rank_sample_seed(base["sample_seeds"][0], rank)
     s_np = gi.make_samples(seed, n) if args.samples == "prior" else gi.make_concentrated_samples(seed, n)
     ctx = ile.Context(base)
     if args.variant:
@@ -254,10 +275,7 @@ def main():
     e2e_wall = time.perf_counter() - t0
     e2e_ms = max(e2e_ms, e2e_wall * 1e3)        # the call synchronises: wall clock and device time agree; take the larger
 
-    t = torch.tensor([step_ms, eval_ms, e2e_ms], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    step_ms, eval_ms, e2e_ms = (float(x) for x in t.cpu())
+    step_ms, eval_ms, e2e_ms = max_over_ranks([step_ms, eval_ms, e2e_ms], "cuda")
 
     if rank == 0:
         K, M, n_t = base["n_det"], base["n_modes"], base["n_t"]

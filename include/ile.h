@@ -107,6 +107,15 @@ int ile_evidence(ile_ctx *ctx, int32_t n_segments, int64_t n_per_segment, const 
 /* Set n_segments evidence states (device [n_segments][3]) to (-inf, 0, 0). */
 int ile_evidence_reset(ile_ctx *ctx, int32_t n_segments, double *state, void *cuda_stream);
 
+/* Combine n_states evidence states of the same n_segments segments -- the sums of eq. 4 (L42-L47) taken over disjoint
+ * parts of one sample set, e.g. by independent workers (L134-L141) or by several GPUs: states_in is device
+ * [n_states][n_segments][3] doubles, each as ile_evidence leaves it.  Writes the merged state to state_out (device
+ * [n_segments][3], may alias states_in[0], may be NULL) and lnZ / n_eff (device, n_segments doubles; n_eff may be NULL)
+ * exactly as one ile_evidence call over the union would.  The only data a multi-GPU run of one intrinsic point has to
+ * exchange is these 24 bytes per segment and rank. */
+int ile_evidence_merge(ile_ctx *ctx, int32_t n_segments, int32_t n_states, const double *states_in, double *state_out,
+                       double *lnZ, double *n_eff, void *cuda_stream);
+
 /* Whole hot path from HOST buffers, for callers that keep samples on the host (the paper's workflow, L97: blocks
  * generated on the CPU and transferred to the board): H2D copy of the seven sample arrays (+ log_w), ile_eval,
  * ile_evidence, D2H of lnL_margT (if not NULL), lnZ and n_eff.  Host arrays of n doubles each; pinned memory makes

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libile_b200.so")
 _lib = None
 
 SAMPLE_FIELDS = ("ra", "dec", "t_ref", "phi_ref", "psi", "incl", "dist_mpc")
-EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_run_host", "ile_status",
+EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_evidence_merge", "ile_run_host", "ile_status",
            "ile_set_variant", "ile_launch_count", "ile_measure_fp64_peak", "ile_destroy", "ile_strerror")
 
 
@@ -56,6 +56,7 @@ def load():
     L.ile_eval_all.argtypes = [vp, i64] + [vp] * 7 + [vp, vp, vp]
     L.ile_evidence.argtypes = [vp, i32, i64, vp, vp, vp, vp, vp, vp]
     L.ile_evidence_reset.argtypes = [vp, i32, vp, vp]
+    L.ile_evidence_merge.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
     L.ile_run_host.argtypes = [vp, i32, i64] + [vp] * 7 + [vp, vp, dp, dp, vp]
     L.ile_status.argtypes = [vp, ctypes.POINTER(i64), ctypes.c_int, vp]
     L.ile_set_variant.argtypes = [vp, i32]
@@ -190,6 +191,20 @@ class Context:
                                    _ptr(lnZ), _ptr(neff), _stream_ptr(stream)), "ile_evidence")
         return lnZ, neff
 
+    def evidence_merge(self, states, stream=None):
+        """ile_evidence_merge: states [n_states][n_segments][3] (CUDA float64, e.g. gathered from all ranks by
+        gather_evidence_states) -> (merged state [n_segments][3], lnZ [n_segments], n_eff [n_segments])."""
+        import torch
+
+        assert states.is_cuda and states.dtype == torch.float64 and states.is_contiguous() and states.dim() == 3 and states.shape[2] == 3
+        n_states, n_seg = int(states.shape[0]), int(states.shape[1])
+        out = torch.empty((n_seg, 3), dtype=torch.float64, device=states.device)
+        lnZ = torch.empty(n_seg, dtype=torch.float64, device=states.device)
+        neff = torch.empty(n_seg, dtype=torch.float64, device=states.device)
+        _check(load().ile_evidence_merge(self._h, n_seg, n_states, _ptr(states), _ptr(out), _ptr(lnZ), _ptr(neff),
+                                         _stream_ptr(stream)), "ile_evidence_merge")
+        return out, lnZ, neff
+
     def new_state(self, n_segments: int = 1, device="cuda", stream=None):
         import torch
 
@@ -221,6 +236,19 @@ class Context:
         if code not in (0, -5):
             raise IleError(code, "ile_status")
         return int(v.value), code
+
+
+def gather_evidence_states(state, group=None):
+    """Plumbing for several GPUs working on ONE intrinsic point: all-gather every rank's evidence state
+    ([n_segments][3], as ile_evidence leaves it) -> [world][n_segments][3] on every rank, ready for
+    Context.evidence_merge.  No arithmetic here; works with any torch.distributed backend (nccl on GPUs, gloo on CPU)."""
+    import torch
+    import torch.distributed as dist
+
+    world = dist.get_world_size(group)
+    out = [torch.empty_like(state) for _ in range(world)]
+    dist.all_gather(out, state.contiguous(), group=group)
+    return torch.stack(out, 0).contiguous()
 
 
 def samples_to_device(samples_np, device="cuda"):

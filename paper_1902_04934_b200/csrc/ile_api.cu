@@ -434,6 +434,17 @@ extern "C" int ile_evidence(ile_ctx *c, int32_t n_segments, int64_t n_per_segmen
     return ILE_OK;
 }
 
+extern "C" int ile_evidence_merge(ile_ctx *c, int32_t n_segments, int32_t n_states, const double *states_in, double *state_out,
+                                  double *lnZ, double *n_eff, void *cuda_stream)
+{
+    if (!c || n_segments < 1 || n_states < 1 || !states_in || !lnZ) return ILE_ERR_BAD_ARGUMENT;
+    int nl = 0;
+    cudaError_t e = ile_launch_evidence_merge(n_segments, n_states, states_in, state_out, lnZ, n_eff, (cudaStream_t)cuda_stream, &nl);
+    c->launches += nl;
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ILE_OK;
+}
+
 extern "C" int ile_evidence_reset(ile_ctx *c, int32_t n_segments, double *state, void *cuda_stream)
 {
     if (!c || n_segments < 1 || !state) return ILE_ERR_BAD_ARGUMENT;

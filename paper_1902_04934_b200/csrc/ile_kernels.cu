@@ -260,6 +260,36 @@ __global__ void ile_evidence_reset_kernel(int32_t n_segments, double *state)
     }
 }
 
+// states_in [n_states][n_segments][3] -> merged state, lnZ, n_eff: one thread per segment
+__global__ void ile_evidence_merge_kernel(int32_t n_segments, int32_t n_states, const double *__restrict__ states_in,
+                                          double *state_out, double *__restrict__ lnZ, double *__restrict__ n_eff)
+{
+    const int seg = blockIdx.x * blockDim.x + threadIdx.x;
+    if (seg >= n_segments) return;
+    double m = -CUDART_INF, sm = 0.0, cnt = 0.0;
+    for (int r = 0; r < n_states; ++r) {
+        const double *st = states_in + ((size_t)r * n_segments + seg) * 3;
+        ev_merge(m, sm, st[0], st[1]);
+        cnt += st[2];
+    }
+    if (state_out) {
+        state_out[seg * 3 + 0] = m;
+        state_out[seg * 3 + 1] = sm;
+        state_out[seg * 3 + 2] = cnt;
+    }
+    const bool ok = m > -CUDART_INF;
+    lnZ[seg] = ok ? m + log(sm) - log(cnt) : -CUDART_INF;
+    if (n_eff) n_eff[seg] = ok ? sm : 0.0;
+}
+
+cudaError_t ile_launch_evidence_merge(int32_t n_segments, int32_t n_states, const double *states_in, double *state_out,
+                                      double *lnZ, double *n_eff, cudaStream_t st, int *n_launches)
+{
+    ile_evidence_merge_kernel<<<(n_segments + 127) / 128, 128, 0, st>>>(n_segments, n_states, states_in, state_out, lnZ, n_eff);
+    if (n_launches) *n_launches += 1;
+    return cudaGetLastError();
+}
+
 int32_t ile_evidence_blocks_per_segment(int32_t n_segments, int64_t n_per_segment, int32_t sm_count)
 {
     int64_t want = (n_per_segment + EV_PER * EV_THREADS - 1) / (EV_PER * EV_THREADS);  // one tile per block while the grid allows

@@ -133,6 +133,8 @@ cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const
                                 double *state, double *lnZ, double *n_eff, double *partials, int32_t blocks_per_seg,
                                 cudaStream_t st, int *n_launches);
 int32_t ile_evidence_blocks_per_segment(int32_t n_segments, int64_t n_per_segment, int32_t sm_count);
+cudaError_t ile_launch_evidence_merge(int32_t n_segments, int32_t n_states, const double *states_in, double *state_out,
+                                      double *lnZ, double *n_eff, cudaStream_t st, int *n_launches);
 cudaError_t ile_launch_evidence_reset(int32_t n_segments, double *state, cudaStream_t st, int *n_launches);
 
 cudaError_t ile_launch_fp64_peak(int32_t iters, int32_t sm_count, double *sink, cudaStream_t st);

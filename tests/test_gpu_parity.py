@@ -331,3 +331,44 @@ def test_run_host_matches_device_path(gpu_lib):
     assert out2 is None and rel_err([oracle.evidence(ref)[0]], [lnZ2]) <= TOL
     assert ctx.launch_count >= 6
     ctx.close()
+
+
+def test_evidence_merge_of_split_batch_equals_whole(gpu_lib):
+    """ile_evidence_merge: states of disjoint parts of one sample set merge to the evidence of the whole (what several
+    GPUs sharing one intrinsic point exchange); also across segments and with an empty (all -inf) part."""
+    import torch
+
+    cfg = gi.make_config(1, n=30_000)
+    s = gi.make_samples(cfg["sample_seeds"][0], cfg["n"])
+    lw = gi.make_log_weights(3, cfg["n"])
+    ctx = gpu_lib.Context(cfg)
+    lnL, _ = ctx.eval(to_dev(s))
+    lwd = torch.from_numpy(lw).cuda()
+    cuts = [0, 7_001, 7_001 + 16_384, 30_000]
+    states = []
+    for a, b in zip(cuts[:-1], cuts[1:]):
+        st = ctx.new_state(1)
+        ctx.evidence(lnL[a:b].contiguous(), lwd[a:b].contiguous(), state=st)
+        states.append(st)
+    dead = ctx.new_state(1)  # a rank whose samples were all out of range
+    ctx.evidence(torch.full((5,), float("-inf"), dtype=torch.float64, device="cuda"), None, state=dead)
+    states.append(dead)
+    merged, lnZ, neff = ctx.evidence_merge(torch.stack(states, 0).contiguous())
+    ref, _, _ = oracle.eval_batch(cfg, s, n_threads=ORACLE_THREADS)
+    e = ref + lw
+    m = e.max()
+    rN = float(np.sum(np.exp(e - m)))
+    rZ = m + np.log(rN) - np.log(cfg["n"] + 5)  # the dead part still counts its 5 samples (eq. 4: 1/n of ALL draws)
+    assert rel_err([rZ], lnZ.cpu().numpy()) <= TOL
+    assert rel_err([rN], neff.cpu().numpy()) <= TOL
+    assert merged.cpu().numpy()[0, 2] == cfg["n"] + 5
+    ctx.close()
+
+
+@pytest.mark.parametrize("variant", [1, 2, 3, 4])
+def test_every_variant_matches_the_oracle(gpu_lib, variant):
+    """ile_set_variant: each evaluation kernel family on the same 20,000 samples of config 1 (indices bit-exact, values
+    within TOL); variant 0 (automatic) is what every other test and bench.py run."""
+    cfg = gi.make_config(1, n=20_000)
+    s = gi.make_samples(cfg["sample_seeds"][0], cfg["n"])
+    full_compare(gpu_lib, cfg, s, variant=variant)
