@@ -156,9 +156,10 @@ def run_reference(args, rank: int):
 def workload_config(cfg, n, args, extra=None):
     c = {"workload": f"BASELINE.json configs[{cfg['config_id']}]: {cfg['n_det']} detectors ({','.join(cfg['dets'])}), "
                      f"{cfg['n_modes']} modes (l<= {int(max(cfg['l']))}), Q {cfg['n_q']} complex128 @ {int(cfg['fs_hz'])} Hz, "
-                     f"{n} extrinsic samples/step/GPU, {cfg['n_t']} time bins",
-         "n_det": cfg["n_det"], "n_modes": cfg["n_modes"], "n_q": cfg["n_q"], "n_t": cfg["n_t"], "samples_per_step_per_gpu": n,
-         "parallelism": f"independent intrinsic points, 1 per GPU x{args.gpus}", "l2": "flushed between timed steps (256 MiB write)"}
+                     f"{cfg['n_points']} intrinsic point(s) x {n} extrinsic samples/step/GPU, {cfg['n_t']} time bins",
+         "n_det": cfg["n_det"], "n_modes": cfg["n_modes"], "n_q": cfg["n_q"], "n_t": cfg["n_t"],
+         "samples_per_step_per_gpu": n * cfg["n_points"], "points_per_gpu": cfg["n_points"],
+         "parallelism": f"independent intrinsic points, {cfg['n_points']} per GPU x{args.gpus}", "l2": "flushed between timed steps (256 MiB write)"}
     if extra:
         c.update(extra)
     return c
@@ -174,6 +175,7 @@ def main():
     ap.add_argument("--config", type=int, default=1)
     ap.add_argument("--n", type=int, default=None, help="samples per step per GPU (default: the config's)")
     ap.add_argument("--variant", type=int, default=0)
+    ap.add_argument("--points", type=int, default=1, help="intrinsic points evaluated concurrently per step (config 4: 256), ile_eval_all")
     ap.add_argument("--samples", default="prior", choices=["prior", "concentrated"])
     ap.add_argument("--ref-samples-per-step", type=int, default=100_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -204,7 +206,8 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     # ---- workload: one intrinsic point and one batch per rank (independent workers)
-    base = gi.make_config(args.config, n_points=1)
+    P = max(1, args.points)
+    base = gi.make_config(args.config, n_points=P)
     n = args.n if args.n is not None else base["n"]
     if rank > 0:  # a different seeded intrinsic point per rank, same recipe
         c = gi.CONFIGS[args.config]
@@ -212,25 +215,48 @@ def main():
         Q, U, V, meta = gi.make_point(rank_point_seed(gi.point_seed(args.config, 0), rank), c["dets"], c["modes"], c["n_q"], snr, admix=c["admix"])
         base["Q"], base["U"], base["V"] = Q[None], U[None], V[None]
     seed = rank_sample_seed(base["sample_seeds"][0], rank)
-    s_np = gi.make_samples(seed, n) if args.samples == "prior" else gi.make_concentrated_samples(seed, n)
+    mk = gi.make_samples if args.samples == "prior" else gi.make_concentrated_samples
+    if P == 1:
+        s_np = mk(seed, n)
+    else:  # [P][n]: every point its own seeded batch
+        parts = [mk(rank_sample_seed(base["sample_seeds"][p], rank), n) for p in range(P)]
+        s_np = {k: np.ascontiguousarray(np.concatenate([q[k] for q in parts])) for k in parts[0]}
     ctx = ile.Context(base)
     if args.variant:
         ctx.set_variant(args.variant)
     dev = ile.samples_to_device(s_np)
     host = {k: torch.from_numpy(v).pin_memory() for k, v in s_np.items()}
     host_out = torch.empty(n, dtype=torch.float64).pin_memory()
-    lnL = torch.empty(n, dtype=torch.float64, device="cuda")
+    lnL = torch.empty(P * n, dtype=torch.float64, device="cuda")
+    host_out = torch.empty(P * n, dtype=torch.float64).pin_memory() if P > 1 else host_out
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     stream = torch.cuda.current_stream()
 
+    def do_eval():
+        if P == 1:
+            ctx.eval(dev, want_idx=False, out=lnL)
+        else:
+            ctx.eval_all(dev, want_idx=False, out=lnL.view(P, n))
+
+    def do_e2e():
+        if P == 1:
+            return ctx.run_host(host, None, out_host=host_out)
+        # several points: H2D of the [P][n] sample arrays, ile_eval_all + ile_evidence, D2H of lnL_margT, lnZ, n_eff
+        d = {k: dev[k].copy_(host[k], non_blocking=True) for k in host}
+        ctx.eval_all(d, want_idx=False, out=lnL.view(P, n))
+        z, ne = ctx.evidence(lnL, n_segments=P)
+        host_out.copy_(lnL, non_blocking=True)
+        zc, nc = z.cpu(), ne.cpu()
+        return host_out, zc, nc
+
     def step():
-        ctx.eval(dev, want_idx=False, out=lnL)
-        return ctx.evidence(lnL)
+        do_eval()
+        return ctx.evidence(lnL, n_segments=P)
 
     for _ in range(args.warmup):
         flush.fill_(1)
         step()
-        ctx.run_host(host, None, out_host=host_out)
+        do_e2e()
     torch.cuda.synchronize()
 
     peak_tflops, _ = ile.measure_fp64_peak(1 << 15)
@@ -248,9 +274,9 @@ def main():
     for i in range(args.steps):
         flush.fill_(i & 1)                      # L2 flush, outside the event pair
         ev[i][0].record(stream)
-        ctx.eval(dev, want_idx=False, out=lnL)
+        do_eval()
         ev[i][1].record(stream)
-        lnZ, neff = ctx.evidence(lnL)
+        lnZ, neff = ctx.evidence(lnL, n_segments=P)
         ev[i][2].record(stream)
     torch.cuda.synchronize()
     wall = time.perf_counter() - wall0
@@ -268,7 +294,7 @@ def main():
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     e0.record(stream)
     for i in range(args.steps):
-        _, lnZ_h, neff_h = ctx.run_host(host, None, out_host=host_out)
+        _, lnZ_h, neff_h = do_e2e()
     e1.record(stream)
     torch.cuda.synchronize()
     e2e_ms = e0.elapsed_time(e1)
@@ -280,9 +306,9 @@ def main():
     if rank == 0:
         K, M, n_t = base["n_det"], base["n_modes"], base["n_t"]
         w = dfma_per_sample(K, M, n_t)
-        value = world * n * args.steps / (step_ms * 1e-3)
+        value = world * P * n * args.steps / (step_ms * 1e-3)
         eval_avg_ms = eval_ms / args.steps
-        achieved = 2.0 * w * n / (eval_avg_ms * 1e-3) * 1e-12
+        achieved = 2.0 * w * P * n / (eval_avg_ms * 1e-3) * 1e-12
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": step_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -292,16 +318,17 @@ def main():
                          "traffic": read_traffic_bytes(), "kernel": "ile_eval (steps 1-6)", "kernel_ms": eval_avg_ms,
                          "dfma_equiv_per_sample": w, "peak_source": "ile_measure_fp64_peak: register-resident DFMA chains, measured in this run "
                          "(nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2 TFLOP/s)"},
-            "e2e": {"value": world * n * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 7 * 8 * n,
-                    "d2h_bytes_per_step": 8 * n + 16, "ms_per_step": e2e_ms / args.steps, "api": "ile_run_host (pinned host buffers)"},
+            "e2e": {"value": world * P * n * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 7 * 8 * P * n,
+                    "d2h_bytes_per_step": 8 * P * n + 16 * P, "ms_per_step": e2e_ms / args.steps,
+                    "api": "ile_run_host (pinned host buffers)" if P == 1 else "pinned H2D + ile_eval_all + ile_evidence + D2H"},
             "gpu_launches": int(launches), "clocks": sampler.summary(), "wall_ms_per_step": wall / args.steps * 1e3,
-            "lnZ": float(lnZ.item()), "n_eff": float(neff.item()), "n_out_of_range": int(n_bad),
+            "lnZ": float(lnZ[0].item()), "n_eff": float(neff[0].item()), "n_out_of_range": int(n_bad),
         }
         if not args.no_cpu_baseline:
             import oracle  # cpu_baseline leg: the one place bench.py's product arm may execute oracle/
 
             cores = os.cpu_count() or 1
-            n_cpu = min(n, 100_000)
+            n_cpu = min(n, 100_000)  # of intrinsic point 0
             sub = {k: v[:n_cpu] for k, v in s_np.items()}
             passes = 4
             oracle.eval_batch(base, {k: v[:2000] for k, v in s_np.items()}, n_threads=cores)  # page in / spin up

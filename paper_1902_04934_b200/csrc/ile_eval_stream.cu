@@ -567,6 +567,8 @@ cudaError_t ile_launch_pack_q_stream(const IleSizes &sz, const IleStreamPlan &pl
 // group of 8 consecutive slots never mixes two (d1, d2) cells
 // ------------------------------------------------------------------------------------------------------------
 #define SS_THREADS 1024 /* scan kernel of multi-point launches */
+#define SS_BIG 64       /* a cell with more groups than this is written to the group list by the whole block */
+#define SS_NBIG 256
 #ifndef IX_THREADS
 #define IX_THREADS 1024
 #endif
@@ -723,9 +725,13 @@ __device__ void ss_scan_point(const IleScanArgs &A, int pt, uint32_t *__restrict
         wsum[lane] = xi - x;
     }
     __syncthreads();
+    __shared__ uint3 big[SS_NBIG];
+    __shared__ uint32_t nbig;
+    if (threadIdx.x == 0) nbig = 0;
+    __syncthreads();
     // the list is assembled in shared memory when it fits (scattered 4-byte global stores cost a cycle each), then copied out
     const bool staged = (tot >> 3) <= (uint32_t)A.stage;
-    int32_t *__restrict__ dst = staged ? reinterpret_cast<int32_t *>(ad + nseg) : go;
+    int32_t *__restrict__ dst = staged ? reinterpret_cast<int32_t *>(h + ((ncell + 1 + nseg + 3) & ~3)) : go;
     uint32_t run = wsum[warp] + inc - loc;
     {
         int b = qlo / nseg, sgm = qlo - b * nseg;
@@ -733,13 +739,29 @@ __device__ void ss_scan_point(const IleScanArgs &A, int pt, uint32_t *__restrict
             const int c = sgm * n0 + b;
             const uint32_t p0 = h[c] + ad[sgm], p1 = h[c + 1] + ad[sgm];
             const uint32_t g0 = (p0 + 7u) >> 3, g1 = (p1 + 7u) >> 3;
+            if (g1 - g0 > SS_BIG) {  // a crowded cell (concentrated samples): left to the whole block
+                const uint32_t e = atomicAdd(&nbig, 1u);
+                if (e < SS_NBIG) {
+                    big[e] = make_uint3(run, g0, g1 - g0);
+                    run += g1 - g0;
+                    if (++sgm == nseg) sgm = 0, ++b;
+                    continue;
+                }
+            }
             for (uint32_t g = g0; g < g1; ++g) dst[run++] = (int32_t)g;
             if (++sgm == nseg) sgm = 0, ++b;
         }
     }
+    __syncthreads();
+    for (uint32_t e = 0; e < min(nbig, (uint32_t)SS_NBIG); ++e) {
+        const uint3 w = big[e];
+        for (uint32_t i = threadIdx.x; i < w.z; i += NT) dst[w.x + i] = (int32_t)(w.y + i);
+    }
     if (staged) {
         __syncthreads();
-        for (uint32_t i = threadIdx.x; i < (tot >> 3); i += NT) go[i] = dst[i];
+        // 16-byte stores (gorder rows and the staging area are 16-byte aligned; the tail past the list is scratch)
+        const uint32_t n4 = ((tot >> 3) + 3) >> 2;
+        for (uint32_t i = threadIdx.x; i < n4; i += NT) reinterpret_cast<int4 *>(go)[i] = reinterpret_cast<const int4 *>(dst)[i];
     }
 }
 
@@ -788,7 +810,11 @@ __global__ void __launch_bounds__(IX_THREADS)
             c = seg * sp.n0 + (i0[0] >> sp.g0);  // 0 <= i0_0 <= n_q - n_t here
         }
         cell[s] = c;
-        atomicAdd(&A.hist[(size_t)pt * sp.ncell + c], 1u);
+        // warp-aggregated: lanes with the same counter send ONE atomic (late in a run the adaptive sampler's draws
+        // crowd into a handful of cells, L47, L109, and one atomic per sample on the same address serialises in L2)
+        const unsigned long long key = (unsigned long long)pt * sp.ncell + c;
+        const unsigned peers = __match_any_sync(__activemask(), key);
+        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&A.hist[key], (uint32_t)__popc(peers));
     }
     if (FUSED) {
         extern __shared__ uint32_t ss_h[];
@@ -823,8 +849,15 @@ __global__ void __launch_bounds__(IX_THREADS) ile_stream_scatter_kernel(long lon
     for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n_total; s += (long long)gridDim.x * blockDim.x) {
         const int pt = (int)(s / n_per_point);
         const int c = cell[s];
-        if (c == ncell - 1) continue;  // out of range: lnL = -inf was written by the setup kernel
-        const uint32_t pos = atomicAdd(&offs[(size_t)pt * ncell + c], 1u) + adj[(size_t)pt * nseg + c / n0];
+        if (c == ncell - 1) continue;  // out of range: lnL = -inf was written by the index kernel
+        // warp-aggregated claim: the first lane of every set of lanes with the same counter takes the whole set's places
+        const unsigned long long key = (unsigned long long)pt * ncell + c;
+        const unsigned peers = __match_any_sync(__activemask(), key);
+        const int lane = threadIdx.x & 31, leader = __ffs(peers) - 1;
+        uint32_t first = 0;
+        if (lane == leader) first = atomicAdd(&offs[key], (uint32_t)__popc(peers));
+        first = __shfl_sync(peers, first, leader);
+        const uint32_t pos = first + (uint32_t)__popc(peers & ((1u << lane) - 1u)) + adj[(size_t)pt * nseg + c / n0];
         slots[(size_t)pt * slot_cap + pos] = (int32_t)(s - (long long)pt * n_per_point);
     }
 }
@@ -875,7 +908,7 @@ bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per
     for (;; ++g0) {
         sp.n0 = ((sz.n_q - sz.n_t) >> g0) + 1;
         const long long nc = (long long)sp.n0 * sp.n1 * sp.n2 + 1;
-        if ((nc + 1 + (long long)sp.n1 * sp.n2) * 4 <= (long long)sz.max_smem_optin - 2048) {  // the scan kernel keeps a point's histogram in shared memory
+        if ((nc + 1 + (long long)sp.n1 * sp.n2) * 4 <= (long long)sz.max_smem_optin - 8192 - 64) {  // the scan kernel keeps a point's histogram in shared memory
             sp.ncell = (int32_t)nc;
             break;
         }
@@ -944,17 +977,17 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     sa.gcum = ss.gcum;
     sa.gorder = ss.gorder;
     sa.gcap = ss.slot_cap / 8;
-    size_t scan_smem = ((size_t)sp.ncell + 1 + nseg) * sizeof(uint32_t);
+    size_t scan_smem = (((size_t)sp.ncell + 1 + nseg + 3) & ~(size_t)3) * sizeof(uint32_t);
     {
-        const size_t room = (size_t)(sz.max_smem_optin - 1024) - scan_smem, want = (size_t)sa.gcap * sizeof(int32_t);
+        const size_t room = (size_t)(sz.max_smem_optin - 8192) - scan_smem, want = (size_t)sa.gcap * sizeof(int32_t);
         sa.stage = want <= room ? (int32_t)sa.gcap : 0;
         if (sa.stage) scan_smem += want;
     }
     static bool scan_attr = false;
     if (!scan_attr) {
-        e = cudaFuncSetAttribute(ile_stream_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 1024);
+        e = cudaFuncSetAttribute(ile_stream_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 8192);
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(ile_stream_index_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 1024);
+        e = cudaFuncSetAttribute(ile_stream_index_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 8192);
         if (e != cudaSuccess) return e;
         scan_attr = true;
     }
