@@ -27,7 +27,7 @@ struct ile_ctx {
     bool mma_ok;
     IleMmaPlan mp;
     double *dQp;
-    int64_t chunk_samples;  // samples per launch group: keeps the record scratch L2-resident
+    int64_t chunk_samples;  // samples per launch group (bounds the scratch: <= 2 GiB of records, <= 2^20 samples)
     IleMmaScratch sc;
     size_t sc_samples, sc_hist;  // capacities (samples, histogram words)
     int32_t sc_points;
@@ -48,6 +48,12 @@ static int cuda_fail(cudaError_t e)
     snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error %d: %s", (int)e, cudaGetErrorString(e));
     return ILE_ERR_CUDA;
 }
+#ifndef ILE_CHUNK_BYTES
+#define ILE_CHUNK_BYTES (2048u << 20) /* record scratch per launch group: bigger groups sort into tighter windows and pay one pre-pass */
+#endif
+#ifndef ILE_CHUNK_MAX
+#define ILE_CHUNK_MAX 1048576
+#endif
 #define CK(call)                                  \
     do {                                          \
         cudaError_t e__ = (call);                 \
@@ -168,8 +174,8 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
         CKC(cudaMalloc(&c->dQp, nQp * sizeof(double)));
         CKC(ile_launch_pack_q(c->sz, c->mp, cfg->n_points, c->dQ, c->dQp, 0));
         CKC(cudaDeviceSynchronize());
-        int64_t cs = (int64_t)(64u << 20) / ((int64_t)c->mp.recg * 8);
-        cs = cs < 16384 ? 16384 : cs > 262144 ? 262144 : cs;
+        int64_t cs = (int64_t)ILE_CHUNK_BYTES / ((int64_t)c->mp.recg * 8);
+        cs = cs < 16384 ? 16384 : cs > ILE_CHUNK_MAX ? ILE_CHUNK_MAX : cs;
         c->chunk_samples = cs;
     }
     c->sc_recg = c->mma_ok ? c->mp.recg : 0;
@@ -184,8 +190,8 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
         CKC(cudaDeviceSynchronize());
         if (cfg->n_det * c->spl.cp > c->sc_recg) c->sc_recg = cfg->n_det * c->spl.cp;
         if (!c->mma_ok) {
-            int64_t cs = (int64_t)(64u << 20) / ((int64_t)c->sc_recg * 8);
-            c->chunk_samples = cs < 16384 ? 16384 : cs > 262144 ? 262144 : cs;
+            int64_t cs = (int64_t)ILE_CHUNK_BYTES / ((int64_t)c->sc_recg * 8);
+            c->chunk_samples = cs < 16384 ? 16384 : cs > ILE_CHUNK_MAX ? ILE_CHUNK_MAX : cs;
         }
     }
 #undef CKC
