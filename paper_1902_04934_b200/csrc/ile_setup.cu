@@ -64,7 +64,7 @@ cudaError_t ile_launch_pack_q(const IleSizes &sz, const IleMmaPlan &mp, int32_t 
 // SORT = false (variant 4): coefficients and quadratic term only -- window starts, cell keys and the histogram come
 // from ile_index_kernel, which runs concurrently on the caller's stream.
 template <int MMAX, bool SORT>
-__global__ void __launch_bounds__(SETUP_THREADS, SETUP_MINB)
+__global__ void __launch_bounds__(SETUP_THREADS, (MMAX <= 5 ? SETUP_MINB : MMAX <= 12 ? 3 : 2))
     ile_setup_kernel(const __grid_constant__ IleDevParams P, const __grid_constant__ IleEvalArgs a, const int32_t cp,
                      const __grid_constant__ IleSortPlan sp, const __grid_constant__ IleMmaScratch sc)
 {
@@ -297,6 +297,7 @@ void ile_launch_setup_coef(const IleSizes &sz, const IleDevParams &hp, const Ile
     if (M <= 2) setup_launch_t<2, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
     else if (M <= 5) setup_launch_t<5, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
     else if (M <= 12) setup_launch_t<12, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
+    else if (M <= 21) setup_launch_t<21, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
     else setup_launch_t<ILE_MAX_MODES, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
 }
 
