@@ -39,6 +39,8 @@ struct ile_ctx {
     double *dQs;
     IleStreamScratch ss;
     size_t ss_slots, ss_adj, ss_gcum, ss_gorder;  // capacities in words
+    cudaStream_t copy_stream;  // ile_run_host: second H2D queue
+    cudaEvent_t ev_copy_go, ev_copy_done;
 };
 
 static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
@@ -184,6 +186,9 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
         CKC(cudaStreamCreateWithFlags(&c->ss.aux, cudaStreamNonBlocking));
         CKC(cudaEventCreateWithFlags(&c->ss.ev_fork, cudaEventDisableTiming));
         CKC(cudaEventCreateWithFlags(&c->ss.ev_join, cudaEventDisableTiming));
+        CKC(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+        CKC(cudaEventCreateWithFlags(&c->ev_copy_go, cudaEventDisableTiming));
+        CKC(cudaEventCreateWithFlags(&c->ev_copy_done, cudaEventDisableTiming));
         const size_t nQs = (size_t)cfg->n_points * cfg->n_det * c->spl.ks * c->spl.nqp * 4;
         CKC(cudaMalloc(&c->dQs, nQs * sizeof(double)));
         CKC(ile_launch_pack_q_stream(c->sz, c->spl, cfg->n_points, c->dQ, c->dQs, 0));
@@ -226,6 +231,9 @@ extern "C" void ile_destroy(ile_ctx *c)
     if (c->ss.aux) cudaStreamDestroy(c->ss.aux);
     if (c->ss.ev_fork) cudaEventDestroy(c->ss.ev_fork);
     if (c->ss.ev_join) cudaEventDestroy(c->ss.ev_join);
+    if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
+    if (c->ev_copy_go) cudaEventDestroy(c->ev_copy_go);
+    if (c->ev_copy_done) cudaEventDestroy(c->ev_copy_done);
     if (c->h_small) cudaFreeHost(c->h_small);
     delete c;
 }
@@ -480,11 +488,25 @@ extern "C" int ile_run_host(ile_ctx *c, int32_t point, int64_t n, const double *
     }
     double *d = c->d_stage;
     const double *src[8] = {ra, dec, t_ref, phi_ref, psi, incl, dist_mpc, log_w};
-    for (int i = 0; i < 8; ++i)
-        if (src[i]) CK(cudaMemcpyAsync(d + (size_t)i * n, src[i], (size_t)n * sizeof(double), cudaMemcpyHostToDevice, st));
+    // The sort needs ra, dec, t_ref only.  When the streaming variant will run as ONE launch group, the other arrays are
+    // copied on a second queue and only the coefficient kernel (side stream) waits for them: their transfer overlaps the
+    // index kernel, the scan and the scatter.
+    const bool split = c->copy_stream && (c->variant == 4 || (c->variant == 0 && c->stream_ok && n >= 16384)) && n <= c->chunk_samples;
+    for (int i = 0; i < 3; ++i) CK(cudaMemcpyAsync(d + (size_t)i * n, src[i], (size_t)n * sizeof(double), cudaMemcpyHostToDevice, st));
+    cudaStream_t late = split ? c->copy_stream : st;
+    if (split) {
+        CK(cudaEventRecord(c->ev_copy_go, st));  // the staging buffer is free once the stream gets here
+        CK(cudaStreamWaitEvent(late, c->ev_copy_go, 0));
+    }
+    for (int i = 3; i < 8; ++i)
+        if (src[i]) CK(cudaMemcpyAsync(d + (size_t)i * n, src[i], (size_t)n * sizeof(double), cudaMemcpyHostToDevice, late));
+    if (split) CK(cudaEventRecord(c->ev_copy_done, late));
     double *d_out = d + (size_t)8 * n;
+    c->ss.ev_late = split ? c->ev_copy_done : nullptr;
     int r = eval_dispatch(c, point, 1, n, d, d + n, d + 2 * n, d + 3 * n, d + 4 * n, d + 5 * n, d + 6 * n, d_out, nullptr, st);
+    c->ss.ev_late = nullptr;
     if (r != ILE_OK) return r;
+    if (split) CK(cudaStreamWaitEvent(st, c->ev_copy_done, 0));  // log_w for the evidence (already implied by the join)
     r = ile_evidence(c, 1, n, d_out, log_w ? d + 7 * n : nullptr, nullptr, c->d_small, c->d_small + 1, st);
     if (r != ILE_OK) return r;
     if (lnL_margT) CK(cudaMemcpyAsync(lnL_margT, d_out, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, st));

@@ -1008,6 +1008,10 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     }
     e = cudaStreamWaitEvent(ss.aux, ss.ev_fork, 0);
     if (e != cudaSuccess) return e;
+    if (ss.ev_late) {  // ile_run_host: those arrays are still being copied on the copy stream
+        e = cudaStreamWaitEvent(ss.aux, ss.ev_late, 0);
+        if (e != cudaSuccess) return e;
+    }
 #ifndef DBG_SKIP_SETUP
     ile_launch_setup_coef(sz, hp, a, pl.cp, sp, sc, ss.aux);
 #endif

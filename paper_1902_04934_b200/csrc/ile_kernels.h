@@ -115,6 +115,7 @@ struct IleStreamScratch {
     int64_t slot_cap;   // slots per point (multiple of 8)
     cudaStream_t aux;   // side stream: the coefficient kernel runs there while the caller's stream sorts
     cudaEvent_t ev_fork, ev_join;
+    cudaEvent_t ev_late;  // if not NULL: the arrays the coefficient kernel reads (phi_ref, psi, incl, dist) arrive with this event
 };
 
 bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point, IleStreamPlan *out, IleSortPlan *sp);
