@@ -39,6 +39,9 @@ struct ile_ctx {
     double *dQs;
     IleStreamScratch ss;
     size_t ss_slots, ss_adj, ss_gcum, ss_gorder;  // capacities in words
+    double *d_quad_mats;  // packed real representations of U, V for the FP64-MMA quadratic forms (M >= ILE_QUAD_MMA_MIN_MODES)
+    double *d_qform;      // [n][K][3]
+    size_t qform_cap;     // samples
     cudaStream_t copy_stream;  // ile_run_host: second H2D queue
     cudaEvent_t ev_copy_go, ev_copy_done;
 };
@@ -52,6 +55,9 @@ static int cuda_fail(cudaError_t e)
 }
 #ifndef ILE_CHUNK_BYTES
 #define ILE_CHUNK_BYTES (2048u << 20) /* record scratch per launch group: bigger groups sort into tighter windows and pay one pre-pass */
+#endif
+#ifndef ILE_QUAD_MMA_MIN_MODES
+#define ILE_QUAD_MMA_MIN_MODES 8
 #endif
 #ifndef ILE_CHUNK_MAX
 #define ILE_CHUNK_MAX 1048576
@@ -183,6 +189,27 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     c->sc_recg = c->mma_ok ? c->mp.recg : 0;
     c->stream_ok = ile_stream_plan(c->sz, c->hparams, 0, &c->spl, &c->ssp);
     if (c->stream_ok) {
+        if (cfg->n_modes >= ILE_QUAD_MMA_MIN_MODES) {
+            const size_t nd = ile_quad_pack_doubles(cfg->n_points, cfg->n_det, cfg->n_modes);
+            double *hm = new (std::nothrow) double[nd];
+            double2 *hU = new (std::nothrow) double2[nU], *hV = new (std::nothrow) double2[nU];
+            if (!hm || !hU || !hV) {
+                delete[] hm, delete[] hU, delete[] hV;
+                ile_destroy(c);
+                return ILE_ERR_CUDA;
+            }
+            cudaError_t e1 = cudaMemcpy(hU, c->dU, nU * sizeof(double2), cudaMemcpyDeviceToHost);
+            cudaError_t e2 = cudaMemcpy(hV, c->dV, nU * sizeof(double2), cudaMemcpyDeviceToHost);
+            cudaError_t e3 = cudaMalloc(&c->d_quad_mats, nd * sizeof(double));
+            if (e1 == cudaSuccess && e2 == cudaSuccess && e3 == cudaSuccess) {
+                ile_quad_pack_host(cfg->n_points, cfg->n_det, cfg->n_modes, hU, hV, hm);
+                e3 = cudaMemcpy(c->d_quad_mats, hm, nd * sizeof(double), cudaMemcpyHostToDevice);
+            }
+            delete[] hm, delete[] hU, delete[] hV;
+            CKC(e1);
+            CKC(e2);
+            CKC(e3);
+        }
         CKC(cudaStreamCreateWithFlags(&c->ss.aux, cudaStreamNonBlocking));
         CKC(cudaEventCreateWithFlags(&c->ss.ev_fork, cudaEventDisableTiming));
         CKC(cudaEventCreateWithFlags(&c->ss.ev_join, cudaEventDisableTiming));
@@ -228,6 +255,8 @@ extern "C" void ile_destroy(ile_ctx *c)
     cudaFree(c->ss.adj);
     cudaFree(c->ss.gcum);
     cudaFree(c->ss.gorder);
+    cudaFree(c->d_quad_mats);
+    cudaFree(c->d_qform);
     if (c->ss.aux) cudaStreamDestroy(c->ss.aux);
     if (c->ss.ev_fork) cudaEventDestroy(c->ss.ev_fork);
     if (c->ss.ev_join) cudaEventDestroy(c->ss.ev_join);
@@ -312,6 +341,20 @@ static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
     }
     c->ss.Qs = c->dQs;
     c->ss.slot_cap = slot_cap;
+    // many modes: the quadratic forms run as an FP64-MMA contraction in front of the coefficient kernel (side stream)
+    const bool quad_mma = c->d_quad_mats && (a.n_points == 1 || (a.n_per_point & 7) == 0);
+    if (quad_mma) {
+        const size_t ns = (size_t)a.n_per_point * a.n_points;
+        if (ns > c->qform_cap) {
+            CK(cudaStreamSynchronize(st));
+            cudaFree(c->d_qform);
+            c->d_qform = nullptr, c->qform_cap = 0;
+            CK(cudaMalloc(&c->d_qform, ns * c->sz.n_det * 3 * sizeof(double)));
+            c->qform_cap = ns;
+        }
+    }
+    c->sc.qform = quad_mma ? c->d_qform : nullptr;
+    c->ss.quad_mats = quad_mma ? c->d_quad_mats : nullptr;
     int nl = 0;
     cudaError_t e = ile_launch_eval_stream(c->sz, c->hparams, a, c->spl, sp, c->sc, c->ss, st, &nl);
     c->launches += nl;

@@ -382,6 +382,15 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
         // fragments in registers one step ahead while they fit (PIPE); otherwise loaded where they are used
         constexpr bool PIPE = KS <= ST_PIPE_MAXKS;
         double af[K][2][PIPE ? KS : 1];  // [k][block of the pair][k-step]; k = 0 is detector 0
+        // too many k-steps for that: two chain-sized buffers, the fragments of chain i + 1 are loaded while chain i runs.
+        // Chains of a step in order: (k = 1, bb = 0), (1, 1), ..., (K - 1, 1), (0, 0), (0, 1); 2K of them, so buffer parity
+        // is the same in every step.
+        double fa[2][PIPE ? 1 : KS];
+        auto ldchain = [&](auto BUF, int k, int bb) {
+            constexpr int B = decltype(BUF)::value;
+#pragma unroll
+            for (int s = 0; s < KS; ++s) fa[B][PIPE ? 0 : s] = __ldg(pk[k] + s * nqp4 + bb * 32);
+        };
         if (PIPE) {
 #pragma unroll
             for (int k = 0; k < K; ++k) {
@@ -391,6 +400,8 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
                     for (int s = 0; s < KS; ++s) af[k][bb][PIPE ? s : 0] = __ldg(pk[k] + s * nqp4 + bb * 32);
                 pk[k] += 64;
             }
+        } else {
+            ldchain(std::integral_constant<int, 0>(), K > 1 ? 1 : 0, 0);
         }
 
         // ---- the stream.  One step = two blocks (t0, t0 + 1): the shifted detectors' MMAs of blocks t0 + NC, t0 + NC + 1
@@ -420,16 +431,18 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
 #pragma unroll
                 for (int bb = 0; bb < 2; ++bb) {
                     double c0 = 0.0, c1 = 0.0;
+                    if (!PIPE) {  // next chain: (k, 1), (k + 1, 0) or detector 0's first
+                        if (bb == 0) ldchain(std::integral_constant<int, 1>(), k, 1);
+                        else ldchain(std::integral_constant<int, 0>(), k + 1 < K ? k + 1 : 0, 0);
+                    }
 #pragma unroll
-                    for (int s = 0; s < KS; ++s)
-                        st_dmma(c0, c1, PIPE ? af[k][bb][PIPE ? s : 0] : __ldg(pk[k] + s * nqp4 + bb * 32), bf[k][s]);
+                    for (int s = 0; s < KS; ++s) st_dmma(c0, c1, PIPE ? af[k][bb][PIPE ? s : 0] : fa[bb][PIPE ? 0 : s], bf[k][s]);
                     ring[k - 1][(2 * P + NC + bb) % 4][0] = c0;
                     ring[k - 1][(2 * P + NC + bb) % 4][1] = c1;
                 }
             }
 #pragma unroll
             for (int k = 1; k < K; ++k) {
-                pk[k] += PIPE ? 0 : 64;
                 if (PIPE) {
 #pragma unroll
                     for (int bb = 0; bb < 2; ++bb)
@@ -467,13 +480,20 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
             }
 #pragma unroll
             for (int bb = 0; bb < 2; ++bb) {
+                if (!PIPE) {
+                    if (bb == 0) {
+                        ldchain(std::integral_constant<int, 1>(), 0, 1);
+                    } else {  // the step is over for the pointers: the next chain is the next step's first
 #pragma unroll
-                for (int s = 0; s < KS; ++s)
-                    st_dmma(z[bb][0], z[bb][1], PIPE ? af[0][bb][PIPE ? s : 0] : __ldg(pk[0] + s * nqp4 + bb * 32), bf[0][s]);
+                        for (int k = 0; k < K; ++k) pk[k] += 64;
+                        ldchain(std::integral_constant<int, 0>(), K > 1 ? 1 : 0, 0);
+                    }
+                }
+#pragma unroll
+                for (int s = 0; s < KS; ++s) st_dmma(z[bb][0], z[bb][1], PIPE ? af[0][bb][PIPE ? s : 0] : fa[bb][PIPE ? 0 : s], bf[0][s]);
                 lin[bb][0] = z[bb][0];
                 lin[bb][1] = z[bb][1];
             }
-            pk[0] += PIPE ? 0 : 64;
             if (PIPE) {
 #pragma unroll
                 for (int bb = 0; bb < 2; ++bb)
@@ -1013,6 +1033,11 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
         if (e != cudaSuccess) return e;
     }
 #ifndef DBG_SKIP_SETUP
+    if (ss.quad_mats && sc.qform) {
+        e = ile_launch_quad_mma(sz, hp, a, ss.quad_mats, sc.qform, ss.aux);
+        if (e != cudaSuccess) return e;
+        ++nl;
+    }
     ile_launch_setup_coef(sz, hp, a, pl.cp, sp, sc, ss.aux);
 #endif
     ++nl;

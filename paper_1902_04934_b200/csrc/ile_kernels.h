@@ -82,6 +82,7 @@ struct IleMmaScratch {
     int32_t *perm;     // [n]
     uint32_t *hist;    // [n_points][ncell]
     int32_t *ngood;    // [n_points]
+    double *qform;     // [n][K][3] quadratic forms from the FP64-MMA kernel, or NULL (the coefficient kernel computes them)
 };
 
 bool ile_mma_plan(const IleSizes &sz, IleMmaPlan *out);
@@ -115,6 +116,7 @@ struct IleStreamScratch {
     int64_t slot_cap;   // slots per point (multiple of 8)
     cudaStream_t aux;   // side stream: the coefficient kernel runs there while the caller's stream sorts
     cudaEvent_t ev_fork, ev_join;
+    const double *quad_mats;  // packed U, V for ile_launch_quad_mma, or NULL
     cudaEvent_t ev_late;  // if not NULL: the arrays the coefficient kernel reads (phi_ref, psi, incl, dist) arrive with this event
 };
 
@@ -128,6 +130,12 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
 // variant 4: coefficients a F_k Y_lm and quadratic term of every sample (steps 1, 3, 4), no sorting work
 void ile_launch_setup_coef(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, int32_t cp, const IleSortPlan &sp,
                            const IleMmaScratch &sc, cudaStream_t st);
+
+// step 4 for many modes (ile_quad_mma.cu): packed real representations of U, V and the batched quadratic forms
+size_t ile_quad_pack_doubles(int32_t n_points, int32_t K, int32_t M);
+void ile_quad_pack_host(int32_t n_points, int32_t K, int32_t M, const double2 *U, const double2 *V, double *out);
+cudaError_t ile_launch_quad_mma(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const double *mats, double *qform,
+                                cudaStream_t st);
 
 // evidence: two kernels (per-block partials, then per-segment combine with the carried state)
 cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const double *lnL, const double *log_w,

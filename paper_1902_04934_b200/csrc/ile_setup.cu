@@ -63,7 +63,7 @@ cudaError_t ile_launch_pack_q(const IleSizes &sz, const IleMmaPlan &mp, int32_t 
 
 // SORT = false (variant 4): coefficients and quadratic term only -- window starts, cell keys and the histogram come
 // from ile_index_kernel, which runs concurrently on the caller's stream.
-template <int MMAX, bool SORT>
+template <int MMAX, bool SORT, bool QF>
 __global__ void __launch_bounds__(SETUP_THREADS, (MMAX <= 5 ? SETUP_MINB : MMAX <= 12 ? 3 : 2))
     ile_setup_kernel(const __grid_constant__ IleDevParams P, const __grid_constant__ IleEvalArgs a, const int32_t cp,
                      const __grid_constant__ IleSortPlan sp, const __grid_constant__ IleMmaScratch sc)
@@ -114,27 +114,33 @@ __global__ void __launch_bounds__(SETUP_THREADS, (MMAX <= 5 ? SETUP_MINB : MMAX 
             const double2 F = ile_antenna(P.det_tensor[k], g);
             double yuy = 0.0;
             double2 yvy = make_double2(0.0, 0.0);
+            if (QF) {  // many modes: Y^dagger U_k Y and Y^T V_k Y come from the FP64-MMA kernel (ile_quad_mma.cu)
+                const double *__restrict__ q = sc.qform + ((size_t)s * K + k) * 3;
+                yuy = q[0];
+                yvy = make_double2(q[1], q[2]);
+            } else {
 #pragma unroll
-            for (int p = 0; p < MMAX; ++p) {
-                if (p < M) {
-                    double2 tu = make_double2(0.0, 0.0), tv = make_double2(0.0, 0.0);
-                    const double2 *Ur = U + ((size_t)k * M + p) * M;
-                    const double2 *Vr = V + ((size_t)k * M + p) * M;
+                for (int p = 0; p < MMAX; ++p) {
+                    if (p < M) {
+                        double2 tu = make_double2(0.0, 0.0), tv = make_double2(0.0, 0.0);
+                        const double2 *Ur = U + ((size_t)k * M + p) * M;
+                        const double2 *Vr = V + ((size_t)k * M + p) * M;
 #pragma unroll
-                    for (int q = 0; q < MMAX; ++q) {
-                        if (q < M) {
-                            const double2 Yq = Y[q], u = __ldg(Ur + q), v = __ldg(Vr + q);
-                            tu.x += u.x * Yq.x - u.y * Yq.y;
-                            tu.y += u.x * Yq.y + u.y * Yq.x;
-                            tv.x += v.x * Yq.x - v.y * Yq.y;
-                            tv.y += v.x * Yq.y + v.y * Yq.x;
+                        for (int q = 0; q < MMAX; ++q) {
+                            if (q < M) {
+                                const double2 Yq = Y[q], u = __ldg(Ur + q), v = __ldg(Vr + q);
+                                tu.x += u.x * Yq.x - u.y * Yq.y;
+                                tu.y += u.x * Yq.y + u.y * Yq.x;
+                                tv.x += v.x * Yq.x - v.y * Yq.y;
+                                tv.y += v.x * Yq.y + v.y * Yq.x;
+                            }
                         }
+                        const double2 Yp = Y[p];
+                        yuy += Yp.x * tu.x + Yp.y * tu.y;  // Re(conj(Y_p) (U Y)_p): U not assumed Hermitian (reading R15)
+                        const double2 t = ile_cmul(Yp, tv);
+                        yvy.x += t.x;
+                        yvy.y += t.y;
                     }
-                    const double2 Yp = Y[p];
-                    yuy += Yp.x * tu.x + Yp.y * tu.y;  // Re(conj(Y_p) (U Y)_p): U not assumed Hermitian (reading R15)
-                    const double2 t = ile_cmul(Yp, tv);
-                    yvy.x += t.x;
-                    yvy.y += t.y;
                 }
             }
             const double F2 = F.x * F.x + F.y * F.y;
@@ -277,11 +283,11 @@ IleSortPlan ile_sort_plan(const IleSizes &sz, const IleDevParams &hp, long long 
     return sp;
 }
 
-template <int MMAX, bool SORT = true>
+template <int MMAX, bool SORT = true, bool QF = false>
 static void setup_launch_t(unsigned blocks, const IleDevParams &hp, const IleEvalArgs &a, const IleMmaPlan &mp,
                            const IleSortPlan &sp, const IleMmaScratch &sc, cudaStream_t st)
 {
-    ile_setup_kernel<MMAX, SORT><<<blocks, SETUP_THREADS, 0, st>>>(hp, a, mp.cp, sp, sc);
+    ile_setup_kernel<MMAX, SORT, QF><<<blocks, SETUP_THREADS, 0, st>>>(hp, a, mp.cp, sp, sc);
 }
 
 void ile_launch_setup_coef(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, int32_t cp, const IleSortPlan &sp,
@@ -294,7 +300,11 @@ void ile_launch_setup_coef(const IleSizes &sz, const IleDevParams &hp, const Ile
     IleMmaPlan mp;
     mp.cp = cp;
     const int M = sz.n_modes;
-    if (M <= 2) setup_launch_t<2, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
+    if (sc.qform) {  // the quadratic forms were computed by ile_launch_quad_mma
+        if (M <= 12) setup_launch_t<12, false, true>((unsigned)blocks, hp, a, mp, sp, sc, st);
+        else if (M <= 21) setup_launch_t<21, false, true>((unsigned)blocks, hp, a, mp, sp, sc, st);
+        else setup_launch_t<ILE_MAX_MODES, false, true>((unsigned)blocks, hp, a, mp, sp, sc, st);
+    } else if (M <= 2) setup_launch_t<2, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
     else if (M <= 5) setup_launch_t<5, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
     else if (M <= 12) setup_launch_t<12, false>((unsigned)blocks, hp, a, mp, sp, sc, st);
     else if (M <= 21) setup_launch_t<21, false>((unsigned)blocks, hp, a, mp, sp, sc, st);

@@ -372,3 +372,15 @@ def test_every_variant_matches_the_oracle(gpu_lib, variant):
     cfg = gi.make_config(1, n=20_000)
     s = gi.make_samples(cfg["sample_seeds"][0], cfg["n"])
     full_compare(gpu_lib, cfg, s, variant=variant)
+
+
+def test_many_modes_quadratic_term_as_mma_with_generic_U_V(gpu_lib):
+    """21 modes through the streaming variant (n >= 16384): the quadratic term runs as the FP64-MMA contraction of
+    ile_quad_mma.cu.  U deliberately not Hermitian, V not symmetric (reading R15); ragged sample count (not a multiple
+    of 8) so the last group of 8 is partial."""
+    cfg = gi.make_config(2, n=20_003)
+    rng = np.random.default_rng(21)
+    cfg["U"] = cfg["U"] * (1.0 + 0.3 * rng.standard_normal(cfg["U"].shape)) + 20j * rng.standard_normal(cfg["U"].shape)
+    cfg["V"] = cfg["V"] + 10.0 * (rng.standard_normal(cfg["V"].shape) + 1j * rng.standard_normal(cfg["V"].shape))
+    s = gi.make_samples(99, cfg["n"])
+    full_compare(gpu_lib, cfg, s, variant=4)
