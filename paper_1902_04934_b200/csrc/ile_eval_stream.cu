@@ -641,6 +641,7 @@ struct IleScanArgs {
     uint32_t *ngr;    // [n_points]
     int32_t *gcum;    // [n_points + 1]
     int32_t *gorder;  // [n_points][gcap]
+    int32_t *slots;   // [n_points][8 gcap]: the scan marks the padding at the end of every segment with -1
     long long gcap;
     int32_t stage;    // words of shared memory behind the histogram for assembling the group list (0: none)
 };
@@ -700,7 +701,10 @@ __device__ void ss_scan_point(const IleScanArgs &A, int pt, uint32_t *__restrict
     const uint32_t tot = ss_block_scan<NT>(ad, nseg, wsum);
     __syncthreads();
     for (int s = threadIdx.x; s < nseg; s += NT) {
-        ad[s] -= h[(size_t)s * n0];
+        const uint32_t first = h[(size_t)s * n0], cnt = h[(size_t)(s + 1) * n0] - first;
+        int32_t *sl = A.slots + (size_t)pt * 8 * A.gcap + ad[s];  // ad[s] is still the segment's padded base here
+        for (uint32_t i = cnt; i < ((cnt + 7u) & ~7u); ++i) sl[i] = -1;
+        ad[s] -= first;
         adg[s] = ad[s];
     }
     if (threadIdx.x == 0) {
@@ -982,10 +986,8 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     if (a.n_per_point <= 0 || a.n_points <= 0) return cudaSuccess;
     const long long n_total = a.n_per_point * a.n_points;
     const int nseg = sp.n1 * sp.n2;
-    // histogram + claim counters of the streaming kernel (right behind the histograms), then the slot table
+    // histogram + claim counters of the streaming kernel (right behind the histograms)
     cudaError_t e = cudaMemsetAsync(sc.hist, 0, ((size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES) * sizeof(uint32_t), st);
-    if (e != cudaSuccess) return e;
-    e = cudaMemsetAsync(ss.slots, 0xFF, (size_t)a.n_points * ss.slot_cap * sizeof(int32_t), st);
     if (e != cudaSuccess) return e;
     // window starts + histogram on the caller's stream; a single point's scan runs in the index kernel's last block
     IleScanArgs sa;
@@ -996,6 +998,7 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     sa.ngr = reinterpret_cast<uint32_t *>(ss.gcum) + a.n_points + 1;
     sa.gcum = ss.gcum;
     sa.gorder = ss.gorder;
+    sa.slots = ss.slots;
     sa.gcap = ss.slot_cap / 8;
     size_t scan_smem = (((size_t)sp.ncell + 1 + nseg + 3) & ~(size_t)3) * sizeof(uint32_t);
     {
