@@ -79,7 +79,7 @@ def detector_arrays(dets):
 
 
 def make_point(seed: int, dets, modes, n_q: int, snr: float, *, fs_hz: float = FS_HZ,
-               admix: float = 0.0, truth_response=None, noise: bool = True):
+               admix: float = 0.0, truth_response=None, noise: bool = True, spectra: bool = False):
     """One intrinsic point: Q [K][M][n_q], U [K][M][M], V [K][M][M] (complex128, C order) + metadata.
 
     Frequency-domain recipe.  With the whitened mode spectra
@@ -145,15 +145,20 @@ def make_point(seed: int, dets, modes, n_q: int, snr: float, *, fs_hz: float = F
     Q = np.empty((K, M, n_q), dtype=np.complex128)
     U = np.empty((K, M, M), dtype=np.complex128)
     V = np.empty((K, M, M), dtype=np.complex128)
+    D = np.empty((K, n_q), dtype=np.complex128)
     for k in range(K):
         d = signal(X[k], k)
         if noise:
             d = d + np.fft.fft(rng.standard_normal(n_q)) / np.sqrt(n_q)
+        D[k] = d
         U[k] = X[k].conj().T @ X[k]
         V[k] = X[k].T @ X[k][neg]
         spec = np.conj(X[k]) * (d * np.exp(2j * np.pi * f * t0_q_s))[:, None]       # [n_q][M]
         Q[k] = (np.fft.ifft(spec, axis=0) * n_q).T
     meta = dict(seed=seed, snr=float(snr), t0_q_s=t0_q_s, fs_hz=fs_hz, truth=dict(y=y, resp=resp, tau_samples=tau, a0=a0))
+    if spectra:  # inputs of the overlap pre-computation (eq. 8): whitened mode spectra [K][M][n_q] and data [K][n_q], FFT order
+        meta["x"] = np.ascontiguousarray(np.transpose(X, (0, 2, 1)))
+        meta["d"] = np.ascontiguousarray(D)
     return np.ascontiguousarray(Q), np.ascontiguousarray(U), np.ascontiguousarray(V), meta
 
 
