@@ -116,6 +116,17 @@ int ile_evidence_reset(ile_ctx *ctx, int32_t n_segments, double *state, void *cu
 int ile_evidence_merge(ile_ctx *ctx, int32_t n_segments, int32_t n_states, const double *states_in, double *state_out,
                        double *lnZ, double *n_eff, void *cuda_stream);
 
+/* Overlap pre-computation of n_points intrinsic points (eq. 8a-c: Q_{k,lm}(t) = <h_lm|d_k>(t), U_k = <h_lm|h_l'm'>,
+ * V_k = <h_lm^*|h_l'm'>) -- what ile_create takes as input, made on the GPU.  Discrete two-sided setting: n_q samples at
+ * fs_hz, FFT-order frequency grid f_n = n' fs_hz / n_q (n' the signed index), whitened spectra, <a|b> = sum_n conj(a[n]) b[n]:
+ *   Q[p][k][m][i] = sum_n conj(x[p][k][m][n]) d[p][k][n] exp(+2 pi i f_n (t0_q_s + i / fs_hz))   (one inverse FFT per series)
+ *   U[p][k][a][b] = sum_n conj(x[p][k][a][n]) x[p][k][b][n],   V[p][k][a][b] = sum_n x[p][k][a][(-n) mod n_q] x[p][k][b][n]
+ * x: device complex128 [P][K][M][n_q]; d: device complex128 [P][K][n_q]; Q, U, V: device outputs, caller-owned, shapes as
+ * ile_create reads them.  n_q must be a power of two, 2..8192 (else ILE_ERR_UNSUPPORTED).  Asynchronous on cuda_stream;
+ * needs no context. */
+int ile_precompute(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_q, double fs_hz, double t0_q_s, const void *x,
+                   const void *d, void *Q, void *U, void *V, void *cuda_stream);
+
 /* Whole hot path from HOST buffers, for callers that keep samples on the host (the paper's workflow, L97: blocks
  * generated on the CPU and transferred to the board): H2D copy of the seven sample arrays (+ log_w), ile_eval,
  * ile_evidence, D2H of lnL_margT (if not NULL), lnZ and n_eff.  Host arrays of n doubles each; pinned memory makes

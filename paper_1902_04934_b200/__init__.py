@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libile_b200.so")
 _lib = None
 
 SAMPLE_FIELDS = ("ra", "dec", "t_ref", "phi_ref", "psi", "incl", "dist_mpc")
-EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_evidence_merge", "ile_run_host", "ile_status",
+EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_evidence_merge", "ile_precompute", "ile_run_host", "ile_status",
            "ile_set_variant", "ile_launch_count", "ile_measure_fp64_peak", "ile_destroy", "ile_strerror")
 
 
@@ -57,6 +57,7 @@ def load():
     L.ile_evidence.argtypes = [vp, i32, i64, vp, vp, vp, vp, vp, vp]
     L.ile_evidence_reset.argtypes = [vp, i32, vp, vp]
     L.ile_evidence_merge.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
+    L.ile_precompute.argtypes = [i32, i32, i32, i32, ctypes.c_double, ctypes.c_double, vp, vp, vp, vp, vp, vp]
     L.ile_run_host.argtypes = [vp, i32, i64] + [vp] * 7 + [vp, vp, dp, dp, vp]
     L.ile_status.argtypes = [vp, ctypes.POINTER(i64), ctypes.c_int, vp]
     L.ile_set_variant.argtypes = [vp, i32]
@@ -236,6 +237,22 @@ class Context:
         if code not in (0, -5):
             raise IleError(code, "ile_status")
         return int(v.value), code
+
+
+def precompute(x, d, fs_hz: float, t0_q_s: float, stream=None):
+    """ile_precompute: whitened mode spectra x [P][K][M][N] and data spectra d [P][K][N] (CUDA complex128, FFT order)
+    -> (Q [P][K][M][N], U [P][K][M][M], V [P][K][M][M]) CUDA complex128 tensors, the inputs of ile_create (eq. 8a-c)."""
+    import torch
+
+    assert x.is_cuda and d.is_cuda and x.dtype == torch.complex128 and d.dtype == torch.complex128
+    assert x.is_contiguous() and d.is_contiguous() and x.dim() == 4 and d.dim() == 3 and tuple(d.shape) == (x.shape[0], x.shape[1], x.shape[3])
+    P, K, M, N = (int(v) for v in x.shape)
+    Q = torch.empty((P, K, M, N), dtype=torch.complex128, device=x.device)
+    U = torch.empty((P, K, M, M), dtype=torch.complex128, device=x.device)
+    V = torch.empty((P, K, M, M), dtype=torch.complex128, device=x.device)
+    _check(load().ile_precompute(P, K, M, N, float(fs_hz), float(t0_q_s), _ptr(x), _ptr(d), _ptr(Q), _ptr(U), _ptr(V),
+                                 _stream_ptr(stream)), "ile_precompute")
+    return Q, U, V
 
 
 def gather_evidence_states(state, group=None):

@@ -137,6 +137,10 @@ void ile_quad_pack_host(int32_t n_points, int32_t K, int32_t M, const double2 *U
 cudaError_t ile_launch_quad_mma(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const double *mats, double *qform,
                                 cudaStream_t st);
 
+// overlap pre-computation (ile_precompute.cu)
+cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_t N, double fs_hz, double t0_q_s, const double2 *x,
+                                  const double2 *d, double2 *Q, double2 *U, double2 *V, int32_t max_smem_optin, cudaStream_t st);
+
 // evidence: two kernels (per-block partials, then per-segment combine with the carried state)
 cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const double *lnL, const double *log_w,
                                 double *state, double *lnZ, double *n_eff, double *partials, int32_t blocks_per_seg,
