@@ -153,6 +153,63 @@ def run_reference(args, rank: int):
     print(json.dumps(line), flush=True)
 
 
+def run_precompute(args, rank: int):
+    """SURVEY.md §8(f) NEXT-1, single GPU: ile_precompute over --points intrinsic points of --config's shape per step.
+    HBM-bound by construction (every spectrum is read once, every Q written once); roofline against MEASURED_PEAKS.json."""
+    if rank != 0:
+        return
+    import numpy as np
+    import torch
+
+    import ile_inputs as gi
+    import paper_1902_04934_b200 as ile
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    ile.load()
+    c = gi.CONFIGS[args.config]
+    P = max(1, args.points)
+    snr = c["snr"] if not isinstance(c["snr"], tuple) else 20.0
+    _, _, _, meta = gi.make_point(gi.point_seed(args.config, 0), c["dets"], c["modes"], c["n_q"], snr, admix=c["admix"], spectra=True)
+    rng = np.random.Generator(np.random.PCG64(4934))
+    x = torch.from_numpy(np.ascontiguousarray(np.broadcast_to(meta["x"], (P,) + meta["x"].shape))).cuda()
+    d = torch.from_numpy(np.ascontiguousarray(np.broadcast_to(meta["d"], (P,) + meta["d"].shape))).cuda()
+    x = x * torch.from_numpy(1.0 + 0.01 * rng.standard_normal(P)).cuda().view(P, 1, 1, 1)  # P different points of one shape
+    K, M, N = x.shape[1:]
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    for _ in range(max(args.warmup, 3)):
+        ile.precompute(x, d, meta["fs_hz"], meta["t0_q_s"])
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    sampler = ClockSampler(0)
+    sampler.start()
+    for i in range(args.steps):
+        flush.fill_(i & 1)
+        ev[i][0].record()
+        ile.precompute(x, d, meta["fs_hz"], meta["t0_q_s"])
+        ev[i][1].record()
+    torch.cuda.synchronize()
+    sampler.stop_flag = True
+    ms = sum(a.elapsed_time(b) for a, b in ev) / args.steps
+    nbytes = 16 * P * K * (2 * M * N + N + 2 * M * M)  # x in, d in, Q out, U and V out
+    peak = None
+    try:
+        peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+        src = "MEASURED_PEAKS.json hbm_gbs"
+    except Exception:
+        peak, src = 6550.0, "B200_PROFILING.md fallback"
+    ach = nbytes / (ms * 1e-3) * 1e-9
+    line = {"metric": "overlap pre-computation (eq. 8: Q, U, V) intrinsic points/sec", "value": P / (ms * 1e-3), "unit": "points/s",
+            "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "c128", "data": "synthetic",
+            "config": {"workload": f"ile_precompute: {P} intrinsic point(s) of BASELINE.json configs[{args.config}]'s shape "
+                                   f"({K} detectors, {M} modes, {N}-point spectra)", "l2": "flushed between timed steps (256 MiB write)"},
+            "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
+                         "kernel": "ile_overlap_tables_kernel + ile_overlap_q_kernel + ile_overlap_uv_kernel", "peak_source": src, "algorithmic_bytes": nbytes},
+            "gpu_launches": 3 * args.steps, "clocks": sampler.summary()}
+    print(json.dumps(line), flush=True)
+
+
 def workload_config(cfg, n, args, extra=None):
     c = {"workload": f"BASELINE.json configs[{cfg['config_id']}]: {cfg['n_det']} detectors ({','.join(cfg['dets'])}), "
                      f"{cfg['n_modes']} modes (l<= {int(max(cfg['l']))}), Q {cfg['n_q']} complex128 @ {int(cfg['fs_hz'])} Hz, "
@@ -179,6 +236,8 @@ def main():
     ap.add_argument("--samples", default="prior", choices=["prior", "concentrated"])
     ap.add_argument("--ref-samples-per-step", type=int, default=100_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--stage", default="hotpath", choices=["hotpath", "precompute"],
+                    help="precompute: time ile_precompute (eq. 8: Q, U, V of --points intrinsic points) instead of the hot path")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -189,6 +248,9 @@ def main():
         if args.steps > 20:
             args.steps = 20
         run_reference(args, rank)
+        return
+    if args.stage == "precompute":
+        run_precompute(args, rank)
         return
 
     import numpy as np

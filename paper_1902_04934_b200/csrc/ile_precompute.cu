@@ -7,19 +7,126 @@
 // "After the port it is what dominates for BNS" (L97, L175): one inverse FFT per (point, detector, mode) and M^2 dot
 // products per (point, detector).
 //
-//   ile_overlap_q_kernel   one block per series: spectrum product and the start-time phase on load (bit-reversed into shared
-//                          memory), in-place radix-2 decimation-in-time butterflies with a twiddle table in shared memory,
-//                          natural-order store.  N a power of two, 2 <= N <= 8192 (16 N + 8 N bytes of shared memory).
-//   ile_overlap_uv_kernel  one block per (a, b, detector, point): both sums in one pass over n, warp-shuffle then block-level
-//                          reduction.
+//   ile_overlap_tables_kernel      twiddles exp(2 pi i j / N) and start-time phases exp(2 pi i f_n t0_Q), once per (N, t0_Q)
+//   ile_overlap_q_stockham_kernel  N <= 4096, one block per series: spectrum product and start-time phase on load, Stockham
+//                                  autosort radix-4 passes (+ one radix-2) between two shared-memory buffers, natural order in
+//                                  and out; elements per thread known at compile time
+//   ile_overlap_q_kernel           N = 8192: in-place radix-2 with a bit-reversed load (one buffer fits shared memory)
+//   ile_overlap_uv_kernel          one block per (detector, point): the M series staged through shared memory chunk by chunk
+//                                  with the mirrored chunk; every pair (a, b) summed by one warp
 #include "ile_kernels.h"
 
 #define PC_THREADS 256
 
 __device__ __forceinline__ double2 pc_cmul(double2 a, double2 b) { return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x); }
 
+// tab[0 .. N/2) = twiddles exp(+2 pi i j / N); tab[N/2 .. N/2 + N) = start-time phases exp(2 pi i f_n t0_Q), f_n = n' f_s / N
+// (the same for every series of the call: computed once instead of 1.5 sincospi per point and series)
+__global__ void __launch_bounds__(PC_THREADS) ile_overlap_tables_kernel(int32_t N, double fs_t0_over_n, double2 *__restrict__ tab)
+{
+    const int j = blockIdx.x * blockDim.x + threadIdx.x;
+    double s, c;
+    if (j < N / 2) {
+        sincospi(2.0 * (double)j / (double)N, &s, &c);
+        tab[j] = make_double2(c, s);
+    }
+    if (j < N) {
+        const int np = j < (N + 1) / 2 ? j : j - N;  // signed index
+        sincospi(2.0 * (double)np * fs_t0_over_n, &s, &c);
+        tab[N / 2 + j] = make_double2(c, s);
+    }
+}
+
+// W_N^m = exp(+2 pi i m / N) for 0 <= m < N from the half-length table
+__device__ __forceinline__ double2 pc_tw(const double2 *__restrict__ tab, int N, int m)
+{
+    const bool hi = m >= N / 2;
+    const double2 w = __ldg(tab + (hi ? m - N / 2 : m));
+    return hi ? make_double2(-w.x, -w.y) : w;
+}
+
+// Stockham autosort form (N <= 4096): natural order in and out through two ping-pong buffers, no bit reversal.  Stage with
+// completed sub-transforms of length ns: u = in[j], v = W^(k N / 2ns) in[j + N/2], k = j mod ns;
+// out[(j - k) 2 + k] = u + v, out[... + ns] = u - v.  EPT = N / PC_THREADS elements per thread, compile-time, so that the
+// global loads of a thread are all in flight at once and the butterflies of a stage are independent instruction streams
+// (EPT = 0: any N < 2 PC_THREADS, plain loops).  Twiddles come from the table through L1.
+template <int EPT>
 __global__ void __launch_bounds__(PC_THREADS)
-    ile_overlap_q_kernel(int32_t M, int32_t N, int32_t log2n, double fs_t0_over_n, const double2 *__restrict__ x,
+    ile_overlap_q_stockham_kernel(int32_t M, int32_t N, int32_t log2n, const double2 *__restrict__ tab, const double2 *__restrict__ x,
+                                  const double2 *__restrict__ d, double2 *__restrict__ Q)
+{
+    extern __shared__ double2 pc_sm[];
+    double2 *in = pc_sm, *out = pc_sm + N;
+    const size_t series = blockIdx.x;  // (point * K + k) * M + mode
+    const double2 *xs = x + series * N;
+    const double2 *ds = d + (series / M) * N;
+    if (EPT > 0) {
+        double2 xv[EPT > 0 ? EPT : 1], dv[EPT > 0 ? EPT : 1], pv[EPT > 0 ? EPT : 1];
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            const int n = e * PC_THREADS + threadIdx.x;
+            xv[e] = __ldcs(xs + n), dv[e] = __ldg(ds + n), pv[e] = __ldg(tab + N / 2 + n);
+        }
+#pragma unroll
+        for (int e = 0; e < EPT; ++e) {
+            const double2 w = pc_cmul(dv[e], pv[e]);
+            in[e * PC_THREADS + threadIdx.x] = make_double2(xv[e].x * w.x + xv[e].y * w.y, xv[e].x * w.y - xv[e].y * w.x);  // conj(x) d
+        }
+    } else {
+        for (int n = threadIdx.x; n < N; n += PC_THREADS) {
+            const double2 xv = xs[n], w = pc_cmul(ds[n], tab[N / 2 + n]);
+            in[n] = make_double2(xv.x * w.x + xv.y * w.y, xv.x * w.y - xv.y * w.x);
+        }
+    }
+    __syncthreads();
+    // radix-4 passes (each element goes through shared memory once per pass: the transform is bound by the 16-byte shared
+    // accesses, 4 wavefronts per warp instruction), then one radix-2 pass when log2 N is odd
+    const int T4 = N >> 2;
+    int ns = 1;
+    for (; ns * 4 <= N; ns <<= 2) {
+        const int tws = N / (4 * ns);  // W_N^(r k tws) = exp(2 pi i r k / (4 ns))
+        auto pass4 = [&](int j) {
+            const int k = j & (ns - 1), j0 = ((j - k) << 2) + k;
+            double2 u0 = in[j], u1 = in[j + T4], u2 = in[j + 2 * T4], u3 = in[j + 3 * T4];
+            if (ns > 1) {
+                u1 = pc_cmul(pc_tw(tab, N, k * tws), u1);
+                u2 = pc_cmul(pc_tw(tab, N, 2 * k * tws), u2);
+                u3 = pc_cmul(pc_tw(tab, N, 3 * k * tws), u3);
+            }
+            const double2 v0 = make_double2(u0.x + u2.x, u0.y + u2.y), v1 = make_double2(u0.x - u2.x, u0.y - u2.y);
+            const double2 v2 = make_double2(u1.x + u3.x, u1.y + u3.y);
+            const double2 v3 = make_double2(-(u1.y - u3.y), u1.x - u3.x);  // (u1 - u3) * (+i): inverse transform
+            out[j0] = make_double2(v0.x + v2.x, v0.y + v2.y);
+            out[j0 + ns] = make_double2(v1.x + v3.x, v1.y + v3.y);
+            out[j0 + 2 * ns] = make_double2(v0.x - v2.x, v0.y - v2.y);
+            out[j0 + 3 * ns] = make_double2(v1.x - v3.x, v1.y - v3.y);
+        };
+        if (EPT >= 4) {
+#pragma unroll
+            for (int e = 0; e < EPT / 4; ++e) pass4(e * PC_THREADS + threadIdx.x);
+        } else {
+            for (int j = threadIdx.x; j < T4; j += PC_THREADS) pass4(j);
+        }
+        __syncthreads();
+        double2 *t = in;
+        in = out, out = t;
+    }
+    if (ns < N) {  // ns = N / 2
+        for (int j = threadIdx.x; j < N / 2; j += PC_THREADS) {
+            const double2 u = in[j], v = pc_cmul(__ldg(tab + j), in[j + N / 2]);  // k = j, W_N^k
+            out[j] = make_double2(u.x + v.x, u.y + v.y);
+            out[j + ns] = make_double2(u.x - v.x, u.y - v.y);
+        }
+        __syncthreads();
+        double2 *t = in;
+        in = out, out = t;
+    }
+    double2 *q = Q + series * N;
+    for (int i = threadIdx.x; i < N; i += PC_THREADS) __stcs(q + i, in[i]);
+}
+
+__global__ void __launch_bounds__(PC_THREADS)
+    ile_overlap_q_kernel(int32_t M, int32_t N, int32_t log2n, const double2 *__restrict__ tab, const double2 *__restrict__ x,
                          const double2 *__restrict__ d, double2 *__restrict__ Q)
 {
     extern __shared__ double2 pc_sm[];
@@ -28,16 +135,9 @@ __global__ void __launch_bounds__(PC_THREADS)
     const size_t series = blockIdx.x;             // (point * K + k) * M + mode
     const double2 *xs = x + series * N;
     const double2 *ds = d + (series / M) * N;
-    for (int j = threadIdx.x; j < N / 2; j += PC_THREADS) {
-        double s, c;
-        sincospi(2.0 * (double)j / (double)N, &s, &c);
-        W[j] = make_double2(c, s);
-    }
+    for (int j = threadIdx.x; j < N / 2; j += PC_THREADS) W[j] = tab[j];
     for (int n = threadIdx.x; n < N; n += PC_THREADS) {
-        const int np = n < (N + 1) / 2 ? n : n - N;  // signed index
-        double s, c;
-        sincospi(2.0 * (double)np * fs_t0_over_n, &s, &c);  // exp(2 pi i f_n t0_Q), f_n = n' f_s / N
-        const double2 xv = xs[n], dv = pc_cmul(ds[n], make_double2(c, s));
+        const double2 xv = __ldcs(xs + n), dv = pc_cmul(ds[n], tab[N / 2 + n]);
         const double2 v = make_double2(xv.x * dv.x + xv.y * dv.y, xv.x * dv.y - xv.y * dv.x);  // conj(x) d
         a[__brev((unsigned)n) >> (32 - log2n)] = v;
     }
@@ -53,38 +153,59 @@ __global__ void __launch_bounds__(PC_THREADS)
         __syncthreads();
     }
     double2 *q = Q + series * N;
-    for (int i = threadIdx.x; i < N; i += PC_THREADS) q[i] = a[i];
+    for (int i = threadIdx.x; i < N; i += PC_THREADS) __stcs(q + i, a[i]);
 }
 
+// One block per (point, detector).  The M series are staged through shared memory in chunks of C frequencies together with
+// the mirrored chunk (x_a[-n]); warp w owns the pairs (a, b) with index = w mod 8, its lanes walk the chunk, the chunk's
+// partial sums are reduced by shuffles and added to the pair's accumulator in shared memory.  x is read from HBM once.
 __global__ void __launch_bounds__(PC_THREADS)
-    ile_overlap_uv_kernel(int32_t M, int32_t N, const double2 *__restrict__ x, double2 *__restrict__ U, double2 *__restrict__ V)
+    ile_overlap_uv_kernel(int32_t M, int32_t N, int32_t C, const double2 *__restrict__ x, double2 *__restrict__ U, double2 *__restrict__ V)
 {
-    __shared__ double red[4][PC_THREADS / 32];
-    const int a = blockIdx.x / M, b = blockIdx.x % M;
-    const size_t pk = blockIdx.y;  // point * K + k
-    const double2 *xa = x + (pk * M + a) * N, *xb = x + (pk * M + b) * N;
-    double ur = 0.0, ui = 0.0, vr = 0.0, vi = 0.0;
-    for (int n = threadIdx.x; n < N; n += PC_THREADS) {
-        const double2 p = xa[n], m = xa[(N - n) & (N - 1)], q = xb[n];
-        ur += p.x * q.x + p.y * q.y;  // conj(x_a) x_b
-        ui += p.x * q.y - p.y * q.x;
-        vr += m.x * q.x - m.y * q.y;  // x_a(-f) x_b(f)
-        vi += m.x * q.y + m.y * q.x;
-    }
-    double v[4] = {ur, ui, vr, vi};
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    extern __shared__ double2 pc_sm[];
+    double2 *xs = pc_sm;                // [M][C]   x_a[c0 + i]
+    double2 *xr = pc_sm + (size_t)M * C;  // [M][C]   x_a[(N - c0 - i) mod N]
+    double *acc = reinterpret_cast<double *>(pc_sm + 2 * (size_t)M * C);  // [M*M][4]
+    const size_t pk = blockIdx.x;  // point * K + k
+    const double2 *xk = x + pk * M * N;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, npairs = M * M;
+    for (int i = threadIdx.x; i < 4 * npairs; i += PC_THREADS) acc[i] = 0.0;
+    for (int c0 = 0; c0 < N; c0 += C) {
+        __syncthreads();  // the previous chunk has been consumed (and acc is initialised)
+#pragma unroll 4
+        for (int e = threadIdx.x; e < M * C; e += PC_THREADS) {
+            const int a = e / C, i = e - a * C;
+            xs[e] = xk[(size_t)a * N + c0 + i];
+            xr[e] = xk[(size_t)a * N + ((N - c0 - i) & (N - 1))];
+        }
+        __syncthreads();
+        for (int pr = warp; pr < npairs; pr += PC_THREADS / 32) {
+            const int a = pr / M, b = pr - a * M;
+            double ur = 0.0, ui = 0.0, vr = 0.0, vi = 0.0;
+#pragma unroll 4
+            for (int i = lane; i < C; i += 32) {
+                const double2 p = xs[a * C + i], m = xr[a * C + i], q = xs[b * C + i];
+                ur += p.x * q.x + p.y * q.y;  // conj(x_a) x_b
+                ui += p.x * q.y - p.y * q.x;
+                vr += m.x * q.x - m.y * q.y;  // x_a(-f) x_b(f)
+                vi += m.x * q.y + m.y * q.x;
+            }
 #pragma unroll
-    for (int c = 0; c < 4; ++c) {
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) v[c] += __shfl_xor_sync(0xffffffffu, v[c], o);
-        if (lane == 0) red[c][warp] = v[c];
+            for (int o = 16; o > 0; o >>= 1) {
+                ur += __shfl_xor_sync(0xffffffffu, ur, o);
+                ui += __shfl_xor_sync(0xffffffffu, ui, o);
+                vr += __shfl_xor_sync(0xffffffffu, vr, o);
+                vi += __shfl_xor_sync(0xffffffffu, vi, o);
+            }
+            if (lane == 0) {  // the pair belongs to this warp alone
+                acc[4 * pr + 0] += ur, acc[4 * pr + 1] += ui, acc[4 * pr + 2] += vr, acc[4 * pr + 3] += vi;
+            }
+        }
     }
     __syncthreads();
-    if (threadIdx.x < 4) {
-        double s = 0.0;
-        for (int w = 0; w < PC_THREADS / 32; ++w) s += red[threadIdx.x][w];
-        double *out = reinterpret_cast<double *>((threadIdx.x < 2 ? U : V) + (pk * M + a) * M + b);
-        out[threadIdx.x & 1] = s;
+    for (int pr = threadIdx.x; pr < npairs; pr += PC_THREADS) {
+        U[pk * npairs + pr] = make_double2(acc[4 * pr + 0], acc[4 * pr + 1]);
+        V[pk * npairs + pr] = make_double2(acc[4 * pr + 2], acc[4 * pr + 3]);
     }
 }
 
@@ -94,12 +215,51 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
     int log2n = 0;
     while ((1 << log2n) < N) ++log2n;
     if ((1 << log2n) != N || N < 2 || N > 8192) return cudaErrorInvalidValue;
-    const size_t smem = (size_t)N * 16 + (size_t)(N / 2) * 16;
+    const bool stockham = N <= 4096;
+    const size_t smem = stockham ? (size_t)2 * N * 16 : (size_t)N * 16 + (size_t)(N / 2) * 16;
     if (smem > (size_t)max_smem_optin) return cudaErrorInvalidValue;
-    cudaError_t e = cudaFuncSetAttribute(ile_overlap_q_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    auto stock = [&](auto kern, unsigned grid, const double2 *tab) {
+        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        kern<<<grid, PC_THREADS, smem, st>>>(M, N, log2n, tab, x, d, Q);
+        return cudaSuccess;
+    };
+    cudaError_t e = cudaSuccess;
+    if (!stockham) e = cudaFuncSetAttribute(ile_overlap_q_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    ile_overlap_q_kernel<<<(unsigned)((size_t)n_points * K * M), PC_THREADS, smem, st>>>(M, N, log2n, fs_hz * t0_q_s / (double)N, x, d, Q);
-    dim3 grid((unsigned)(M * M), (unsigned)(n_points * K));
-    ile_overlap_uv_kernel<<<grid, PC_THREADS, 0, st>>>(M, N, x, U, V);
+    // chunk of the U, V kernel: 2 M C staged values + the accumulators must fit one block's shared memory
+    int C = N < 256 ? N : 256;
+    while (C > 32 && (size_t)2 * M * C * 16 + (size_t)M * M * 32 > (size_t)max_smem_optin - 1024) C >>= 1;
+    const size_t smem_uv = (size_t)2 * M * C * 16 + (size_t)M * M * 32;
+    e = cudaFuncSetAttribute(ile_overlap_uv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_uv);
+    if (e != cudaSuccess) return e;
+    // twiddles and start-time phases: one table per device, recomputed (in stream order) when the grid or the start time
+    // changes.  Calls for DIFFERENT (n_q, fs t0) must not run concurrently on two streams of one device.
+    static double2 *g_tab[64] = {nullptr};
+    static int g_tab_n[64] = {0};
+    static double g_tab_alpha[64] = {0.0};
+    int dev = 0;
+    e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    if (!g_tab[dev]) {
+        e = cudaMalloc(&g_tab[dev], (size_t)(4096 + 8192) * sizeof(double2));
+        if (e != cudaSuccess) return e;
+    }
+    double2 *tab = g_tab[dev];
+    const double alpha = fs_hz * t0_q_s / (double)N;
+    if (g_tab_n[dev] != N || g_tab_alpha[dev] != alpha) {
+        ile_overlap_tables_kernel<<<(N + PC_THREADS - 1) / PC_THREADS, PC_THREADS, 0, st>>>(N, alpha, tab);
+        g_tab_n[dev] = N, g_tab_alpha[dev] = alpha;
+    }
+    const unsigned n_series = (unsigned)((size_t)n_points * K * M);
+    if (!stockham) ile_overlap_q_kernel<<<n_series, PC_THREADS, smem, st>>>(M, N, log2n, tab, x, d, Q);
+    else if (N == 16 * PC_THREADS) e = stock(ile_overlap_q_stockham_kernel<16>, n_series, tab);
+    else if (N == 8 * PC_THREADS) e = stock(ile_overlap_q_stockham_kernel<8>, n_series, tab);
+    else if (N == 4 * PC_THREADS) e = stock(ile_overlap_q_stockham_kernel<4>, n_series, tab);
+    else if (N == 2 * PC_THREADS) e = stock(ile_overlap_q_stockham_kernel<2>, n_series, tab);
+    else e = stock(ile_overlap_q_stockham_kernel<0>, n_series, tab);
+    if (e != cudaSuccess) return e;
+    ile_overlap_uv_kernel<<<(unsigned)(n_points * K), PC_THREADS, smem_uv, st>>>(M, N, C, x, U, V);
     return cudaGetLastError();
 }
