@@ -12,8 +12,7 @@
 //                                  autosort radix-4 passes (+ one radix-2) between two shared-memory buffers, natural order in
 //                                  and out; elements per thread known at compile time
 //   ile_overlap_q_kernel           N = 8192: in-place radix-2 with a bit-reversed load (one buffer fits shared memory)
-//   ile_overlap_uv_kernel          one block per (detector, point): the M series staged through shared memory chunk by chunk
-//                                  with the mirrored chunk; every pair (a, b) summed by one warp
+//   ile_overlap_uv_kernel          one block per (detector, point): register-blocked tiles of pairs (a, b), lanes over frequencies
 #include "ile_kernels.h"
 
 #define PC_THREADS 256
@@ -156,51 +155,67 @@ __global__ void __launch_bounds__(PC_THREADS)
     for (int i = threadIdx.x; i < N; i += PC_THREADS) __stcs(q + i, a[i]);
 }
 
-// One block per (point, detector).  The M series are staged through shared memory in chunks of C frequencies together with
-// the mirrored chunk (x_a[-n]); warp w owns the pairs (a, b) with index = w mod 8, its lanes walk the chunk, the chunk's
-// partial sums are reduced by shuffles and added to the pair's accumulator in shared memory.  x is read from HBM once.
-__global__ void __launch_bounds__(PC_THREADS)
-    ile_overlap_uv_kernel(int32_t M, int32_t N, int32_t C, const double2 *__restrict__ x, double2 *__restrict__ U, double2 *__restrict__ V)
+// One block per (point, detector).  Work items = (tile of PC_TA rows a, tile of PC_TB columns b, slice of the frequency
+// axis), dealt to the warps round robin.  A lane takes one frequency at a time: x_a[n] and x_a[-n] of the tile's rows and
+// x_b[n] of its columns go to registers (coalesced 16-byte loads; the block's warps re-read the same 100-odd KB, which
+// L1 serves) and all PC_TA x PC_TB pairs are updated from registers -- 8 FMA per pair and frequency, 9 loads per 72 FMA.
+// The items' sums are reduced by shuffles and added to the pair's accumulator in shared memory.
+#define PC_TA 3
+#define PC_TB 3
+__global__ void __launch_bounds__(PC_THREADS, 2)
+    ile_overlap_uv_kernel(int32_t M, int32_t N, int32_t nsplit, const double2 *__restrict__ x, double2 *__restrict__ U, double2 *__restrict__ V)
 {
     extern __shared__ double2 pc_sm[];
-    double2 *xs = pc_sm;                // [M][C]   x_a[c0 + i]
-    double2 *xr = pc_sm + (size_t)M * C;  // [M][C]   x_a[(N - c0 - i) mod N]
-    double *acc = reinterpret_cast<double *>(pc_sm + 2 * (size_t)M * C);  // [M*M][4]
-    const size_t pk = blockIdx.x;  // point * K + k
+    double *acc = reinterpret_cast<double *>(pc_sm);  // [M*M][4]
+    const size_t pk = blockIdx.x;                     // point * K + k
     const double2 *xk = x + pk * M * N;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, npairs = M * M;
     for (int i = threadIdx.x; i < 4 * npairs; i += PC_THREADS) acc[i] = 0.0;
-    for (int c0 = 0; c0 < N; c0 += C) {
-        __syncthreads();  // the previous chunk has been consumed (and acc is initialised)
-#pragma unroll 4
-        for (int e = threadIdx.x; e < M * C; e += PC_THREADS) {
-            const int a = e / C, i = e - a * C;
-            xs[e] = xk[(size_t)a * N + c0 + i];
-            xr[e] = xk[(size_t)a * N + ((N - c0 - i) & (N - 1))];
-        }
-        __syncthreads();
-        for (int pr = warp; pr < npairs; pr += PC_THREADS / 32) {
-            const int a = pr / M, b = pr - a * M;
-            double ur = 0.0, ui = 0.0, vr = 0.0, vi = 0.0;
-#pragma unroll 4
-            for (int i = lane; i < C; i += 32) {
-                const double2 p = xs[a * C + i], m = xr[a * C + i], q = xs[b * C + i];
-                ur += p.x * q.x + p.y * q.y;  // conj(x_a) x_b
-                ui += p.x * q.y - p.y * q.x;
-                vr += m.x * q.x - m.y * q.y;  // x_a(-f) x_b(f)
-                vi += m.x * q.y + m.y * q.x;
+    __syncthreads();
+    const int ta = (M + PC_TA - 1) / PC_TA, tb = (M + PC_TB - 1) / PC_TB, items = ta * tb * nsplit;
+    const int slice = ((N + nsplit - 1) / nsplit + 31) & ~31;
+    for (int it = warp; it < items; it += PC_THREADS / 32) {
+        const int sp = it % nsplit, tile = it / nsplit, a0 = (tile / tb) * PC_TA, b0 = (tile % tb) * PC_TB;
+        const int lo = sp * slice, hi = min(lo + slice, N);
+        double su[PC_TA][PC_TB][4];
+#pragma unroll
+        for (int i = 0; i < PC_TA; ++i)
+#pragma unroll
+            for (int j = 0; j < PC_TB; ++j) su[i][j][0] = su[i][j][1] = su[i][j][2] = su[i][j][3] = 0.0;
+#pragma unroll 2
+        for (int n = lo + lane; n < hi; n += 32) {
+            const int nm = (N - n) & (N - 1);
+            double2 p[PC_TA], m[PC_TA], q[PC_TB];
+#pragma unroll
+            for (int i = 0; i < PC_TA; ++i) {
+                const int a = min(a0 + i, M - 1);  // rows past M repeat the last one; their sums are dropped
+                p[i] = __ldg(xk + (size_t)a * N + n);
+                m[i] = __ldg(xk + (size_t)a * N + nm);
             }
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                ur += __shfl_xor_sync(0xffffffffu, ur, o);
-                ui += __shfl_xor_sync(0xffffffffu, ui, o);
-                vr += __shfl_xor_sync(0xffffffffu, vr, o);
-                vi += __shfl_xor_sync(0xffffffffu, vi, o);
-            }
-            if (lane == 0) {  // the pair belongs to this warp alone
-                acc[4 * pr + 0] += ur, acc[4 * pr + 1] += ui, acc[4 * pr + 2] += vr, acc[4 * pr + 3] += vi;
-            }
+            for (int j = 0; j < PC_TB; ++j) q[j] = __ldg(xk + (size_t)min(b0 + j, M - 1) * N + n);
+#pragma unroll
+            for (int i = 0; i < PC_TA; ++i)
+#pragma unroll
+                for (int j = 0; j < PC_TB; ++j) {
+                    su[i][j][0] += p[i].x * q[j].x + p[i].y * q[j].y;  // conj(x_a) x_b
+                    su[i][j][1] += p[i].x * q[j].y - p[i].y * q[j].x;
+                    su[i][j][2] += m[i].x * q[j].x - m[i].y * q[j].y;  // x_a(-f) x_b(f)
+                    su[i][j][3] += m[i].x * q[j].y + m[i].y * q[j].x;
+                }
         }
+#pragma unroll
+        for (int i = 0; i < PC_TA; ++i)
+#pragma unroll
+            for (int j = 0; j < PC_TB; ++j) {
+#pragma unroll
+                for (int c = 0; c < 4; ++c) {
+                    double v = su[i][j][c];
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                    if (lane == 0 && a0 + i < M && b0 + j < M) atomicAdd(&acc[4 * ((a0 + i) * M + b0 + j) + c], v);
+                }
+            }
     }
     __syncthreads();
     for (int pr = threadIdx.x; pr < npairs; pr += PC_THREADS) {
@@ -227,12 +242,11 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
     cudaError_t e = cudaSuccess;
     if (!stockham) e = cudaFuncSetAttribute(ile_overlap_q_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    // chunk of the U, V kernel: 2 M C staged values + the accumulators must fit one block's shared memory
-    int C = N < 256 ? N : 256;
-    while (C > 32 && (size_t)2 * M * C * 16 + (size_t)M * M * 32 > (size_t)max_smem_optin - 1024) C >>= 1;
-    const size_t smem_uv = (size_t)2 * M * C * 16 + (size_t)M * M * 32;
-    e = cudaFuncSetAttribute(ile_overlap_uv_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_uv);
-    if (e != cudaSuccess) return e;
+    // U, V kernel: enough frequency slices that a block's 8 warps all have work items
+    const int tiles = ((M + PC_TA - 1) / PC_TA) * ((M + PC_TB - 1) / PC_TB);
+    int nsplit = (PC_THREADS / 32 + tiles - 1) / tiles;
+    while (nsplit > 1 && N / nsplit < 32) --nsplit;
+    const size_t smem_uv = (size_t)M * M * 32;
     // twiddles and start-time phases: one table per device, recomputed (in stream order) when the grid or the start time
     // changes.  Calls for DIFFERENT (n_q, fs t0) must not run concurrently on two streams of one device.
     static double2 *g_tab[64] = {nullptr};
@@ -260,6 +274,6 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
     else if (N == 2 * PC_THREADS) e = stock(ile_overlap_q_stockham_kernel<2>, n_series, tab);
     else e = stock(ile_overlap_q_stockham_kernel<0>, n_series, tab);
     if (e != cudaSuccess) return e;
-    ile_overlap_uv_kernel<<<(unsigned)(n_points * K), PC_THREADS, smem_uv, st>>>(M, N, C, x, U, V);
+    ile_overlap_uv_kernel<<<(unsigned)(n_points * K), PC_THREADS, smem_uv, st>>>(M, N, nsplit, x, U, V);
     return cudaGetLastError();
 }
