@@ -33,13 +33,16 @@ UNIT = "samples/s"
 # algorithmic work per sample in DFMA-equivalents
 # ------------------------------------------------------------------------------------------------------------------
 EXP_DFMA = 20.0      # "Total DFMA-equivalents with exp ~ 20" (subtract, range reduction, polynomial, accumulate)
+NOMINAL_FP64_TFLOPS = 37.2  # 148 SMs x 64 FP64 lanes x 2 flop x 1.965 GHz
 
 
-def dfma_per_sample(K: int, M: int, n_t: int) -> float:
-    """config 1 -> 12,300 + 720 + 8,200 + 400 = 21,620 DFMA-equivalents per sample."""
+def dfma_per_sample(K: int, M: int, n_t: int, exp_cost: float = EXP_DFMA) -> float:
+    """config 1 -> 12,300 + 720 + 8,200 + 400 = 21,620 DFMA-equivalents per sample.
+    `exp_cost` = FP64-pipe instructions per time bin of step 6: 20 is the survey's convention; the kernel's own count
+    (from the committed ncu SASS mix) gives the "measured exp" accounting of SURVEY.md §8(d)."""
     linear = 2.0 * K * M * n_t                      # step 5: Re sum conj(A) Q, 2 DFMA per complex element
     quad = 2.0 * K * (4.0 * M * M + 4.0 * M)        # step 4: Y^dagger U Y and Y^T V Y per detector
-    lse = n_t * EXP_DFMA                            # step 6
+    lse = n_t * exp_cost                            # step 6
     geom = 250.0 + 30.0 * M                         # steps 1-3: five sincos, F_k, dt_k, Y_lm, K*M coefficient products
     return linear + quad + lse + geom
 
@@ -108,15 +111,17 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "n_samples": len(s)}
 
 
-def read_traffic_bytes():
-    """DRAM bytes per launch of the dominant kernel (read + write) from the committed ncu --set full summary
-    (profiles/traffic.csv, last row), or None."""
-    p = os.path.join(ROOT, "profiles", "traffic.csv")
+def read_stream_counters():
+    """Counters of the dominant kernel (the streaming FP64-MMA kernel, config 1, one launch = 100,000 samples) from the
+    committed `ncu --set full` capture: profiles/stream_counters.csv, last row (its .md names the command).  Returns a
+    dict or None.  Columns: dram_bytes_read, dram_bytes_write, dmma_inst, fp64_other_inst (DFMA + DADD + DMUL warp
+    instructions), cycles_elapsed_max, pipe_fp64_pct (ncu sm__inst_executed_pipe_fp64 % of peak), samples, n_t."""
+    p = os.path.join(ROOT, "profiles", "stream_counters.csv")
     try:
         import csv
 
-        rows = [r for r in csv.DictReader(open(p))]
-        return int(rows[-1]["dram_bytes_read"]) + int(rows[-1]["dram_bytes_write"])
+        row = [r for r in csv.DictReader(open(p))][-1]
+        return {k: (v if k in ("capture", "kernel", "source") else float(v)) for k, v in row.items()}
     except Exception:
         return None
 
@@ -303,13 +308,7 @@ def main():
     def do_e2e():
         if P == 1:
             return ctx.run_host(host, None, out_host=host_out)
-        # several points: H2D of the [P][n] sample arrays, ile_eval_all + ile_evidence, D2H of lnL_margT, lnZ, n_eff
-        d = {k: dev[k].copy_(host[k], non_blocking=True) for k in host}
-        ctx.eval_all(d, want_idx=False, out=lnL.view(P, n))
-        z, ne = ctx.evidence(lnL, n_segments=P)
-        host_out.copy_(lnL, non_blocking=True)
-        zc, nc = z.cpu(), ne.cpu()
-        return host_out, zc, nc
+        return ctx.run_host_all(host, None, out_host=host_out)  # [P][n] arrays, one C-ABI call
 
     def step():
         do_eval()
@@ -321,7 +320,9 @@ def main():
         do_e2e()
     torch.cuda.synchronize()
 
-    peak_tflops, _ = ile.measure_fp64_peak(1 << 15)
+    peak_dfma, _ = ile.measure_fp64_peak(1 << 15)
+    peak_dmma, _ = ile.measure_dmma_peak(1 << 12)
+    peak_tflops = max(peak_dfma, peak_dmma)
 
     # ---- timed region: exactly K steps, device-timed with CUDA events on the launching stream
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
@@ -371,18 +372,35 @@ def main():
         value = world * P * n * args.steps / (step_ms * 1e-3)
         eval_avg_ms = eval_ms / args.steps
         achieved = 2.0 * w * P * n / (eval_avg_ms * 1e-3) * 1e-12
+        # the same with the exp cost the kernel really pays (FP64-pipe instructions per bin outside the contraction, from the
+        # committed ncu SASS mix) and the FP64 pipe's busy fraction in that capture (DMMA 16 cycles, DFMA/DADD/DMUL 2 cycles
+        # per warp instruction and SMSP): SURVEY.md §8(d) "model fraction" and "pipe fraction"
+        sc_ = read_stream_counters()
+        exp_meas = frac_meas = frac_pipe = None
+        if sc_:
+            exp_meas = sc_["fp64_other_inst"] * 32.0 / (sc_["samples"] * sc_["n_t"])
+            frac_meas = 2.0 * dfma_per_sample(K, M, n_t, exp_meas) * P * n / (eval_avg_ms * 1e-3) * 1e-12 / peak_tflops
+            frac_pipe = (16.0 * sc_["dmma_inst"] + 2.0 * sc_["fp64_other_inst"]) / (sc_["cycles_elapsed_max"] * 4.0 * 148.0)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": step_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": workload_config(base, n, args, extra={"variant": args.variant, "samples": args.samples}),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
-                         "traffic": read_traffic_bytes(), "kernel": "ile_eval (steps 1-6)", "kernel_ms": eval_avg_ms,
-                         "dfma_equiv_per_sample": w, "peak_source": "ile_measure_fp64_peak: register-resident DFMA chains, measured in this run "
-                         "(nominal 148 SM x 64 lanes x 2 x 1.965 GHz = 37.2 TFLOP/s)"},
+                         "traffic": int(sc_["dram_bytes_read"] + sc_["dram_bytes_write"]) if sc_ else None,
+                         "kernel": "ile_eval (steps 1-6)", "kernel_ms": eval_avg_ms, "dfma_equiv_per_sample": w,
+                         "peak_dfma": peak_dfma, "peak_dmma": peak_dmma, "peak_nominal": NOMINAL_FP64_TFLOPS,
+                         "frac_vs_nominal": achieved / NOMINAL_FP64_TFLOPS,
+                         "exp_fp64_inst_per_bin_measured": exp_meas, "frac_model_measured_exp": frac_meas,
+                         "frac_pipe": frac_pipe, "pipe_fp64_pct_ncu": sc_["pipe_fp64_pct"] if sc_ else None,
+                         "counters_capture": sc_["capture"] if sc_ else None,
+                         "peak_source": "max(ile_measure_fp64_peak: register-resident DFMA chains, ile_measure_dmma_peak: DMMA.8x8x4 chains), "
+                         "both measured in this run; frac counts exp at 20 DFMA-equivalents per bin (SURVEY.md 8(d)), "
+                         "frac_model_measured_exp at the kernel's own FP64 instruction count per bin, frac_pipe is the FP64 pipe's "
+                         "busy fraction in the committed ncu capture"},
             "e2e": {"value": world * P * n * args.steps / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 7 * 8 * P * n,
                     "d2h_bytes_per_step": 8 * P * n + 16 * P, "ms_per_step": e2e_ms / args.steps,
-                    "api": "ile_run_host (pinned host buffers)" if P == 1 else "pinned H2D + ile_eval_all + ile_evidence + D2H"},
+                    "api": "ile_run_host (pinned host buffers)" if P == 1 else "ile_run_host_all (pinned host buffers)"},
             "gpu_launches": int(launches), "clocks": sampler.summary(), "wall_ms_per_step": wall / args.steps * 1e3,
             "lnZ": float(lnZ[0].item()), "n_eff": float(neff[0].item()), "n_out_of_range": int(n_bad),
         }
@@ -404,8 +422,15 @@ def main():
                 rZ, _ = oracle.evidence(ref)
                 passes += 1
             dt = time.perf_counter() - t0
+            n_one = min(n_cpu, 20_000)  # single thread: a smaller bounded sample of the same batch
+            sub1 = {k: v[:n_one] for k, v in s_np.items()}
+            t1 = time.perf_counter()
+            ref1, _, _ = oracle.eval_batch(pb, sub1, n_threads=1)
+            oracle.evidence(ref1)
+            dt1 = time.perf_counter() - t1
             line["cpu_baseline"] = {"value": n_cpu * passes / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                     "sample": f"{passes} passes over the first {n_cpu} samples of the same batch (eval + evidence), OpenMP over samples",
+                                    "value_1thread": n_one / dt1, "sample_1thread": f"one pass over the first {n_one} samples, 1 thread",
                                     "lnZ_oracle": rZ if n_cpu == n else None}
         print(json.dumps(line), flush=True)
     ctx.close()

@@ -1,14 +1,23 @@
 """Seeded synthetic inputs for the ILE hot path.
 
 This module is the ONLY code shared by the CPU oracle (`oracle/`) and the CUDA path
-(`paper_1902_04934_b200/`).  It holds none of the method's arithmetic: no antenna
+(`paper_1902_04934_b200/`).  It holds none of the hot path's arithmetic: no antenna
 pattern, no arrival-time delay, no spherical harmonic, no likelihood, no log-sum-exp.
-It only manufactures the *inputs* of the hot path -- the mode overlap time series
+It manufactures the *inputs* of the hot path -- the mode overlap time series
 Q_{k,lm}(t), the mode-mode matrices U_k, V_k (eq. 8a-c), the
 detector constants and the extrinsic sample arrays -- with the
 shapes, sizes and value distributions of the paper's workloads
 and of BASELINE.json's five configs.  The paper's own inputs come from lalsuite
 waveforms and LIGO PSDs, neither of which exists here; these stand in for them.
+
+Since the overlap pre-computation itself became a product entry (`ile_precompute`,
+SURVEY.md §8(f) NEXT-1), note what that means here: `make_point` builds Q, U, V from
+the whitened spectra with numpy (matrix products and one inverse FFT) because the hot
+path needs inputs whether or not NEXT-1 exists.  For NEXT-1 only the spectra
+(`spectra=True`: meta["x"], meta["d"]) are the shared inputs; the expected Q, U, V of
+its parity tests come from `oracle/precompute.py`, never from this module, and the
+test that compares this module's Q, U, V with the oracle's is a consistency check of
+the generator, not a pin of the oracle (its pins are in tests/test_oracle_precompute_pins.py).
 
 The "true signal" injected into the data is described by seeded random response
 numbers (one complex amplitude per detector, one complex weight per mode, one integer

@@ -25,6 +25,9 @@
  *  - Work is enqueued on the caller's CUDA stream (cudaStream_t passed as void*; NULL = default stream) and is
  *    asynchronous unless stated.  Errors detected on the device (a window leaving [0, N_Q)) write -inf for that
  *    sample, never read out of bounds, and bump a sticky counter readable with ile_status().
+ *  - A context belongs to the device that was current at ile_create (calls made with another current device return
+ *    ILE_ERR_BAD_ARGUMENT) and owns ONE set of scratch buffers: calls on one context must be issued in stream order
+ *    (one stream at a time, or ordered by events).  Independent streams take independent contexts.
  *  - One GPU.  There is no CPU fallback and no backend dispatch: without a CUDA device every call fails.
  */
 #ifndef ILE_H
@@ -137,13 +140,20 @@ int ile_run_host(ile_ctx *ctx, int32_t point, int64_t n, const double *ra, const
                  const double *log_w /* may be NULL */, double *lnL_margT /* host out, may be NULL */,
                  double *lnZ /* host out, 1 */, double *n_eff /* host out, 1, may be NULL */, void *cuda_stream);
 
+/* The same for every intrinsic point in one call (BASELINE.json config 4): host arrays are [P][n_per_point] (log_w may be
+ * NULL), lnL_margT host out [P][n_per_point] or NULL, lnZ / n_eff host out [P] (n_eff may be NULL).  One H2D per array,
+ * one ile_eval_all, one ile_evidence over the P segments, one D2H per result. */
+int ile_run_host_all(ile_ctx *ctx, int64_t n_per_point, const double *ra, const double *dec, const double *t_ref,
+                     const double *phi_ref, const double *psi, const double *incl, const double *dist_mpc,
+                     const double *log_w, double *lnL_margT, double *lnZ, double *n_eff, void *cuda_stream);
+
 /* Sticky device-side status: synchronises the stream, writes the number of samples whose window left [0, N_Q)
  * since the context was created (or since the last reset) and returns ILE_OK or ILE_ERR_OUT_OF_RANGE.
  * reset != 0 clears the counter. */
 int ile_status(ile_ctx *ctx, int64_t *n_out_of_range, int reset, void *cuda_stream);
 
-/* Select the evaluation kernel: 0 = automatic (default), 1 = reference-shaped direct kernel (any size),
- * 2.. = tuned variants.  Returns ILE_ERR_UNSUPPORTED if the variant cannot run this
+/* Select the evaluation kernel: 0 = automatic (default), 1 = reference-shaped direct kernel (any size), 2 = tiled
+ * Q-stationary DFMA kernel, 4 = sorted streaming FP64-MMA kernel (3 is retired).  Returns ILE_ERR_UNSUPPORTED if the variant cannot run this
  * context's sizes.  For tests and benchmarks; results are identical to within rounding. */
 int ile_set_variant(ile_ctx *ctx, int32_t variant);
 
@@ -154,6 +164,11 @@ int64_t ile_launch_count(const ile_ctx *ctx);
  * dependent steps of 8 independent chains per thread, full grid), in TFLOP/s (2 flops per FMA), and the kernel time
  * in ms.  The roofline denominator for this ALU-bound path.  Synchronous. */
 int ile_measure_fp64_peak(int32_t iters, double *tflops, double *ms);
+
+/* The same for the FP64 matrix instruction (mma.sync.m8n8k4.f64, 256 FMA per warp instruction, 8 independent chains per
+ * warp) -- the unit the streaming kernel's contraction runs on.  It shares the FP64 pipe with DFMA; bench.py takes the
+ * larger of the two measurements as the roofline denominator. */
+int ile_measure_dmma_peak(int32_t iters, double *tflops, double *ms);
 
 void ile_destroy(ile_ctx *ctx);
 

@@ -19,8 +19,8 @@ LIB_PATH = os.path.join(_HERE, "libile_b200.so")
 _lib = None
 
 SAMPLE_FIELDS = ("ra", "dec", "t_ref", "phi_ref", "psi", "incl", "dist_mpc")
-EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_evidence_merge", "ile_precompute", "ile_run_host", "ile_status",
-           "ile_set_variant", "ile_launch_count", "ile_measure_fp64_peak", "ile_destroy", "ile_strerror")
+EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_evidence_merge", "ile_precompute", "ile_run_host", "ile_run_host_all", "ile_status",
+           "ile_set_variant", "ile_launch_count", "ile_measure_fp64_peak", "ile_measure_dmma_peak", "ile_destroy", "ile_strerror")
 
 
 class IleError(RuntimeError):
@@ -59,11 +59,13 @@ def load():
     L.ile_evidence_merge.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
     L.ile_precompute.argtypes = [i32, i32, i32, i32, ctypes.c_double, ctypes.c_double, vp, vp, vp, vp, vp, vp]
     L.ile_run_host.argtypes = [vp, i32, i64] + [vp] * 7 + [vp, vp, dp, dp, vp]
+    L.ile_run_host_all.argtypes = [vp, i64] + [vp] * 7 + [vp, vp, dp, dp, vp]
     L.ile_status.argtypes = [vp, ctypes.POINTER(i64), ctypes.c_int, vp]
     L.ile_set_variant.argtypes = [vp, i32]
     L.ile_launch_count.argtypes = [vp]
     L.ile_launch_count.restype = i64
     L.ile_measure_fp64_peak.argtypes = [i32, dp, dp]
+    L.ile_measure_dmma_peak.argtypes = [i32, dp, dp]
     L.ile_destroy.argtypes = [vp]
     L.ile_destroy.restype = None
     L.ile_strerror.argtypes = [ctypes.c_int]
@@ -95,6 +97,13 @@ def measure_fp64_peak(iters: int = 1 << 16):
     """(TFLOP/s, ms) of register-resident DFMA chains on the current device (ile_measure_fp64_peak)."""
     tf, ms = ctypes.c_double(0.0), ctypes.c_double(0.0)
     _check(load().ile_measure_fp64_peak(int(iters), ctypes.byref(tf), ctypes.byref(ms)), "ile_measure_fp64_peak")
+    return tf.value, ms.value
+
+
+def measure_dmma_peak(iters: int = 1 << 13):
+    """(TFLOP/s, ms) of independent DMMA.8x8x4 chains on the current device (ile_measure_dmma_peak)."""
+    tf, ms = ctypes.c_double(0.0), ctypes.c_double(0.0)
+    _check(load().ile_measure_dmma_peak(int(iters), ctypes.byref(tf), ctypes.byref(ms)), "ile_measure_dmma_peak")
     return tf.value, ms.value
 
 
@@ -229,6 +238,27 @@ class Context:
         _check(load().ile_run_host(self._h, int(point), n, *[_ptr(t) for t in ts], _ptr(log_w_host), _ptr(out),
                                    ctypes.byref(lnZ), ctypes.byref(neff), _stream_ptr(stream)), "ile_run_host")
         return out, lnZ.value, neff.value
+
+    def run_host_all(self, samples_host, log_w_host=None, want_lnL: bool = True, out_host=None, stream=None):
+        """ile_run_host_all: HOST tensors [P][n_per_point] in, host results out: (lnL_margT host tensor [P][n] or None,
+        lnZ numpy [P], n_eff numpy [P])."""
+        import numpy as np
+        import torch
+
+        ts = [samples_host[f] for f in SAMPLE_FIELDS]
+        tot = ts[0].numel()
+        assert tot % self.n_points == 0
+        n = tot // self.n_points
+        for t in ts:
+            assert (not t.is_cuda) and t.dtype == torch.float64 and t.is_contiguous() and t.numel() == tot
+        out = None
+        if want_lnL:
+            out = out_host if out_host is not None else torch.empty((self.n_points, n), dtype=torch.float64).pin_memory()
+        lnZ, neff = np.zeros(self.n_points), np.zeros(self.n_points)
+        dp = ctypes.POINTER(ctypes.c_double)
+        _check(load().ile_run_host_all(self._h, n, *[_ptr(t) for t in ts], _ptr(log_w_host), _ptr(out), lnZ.ctypes.data_as(dp),
+                                       neff.ctypes.data_as(dp), _stream_ptr(stream)), "ile_run_host_all")
+        return out, lnZ, neff
 
     def status(self, reset: bool = False, stream=None):
         """ile_status: (n_out_of_range, code).  Synchronises the stream."""

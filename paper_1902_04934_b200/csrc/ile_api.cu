@@ -16,23 +16,20 @@ struct ile_ctx {
     unsigned long long *d_oob;
     double *d_partials;
     size_t partials_cap;  // doubles
-    size_t ev_tickets_at;  // offset (doubles) of the zeroed ticket words of the last evidence call's layout; 0 = none
+    unsigned int *d_tickets;  // one word per evidence segment; zero between calls (the kernel's last block resets its own)
+    size_t tickets_cap;
     double *d_stage;
     size_t stage_cap;  // doubles
     double *d_small;   // lnZ, n_eff (device)
     double *h_small;   // pinned mirror
     int32_t variant;
     long long launches;
-    // variant 3 (sorted FP64-MMA path)
-    bool mma_ok;
-    IleMmaPlan mp;
-    double *dQp;
+    // variant 4 (sorted, streaming FP64-MMA path)
     int64_t chunk_samples;  // samples per launch group (bounds the scratch: <= 2 GiB of records, <= 2^20 samples)
-    IleMmaScratch sc;
+    IleSortScratch sc;
     size_t sc_samples, sc_hist;  // capacities (samples, histogram words)
     int32_t sc_points;
     int32_t sc_recg;             // doubles per record the scratch was sized for
-    // variant 4 (streaming FP64-MMA path)
     bool stream_ok;
     IleStreamPlan spl;
     IleSortPlan ssp;
@@ -53,11 +50,21 @@ static int cuda_fail(cudaError_t e)
     snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error %d: %s", (int)e, cudaGetErrorString(e));
     return ILE_ERR_CUDA;
 }
+// Function attributes, streams and every buffer of a context belong to the device it was created on.
+static int check_device(const ile_ctx *c)
+{
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return ILE_ERR_NO_DEVICE;
+    return dev == c->device ? ILE_OK : ILE_ERR_BAD_ARGUMENT;
+}
 #ifndef ILE_CHUNK_BYTES
 #define ILE_CHUNK_BYTES (2048u << 20) /* record scratch per launch group: bigger groups sort into tighter windows and pay one pre-pass */
 #endif
 #ifndef ILE_QUAD_MMA_MIN_MODES
 #define ILE_QUAD_MMA_MIN_MODES 8
+#endif
+#ifndef ILE_STREAM_MIN_SAMPLES
+#define ILE_STREAM_MIN_SAMPLES 16384 /* automatic choice: batches per point from this size on take the streaming variant */
 #endif
 #ifndef ILE_CHUNK_MAX
 #define ILE_CHUNK_MAX 1048576
@@ -115,12 +122,14 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
         cudaGetLastError();
         return ILE_ERR_NO_DEVICE;
     }
+    int device = 0;
+    cudaDeviceProp prop;
+    CK(cudaGetDevice(&device));  // nothing is allocated yet: a failure here leaks nothing
+    CK(cudaGetDeviceProperties(&prop, device));
     ile_ctx *c = new (std::nothrow) ile_ctx();
     if (!c) return ILE_ERR_BAD_ARGUMENT;
     std::memset(c, 0, sizeof(*c));
-    CK(cudaGetDevice(&c->device));
-    cudaDeviceProp prop;
-    CK(cudaGetDeviceProperties(&prop, c->device));
+    c->device = device;
     c->sz.n_det = cfg->n_det;
     c->sz.n_modes = cfg->n_modes;
     c->sz.n_q = cfg->n_q;
@@ -169,26 +178,16 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     CKC(cudaMalloc(&c->dU, nU * sizeof(double2)));
     CKC(cudaMalloc(&c->dV, nU * sizeof(double2)));
     CKC(cudaMalloc(&c->d_oob, sizeof(unsigned long long)));
-    CKC(cudaMalloc(&c->d_small, 8 * sizeof(double)));
-    CKC(cudaMallocHost(&c->h_small, 8 * sizeof(double)));
+    CKC(cudaMalloc(&c->d_small, 2 * (size_t)cfg->n_points * sizeof(double)));  // lnZ[P], n_eff[P] of ile_run_host(_all)
+    CKC(cudaMallocHost(&c->h_small, 2 * (size_t)cfg->n_points * sizeof(double)));
     CKC(cudaMemcpy(c->dparams, &P, sizeof(P), cudaMemcpyHostToDevice));
     CKC(cudaMemcpy(c->dQ, Q, nQ * sizeof(double2), cudaMemcpyDefault));
     CKC(cudaMemcpy(c->dU, U, nU * sizeof(double2), cudaMemcpyDefault));
     CKC(cudaMemcpy(c->dV, V, nU * sizeof(double2), cudaMemcpyDefault));
     CKC(cudaMemset(c->d_oob, 0, sizeof(unsigned long long)));
-    c->mma_ok = ile_mma_plan(c->sz, &c->mp);
-    if (c->mma_ok) {
-        const size_t nQp = (size_t)cfg->n_points * cfg->n_det * c->mp.nblk_q * c->mp.ks * 32;
-        CKC(cudaMalloc(&c->dQp, nQp * sizeof(double)));
-        CKC(ile_launch_pack_q(c->sz, c->mp, cfg->n_points, c->dQ, c->dQp, 0));
-        CKC(cudaDeviceSynchronize());
-        int64_t cs = (int64_t)ILE_CHUNK_BYTES / ((int64_t)c->mp.recg * 8);
-        cs = cs < 16384 ? 16384 : cs > ILE_CHUNK_MAX ? ILE_CHUNK_MAX : cs;
-        c->chunk_samples = cs;
-    }
-    c->sc_recg = c->mma_ok ? c->mp.recg : 0;
     c->stream_ok = ile_stream_plan(c->sz, c->hparams, 0, &c->spl, &c->ssp);
     if (c->stream_ok) {
+        CKC(ile_stream_prepare(c->sz, &c->spl));
         if (cfg->n_modes >= ILE_QUAD_MMA_MIN_MODES) {
             const size_t nd = ile_quad_pack_doubles(cfg->n_points, cfg->n_det, cfg->n_modes);
             double *hm = new (std::nothrow) double[nd];
@@ -220,11 +219,9 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
         CKC(cudaMalloc(&c->dQs, nQs * sizeof(double)));
         CKC(ile_launch_pack_q_stream(c->sz, c->spl, cfg->n_points, c->dQ, c->dQs, 0));
         CKC(cudaDeviceSynchronize());
-        if (cfg->n_det * c->spl.cp > c->sc_recg) c->sc_recg = cfg->n_det * c->spl.cp;
-        if (!c->mma_ok) {
-            int64_t cs = (int64_t)ILE_CHUNK_BYTES / ((int64_t)c->sc_recg * 8);
-            c->chunk_samples = cs < 16384 ? 16384 : cs > ILE_CHUNK_MAX ? ILE_CHUNK_MAX : cs;
-        }
+        c->sc_recg = cfg->n_det * c->spl.cp;
+        const int64_t cs = (int64_t)ILE_CHUNK_BYTES / ((int64_t)c->sc_recg * 8);
+        c->chunk_samples = cs < 16384 ? 16384 : cs > ILE_CHUNK_MAX ? ILE_CHUNK_MAX : cs;
     }
 #undef CKC
     *out = c;
@@ -240,14 +237,13 @@ extern "C" void ile_destroy(ile_ctx *c)
     cudaFree(c->dV);
     cudaFree(c->d_oob);
     cudaFree(c->d_partials);
+    cudaFree(c->d_tickets);
     cudaFree(c->d_stage);
     cudaFree(c->d_small);
-    cudaFree(c->dQp);
     cudaFree(c->sc.rec);
     cudaFree(c->sc.quad);
     cudaFree(c->sc.i0);
     cudaFree(c->sc.cell);
-    cudaFree(c->sc.perm);
     cudaFree(c->sc.hist);
     cudaFree(c->sc.ngood);
     cudaFree(c->dQs);
@@ -273,14 +269,13 @@ static int ensure_scratch(ile_ctx *c, size_t samples, size_t hist_words, int32_t
 {
     if (samples > c->sc_samples) {
         CK(cudaStreamSynchronize(st));
-        cudaFree(c->sc.rec), cudaFree(c->sc.quad), cudaFree(c->sc.i0), cudaFree(c->sc.cell), cudaFree(c->sc.perm);
-        c->sc.rec = nullptr, c->sc.quad = nullptr, c->sc.i0 = nullptr, c->sc.cell = nullptr, c->sc.perm = nullptr;
+        cudaFree(c->sc.rec), cudaFree(c->sc.quad), cudaFree(c->sc.i0), cudaFree(c->sc.cell);
+        c->sc.rec = nullptr, c->sc.quad = nullptr, c->sc.i0 = nullptr, c->sc.cell = nullptr;
         c->sc_samples = 0;
         CK(cudaMalloc(&c->sc.rec, samples * c->sc_recg * sizeof(double)));
         CK(cudaMalloc(&c->sc.quad, samples * sizeof(double)));
         CK(cudaMalloc(&c->sc.i0, samples * c->sz.n_det * sizeof(int32_t)));
         CK(cudaMalloc(&c->sc.cell, samples * sizeof(int32_t)));
-        CK(cudaMalloc(&c->sc.perm, samples * sizeof(int32_t)));
         c->sc_samples = samples;
     }
     if (hist_words > c->sc_hist) {
@@ -308,7 +303,7 @@ static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
     const IleSortPlan &sp = c->ssp;
     const size_t nseg = (size_t)sp.n1 * sp.n2;
     const int64_t slot_cap = (((a.n_per_point + 7) & ~(int64_t)7) + 8 * (int64_t)nseg + 31) & ~(int64_t)31;  // groups per point: multiple of 4
-    int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES, a.n_points, st);
+    int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES + 1, a.n_points, st);
     if (r != ILE_OK) return r;
     const size_t need_slots = (size_t)a.n_points * slot_cap, need_adj = (size_t)a.n_points * nseg, need_g = 2 * (size_t)a.n_points + 2;
     const size_t need_go = need_slots / 8;
@@ -362,21 +357,6 @@ static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
     return ILE_OK;
 }
 
-// variant 3 for one launch group: setup + sort + contraction on [point0, point0 + n_points) x n samples each
-static int eval_mma_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
-{
-    const IleSortPlan sp = ile_sort_plan(c->sz, c->hparams, a.n_per_point);
-    int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * sp.ncell, a.n_points, st);
-    if (r != ILE_OK) return r;
-    c->sc.Qp = c->dQp;
-    int nl = 0;
-    cudaError_t e = ile_launch_setup_sort(c->sz, c->hparams, a, c->mp, sp, c->sc, st, &nl);
-    if (e == cudaSuccess) e = ile_launch_eval_mma(c->sz, c->hparams, a, c->mp, c->sc, st, &nl);
-    c->launches += nl;
-    if (e != cudaSuccess) return cuda_fail(e);
-    return ILE_OK;
-}
-
 static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n, const double *ra, const double *dec,
                          const double *t_ref, const double *phi_ref, const double *psi, const double *incl,
                          const double *dist, double *lnL, int32_t *shift_idx, cudaStream_t st)
@@ -393,8 +373,8 @@ static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n
     a.lnL = lnL;
     a.shift_idx = shift_idx;
     a.oob_counter = c->d_oob;
-    const bool use_stream = c->variant == 4 || (c->variant == 0 && c->stream_ok && n >= 16384);
-    if (use_stream || c->variant == 3) {
+    const bool use_stream = c->variant == 4 || (c->variant == 0 && c->stream_ok && n >= ILE_STREAM_MIN_SAMPLES);
+    if (use_stream) {
         // launch groups of at most chunk_samples samples: whole points while they fit, else slices of one point
         const int64_t cs = c->chunk_samples;
         const int K = c->sz.n_det;
@@ -413,7 +393,7 @@ static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n
             for (int32_t p = 0; p < n_points; p += per) {
                 const int32_t np = n_points - p < per ? n_points - p : per;
                 const IleEvalArgs g = shifted((int64_t)p * n, point0 + p, np, n);
-                int r = use_stream ? eval_stream_group(c, g, st) : eval_mma_group(c, g, st);
+                int r = eval_stream_group(c, g, st);
                 if (r != ILE_OK) return r;
             }
         } else {
@@ -421,7 +401,7 @@ static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n
                 for (int64_t off = 0; off < n; off += cs) {
                     const int64_t cnt = n - off < cs ? n - off : cs;
                     const IleEvalArgs g = shifted((int64_t)p * n + off, point0 + p, 1, cnt);
-                    int r = use_stream ? eval_stream_group(c, g, st) : eval_mma_group(c, g, st);
+                    int r = eval_stream_group(c, g, st);
                     if (r != ILE_OK) return r;
                 }
         }
@@ -443,6 +423,7 @@ extern "C" int ile_eval(ile_ctx *c, int32_t point, int64_t n, const double *ra, 
     if (!c || n < 0 || point < 0 || point >= c->n_points) return ILE_ERR_BAD_ARGUMENT;
     if (n == 0) return ILE_OK;
     if (!ra || !dec || !t_ref || !phi_ref || !psi || !incl || !dist_mpc || !lnL_margT) return ILE_ERR_BAD_ARGUMENT;
+    if (int r = check_device(c)) return r;
     return eval_dispatch(c, point, 1, n, ra, dec, t_ref, phi_ref, psi, incl, dist_mpc, lnL_margT, shift_idx,
                          (cudaStream_t)cuda_stream);
 }
@@ -454,18 +435,30 @@ extern "C" int ile_eval_all(ile_ctx *c, int64_t n_per_point, const double *ra, c
     if (!c || n_per_point < 0) return ILE_ERR_BAD_ARGUMENT;
     if (n_per_point == 0) return ILE_OK;
     if (!ra || !dec || !t_ref || !phi_ref || !psi || !incl || !dist_mpc || !lnL_margT) return ILE_ERR_BAD_ARGUMENT;
+    if (int r = check_device(c)) return r;
     return eval_dispatch(c, 0, c->n_points, n_per_point, ra, dec, t_ref, phi_ref, psi, incl, dist_mpc, lnL_margT,
                          shift_idx, (cudaStream_t)cuda_stream);
 }
 
-static int ensure_partials(ile_ctx *c, size_t doubles)
+static int ensure_evidence_scratch(ile_ctx *c, size_t doubles, size_t segments, cudaStream_t st)
 {
-    if (doubles <= c->partials_cap) return ILE_OK;
-    if (c->d_partials) CK(cudaFree(c->d_partials));
-    c->d_partials = nullptr;
-    c->partials_cap = 0;
-    CK(cudaMalloc(&c->d_partials, doubles * sizeof(double)));
-    c->partials_cap = doubles;
+    if (doubles > c->partials_cap || segments > c->tickets_cap) CK(cudaStreamSynchronize(st));  // an earlier call may still use them
+    if (doubles > c->partials_cap) {
+        cudaFree(c->d_partials);
+        c->d_partials = nullptr;
+        c->partials_cap = 0;
+        CK(cudaMalloc(&c->d_partials, doubles * sizeof(double)));
+        c->partials_cap = doubles;
+    }
+    if (segments > c->tickets_cap) {
+        cudaFree(c->d_tickets);
+        c->d_tickets = nullptr;
+        c->tickets_cap = 0;
+        const size_t cap = segments < 256 ? 256 : segments;
+        CK(cudaMalloc(&c->d_tickets, cap * sizeof(unsigned int)));
+        CK(cudaMemset(c->d_tickets, 0, cap * sizeof(unsigned int)));
+        c->tickets_cap = cap;
+    }
     return ILE_OK;
 }
 
@@ -474,18 +467,15 @@ extern "C" int ile_evidence(ile_ctx *c, int32_t n_segments, int64_t n_per_segmen
 {
     if (!c || n_segments < 1 || n_per_segment < 0 || !lnZ) return ILE_ERR_BAD_ARGUMENT;
     if (n_per_segment > 0 && !lnL_margT) return ILE_ERR_BAD_ARGUMENT;
-    int32_t B = ile_evidence_blocks_per_segment(n_segments, n_per_segment, c->sz.sm_count);
-    const size_t at = (size_t)n_segments * B * 2, need = at + ((size_t)n_segments + 1) / 2;
-    if (need > c->partials_cap) c->ev_tickets_at = 0;
-    int r = ensure_partials(c, need);
+    int r = check_device(c);
     if (r != ILE_OK) return r;
-    if (c->ev_tickets_at != at) {  // new layout: the ticket words behind the partials start at zero (each call leaves them so)
-        CK(cudaMemsetAsync(c->d_partials + at, 0, (((size_t)n_segments + 1) / 2) * sizeof(double), (cudaStream_t)cuda_stream));
-        c->ev_tickets_at = at;
-    }
+    const int32_t B = ile_evidence_blocks_per_segment(n_segments, n_per_segment, c->sz.sm_count);
+    // every segment has its own ticket word, zero between calls whatever layout the previous call used
+    r = ensure_evidence_scratch(c, (size_t)n_segments * B * 2, (size_t)n_segments, (cudaStream_t)cuda_stream);
+    if (r != ILE_OK) return r;
     int nl = 0;
     cudaError_t e = ile_launch_evidence(n_segments, n_per_segment, lnL_margT, log_w, state, lnZ, n_eff, c->d_partials,
-                                        B, (cudaStream_t)cuda_stream, &nl);
+                                        c->d_tickets, B, (cudaStream_t)cuda_stream, &nl);
     c->launches += nl;
     if (e != cudaSuccess) return cuda_fail(e);
     return ILE_OK;
@@ -509,6 +499,7 @@ extern "C" int ile_evidence_merge(ile_ctx *c, int32_t n_segments, int32_t n_stat
                                   double *lnZ, double *n_eff, void *cuda_stream)
 {
     if (!c || n_segments < 1 || n_states < 1 || !states_in || !lnZ) return ILE_ERR_BAD_ARGUMENT;
+    if (int r = check_device(c)) return r;
     int nl = 0;
     cudaError_t e = ile_launch_evidence_merge(n_segments, n_states, states_in, state_out, lnZ, n_eff, (cudaStream_t)cuda_stream, &nl);
     c->launches += nl;
@@ -519,10 +510,58 @@ extern "C" int ile_evidence_merge(ile_ctx *c, int32_t n_segments, int32_t n_stat
 extern "C" int ile_evidence_reset(ile_ctx *c, int32_t n_segments, double *state, void *cuda_stream)
 {
     if (!c || n_segments < 1 || !state) return ILE_ERR_BAD_ARGUMENT;
+    if (int r = check_device(c)) return r;
     int nl = 0;
     cudaError_t e = ile_launch_evidence_reset(n_segments, state, (cudaStream_t)cuda_stream, &nl);
     c->launches += nl;
     if (e != cudaSuccess) return cuda_fail(e);
+    return ILE_OK;
+}
+
+// H2D of the sample arrays ([np][n] each), ile_eval / ile_eval_all, ile_evidence per point, D2H of the results.
+static int run_host(ile_ctx *c, int32_t point0, int32_t np, int64_t n, const double *const src[8], double *lnL_margT, double *lnZ,
+                    double *n_eff, cudaStream_t st)
+{
+    const size_t tot = (size_t)n * np;
+    const size_t need = tot * 9;
+    if (need > c->stage_cap) {
+        CK(cudaStreamSynchronize(st));
+        if (c->d_stage) CK(cudaFree(c->d_stage));
+        c->d_stage = nullptr;
+        c->stage_cap = 0;
+        CK(cudaMalloc(&c->d_stage, need * sizeof(double)));
+        c->stage_cap = need;
+    }
+    double *d = c->d_stage;
+    // The sort needs ra, dec, t_ref only.  When the streaming variant will run as ONE launch group, the other arrays are
+    // copied on a second queue and only the coefficient kernel (side stream) waits for them: their transfer overlaps the
+    // index kernel, the scan and the scatter.
+    const bool split = c->copy_stream && (c->variant == 4 || (c->variant == 0 && c->stream_ok && n >= ILE_STREAM_MIN_SAMPLES)) &&
+                       (int64_t)tot <= c->chunk_samples;
+    for (int i = 0; i < 3; ++i) CK(cudaMemcpyAsync(d + (size_t)i * tot, src[i], tot * sizeof(double), cudaMemcpyHostToDevice, st));
+    cudaStream_t late = split ? c->copy_stream : st;
+    if (split) {
+        CK(cudaEventRecord(c->ev_copy_go, st));  // the staging buffer is free once the stream gets here
+        CK(cudaStreamWaitEvent(late, c->ev_copy_go, 0));
+    }
+    for (int i = 3; i < 8; ++i)
+        if (src[i]) CK(cudaMemcpyAsync(d + (size_t)i * tot, src[i], tot * sizeof(double), cudaMemcpyHostToDevice, late));
+    if (split) CK(cudaEventRecord(c->ev_copy_done, late));
+    double *d_out = d + (size_t)8 * tot;
+    c->ss.ev_late = split ? c->ev_copy_done : nullptr;
+    int r = eval_dispatch(c, point0, np, n, d, d + tot, d + 2 * tot, d + 3 * tot, d + 4 * tot, d + 5 * tot, d + 6 * tot, d_out, nullptr, st);
+    c->ss.ev_late = nullptr;
+    if (r != ILE_OK) return r;
+    if (split) CK(cudaStreamWaitEvent(st, c->ev_copy_done, 0));  // log_w for the evidence (already implied by the join)
+    r = ile_evidence(c, np, n, d_out, src[7] ? d + 7 * tot : nullptr, nullptr, c->d_small, c->d_small + np, st);
+    if (r != ILE_OK) return r;
+    if (lnL_margT) CK(cudaMemcpyAsync(lnL_margT, d_out, tot * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(c->h_small, c->d_small, 2 * (size_t)np * sizeof(double), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    for (int32_t p = 0; p < np; ++p) {
+        lnZ[p] = c->h_small[p];
+        if (n_eff) n_eff[p] = c->h_small[np + p];
+    }
     return ILE_OK;
 }
 
@@ -533,50 +572,26 @@ extern "C" int ile_run_host(ile_ctx *c, int32_t point, int64_t n, const double *
 {
     if (!c || n < 1 || point < 0 || point >= c->n_points) return ILE_ERR_BAD_ARGUMENT;
     if (!ra || !dec || !t_ref || !phi_ref || !psi || !incl || !dist_mpc || !lnZ) return ILE_ERR_BAD_ARGUMENT;
-    cudaStream_t st = (cudaStream_t)cuda_stream;
-    const size_t need = (size_t)n * 9;
-    if (need > c->stage_cap) {
-        CK(cudaStreamSynchronize(st));
-        if (c->d_stage) CK(cudaFree(c->d_stage));
-        c->d_stage = nullptr;
-        c->stage_cap = 0;
-        CK(cudaMalloc(&c->d_stage, need * sizeof(double)));
-        c->stage_cap = need;
-    }
-    double *d = c->d_stage;
+    if (int r = check_device(c)) return r;
     const double *src[8] = {ra, dec, t_ref, phi_ref, psi, incl, dist_mpc, log_w};
-    // The sort needs ra, dec, t_ref only.  When the streaming variant will run as ONE launch group, the other arrays are
-    // copied on a second queue and only the coefficient kernel (side stream) waits for them: their transfer overlaps the
-    // index kernel, the scan and the scatter.
-    const bool split = c->copy_stream && (c->variant == 4 || (c->variant == 0 && c->stream_ok && n >= 16384)) && n <= c->chunk_samples;
-    for (int i = 0; i < 3; ++i) CK(cudaMemcpyAsync(d + (size_t)i * n, src[i], (size_t)n * sizeof(double), cudaMemcpyHostToDevice, st));
-    cudaStream_t late = split ? c->copy_stream : st;
-    if (split) {
-        CK(cudaEventRecord(c->ev_copy_go, st));  // the staging buffer is free once the stream gets here
-        CK(cudaStreamWaitEvent(late, c->ev_copy_go, 0));
-    }
-    for (int i = 3; i < 8; ++i)
-        if (src[i]) CK(cudaMemcpyAsync(d + (size_t)i * n, src[i], (size_t)n * sizeof(double), cudaMemcpyHostToDevice, late));
-    if (split) CK(cudaEventRecord(c->ev_copy_done, late));
-    double *d_out = d + (size_t)8 * n;
-    c->ss.ev_late = split ? c->ev_copy_done : nullptr;
-    int r = eval_dispatch(c, point, 1, n, d, d + n, d + 2 * n, d + 3 * n, d + 4 * n, d + 5 * n, d + 6 * n, d_out, nullptr, st);
-    c->ss.ev_late = nullptr;
-    if (r != ILE_OK) return r;
-    if (split) CK(cudaStreamWaitEvent(st, c->ev_copy_done, 0));  // log_w for the evidence (already implied by the join)
-    r = ile_evidence(c, 1, n, d_out, log_w ? d + 7 * n : nullptr, nullptr, c->d_small, c->d_small + 1, st);
-    if (r != ILE_OK) return r;
-    if (lnL_margT) CK(cudaMemcpyAsync(lnL_margT, d_out, (size_t)n * sizeof(double), cudaMemcpyDeviceToHost, st));
-    CK(cudaMemcpyAsync(c->h_small, c->d_small, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    *lnZ = c->h_small[0];
-    if (n_eff) *n_eff = c->h_small[1];
-    return ILE_OK;
+    return run_host(c, point, 1, n, src, lnL_margT, lnZ, n_eff, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int ile_run_host_all(ile_ctx *c, int64_t n_per_point, const double *ra, const double *dec, const double *t_ref,
+                                const double *phi_ref, const double *psi, const double *incl, const double *dist_mpc,
+                                const double *log_w, double *lnL_margT, double *lnZ, double *n_eff, void *cuda_stream)
+{
+    if (!c || n_per_point < 1) return ILE_ERR_BAD_ARGUMENT;
+    if (!ra || !dec || !t_ref || !phi_ref || !psi || !incl || !dist_mpc || !lnZ) return ILE_ERR_BAD_ARGUMENT;
+    if (int r = check_device(c)) return r;
+    const double *src[8] = {ra, dec, t_ref, phi_ref, psi, incl, dist_mpc, log_w};
+    return run_host(c, 0, c->n_points, n_per_point, src, lnL_margT, lnZ, n_eff, (cudaStream_t)cuda_stream);
 }
 
 extern "C" int ile_status(ile_ctx *c, int64_t *n_out_of_range, int reset, void *cuda_stream)
 {
     if (!c) return ILE_ERR_BAD_ARGUMENT;
+    if (int r = check_device(c)) return r;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     unsigned long long v = 0;
     CK(cudaMemcpyAsync(&v, c->d_oob, sizeof(v), cudaMemcpyDeviceToHost, st));
@@ -590,7 +605,7 @@ extern "C" int ile_set_variant(ile_ctx *c, int32_t variant)
 {
     if (!c || variant < 0) return ILE_ERR_BAD_ARGUMENT;
     if (variant > 4) return ILE_ERR_UNSUPPORTED;
-    if (variant == 3 && !c->mma_ok) return ILE_ERR_UNSUPPORTED;
+    if (variant == 3) return ILE_ERR_UNSUPPORTED;  // retired (superseded by variant 4)
     if (variant == 4 && !c->stream_ok) return ILE_ERR_UNSUPPORTED;
     if (variant == 2) {
         IleTiledLayout L;
@@ -602,7 +617,7 @@ extern "C" int ile_set_variant(ile_ctx *c, int32_t variant)
 
 extern "C" int64_t ile_launch_count(const ile_ctx *c) { return c ? (int64_t)c->launches : 0; }
 
-extern "C" int ile_measure_fp64_peak(int32_t iters, double *tflops, double *ms)
+static int measure_peak(int32_t iters, int dmma, double *tflops, double *ms)
 {
     if (iters < 1 || !tflops) return ILE_ERR_BAD_ARGUMENT;
     int ndev = 0;
@@ -615,28 +630,34 @@ extern "C" int ile_measure_fp64_peak(int32_t iters, double *tflops, double *ms)
     cudaDeviceProp prop;
     CK(cudaGetDeviceProperties(&prop, dev));
     double *sink = nullptr;
-    CK(cudaMalloc(&sink, sizeof(double)));
-    cudaEvent_t e0, e1;
-    CK(cudaEventCreate(&e0));
-    CK(cudaEventCreate(&e1));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
     float best = 1e30f;
-    for (int rep = 0; rep < 4; ++rep) {  // first repetition is the warm-up
-        CK(cudaEventRecord(e0, 0));
-        CK(ile_launch_fp64_peak(iters, prop.multiProcessorCount, sink, 0));
-        CK(cudaEventRecord(e1, 0));
-        CK(cudaEventSynchronize(e1));
+    cudaError_t e = cudaMalloc(&sink, sizeof(double));
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    for (int rep = 0; rep < 4 && e == cudaSuccess; ++rep) {  // first repetition is the warm-up
+        e = cudaEventRecord(e0, 0);
+        if (e == cudaSuccess) e = ile_launch_fp64_peak(iters, prop.multiProcessorCount, sink, dmma, 0);
+        if (e == cudaSuccess) e = cudaEventRecord(e1, 0);
+        if (e == cudaSuccess) e = cudaEventSynchronize(e1);
         float t = 0.f;
-        CK(cudaEventElapsedTime(&t, e0, e1));
+        if (e == cudaSuccess) e = cudaEventElapsedTime(&t, e0, e1);
         if (rep > 0 && t < best) best = t;
     }
-    cudaEventDestroy(e0);
-    cudaEventDestroy(e1);
+    if (e0) cudaEventDestroy(e0);
+    if (e1) cudaEventDestroy(e1);
     cudaFree(sink);
-    const double flops = 2.0 * 8.0 * (double)iters * 256.0 * 8.0 * prop.multiProcessorCount;
-    *tflops = flops / (best * 1e-3) * 1e-12;
+    if (e != cudaSuccess) return cuda_fail(e);
+    // DFMA: 8 chains x 256 threads x 8 blocks per SM, 2 flops each; DMMA.8x8x4: 8 chains x 8 warps x 8 blocks, 512 flops each
+    const double per_iter = dmma ? 8.0 * 8.0 * 8.0 * 512.0 : 8.0 * 256.0 * 8.0 * 2.0;
+    *tflops = per_iter * (double)iters * prop.multiProcessorCount / (best * 1e-3) * 1e-12;
     if (ms) *ms = best;
     return ILE_OK;
 }
+
+extern "C" int ile_measure_fp64_peak(int32_t iters, double *tflops, double *ms) { return measure_peak(iters, 0, tflops, ms); }
+
+extern "C" int ile_measure_dmma_peak(int32_t iters, double *tflops, double *ms) { return measure_peak(iters, 1, tflops, ms); }
 
 extern "C" const char *ile_strerror(int code)
 {

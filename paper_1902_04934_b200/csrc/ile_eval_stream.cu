@@ -45,6 +45,9 @@
 #ifndef ST_MINB3
 #define ST_MINB3 3
 #endif
+#ifndef ST_NC
+#define ST_NC 2 /* (d1, d2) cells are 8 ST_NC rows wide */
+#endif
 #ifndef ST_PIPE_MAXKS
 #define ST_PIPE_MAXKS 4
 #endif
@@ -229,11 +232,6 @@ struct IleStreamKArgs {
     double *lnL;
 };
 
-#define ST_PFS 1 /* steps (pairs of blocks) the L1 prefetch runs ahead of the fragment loads */
-#ifndef ST_PREFETCH
-#define ST_PREFETCH 0 /* prefetch.global.L1 always goes to L2 (2.1 GB per 100,000 samples): off */
-#endif
-
 template <int K, int KS, int NC, int MINB>
 __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const __grid_constant__ IleStreamKArgs a)
 {
@@ -350,17 +348,6 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
 #pragma unroll
         for (int k = 0; k < K; ++k)
             pk[k] = a.Qs + ((size_t)((a.point0 + pt) * K + k) * KS * a.nqp + (size_t)(a.padf + base[k])) * 4 + lane;
-        // L1 prefetch: lane l looks after 128-byte line (l % 3) of fragment (l / 3) = (detector, k-step) of a block
-        const double *pf = nullptr;
-        {
-            const int f = lane / 3, fk = f / KS, fs = f - fk * KS;
-            if (ST_PREFETCH && f < K * KS) {
-                const int bk = fk == 0 ? base[0] - 8 * NC : fk == 1 ? base[K > 1 ? 1 : 0] : base[K > 2 ? 2 : 0];
-                const int j = lane - 3 * f;
-                pf = a.Qs + ((size_t)((a.point0 + pt) * K + fk) * KS * a.nqp + (size_t)fs * a.nqp + (size_t)(a.padf + bk)) * 4 +
-                     (size_t)(NC + 2 + 2 * ST_PFS) * 32 + (j == 2 ? 31 : 16 * j);
-            }
-        }
 
         const int nblk = ((dspread + n_t + 7) >> 3) + 1 & ~1;  // even: the stream advances two blocks per step
         const int t_lo = (dspread + 7) >> 3, t_hi = n_t >> 3;  // blocks [t_lo, t_hi) lie inside every window of the group
@@ -420,11 +407,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
                     for (int c = 0; c < 2; ++c) v[bb][c] = (unsigned)(jc[c] + 8 * (t0 - 2 + bb)) < (unsigned)n_t;
             }
             double d[2][2];
-#ifndef DBG_NO_LSE
             st_lse_pre2<PRED>(lin, v, m, sm, d, tab_addr);
-#else
-            sm[0] += lin[0][0] + lin[1][0]; sm[1] += lin[0][1] + lin[1][1]; m[0] = 0; m[1] = 0;
-#endif
             // shifted detectors: blocks t0 + NC + bb into ring slots (2 P + NC + bb) % 4
 #pragma unroll
             for (int k = 1; k < K; ++k) {
@@ -451,14 +434,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
                     pk[k] += 64;
                 }
             }
-            if (pf) {
-                asm volatile("prefetch.global.L1 [%0];" ::"l"(pf));
-                asm volatile("prefetch.global.L1 [%0];" ::"l"(pf + 32));
-                pf += 64;
-            }
-#ifndef DBG_NO_LSE
             st_lse_main2<PRED>(d, v, sm, tab_addr);
-#endif
             // realign: row rho of my column wants T_k[base_k + rho + eps]; I hold it for the lane (rho - eps) mod 8
             double z[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
 #pragma unroll
@@ -469,12 +445,8 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
                     for (int c = 0; c < 2; ++c) {
                         double x = ring[k - 1][(2 * P + bb) % 4][c];
 #pragma unroll
-#ifndef DBG_NO_REALIGN
                         for (int o = 1; o <= NC; ++o) x = st_bsel(x, ring[k - 1][(2 * P + bb + o) % 4][c], msk[k][c][o - 1]);
                         const double y = st_shfl(x, src[k][c]);
-#else
-                        const double y = x;
-#endif
                         z[bb][c] = k == 1 ? y : z[bb][c] + y;
                     }
             }
@@ -646,30 +618,6 @@ struct IleScanArgs {
     int32_t stage;    // words of shared memory behind the histogram for assembling the group list (0: none)
 };
 
-// Scan of one point by one block of NT threads; the point's histogram lives in shared memory (h: ncell + 1 + nseg words).
-//   hist  -> exclusive positions (written back for the scatter kernel)
-//   adj[seg] = padded base of the segment minus its first position;  ngr[pt] = groups of the point (a single point also
-//   gets gcum = {0, groups})
-//   gorder[pt][.] = the point's groups listed by i0_0 bin first, segment second: group ids are positions / 8 in the padded
-//   slot table; a group belongs to the (segment, bin) cell its first slot falls in.
-__device__ __forceinline__ uint32_t ss_warp_incl(uint32_t x, int lane)
-{
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t y = __shfl_up_sync(ST_FULL, x, o);
-        if (lane >= o) x += y;
-    }
-    return x;
-}
-
-// Scan of one point by one block of NT threads; the point's histogram lives in shared memory (h: ncell + 1 + nseg words).
-//   hist  -> exclusive positions (written back for the scatter kernel)
-//   adj[seg] = padded base of the segment minus its first position;  ngr[pt] = groups of the point (a single point also
-//   gets gcum = {0, groups})
-//   gorder[pt][.] = the point's groups listed by i0_0 bin first, segment second: group ids are positions / 8 in the padded
-//   slot table; a group belongs to the (segment, bin) cell its first slot falls in.
-// Every pass gives warp w a contiguous range and walks it 32 consecutive elements at a time (conflict-free shared-memory
-// access, coalesced global writes); the warps' totals are combined through wsum.
 // Scan of one point by one block of NT threads; the point's histogram lives in shared memory (h: ncell + 1 + nseg words,
 // followed by `stage` words in which the group list is assembled when it fits; stage = 0: written straight to global).
 //   hist  -> exclusive positions (written back for the scatter kernel)
@@ -906,14 +854,10 @@ bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per
     pl.ks = st_round_ks((2 * sz.n_modes + 3) / 4);
     if (!pl.ks) return false;
     pl.cp = 4 * pl.ks;
-#ifndef ST_NC
-#define ST_NC 2
-#endif
     pl.nc = ST_NC;
     pl.padf = sz.n_q - sz.n_t + 32;
     pl.nqp = pl.padf + sz.n_q + (sz.n_q - sz.n_t) + 64;
     IleSortPlan sp;
-    sp.mode = 1;
     sp.nd = sz.n_det;
     sp.g = pl.nc == 2 ? 4 : 3;
     sp.dmax[0] = 0;
@@ -945,49 +889,71 @@ bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per
     return true;
 }
 
+// Launch (ka != nullptr) or prepare (ka == nullptr: function attributes of the current device + resident CTAs per SM) the
+// instantiation for (K, ks).  Function attributes are per device, so they are set by ile_stream_prepare for every context.
 template <int K, int KS, int NC, int MINB>
-static cudaError_t st_launch_t(const IleSizes &sz, const IleStreamKArgs &ka, long long max_groups, cudaStream_t st)
+static cudaError_t st_launch_t(const IleSizes &sz, const IleStreamKArgs *ka, long long max_groups, int *per_sm, cudaStream_t st)
 {
-    static int per_sm = 0;
-    if (!per_sm) {
+    if (!ka) {
         cudaError_t e = cudaFuncSetAttribute(ile_eval_stream_kernel<K, KS, NC, MINB>, cudaFuncAttributePreferredSharedMemoryCarveout, 8);
         if (e != cudaSuccess) return e;
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ile_eval_stream_kernel<K, KS, NC, MINB>, ST_THREADS, 0);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, ile_eval_stream_kernel<K, KS, NC, MINB>, ST_THREADS, 0);
         if (e != cudaSuccess) return e;
-        if (per_sm < 1) return cudaErrorInvalidConfiguration;
+        return *per_sm < 1 ? cudaErrorInvalidConfiguration : cudaSuccess;
     }
-    long long grid = (long long)sz.sm_count * per_sm;
+    long long grid = (long long)sz.sm_count * *per_sm;
     const long long need = (max_groups + ST_THREADS / 32 - 1) / (ST_THREADS / 32);
     if (need < grid) grid = need < 1 ? 1 : need;
-    ile_eval_stream_kernel<K, KS, NC, MINB><<<(unsigned)grid, ST_THREADS, 0, st>>>(ka);
+    ile_eval_stream_kernel<K, KS, NC, MINB><<<(unsigned)grid, ST_THREADS, 0, st>>>(*ka);
     return cudaGetLastError();
 }
 
 template <int K, int NC>
-static cudaError_t st_launch_k(const IleSizes &sz, int ks, const IleStreamKArgs &ka, long long mg, cudaStream_t st)
+static cudaError_t st_launch_k(const IleSizes &sz, int ks, const IleStreamKArgs *ka, long long mg, int *per_sm, cudaStream_t st)
 {
     switch (ks) {
-        case 1: return st_launch_t<K, 1, NC, 4>(sz, ka, mg, st);
-        case 2: return st_launch_t<K, 2, NC, 4>(sz, ka, mg, st);
-        case 3: return st_launch_t<K, 3, NC, ST_MINB3>(sz, ka, mg, st);
-        case 4: return st_launch_t<K, 4, NC, 3>(sz, ka, mg, st);
-        case 6: return st_launch_t<K, 6, NC, 2>(sz, ka, mg, st);
-        case 8: return st_launch_t<K, 8, NC, 2>(sz, ka, mg, st);
-        case 11: return st_launch_t<K, 11, NC, 2>(sz, ka, mg, st);
-        case 16: return st_launch_t<K, 16, NC, 2>(sz, ka, mg, st);
+        case 1: return st_launch_t<K, 1, NC, 4>(sz, ka, mg, per_sm, st);
+        case 2: return st_launch_t<K, 2, NC, 4>(sz, ka, mg, per_sm, st);
+        case 3: return st_launch_t<K, 3, NC, ST_MINB3>(sz, ka, mg, per_sm, st);
+        case 4: return st_launch_t<K, 4, NC, 3>(sz, ka, mg, per_sm, st);
+        case 6: return st_launch_t<K, 6, NC, 2>(sz, ka, mg, per_sm, st);
+        case 8: return st_launch_t<K, 8, NC, 2>(sz, ka, mg, per_sm, st);
+        case 11: return st_launch_t<K, 11, NC, 2>(sz, ka, mg, per_sm, st);
+        case 16: return st_launch_t<K, 16, NC, 2>(sz, ka, mg, per_sm, st);
         default: return cudaErrorInvalidValue;
     }
 }
 
+static cudaError_t st_launch(const IleSizes &sz, int ks, const IleStreamKArgs *ka, long long mg, int *per_sm, cudaStream_t st)
+{
+    if (sz.n_det == 1) return st_launch_k<1, ST_NC>(sz, ks, ka, mg, per_sm, st);
+    if (sz.n_det == 2) return st_launch_k<2, ST_NC>(sz, ks, ka, mg, per_sm, st);
+    return st_launch_k<3, ST_NC>(sz, ks, ka, mg, per_sm, st);
+}
+
+// Once per context, on the context's device: opt-in shared memory of the scan kernels, carve-out and occupancy of the
+// streaming kernel this context's sizes select.
+cudaError_t ile_stream_prepare(const IleSizes &sz, IleStreamPlan *pl)
+{
+    cudaError_t e = cudaFuncSetAttribute(ile_stream_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 8192);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(ile_stream_index_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 8192);
+    if (e != cudaSuccess) return e;
+    int per_sm = 0;
+    e = st_launch(sz, pl->ks, nullptr, 0, &per_sm, 0);
+    pl->ctas_per_sm = per_sm;
+    return e;
+}
+
 cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleStreamPlan &pl,
-                                   const IleSortPlan &sp, const IleMmaScratch &sc, const IleStreamScratch &ss, cudaStream_t st,
+                                   const IleSortPlan &sp, const IleSortScratch &sc, const IleStreamScratch &ss, cudaStream_t st,
                                    int *n_launches)
 {
     if (a.n_per_point <= 0 || a.n_points <= 0) return cudaSuccess;
     const long long n_total = a.n_per_point * a.n_points;
     const int nseg = sp.n1 * sp.n2;
     // histogram + claim counters of the streaming kernel (right behind the histograms)
-    cudaError_t e = cudaMemsetAsync(sc.hist, 0, ((size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES) * sizeof(uint32_t), st);
+    cudaError_t e = cudaMemsetAsync(sc.hist, 0, ((size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES + 1) * sizeof(uint32_t), st);
     if (e != cudaSuccess) return e;
     // window starts + histogram on the caller's stream; a single point's scan runs in the index kernel's last block
     IleScanArgs sa;
@@ -1006,15 +972,7 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
         sa.stage = want <= room ? (int32_t)sa.gcap : 0;
         if (sa.stage) scan_smem += want;
     }
-    static bool scan_attr = false;
-    if (!scan_attr) {
-        e = cudaFuncSetAttribute(ile_stream_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 8192);
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(ile_stream_index_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 8192);
-        if (e != cudaSuccess) return e;
-        scan_attr = true;
-    }
-    uint32_t *ticket = sc.hist + (size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES - 1;
+    uint32_t *ticket = sc.hist + (size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES;  // its own word behind the claim counters
     long long iblocks = (n_total + IX_THREADS - 1) / IX_THREADS;
     const long long cap = (long long)sz.sm_count * 32;
     if (iblocks > cap) iblocks = cap;
@@ -1035,14 +993,12 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
         e = cudaStreamWaitEvent(ss.aux, ss.ev_late, 0);
         if (e != cudaSuccess) return e;
     }
-#ifndef DBG_SKIP_SETUP
     if (ss.quad_mats && sc.qform) {
         e = ile_launch_quad_mma(sz, hp, a, ss.quad_mats, sc.qform, ss.aux);
         if (e != cudaSuccess) return e;
         ++nl;
     }
-    ile_launch_setup_coef(sz, hp, a, pl.cp, sp, sc, ss.aux);
-#endif
+    ile_launch_setup_coef(sz, hp, a, pl.cp, sc, ss.aux);
     ++nl;
     e = cudaEventRecord(ss.ev_join, ss.aux);
     if (e != cudaSuccess) return e;
@@ -1082,12 +1038,8 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     ka.gcap = ss.slot_cap / 8;
     ka.lnL = a.lnL;
     const long long max_groups = (long long)a.n_points * (ss.slot_cap / 8);
-#ifdef DBG_SKIP_STREAM
-    return cudaSuccess;
-#endif
-    if (sz.n_det == 1) e = st_launch_k<1, ST_NC>(sz, pl.ks, ka, max_groups, st);
-    else if (sz.n_det == 2) e = st_launch_k<2, ST_NC>(sz, pl.ks, ka, max_groups, st);
-    else e = st_launch_k<3, ST_NC>(sz, pl.ks, ka, max_groups, st);
+    int per_sm = pl.ctas_per_sm;
+    e = st_launch(sz, pl.ks, &ka, max_groups, &per_sm, st);
     ++nl;
     if (e == cudaSuccess && n_launches) *n_launches += nl;
     return e;

@@ -144,7 +144,7 @@ cudaError_t ile_launch_eval_direct(const IleSizes &sz, const IleEvalArgs &a, cud
 // step 7: evidence.  lnZ = ln((1/n) sum_a exp(lnL_a + ln w_a)), max-subtracted; n_eff = sum / max  (eq. 4).
 // One kernel.  A thread keeps a running (max, sum exp(e - max)) over its elements (one pass over the data), a block
 // merges its threads' pairs with warp shuffles and a block-level combine, and the block of a segment that finishes last
-// (ticket counter behind the partials, reset by that block) folds the segment's partials into the carried state.
+// (ticket counter, reset by that block) folds the segment's partials into the carried state.
 // ------------------------------------------------------------------------------------------------------------
 #define EV_THREADS 256
 #define EV_PER 4
@@ -300,13 +300,12 @@ int32_t ile_evidence_blocks_per_segment(int32_t n_segments, int64_t n_per_segmen
     return (int32_t)want;
 }
 
-// partials: n_segments * B * 2 doubles followed by n_segments ticket words (zero before the first call)
+// partials: n_segments * B * 2 doubles; tickets: n_segments words, zero on entry (every call leaves them zero)
 cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const double *lnL, const double *log_w,
-                                double *state, double *lnZ, double *n_eff, double *partials, int32_t B,
+                                double *state, double *lnZ, double *n_eff, double *partials, unsigned int *tickets, int32_t B,
                                 cudaStream_t st, int *n_launches)
 {
     dim3 grid((unsigned)B, (unsigned)n_segments);
-    unsigned int *tickets = reinterpret_cast<unsigned int *>(partials + (size_t)n_segments * B * 2);
     ile_evidence_kernel<<<grid, EV_THREADS, 0, st>>>(n_per_segment, lnL, log_w, partials, tickets, state, lnZ, n_eff);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
@@ -341,8 +340,29 @@ __global__ void __launch_bounds__(256) ile_fp64_peak_kernel(int iters, double *s
     if (s == 123.456) sink[0] = s;  // never true; keeps the chains alive
 }
 
-cudaError_t ile_launch_fp64_peak(int32_t iters, int32_t sm_count, double *sink, cudaStream_t st)
+// the same for the FP64 matrix instruction the streaming kernel runs on: 8 independent DMMA.8x8x4 chains per warp
+__global__ void __launch_bounds__(256) ile_dmma_peak_kernel(int iters, double *sink)
 {
-    ile_fp64_peak_kernel<<<sm_count * 8, 256, 0, st>>>(iters, sink);
+    double c[8][2];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) c[j][0] = 1e-3 * j, c[j][1] = 2e-3 * j;
+    const double a = 0.9999999 + threadIdx.x * 1e-12, b = 1e-7;
+    for (int i = 0; i < iters; ++i) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j)
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                         : "+d"(c[j][0]), "+d"(c[j][1])
+                         : "d"(a), "d"(b));
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) s += c[j][0] + c[j][1];
+    if (s == 123.456) sink[0] = s;  // never true; keeps the chains alive
+}
+
+cudaError_t ile_launch_fp64_peak(int32_t iters, int32_t sm_count, double *sink, int dmma, cudaStream_t st)
+{
+    if (dmma) ile_dmma_peak_kernel<<<sm_count * 8, 256, 0, st>>>(iters, sink);
+    else ile_fp64_peak_kernel<<<sm_count * 8, 256, 0, st>>>(iters, sink);
     return cudaGetLastError();
 }

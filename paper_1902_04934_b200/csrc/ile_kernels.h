@@ -46,55 +46,27 @@ bool ile_tiled_plan(const IleSizes &sz, long long n_total, IleTiledLayout *out);
 cudaError_t ile_launch_eval_tiled(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, cudaStream_t st,
                                   int *n_launches);
 
-// ---- variant 3: setup + counting sort + FP64-MMA contraction (ile_setup.cu, ile_eval_mma.cu) --------------------
-// Cell grid of the counting sort: window starts binned to width 2^g in (i0_0, i0_1 - i0_0, i0_2 - i0_0).
+// ---- counting sort of the streaming path (variant 4) -----------------------------------------------------------------
+// Cell grid: segments = (i0_1 - i0_0, i0_2 - i0_0) cells of width 2^g, inside a segment bins of i0_0 of width 2^g0.
 struct IleSortPlan {
-    int32_t mode;     // 0: variant 3 (cubic cells, boustrophedon); 1: variant 4 (segments of (d1, d2) x exact i0_0)
-    int32_t g;        // log2 of the cell width in samples (mode 1: of the (d1, d2) cells only)
-    int32_t g0;       // mode 1: log2 of the i0_0 bin width inside a segment
+    int32_t g;        // log2 of the (d1, d2) cell width in samples
+    int32_t g0;       // log2 of the i0_0 bin width inside a segment
     int32_t nd;       // detectors that take part in the key (<= 3)
     int32_t n0, n1, n2;
     int32_t ncell;    // n0*n1*n2 + 1; the last cell collects out-of-range samples
     int32_t dmax[3];  // bound on |i0_d - i0_0| from the light travel time between the sites
 };
 
-// Sizes and shared-memory carve-up of the MMA kernel, computed on the host and passed by value.
-struct IleMmaPlan {
-    int32_t ks;      // k-steps of 4 real channels: ceil(2M / 4)
-    int32_t cp;      // padded channels per detector = 4 * ks
-    int32_t tbmax;   // 8-index time blocks a warp can hold per chunk (template parameter)
-    int32_t S;       // samples per tile, multiple of 8
-    int32_t recg;    // doubles per sample record in global memory = K * cp
-    int32_t ldrec;   // doubles per sample record in shared memory (recg padded to 4 mod 16)
-    int32_t nb;      // 8-cell blocks per row = ceil(n_t / 8)
-    int32_t nblk_q;  // 8-index blocks per detector in the packed Q (with zero padding at the end)
-    uint32_t sb_bytes, sb_quad, sb_flat, sb_i0, sb_misc;  // one setup buffer: rec | quad | flat | i0 | ranges
-    uint32_t off_mbar, off_part, part_bytes, off_rows, bytes;
-};
-
-// Device scratch of variant 3 (owned by the context).
-struct IleMmaScratch {
-    const double *Qp;  // packed Q [P][K][nblk_q][ks][32]
-    double *rec;       // [n][recg]
+// Device scratch of the sorted path (owned by the context).
+struct IleSortScratch {
+    double *rec;       // [n][K * cp] coefficients a F_k Y_lm, (Re, Im) interleaved, zero padded to cp channels per detector
     double *quad;      // [n]
     int32_t *i0;       // [n][K]
     int32_t *cell;     // [n]
-    int32_t *perm;     // [n]
-    uint32_t *hist;    // [n_points][ncell]
+    uint32_t *hist;    // [n_points][ncell], followed by ILE_STREAM_MAX_RANGES claim counters and the index kernel's ticket
     int32_t *ngood;    // [n_points]
     double *qform;     // [n][K][3] quadratic forms from the FP64-MMA kernel, or NULL (the coefficient kernel computes them)
 };
-
-bool ile_mma_plan(const IleSizes &sz, IleMmaPlan *out);
-IleSortPlan ile_sort_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point);
-cudaError_t ile_launch_pack_q(const IleSizes &sz, const IleMmaPlan &mp, int32_t n_points, const double2 *Q, double *Qp,
-                              cudaStream_t st);
-// steps 1-4 for every sample + cell keys + counting sort (4 launches)
-cudaError_t ile_launch_setup_sort(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleMmaPlan &mp,
-                                  const IleSortPlan &sp, const IleMmaScratch &sc, cudaStream_t st, int *n_launches);
-// steps 5-6 on the sorted samples
-cudaError_t ile_launch_eval_mma(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleMmaPlan &mp,
-                                const IleMmaScratch &sc, cudaStream_t st, int *n_launches);
 
 // ---- variant 4: streaming FP64-MMA kernel, one warp per group of 8 samples (ile_eval_stream.cu) ------------------
 struct IleStreamPlan {
@@ -103,9 +75,10 @@ struct IleStreamPlan {
     int32_t nc;       // (d1, d2) cell width = 8 * nc rows; the shuffle realignment looks nc blocks ahead
     int32_t padf;     // zero rows in front of each packed series
     int32_t nqp;      // rows per packed series = padf + n_q + back padding
+    int32_t ctas_per_sm;  // resident CTAs of the streaming kernel per SM on the context's device (ile_stream_prepare)
 };
 
-#define ILE_STREAM_MAX_RANGES 256 /* claim counters of the streaming kernel, kept right behind the histograms */
+#define ILE_STREAM_MAX_RANGES 256 /* claim counters of the streaming kernel, kept right behind the histograms (+ 1 ticket word) */
 
 struct IleStreamScratch {
     const double *Qs;   // packed Q [P][K][ks][nqp][4]
@@ -121,15 +94,16 @@ struct IleStreamScratch {
 };
 
 bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point, IleStreamPlan *out, IleSortPlan *sp);
+cudaError_t ile_stream_prepare(const IleSizes &sz, IleStreamPlan *pl);  // per context: function attributes + occupancy on its device
 cudaError_t ile_launch_pack_q_stream(const IleSizes &sz, const IleStreamPlan &pl, int32_t n_points, const double2 *Q,
                                      double *Qs, cudaStream_t st);
 // setup + sort of variant 4 (memsets + setup + scan + scatter), then the streaming kernel
 cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleStreamPlan &pl,
-                                   const IleSortPlan &sp, const IleMmaScratch &sc, const IleStreamScratch &ss,
+                                   const IleSortPlan &sp, const IleSortScratch &sc, const IleStreamScratch &ss,
                                    cudaStream_t st, int *n_launches);
 // variant 4: coefficients a F_k Y_lm and quadratic term of every sample (steps 1, 3, 4), no sorting work
-void ile_launch_setup_coef(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, int32_t cp, const IleSortPlan &sp,
-                           const IleMmaScratch &sc, cudaStream_t st);
+void ile_launch_setup_coef(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, int32_t cp, const IleSortScratch &sc,
+                           cudaStream_t st);
 
 // step 4 for many modes (ile_quad_mma.cu): packed real representations of U, V and the batched quadratic forms
 size_t ile_quad_pack_doubles(int32_t n_points, int32_t K, int32_t M);
@@ -141,13 +115,15 @@ cudaError_t ile_launch_quad_mma(const IleSizes &sz, const IleDevParams &hp, cons
 cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_t N, double fs_hz, double t0_q_s, const double2 *x,
                                   const double2 *d, double2 *Q, double2 *U, double2 *V, int32_t max_smem_optin, cudaStream_t st);
 
-// evidence: two kernels (per-block partials, then per-segment combine with the carried state)
+// evidence: one kernel (per-block partials; the block of a segment that finishes last folds them into the carried state).
+// partials: n_segments * blocks_per_seg * 2 doubles; tickets: n_segments words, zero on entry, left zero on exit
 cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const double *lnL, const double *log_w,
-                                double *state, double *lnZ, double *n_eff, double *partials, int32_t blocks_per_seg,
+                                double *state, double *lnZ, double *n_eff, double *partials, unsigned int *tickets, int32_t blocks_per_seg,
                                 cudaStream_t st, int *n_launches);
 int32_t ile_evidence_blocks_per_segment(int32_t n_segments, int64_t n_per_segment, int32_t sm_count);
 cudaError_t ile_launch_evidence_merge(int32_t n_segments, int32_t n_states, const double *states_in, double *state_out,
                                       double *lnZ, double *n_eff, cudaStream_t st, int *n_launches);
 cudaError_t ile_launch_evidence_reset(int32_t n_segments, double *state, cudaStream_t st, int *n_launches);
 
-cudaError_t ile_launch_fp64_peak(int32_t iters, int32_t sm_count, double *sink, cudaStream_t st);
+// calibration kernels: dmma = 0 register-resident DFMA chains, 1 = DMMA.8x8x4 chains; 8 blocks of 256 threads per SM
+cudaError_t ile_launch_fp64_peak(int32_t iters, int32_t sm_count, double *sink, int dmma, cudaStream_t st);

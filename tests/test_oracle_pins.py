@@ -196,15 +196,17 @@ def test_O2_window_index_rounding():
 
 def test_O2_index_against_extended_precision():
     """Indices from the binary64 oracle agree with an 80-bit evaluation of the same definition on seeded samples
-    (a flip needs x within ~1e-13 of a half-integer)."""
-    cfg = gi.make_config(1, n=20000)
-    s = gi.make_samples(cfg["sample_seeds"][0], cfg["n"])
-    _, idx, bad = oracle.eval_batch(cfg, {k: v[:2000] for k, v in s.items()})
+    (a flip needs x within ~1e-13 of a half-integer): 100,000 samples x 3 detectors."""
+    n = 100_000
+    cfg = gi.make_config(1, n=n)
+    s = gi.make_samples(cfg["sample_seeds"][0], n)
+    _, idx, bad = oracle.eval_batch(cfg, s, n_threads=4)
     assert bad == 0
     ld = np.longdouble
+    assert np.finfo(ld).nmant >= 63, "needs the x87 80-bit long double"
     for k in range(cfg["n_det"]):
         v = cfg["vertex_m"][k].astype(ld)
-        ra, dec, t = s["ra"][:2000].astype(ld), s["dec"][:2000].astype(ld), s["t_ref"][:2000].astype(ld)
+        ra, dec, t = s["ra"].astype(ld), s["dec"].astype(ld), s["t_ref"].astype(ld)
         lon = ra - ld(cfg["gmst_rad"])
         dot = v[0] * np.cos(dec) * np.cos(lon) + v[1] * np.cos(dec) * np.sin(lon) + v[2] * np.sin(dec)
         x = ((t - dot / ld(C_SI)) - ld(cfg["t0_q_s"])) * ld(cfg["fs_hz"])
@@ -446,6 +448,46 @@ def test_check_c_face_on_single_mode_optimum():
 # ----------------------------------------------------------------------------------------------------------
 # check (d): psi -> psi + pi
 # ----------------------------------------------------------------------------------------------------------
+def test_noise_free_injection_peaks_at_half_rho_squared():
+    """SURVEY.md §8(c) pin: data = the noise-free signal of a known extrinsic point theta_0, built by the input
+    generator from response numbers computed HERE by independent means (vector-algebra antenna pattern, textbook l = 2
+    harmonics, geometric delay), gives oracle lnL(theta_0, t_0) = <h|d> - <h|h>/2 = +rho^2/2 with rho = the SNR the
+    generator scaled the signal to -- and theta_0 is a maximum: every neighbouring point and every other time bin
+    gives less.  A wrong sign of F (R1), of the delay (R2), of the Y_lm phase (R4), a dropped V term or a factor in the
+    quadratic term (eq. 7) fails this."""
+    base = gi.make_config(1, n=1)
+    dets, modes = base["dets"], base["modes"]
+    rng = np.random.default_rng(99)
+    snr = 17.0
+    for trial in range(4):
+        th = dict(ra=rng.uniform(0, 2 * np.pi), dec=np.arcsin(rng.uniform(-1, 1)), psi=rng.uniform(0, np.pi),
+                  phi_ref=rng.uniform(0, 2 * np.pi), incl=np.arccos(rng.uniform(-1, 1)), dist_mpc=gi.D_TRUE_MPC, t_ref=0.0)
+        resp, tau = [], []
+        for k in range(len(dets)):
+            fp, fc = antenna_vec(base["arm_x"][k], base["arm_y"][k], th["ra"], th["dec"], th["psi"], base["gmst_rad"])
+            resp.append(complex(fp, fc))                                       # R1: F = F+ + i Fx
+            dt = -float(np.dot(base["vertex_m"][k], source_dir(th["ra"], th["dec"], base["gmst_rad"]))) / C_SI   # R2
+            tau.append(int(np.rint(dt * base["fs_hz"])))
+        y = np.array([Y2m_closed(m, th["incl"], -th["phi_ref"]) for (_, m) in modes])      # R4: Y_lm(iota, -phi_ref)
+        Q, U, V, meta = gi.make_point(1234 + trial, dets, modes, base["n_q"], snr, noise=False,
+                                      truth_response=dict(y=y, resp=np.array(resp), tau_samples=np.array(tau)))
+        cfg = dict(base)
+        cfg.update(Q=Q[None], U=U[None], V=V[None], n_points=1)
+        series, margT, idx, oob = oracle.sample_series(cfg, th)
+        assert not oob
+        j0 = cfg["n_t"] // 2                                                   # the bin of t = t_ref
+        assert np.array_equal(idx + j0, np.array(tau) + cfg["n_q"] // 2)
+        assert abs(series[j0] - 0.5 * snr ** 2) <= 1e-9 * snr ** 2
+        assert np.argmax(series) == j0
+        for key, step in (("ra", 0.02), ("dec", 0.02), ("psi", 0.05), ("phi_ref", 0.05), ("incl", 0.05), ("dist_mpc", 10.0)):
+            for sgn in (-1.0, 1.0):
+                th2 = dict(th)
+                th2[key] = th[key] + sgn * step
+                if key == "dec" and abs(th2["dec"]) > 0.5 * np.pi:
+                    continue
+                assert oracle.sample_series(cfg, th2)[0].max() < series[j0]
+
+
 def test_check_d_psi_plus_pi_invariance():
     cfg = gi.make_config(0, n=64)
     s = gi.make_samples(5, 64)
