@@ -215,6 +215,83 @@ def run_precompute(args, rank: int):
     print(json.dumps(line), flush=True)
 
 
+def run_integrate(args, rank: int):
+    """SURVEY.md §8(f) NEXT-2, single GPU: the whole adaptive Monte Carlo integral of one intrinsic point through
+    ile_integrate -- Philox draws, sampling-prior refits, ile_eval and the evidence all on the device; per chunk two
+    doubles cross the bus.  Workload: BASELINE.json configs[--config], chunks of --n samples (default 10,000: the paper's
+    block size, L97 / n_chunk L119), --chunks chunks per step (default 200: N_it = 2e6, L119), adapting in RA, dec and
+    distance after every chunk, no early stop (n_eff threshold = inf) so that every step does the same work."""
+    if rank != 0:
+        return
+    import numpy as np
+    import torch
+
+    import ile_inputs as gi
+    import paper_1902_04934_b200 as ile
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback")
+    ile.load()
+    cfg = gi.make_config(args.config, n_points=1)
+    n_chunk = args.n if args.n is not None else 10_000
+    chunks = args.chunks
+    scfg = dict(seed=4934, n_bins=100, adapt=(True, True, True), floor_frac=0.1, temper=0.5, dist_min_mpc=1.0, dist_max_mpc=1000.0,
+                t_ref_lo_s=-0.05, t_ref_hi_s=0.05)
+    ctx = ile.Context(cfg)
+    if args.variant:
+        ctx.set_variant(args.variant)
+    smp = ile.Sampler(scfg)
+    for _ in range(max(args.warmup, 3)):
+        ile.integrate(ctx, smp, n_chunk, min(chunks, 10), chunks, float("inf"))
+    torch.cuda.synchronize()
+    sampler = ClockSampler(0)
+    l0, s0 = ctx.launch_count, smp.launch_count
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t0 = time.perf_counter()
+    e0.record()
+    for _ in range(args.steps):
+        r = ile.integrate(ctx, smp, n_chunk, chunks, chunks, float("inf"))
+    e1.record()
+    torch.cuda.synchronize()
+    wall = time.perf_counter() - t0
+    sampler.stop_flag = True
+    ms = max(e0.elapsed_time(e1), wall * 1e3) / args.steps      # the call synchronises: device and wall time agree
+    launches = (ctx.launch_count - l0) + (smp.launch_count - s0)
+    K, M, n_t = cfg["n_det"], cfg["n_modes"], cfg["n_t"]
+    w = dfma_per_sample(K, M, n_t)
+    peak = max(ile.measure_fp64_peak(1 << 15)[0], ile.measure_dmma_peak(1 << 12)[0])
+    val = n_chunk * chunks / (ms * 1e-3)
+    ach = 2.0 * w * val * 1e-12
+    line = {"metric": "adaptive Monte Carlo integral (draw + lnL_margT + evidence + refit on the device) samples/sec", "value": val,
+            "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": f"ile_integrate on BASELINE.json configs[{args.config}] ({K} detectors, {M} modes, {n_t} bins): {chunks} chunks "
+                                   f"of {n_chunk} Philox-drawn samples per step, refit of the (RA, dec, distance) sampling prior after every chunk",
+                       "n_chunk": n_chunk, "chunks_per_step": chunks, "variant": args.variant},
+            "roofline": {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+                         "kernel": "whole loop (draw, index/sort, coefficients, contraction + marginalisation, evidence, refit)",
+                         "dfma_equiv_per_sample": w},
+            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 16 * chunks, "ms_per_step": ms,
+                    "api": "ile_integrate (samples are generated on the device: no per-block H2D)"},
+            "gpu_launches": int(launches), "clocks": sampler.summary(), "lnZ": r["lnZ"], "n_eff": r["n_eff"],
+            "us_per_chunk": ms * 1e3 / chunks}
+    if not args.no_cpu_baseline:
+        import oracle  # cpu_baseline leg
+        from oracle import sampler as osm
+
+        cores = os.cpu_count() or 1
+        nchk = 3
+        t0 = time.perf_counter()
+        osm.integrate(scfg, lambda sd: oracle.eval_batch(cfg, sd, n_threads=cores)[0], n_chunk, nchk, nchk, float("inf"))
+        dt = time.perf_counter() - t0
+        line["cpu_baseline"] = {"value": n_chunk * nchk / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                                "sample": f"the first {nchk} chunks of the same run: oracle/sampler.py (numpy) around oracle.eval_batch (OpenMP)"}
+    print(json.dumps(line), flush=True)
+    ctx.close()
+    smp.close()
+
+
 def workload_config(cfg, n, args, extra=None):
     c = {"workload": f"BASELINE.json configs[{cfg['config_id']}]: {cfg['n_det']} detectors ({','.join(cfg['dets'])}), "
                      f"{cfg['n_modes']} modes (l<= {int(max(cfg['l']))}), Q {cfg['n_q']} complex128 @ {int(cfg['fs_hz'])} Hz, "
@@ -241,8 +318,10 @@ def main():
     ap.add_argument("--samples", default="prior", choices=["prior", "concentrated"])
     ap.add_argument("--ref-samples-per-step", type=int, default=100_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--stage", default="hotpath", choices=["hotpath", "precompute"],
-                    help="precompute: time ile_precompute (eq. 8: Q, U, V of --points intrinsic points) instead of the hot path")
+    ap.add_argument("--stage", default="hotpath", choices=["hotpath", "precompute", "integrate"],
+                    help="precompute: time ile_precompute (eq. 8: Q, U, V of --points intrinsic points); integrate: time ile_integrate "
+                         "(the adaptive Monte Carlo loop with on-device sampling) instead of the hot path")
+    ap.add_argument("--chunks", type=int, default=200, help="--stage integrate: chunks per step")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -256,6 +335,11 @@ def main():
         return
     if args.stage == "precompute":
         run_precompute(args, rank)
+        return
+    if args.stage == "integrate":
+        if args.steps > 20:
+            args.steps = 20
+        run_integrate(args, rank)
         return
 
     import numpy as np

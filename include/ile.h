@@ -51,6 +51,7 @@ typedef enum {
 #define ILE_MAX_DET 8    /* K */
 #define ILE_MAX_MODES 32 /* M */
 #define ILE_MAX_L 8      /* largest l of a mode */
+#define ILE_SAMPLER_MAX_BINS 512 /* histogram bins per adaptive dimension */
 
 typedef struct ile_ctx ile_ctx; /* opaque, owned by the library */
 
@@ -171,6 +172,76 @@ int ile_measure_fp64_peak(int32_t iters, double *tflops, double *ms);
 int ile_measure_dmma_peak(int32_t iters, double *tflops, double *ms);
 
 void ile_destroy(ile_ctx *ctx);
+
+/* ---------------------------------------------------------------------------------------------------------------------
+ * On-device Monte Carlo sampler.  PAPER.md eq. 4: Monte Carlo over the extrinsic
+ * parameters, prior uniform in volume and orientation, adaptive sampler of ref. [9]; L97: blocks of samples per likelihood
+ * call; L119, L125: sampling prior in the two sky parameters and distance, regenerated every n_chunk draws from the most
+ * recent chunk; L101: fixed threshold on n_eff; L251: random number generation on the GPU.  Ref. [9] is not part of the
+ * paper: the algorithm is this build's reading (S1-S9), restated in oracle/sampler.py.
+ *   S1 uniforms: Philox4x32-10, counters (index_lo, index_hi, j, 0), j = 0..3, key = seed; 53-bit uniforms in (0, 1)
+ *   S2 unit-cube coordinates: RA/2pi, (sin dec + 1)/2, (t_ref - t_lo)/(t_hi - t_lo), phi_ref/2pi, psi/pi,
+ *      (cos iota + 1)/2, (D^3 - Dmin^3)/(Dmax^3 - Dmin^3): the prior is uniform in them
+ *   S3 sampling prior: piecewise-constant densities h_d on n_bins equal bins for d in {RA, dec, distance} (those enabled),
+ *      every other dimension from the prior; ln w = -sum_d ln h_d[bin_d]
+ *   S6 refit: W_a = exp(temper (lnL_a + ln w_a - max)), H_d[b] = sum rint(W_a 2^40) (integers),
+ *      h_d[b] = (1 - floor) n_bins H_d[b] / sum_b H_d[b] + floor
+ * All sample arrays are device memory; a sampler belongs to the device current at creation and, like a context, serialises
+ * its own scratch (one stream at a time). */
+typedef struct ile_sampler ile_sampler;
+
+typedef struct {
+    uint64_t seed;        /* Philox key */
+    int32_t n_bins;       /* bins per adaptive dimension, 1..ILE_SAMPLER_MAX_BINS */
+    int32_t adapt_ra;     /* != 0: RA is adaptive */
+    int32_t adapt_dec;    /* != 0: declination is adaptive */
+    int32_t adapt_dist;   /* != 0: distance is adaptive */
+    double floor_frac;    /* share of the uniform density mixed into every refit density, [0, 1] */
+    double temper;        /* exponent of the refit weights, > 0 */
+    double dist_min_mpc;  /* prior range of the distance (uniform in volume) */
+    double dist_max_mpc;
+    double t_ref_lo_s;    /* prior range of t_ref (uniform); lo = hi fixes it */
+    double t_ref_hi_s;
+} ile_sampler_config;
+
+/* Create a sampler on the current device with uniform densities (the prior).  Synchronous. */
+int ile_sampler_create(ile_sampler **out, const ile_sampler_config *cfg);
+void ile_sampler_destroy(ile_sampler *s);
+
+/* Densities back to uniform (S9). */
+int ile_sampler_reset(ile_sampler *s, void *cuda_stream);
+
+/* Load densities: h host [3][n_bins] (RA, dec, distance; each should average 1), cumulatives rebuilt on the device.
+ * Synchronises the stream. */
+int ile_sampler_set_tables(ile_sampler *s, const double *h, void *cuda_stream);
+
+/* Read the densities h (host [3][n_bins]) and, if C is not NULL, the cumulatives (host [3][n_bins + 1]).  Synchronises. */
+int ile_sampler_get_tables(ile_sampler *s, double *h, double *C, void *cuda_stream);
+
+/* S1 only: the seven Philox uniforms of samples first_index .. first_index + n - 1 -> u device [n][7]. */
+int ile_sampler_uniforms(ile_sampler *s, int64_t first_index, int64_t n, double *u, void *cuda_stream);
+
+/* S1-S5: draw samples first_index .. first_index + n - 1 from the current sampling prior.  Outputs are device arrays of n
+ * doubles each, laid out as ile_eval reads them; log_w (may be NULL) = ln p - ln p_s, ready for ile_evidence;
+ * bin_idx (may be NULL): device int32 [n][3], the bin of each adaptive dimension (-1 where not adaptive), input of the refit. */
+int ile_sampler_draw(ile_sampler *s, int64_t first_index, int64_t n, double *ra, double *dec, double *t_ref, double *phi_ref,
+                     double *psi, double *incl, double *dist_mpc, double *log_w, int32_t *bin_idx, void *cuda_stream);
+
+/* S6: regenerate the sampling prior from one chunk: bin_idx as ile_sampler_draw wrote it, lnL_margT as ile_eval wrote it,
+ * log_w may be NULL (= 0).  A chunk without a finite sample leaves the densities unchanged. */
+int ile_sampler_refit(ile_sampler *s, int64_t n, const int32_t *bin_idx, const double *lnL_margT, const double *log_w,
+                      void *cuda_stream);
+
+/* Kernels launched on behalf of the sampler since creation. */
+int64_t ile_sampler_launch_count(const ile_sampler *s);
+
+/* S7-S8: the whole adaptive Monte Carlo integral of one intrinsic point on the device -- per chunk c: draw samples
+ * c n_chunk .. (c+1) n_chunk - 1, ile_eval, ile_evidence with the carried state, refit while c < n_adapt_chunks; stop after
+ * the first chunk with n_eff >= n_eff_min or after max_chunks.  Nothing but two doubles per chunk crosses the bus.
+ * The sampler's densities are reset first.  Host outputs: lnZ, n_eff (may be NULL), n_samples (may be NULL) = samples used,
+ * history (may be NULL): [max_chunks][2] running (lnZ, n_eff) after every chunk up to the stop.  Synchronous. */
+int ile_integrate(ile_ctx *ctx, ile_sampler *s, int32_t point, int64_t n_chunk, int32_t max_chunks, int32_t n_adapt_chunks,
+                  double n_eff_min, double *lnZ, double *n_eff, int64_t *n_samples, double *history, void *cuda_stream);
 
 /* Static string for an ile_error; for ILE_ERR_CUDA the message of the most recent CUDA failure in this thread. */
 const char *ile_strerror(int code);

@@ -29,7 +29,7 @@ S4  Draw: for an adaptive dimension, v = uniform i; cumulative C_d[0] = 0, C_d[b
     division and one addition per bin, in this order); b = the largest bin with C_d[b] <= v (clamped to n_bins - 1);
     u_d = (b + (v - C_d[b]) / (h_d[b] / n_bins)) / n_bins, clamped below 1.
 S5  Physical parameters: RA = 2 pi u0, dec = asin(2 u1 - 1), t_ref = t_lo + (t_hi - t_lo) u2, phi_ref = 2 pi u3,
-    psi = pi u4, iota = acos(2 u5 - 1), D = cbrt(Dmin^3 + u6 (Dmax^3 - Dmin^3)).
+    psi = pi u4, iota = acos(2 u5 - 1), D = cbrt(Dmin^3 + u6 (Dmax^3 - Dmin^3)) with X^3 = (X X) X.
 S6  Refit from the most recent chunk (L119): e_a = lnL_margT,a + ln w_a, M = max_a e_a, W_a = exp(temper * (e_a - M));
     per adaptive dimension the integer histogram H_d[b] = sum over the chunk's samples in bin b of rint(W_a * 2^40)
     (integers: the sum does not depend on the order); if sum_b H_d[b] = 0 (no finite sample) the density is kept;
@@ -124,7 +124,8 @@ def draw(cfg, h, first_index: int, n: int):
         bins[:, j] = b
         log_w -= np.log(h[j][b])
     two_pi = 2.0 * math.pi
-    dmin3, dmax3 = float(cfg["dist_min_mpc"]) ** 3, float(cfg["dist_max_mpc"]) ** 3
+    dmin, dmax = float(cfg["dist_min_mpc"]), float(cfg["dist_max_mpc"])
+    dmin3, dmax3 = dmin * dmin * dmin, dmax * dmax * dmax           # two multiplications each (S5)
     s = {
         "ra": two_pi * u[:, 0],
         "dec": np.arcsin(2.0 * u[:, 1] - 1.0),

@@ -20,7 +20,9 @@ _lib = None
 
 SAMPLE_FIELDS = ("ra", "dec", "t_ref", "phi_ref", "psi", "incl", "dist_mpc")
 EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_evidence_merge", "ile_precompute", "ile_run_host", "ile_run_host_all", "ile_status",
-           "ile_set_variant", "ile_launch_count", "ile_measure_fp64_peak", "ile_measure_dmma_peak", "ile_destroy", "ile_strerror")
+           "ile_set_variant", "ile_launch_count", "ile_measure_fp64_peak", "ile_measure_dmma_peak", "ile_destroy", "ile_strerror",
+           "ile_sampler_create", "ile_sampler_destroy", "ile_sampler_reset", "ile_sampler_set_tables", "ile_sampler_get_tables",
+           "ile_sampler_uniforms", "ile_sampler_draw", "ile_sampler_refit", "ile_sampler_launch_count", "ile_integrate")
 
 
 class IleError(RuntimeError):
@@ -32,6 +34,13 @@ class IleError(RuntimeError):
 
 class _Detector(ctypes.Structure):
     _fields_ = [("vertex_m", ctypes.c_double * 3), ("arm_x", ctypes.c_double * 3), ("arm_y", ctypes.c_double * 3)]
+
+
+class _SamplerConfig(ctypes.Structure):
+    _fields_ = [("seed", ctypes.c_uint64), ("n_bins", ctypes.c_int32), ("adapt_ra", ctypes.c_int32), ("adapt_dec", ctypes.c_int32),
+                ("adapt_dist", ctypes.c_int32), ("floor_frac", ctypes.c_double), ("temper", ctypes.c_double),
+                ("dist_min_mpc", ctypes.c_double), ("dist_max_mpc", ctypes.c_double), ("t_ref_lo_s", ctypes.c_double),
+                ("t_ref_hi_s", ctypes.c_double)]
 
 
 class _Config(ctypes.Structure):
@@ -71,7 +80,9 @@ def load():
     L.ile_strerror.argtypes = [ctypes.c_int]
     L.ile_strerror.restype = ctypes.c_char_p
     for name in EXPORTS:
-        if name not in ("ile_launch_count", "ile_destroy", "ile_strerror"):
+        if name not in ("ile_launch_count", "ile_destroy", "ile_strerror",
+           "ile_sampler_create", "ile_sampler_destroy", "ile_sampler_reset", "ile_sampler_set_tables", "ile_sampler_get_tables",
+           "ile_sampler_uniforms", "ile_sampler_draw", "ile_sampler_refit", "ile_sampler_launch_count", "ile_integrate"):
             getattr(L, name).restype = ctypes.c_int
     _lib = L
     return L
@@ -267,6 +278,89 @@ class Context:
         if code not in (0, -5):
             raise IleError(code, "ile_status")
         return int(v.value), code
+
+
+class Sampler:
+    """Owns one ile_sampler (NEXT-2).  cfg: dict(seed, n_bins, adapt (RA, dec, distance), floor_frac, temper, dist_min_mpc,
+    dist_max_mpc, t_ref_lo_s, t_ref_hi_s)."""
+
+    def __init__(self, cfg):
+        self.n_bins = int(cfg["n_bins"])
+        c = _SamplerConfig(int(cfg["seed"]), self.n_bins, int(bool(cfg["adapt"][0])), int(bool(cfg["adapt"][1])),
+                           int(bool(cfg["adapt"][2])), float(cfg["floor_frac"]), float(cfg["temper"]), float(cfg["dist_min_mpc"]),
+                           float(cfg["dist_max_mpc"]), float(cfg["t_ref_lo_s"]), float(cfg["t_ref_hi_s"]))
+        self._h = ctypes.c_void_p()
+        _check(load().ile_sampler_create(ctypes.byref(self._h), ctypes.byref(c)), "ile_sampler_create")
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h.value:
+            load().ile_sampler_destroy(self._h)
+            self._h = ctypes.c_void_p()
+
+    __del__ = close
+
+    @property
+    def launch_count(self) -> int:
+        return int(load().ile_sampler_launch_count(self._h))
+
+    def reset(self, stream=None):
+        _check(load().ile_sampler_reset(self._h, _stream_ptr(stream)), "ile_sampler_reset")
+
+    def set_tables(self, h, stream=None):
+        import numpy as np
+
+        h = np.ascontiguousarray(h, dtype=np.float64)
+        assert h.shape == (3, self.n_bins)
+        _check(load().ile_sampler_set_tables(self._h, ctypes.c_void_p(h.ctypes.data), _stream_ptr(stream)), "ile_sampler_set_tables")
+
+    def get_tables(self, stream=None):
+        import numpy as np
+
+        h, C = np.empty((3, self.n_bins)), np.empty((3, self.n_bins + 1))
+        _check(load().ile_sampler_get_tables(self._h, ctypes.c_void_p(h.ctypes.data), ctypes.c_void_p(C.ctypes.data),
+                                             _stream_ptr(stream)), "ile_sampler_get_tables")
+        return h, C
+
+    def uniforms(self, first_index: int, n: int, stream=None):
+        import torch
+
+        u = torch.empty((n, 7), dtype=torch.float64, device="cuda")
+        _check(load().ile_sampler_uniforms(self._h, int(first_index), int(n), _ptr(u), _stream_ptr(stream)), "ile_sampler_uniforms")
+        return u
+
+    def draw(self, first_index: int, n: int, stream=None):
+        """-> (samples dict of CUDA float64 [n] as Context.eval takes it, log_w [n], bin_idx int32 [n][3])."""
+        import torch
+
+        s = {f: torch.empty(n, dtype=torch.float64, device="cuda") for f in SAMPLE_FIELDS}
+        lw = torch.empty(n, dtype=torch.float64, device="cuda")
+        bins = torch.empty((n, 3), dtype=torch.int32, device="cuda")
+        _check(load().ile_sampler_draw(self._h, int(first_index), int(n), *[_ptr(s[f]) for f in SAMPLE_FIELDS], _ptr(lw), _ptr(bins),
+                                       _stream_ptr(stream)), "ile_sampler_draw")
+        return s, lw, bins
+
+    def refit(self, bins, lnL, log_w=None, stream=None):
+        import torch
+
+        n = lnL.numel()
+        assert bins.is_cuda and bins.dtype == torch.int32 and bins.is_contiguous() and bins.numel() == 3 * n
+        assert lnL.is_cuda and lnL.dtype == torch.float64 and lnL.is_contiguous()
+        assert log_w is None or (log_w.is_cuda and log_w.dtype == torch.float64 and log_w.is_contiguous() and log_w.numel() == n)
+        _check(load().ile_sampler_refit(self._h, n, _ptr(bins), _ptr(lnL), _ptr(log_w), _stream_ptr(stream)), "ile_sampler_refit")
+
+
+def integrate(ctx: "Context", sampler: "Sampler", n_chunk: int, max_chunks: int, n_adapt_chunks: int, n_eff_min: float,
+              point: int = 0, stream=None):
+    """ile_integrate: the adaptive Monte Carlo loop on the device -> dict(lnZ, n_eff, n_samples, n_chunks, history [c][2])."""
+    import numpy as np
+
+    lnZ, neff, ns = ctypes.c_double(0.0), ctypes.c_double(0.0), ctypes.c_int64(0)
+    hist = np.zeros((int(max_chunks), 2))
+    _check(load().ile_integrate(ctx._h, sampler._h, int(point), int(n_chunk), int(max_chunks), int(n_adapt_chunks), float(n_eff_min),
+                                ctypes.byref(lnZ), ctypes.byref(neff), ctypes.byref(ns), ctypes.c_void_p(hist.ctypes.data),
+                                _stream_ptr(stream)), "ile_integrate")
+    nc = int(ns.value) // int(n_chunk)
+    return dict(lnZ=lnZ.value, n_eff=neff.value, n_samples=int(ns.value), n_chunks=nc, history=hist[:nc])
 
 
 def precompute(x, d, fs_hz: float, t0_q_s: float, stream=None):

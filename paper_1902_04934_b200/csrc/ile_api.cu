@@ -50,6 +50,8 @@ static int cuda_fail(cudaError_t e)
     snprintf(g_cuda_msg, sizeof(g_cuda_msg), "CUDA error %d: %s", (int)e, cudaGetErrorString(e));
     return ILE_ERR_CUDA;
 }
+int ile_cuda_fail(cudaError_t e) { return cuda_fail(e); }  // for the other translation units of the C ABI
+int ile_ctx_sm_count(const ile_ctx *c);
 // Function attributes, streams and every buffer of a context belong to the device it was created on.
 static int check_device(const ile_ctx *c)
 {
@@ -616,6 +618,8 @@ extern "C" int ile_set_variant(ile_ctx *c, int32_t variant)
 }
 
 extern "C" int64_t ile_launch_count(const ile_ctx *c) { return c ? (int64_t)c->launches : 0; }
+int ile_ctx_sm_count(const ile_ctx *c) { return c->sz.sm_count; }
+void ile_ctx_add_launches(ile_ctx *c, int n) { c->launches += n; }
 
 static int measure_peak(int32_t iters, int dmma, double *tflops, double *ms)
 {

@@ -111,6 +111,29 @@ void ile_quad_pack_host(int32_t n_points, int32_t K, int32_t M, const double2 *U
 cudaError_t ile_launch_quad_mma(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const double *mats, double *qform,
                                 cudaStream_t st);
 
+// ---- shared by the translation units of the C ABI (ile_api.cu, ile_sampler_api.cu) -----------------------------------------
+int ile_cuda_fail(cudaError_t e);  // records the message for ile_strerror, returns ILE_ERR_CUDA
+int ile_ctx_sm_count(const ile_ctx *c);
+void ile_ctx_add_launches(ile_ctx *c, int n);
+
+// ---- on-device Monte Carlo sampler (ile_sampler.cu; NEXT-2) ------------------------------------------------------------
+struct IleSamplerParams {
+    unsigned long long seed;
+    int32_t n_bins;
+    int32_t adapt[3];  // RA, dec, distance
+    double floor_frac, temper;
+    double t_lo, t_span;      // t_ref = t_lo + t_span u
+    double dmin3, d3_span;    // D = cbrt(dmin3 + u d3_span), dmin3 = Dmin Dmin Dmin
+};
+size_t ile_sampler_table_doubles(int32_t n_bins);  // h [3][n_bins] followed by C [3][n_bins + 1]
+cudaError_t ile_launch_sampler_tables(const IleSamplerParams &P, double *tab, int set_uniform, cudaStream_t st);
+cudaError_t ile_launch_sampler_uniforms(const IleSamplerParams &P, int sm_count, long long first, long long n, double *u, cudaStream_t st);
+cudaError_t ile_launch_sampler_draw(const IleSamplerParams &P, int sm_count, const double *tab, long long first, long long n, double *ra,
+                                    double *dec, double *t_ref, double *phi_ref, double *psi, double *incl, double *dist, double *log_w,
+                                    int32_t *bins, cudaStream_t st);
+cudaError_t ile_launch_sampler_refit(const IleSamplerParams &P, double *tab, long long n, const int32_t *bins, const double *lnL,
+                                     const double *log_w, cudaStream_t st);
+
 // overlap pre-computation (ile_precompute.cu)
 cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_t N, double fs_hz, double t0_q_s, const double2 *x,
                                   const double2 *d, double2 *Q, double2 *U, double2 *V, int32_t max_smem_optin, cudaStream_t st);
