@@ -79,11 +79,22 @@ def load():
     L.ile_destroy.restype = None
     L.ile_strerror.argtypes = [ctypes.c_int]
     L.ile_strerror.restype = ctypes.c_char_p
+    L.ile_sampler_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(_SamplerConfig)]
+    L.ile_sampler_destroy.argtypes = [vp]
+    L.ile_sampler_destroy.restype = None
+    L.ile_sampler_reset.argtypes = [vp, vp]
+    L.ile_sampler_set_tables.argtypes = [vp, vp, vp]
+    L.ile_sampler_get_tables.argtypes = [vp, vp, vp, vp]
+    L.ile_sampler_uniforms.argtypes = [vp, i64, i64, vp, vp]
+    L.ile_sampler_draw.argtypes = [vp, i64, i64] + [vp] * 7 + [vp, vp, vp]
+    L.ile_sampler_refit.argtypes = [vp, i64, vp, vp, vp, vp]
+    L.ile_sampler_launch_count.argtypes = [vp]
+    L.ile_sampler_launch_count.restype = i64
+    L.ile_integrate.argtypes = [vp, vp, i32, i64, i32, i32, ctypes.c_double, dp, dp, ctypes.POINTER(i64), vp, vp]
     for name in EXPORTS:
-        if name not in ("ile_launch_count", "ile_destroy", "ile_strerror",
-           "ile_sampler_create", "ile_sampler_destroy", "ile_sampler_reset", "ile_sampler_set_tables", "ile_sampler_get_tables",
-           "ile_sampler_uniforms", "ile_sampler_draw", "ile_sampler_refit", "ile_sampler_launch_count", "ile_integrate"):
+        if name not in ("ile_launch_count", "ile_destroy", "ile_strerror", "ile_sampler_destroy", "ile_sampler_launch_count"):
             getattr(L, name).restype = ctypes.c_int
+        assert getattr(L, name).argtypes is not None, name
     _lib = L
     return L
 
