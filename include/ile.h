@@ -171,6 +171,32 @@ int ile_measure_fp64_peak(int32_t iters, double *tflops, double *ms);
  * larger of the two measurements as the roofline denominator. */
 int ile_measure_dmma_peak(int32_t iters, double *tflops, double *ms);
 
+/* ---------------------------------------------------------------------------------------------------------------------
+ * Extrinsic posterior harvesting.  PAPER.md L265: "The code also produces reliable extrinsic parameter
+ * distributions ... we harvest joint intrinsic and extrinsic information with a single final iteration."  Readings H1-H3 of
+ * DESIGN.md "NEXT-3", restated in oracle/harvest.py.
+ *
+ * H1 ile_resample: equal-weight posterior samples of the Monte Carlo parameters by SYSTEMATIC resampling of n draws with weights
+ * W_a = exp(lnL_margT[a] + log_w[a]) (eq. 4's integrand): output i (i = 0..n_out-1) is the smallest a whose inclusive cumulative
+ * weight, accumulated in sample order and normalised, exceeds (i + v0) / n_out; v0 in [0, 1) is the caller's single uniform.
+ * lnL_margT, log_w (may be NULL): device, n doubles; ids_out: device int64 [n_out], non-decreasing; every entry -1 when no
+ * sample has a finite weight. */
+int ile_resample(ile_ctx *ctx, int64_t n, const double *lnL_margT, const double *log_w, int64_t n_out, double v0,
+                 int64_t *ids_out, void *cuda_stream);
+
+/* H2, H3 ile_harvest: for n_sel harvested samples of intrinsic point `point` -- sample ids[i] of the n-sample device arrays
+ * (ids device int64 [n_sel], e.g. from ile_resample; NULL = samples 0..n_sel-1) -- the lnL_j series of eq. 7 over the sample's
+ * window is evaluated once more and reduced to
+ *   argmax_bin[i]  the first bin j* of the largest lnL_j and lnL_max[i] = lnL_{j*}   (maximised over time instead of eq. 9's average)
+ *   drawn_bin[i]   (may be NULL) the smallest bin whose inclusive cumulative of exp(lnL_j) reaches v_uniform[i] times the total:
+ *                  a draw of the arrival time from eq. 9's normalised integrand; v_uniform: device, n_sel doubles in (0, 1)
+ * Bin j of a sample means the geocentric time t_ref + (j - floor(N_t/2)) / f_s.  A sample whose window leaves the stored Q
+ * (reading R9) or an id outside [0, n) gives -1, -inf, -1.  All outputs device, n_sel entries. */
+int ile_harvest(ile_ctx *ctx, int32_t point, int64_t n, const double *ra, const double *dec, const double *t_ref,
+                const double *phi_ref, const double *psi, const double *incl, const double *dist_mpc, int64_t n_sel,
+                const int64_t *ids, const double *v_uniform, int32_t *argmax_bin, double *lnL_max, int32_t *drawn_bin,
+                void *cuda_stream);
+
 void ile_destroy(ile_ctx *ctx);
 
 /* ---------------------------------------------------------------------------------------------------------------------

@@ -22,7 +22,8 @@ SAMPLE_FIELDS = ("ra", "dec", "t_ref", "phi_ref", "psi", "incl", "dist_mpc")
 EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_evidence_merge", "ile_precompute", "ile_run_host", "ile_run_host_all", "ile_status",
            "ile_set_variant", "ile_launch_count", "ile_measure_fp64_peak", "ile_measure_dmma_peak", "ile_destroy", "ile_strerror",
            "ile_sampler_create", "ile_sampler_destroy", "ile_sampler_reset", "ile_sampler_set_tables", "ile_sampler_get_tables",
-           "ile_sampler_uniforms", "ile_sampler_draw", "ile_sampler_refit", "ile_sampler_launch_count", "ile_integrate")
+           "ile_sampler_uniforms", "ile_sampler_draw", "ile_sampler_refit", "ile_sampler_launch_count", "ile_integrate",
+           "ile_resample", "ile_harvest")
 
 
 class IleError(RuntimeError):
@@ -91,6 +92,8 @@ def load():
     L.ile_sampler_launch_count.argtypes = [vp]
     L.ile_sampler_launch_count.restype = i64
     L.ile_integrate.argtypes = [vp, vp, i32, i64, i32, i32, ctypes.c_double, dp, dp, ctypes.POINTER(i64), vp, vp]
+    L.ile_resample.argtypes = [vp, i64, vp, vp, i64, ctypes.c_double, vp, vp]
+    L.ile_harvest.argtypes = [vp, i32, i64] + [vp] * 7 + [i64, vp, vp, vp, vp, vp, vp]
     for name in EXPORTS:
         if name not in ("ile_launch_count", "ile_destroy", "ile_strerror", "ile_sampler_destroy", "ile_sampler_launch_count"):
             getattr(L, name).restype = ctypes.c_int
@@ -281,6 +284,33 @@ class Context:
         _check(load().ile_run_host_all(self._h, n, *[_ptr(t) for t in ts], _ptr(log_w_host), _ptr(out), lnZ.ctypes.data_as(dp),
                                        neff.ctypes.data_as(dp), _stream_ptr(stream)), "ile_run_host_all")
         return out, lnZ, neff
+
+    def resample(self, lnL, log_w, n_out: int, v0: float, stream=None):
+        """ile_resample: -> CUDA int64 [n_out] sample ids (systematic resampling by w L_margT)."""
+        import torch
+
+        assert lnL.is_cuda and lnL.dtype == torch.float64 and lnL.is_contiguous()
+        assert log_w is None or (log_w.is_cuda and log_w.dtype == torch.float64 and log_w.is_contiguous() and log_w.numel() == lnL.numel())
+        ids = torch.empty(int(n_out), dtype=torch.int64, device=lnL.device)
+        _check(load().ile_resample(self._h, lnL.numel(), _ptr(lnL), _ptr(log_w), int(n_out), float(v0), _ptr(ids),
+                                   _stream_ptr(stream)), "ile_resample")
+        return ids
+
+    def harvest(self, samples, ids=None, v=None, point: int = 0, stream=None):
+        """ile_harvest: -> (argmax_bin int32 [n_sel], lnL_max [n_sel], drawn_bin int32 [n_sel] or None)."""
+        import torch
+
+        ptrs, n = self._sample_ptrs(samples)
+        n_sel = n if ids is None else ids.numel()
+        assert ids is None or (ids.is_cuda and ids.dtype == torch.int64 and ids.is_contiguous())
+        assert v is None or (v.is_cuda and v.dtype == torch.float64 and v.is_contiguous() and v.numel() == n_sel)
+        dev = samples["ra"].device
+        amax = torch.empty(n_sel, dtype=torch.int32, device=dev)
+        lmax = torch.empty(n_sel, dtype=torch.float64, device=dev)
+        drawn = torch.empty(n_sel, dtype=torch.int32, device=dev) if v is not None else None
+        _check(load().ile_harvest(self._h, int(point), n, *ptrs, n_sel, _ptr(ids), _ptr(v), _ptr(amax), _ptr(lmax), _ptr(drawn),
+                                  _stream_ptr(stream)), "ile_harvest")
+        return amax, lmax, drawn
 
     def status(self, reset: bool = False, stream=None):
         """ile_status: (n_out_of_range, code).  Synchronises the stream."""

@@ -39,6 +39,8 @@ struct ile_ctx {
     double *d_quad_mats;  // packed real representations of U, V for the FP64-MMA quadratic forms (M >= ILE_QUAD_MMA_MIN_MODES)
     double *d_qform;      // [n][K][3]
     size_t qform_cap;     // samples
+    double *d_resample;   // scratch of ile_resample
+    size_t resample_cap;  // doubles
     cudaStream_t copy_stream;  // ile_run_host: second H2D queue
     cudaEvent_t ev_copy_go, ev_copy_done;
 };
@@ -255,6 +257,7 @@ extern "C" void ile_destroy(ile_ctx *c)
     cudaFree(c->ss.gorder);
     cudaFree(c->d_quad_mats);
     cudaFree(c->d_qform);
+    cudaFree(c->d_resample);
     if (c->ss.aux) cudaStreamDestroy(c->ss.aux);
     if (c->ss.ev_fork) cudaEventDestroy(c->ss.ev_fork);
     if (c->ss.ev_join) cudaEventDestroy(c->ss.ev_join);
@@ -588,6 +591,53 @@ extern "C" int ile_run_host_all(ile_ctx *c, int64_t n_per_point, const double *r
     if (int r = check_device(c)) return r;
     const double *src[8] = {ra, dec, t_ref, phi_ref, psi, incl, dist_mpc, log_w};
     return run_host(c, 0, c->n_points, n_per_point, src, lnL_margT, lnZ, n_eff, (cudaStream_t)cuda_stream);
+}
+
+extern "C" int ile_resample(ile_ctx *c, int64_t n, const double *lnL_margT, const double *log_w, int64_t n_out, double v0,
+                            int64_t *ids_out, void *cuda_stream)
+{
+    if (!c || n < 0 || n_out < 0 || !(v0 >= 0.0) || !(v0 < 1.0)) return ILE_ERR_BAD_ARGUMENT;
+    if (n_out == 0) return ILE_OK;
+    if (n == 0 || !lnL_margT || !ids_out) return ILE_ERR_BAD_ARGUMENT;
+    if (int r = check_device(c)) return r;
+    cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t need = ile_resample_scratch_doubles(n);
+    if (need > c->resample_cap) {
+        CK(cudaStreamSynchronize(st));
+        cudaFree(c->d_resample);
+        c->d_resample = nullptr, c->resample_cap = 0;
+        CK(cudaMalloc(&c->d_resample, need * sizeof(double)));
+        c->resample_cap = need;
+    }
+    int nl = 0;
+    cudaError_t e = ile_launch_resample(c->sz, n, lnL_margT, log_w, n_out, v0, c->d_resample, reinterpret_cast<long long *>(ids_out), st, &nl);
+    c->launches += nl;
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ILE_OK;
+}
+
+extern "C" int ile_harvest(ile_ctx *c, int32_t point, int64_t n, const double *ra, const double *dec, const double *t_ref,
+                           const double *phi_ref, const double *psi, const double *incl, const double *dist_mpc, int64_t n_sel,
+                           const int64_t *ids, const double *v_uniform, int32_t *argmax_bin, double *lnL_max, int32_t *drawn_bin,
+                           void *cuda_stream)
+{
+    if (!c || n < 0 || n_sel < 0 || point < 0 || point >= c->n_points) return ILE_ERR_BAD_ARGUMENT;
+    if (n_sel == 0) return ILE_OK;
+    if (!ra || !dec || !t_ref || !phi_ref || !psi || !incl || !dist_mpc || !argmax_bin || !lnL_max) return ILE_ERR_BAD_ARGUMENT;
+    if (drawn_bin && !v_uniform) return ILE_ERR_BAD_ARGUMENT;
+    if (!ids && n_sel > n) return ILE_ERR_BAD_ARGUMENT;
+    if (int r = check_device(c)) return r;
+    IleEvalArgs a;
+    a.params = c->dparams;
+    a.Q = c->dQ, a.U = c->dU, a.V = c->dV;
+    a.point0 = point, a.n_points = 1, a.n_per_point = n;
+    a.ra = ra, a.dec = dec, a.t_ref = t_ref, a.phi_ref = phi_ref, a.psi = psi, a.incl = incl, a.dist = dist_mpc;
+    a.lnL = nullptr, a.shift_idx = nullptr, a.oob_counter = c->d_oob;
+    cudaError_t e = ile_launch_harvest(c->sz, a, n_sel, reinterpret_cast<const long long *>(ids), v_uniform, argmax_bin, lnL_max, drawn_bin,
+                                       (cudaStream_t)cuda_stream);
+    c->launches += 1;
+    if (e != cudaSuccess) return cuda_fail(e);
+    return ILE_OK;
 }
 
 extern "C" int ile_status(ile_ctx *c, int64_t *n_out_of_range, int reset, void *cuda_stream)

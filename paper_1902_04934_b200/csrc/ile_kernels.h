@@ -134,6 +134,13 @@ cudaError_t ile_launch_sampler_draw(const IleSamplerParams &P, int sm_count, con
 cudaError_t ile_launch_sampler_refit(const IleSamplerParams &P, double *tab, long long n, const int32_t *bins, const double *lnL,
                                      const double *log_w, cudaStream_t st);
 
+// ---- extrinsic posterior harvesting (ile_harvest.cu; NEXT-3) -------------------------------------------------------------
+cudaError_t ile_launch_harvest(const IleSizes &sz, const IleEvalArgs &a, long long n_sel, const long long *ids, const double *v_uniform,
+                               int32_t *argmax_bin, double *lnL_max, int32_t *drawn_bin, cudaStream_t st);
+size_t ile_resample_scratch_doubles(long long n);
+cudaError_t ile_launch_resample(const IleSizes &sz, long long n, const double *lnL, const double *log_w, long long n_out, double v0,
+                                double *scratch, long long *ids, cudaStream_t st, int *n_launches);
+
 // overlap pre-computation (ile_precompute.cu)
 cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_t N, double fs_hz, double t0_q_s, const double2 *x,
                                   const double2 *d, double2 *Q, double2 *U, double2 *V, int32_t max_smem_optin, cudaStream_t st);
