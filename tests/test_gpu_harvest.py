@@ -60,7 +60,7 @@ def test_harvest_matches_the_oracle_series(gpu_lib, cid):
     n = 600 if cid < 2 else 150
     cfg = gi.make_config(cid, n=n)
     s = gi.make_samples(cfg["sample_seeds"][0] + 3, n)
-    s["t_ref"][11] = 0.4                                   # out of range: -1 / -inf / -1
+    s["t_ref"][11] = 0.9                                   # out of range: -1 / -inf / -1
     rng = np.random.default_rng(cid)
     v = rng.random(n)
     ctx = gpu_lib.Context(cfg)
