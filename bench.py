@@ -293,7 +293,8 @@ def run_integrate(args, rank: int):
 
 
 def workload_config(cfg, n, args, extra=None):
-    c = {"workload": f"BASELINE.json configs[{cfg['config_id']}]: {cfg['n_det']} detectors ({','.join(cfg['dets'])}), "
+    src = f"BASELINE.json configs[{cfg['config_id']}]" if cfg["config_id"] <= 4 else f"paper window config {cfg['config_id']} (NEXT-4: T = 0.3 s, PAPER.md L86, L121)"
+    c = {"workload": f"{src}: {cfg['n_det']} detectors ({','.join(cfg['dets'])}), "
                      f"{cfg['n_modes']} modes (l<= {int(max(cfg['l']))}), Q {cfg['n_q']} complex128 @ {int(cfg['fs_hz'])} Hz, "
                      f"{cfg['n_points']} intrinsic point(s) x {n} extrinsic samples/step/GPU, {cfg['n_t']} time bins",
          "n_det": cfg["n_det"], "n_modes": cfg["n_modes"], "n_q": cfg["n_q"], "n_t": cfg["n_t"],

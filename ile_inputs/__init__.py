@@ -66,6 +66,16 @@ CONFIGS = {
             snr=20.0, admix=0.0, sweep=(1_000, 10_000, 100_000, 1_000_000, 10_000_000)),
     4: dict(dets=("H1", "L1", "V1"), modes=modes_up_to(2), n_q=2048, n_t=410, n=100_000, n_points=256,
             snr=(8.0, 40.0), admix=0.0),
+    # the paper's own window and rates (not BASELINE.json configs): T = 0.3 s, two
+    # detectors (L109), modes (2,+-2) or (2,+-2),(2,+-1) (Tables I/II, L143-L159), at 4096 Hz and at the legacy 16384 Hz (L121)
+    5: dict(dets=("H1", "L1"), modes=[(2, -2), (2, 2)], n_q=8192, n_t=1229, n=100_000, n_points=1, snr=20.0, admix=0.0,
+            fs_hz=4096.0),
+    6: dict(dets=("H1", "L1"), modes=[(2, -2), (2, -1), (2, 1), (2, 2)], n_q=8192, n_t=1229, n=100_000, n_points=1, snr=20.0,
+            admix=0.0, fs_hz=4096.0),
+    7: dict(dets=("H1", "L1"), modes=[(2, -2), (2, 2)], n_q=32768, n_t=4915, n=100_000, n_points=1, snr=20.0, admix=0.0,
+            fs_hz=16384.0),
+    8: dict(dets=("H1", "L1"), modes=[(2, -2), (2, -1), (2, 1), (2, 2)], n_q=32768, n_t=4915, n=100_000, n_points=1, snr=20.0,
+            admix=0.0, fs_hz=16384.0),
 }
 
 SAMPLE_FIELDS = ("ra", "dec", "t_ref", "phi_ref", "psi", "incl", "dist_mpc")
@@ -224,7 +234,7 @@ def make_config(config_id: int, *, n: int | None = None, n_points: int | None = 
             snr = float(np.random.Generator(np.random.PCG64(seed + 250)).uniform(lo, hi))
         else:
             snr = c["snr"]
-        Q, U, V, meta = make_point(seed, c["dets"], c["modes"], c["n_q"], snr, admix=c["admix"])
+        Q, U, V, meta = make_point(seed, c["dets"], c["modes"], c["n_q"], snr, admix=c["admix"], fs_hz=c.get("fs_hz", FS_HZ))
         Qs.append(Q), Us.append(U), Vs.append(V), metas.append(meta), sseeds.append(seed + 500)
     v, ax, ay = detector_arrays(c["dets"])
     return dict(
@@ -232,6 +242,6 @@ def make_config(config_id: int, *, n: int | None = None, n_points: int | None = 
         Q=np.ascontiguousarray(np.stack(Qs)), U=np.ascontiguousarray(np.stack(Us)), V=np.ascontiguousarray(np.stack(Vs)),
         l=np.array([lm[0] for lm in c["modes"]], dtype=np.int32), m=np.array([lm[1] for lm in c["modes"]], dtype=np.int32),
         n_points=P, n_det=len(c["dets"]), n_modes=len(c["modes"]), n_q=c["n_q"], n_t=c["n_t"],
-        fs_hz=FS_HZ, t0_q_s=metas[0]["t0_q_s"], gmst_rad=GMST_RAD, d_ref_mpc=D_REF_MPC,
+        fs_hz=c.get("fs_hz", FS_HZ), t0_q_s=metas[0]["t0_q_s"], gmst_rad=GMST_RAD, d_ref_mpc=D_REF_MPC,
         vertex_m=v, arm_x=ax, arm_y=ay, n=c["n"] if n is None else n, sample_seeds=sseeds, meta=metas,
     )

@@ -516,3 +516,22 @@ def test_evidence_layouts_on_one_context(gpu_lib):
             assert rel_err([rZ], lnZ[g:g + 1].cpu().numpy()) <= TOL, (n_seg, per, g)
             assert rel_err([rN], neff[g:g + 1].cpu().numpy()) <= TOL, (n_seg, per, g)
     ctx.close()
+
+
+# ---------------------------------------------------------------------------------------------- NEXT-4: the paper's own windows
+@pytest.mark.parametrize("n", [1_500, 20_000])
+@pytest.mark.parametrize("cid", [5, 6, 7, 8])
+def test_paper_windows_T03s_at_4096_and_16384_Hz(gpu_lib, cid, n):
+    """T = 0.3 s with two detectors and 2 or 4 modes (Tables I/II) at 4096 Hz (N_t = 1229,
+    N_Q = 8192) and at the legacy 16384 Hz (N_t = 4915, N_Q = 32768; L121).  1,500 samples take the small-batch kernels,
+    20,000 the sorted streaming FP64-MMA path."""
+    cfg = gi.make_config(cid, n=n)
+    s = gi.make_samples(cfg["sample_seeds"][0], n)
+    full_compare(gpu_lib, cfg, s)
+
+
+def test_paper_window_concentrated_batch_16384_Hz(gpu_lib):
+    """Late-in-the-run shape at the legacy rate: samples crowded around one point (a handful of sort cells, long windows)."""
+    cfg = gi.make_config(8, n=20_000)
+    s = gi.make_concentrated_samples(5150, 20_000)
+    full_compare(gpu_lib, cfg, s, log_w=gi.make_log_weights(2, 20_000))
