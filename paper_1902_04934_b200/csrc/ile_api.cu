@@ -28,14 +28,13 @@ struct ile_ctx {
     int64_t chunk_samples;  // samples per launch group (bounds the scratch: <= 2 GiB of records, <= 2^20 samples)
     IleSortScratch sc;
     size_t sc_samples, sc_hist;  // capacities (samples, histogram words)
-    int32_t sc_points;
     int32_t sc_recg;             // doubles per record the scratch was sized for
     bool stream_ok;
     IleStreamPlan spl;
     IleSortPlan ssp;
     double *dQs;
     IleStreamScratch ss;
-    size_t ss_slots, ss_adj, ss_gcum, ss_gorder;  // capacities in words
+    size_t ss_slots, ss_gcum;  // capacities in words
     double *d_quad_mats;  // packed real representations of U, V for the FP64-MMA quadratic forms (M >= ILE_QUAD_MMA_MIN_MODES)
     double *d_qform;      // [n][K][3]
     size_t qform_cap;     // samples
@@ -249,12 +248,9 @@ extern "C" void ile_destroy(ile_ctx *c)
     cudaFree(c->sc.i0);
     cudaFree(c->sc.cell);
     cudaFree(c->sc.hist);
-    cudaFree(c->sc.ngood);
     cudaFree(c->dQs);
     cudaFree(c->ss.slots);
-    cudaFree(c->ss.adj);
     cudaFree(c->ss.gcum);
-    cudaFree(c->ss.gorder);
     cudaFree(c->d_quad_mats);
     cudaFree(c->d_qform);
     cudaFree(c->d_resample);
@@ -270,7 +266,7 @@ extern "C" void ile_destroy(ile_ctx *c)
 
 // Scratch of the sorted path, grown on demand (never inside a launch sequence that still uses the old buffers: the
 // stream is synchronised first).
-static int ensure_scratch(ile_ctx *c, size_t samples, size_t hist_words, int32_t points, cudaStream_t st)
+static int ensure_scratch(ile_ctx *c, size_t samples, size_t hist_words, cudaStream_t st)
 {
     if (samples > c->sc_samples) {
         CK(cudaStreamSynchronize(st));
@@ -291,14 +287,6 @@ static int ensure_scratch(ile_ctx *c, size_t samples, size_t hist_words, int32_t
         CK(cudaMalloc(&c->sc.hist, hist_words * sizeof(uint32_t)));
         c->sc_hist = hist_words;
     }
-    if (points > c->sc_points) {
-        CK(cudaStreamSynchronize(st));
-        cudaFree(c->sc.ngood);
-        c->sc.ngood = nullptr;
-        c->sc_points = 0;
-        CK(cudaMalloc(&c->sc.ngood, (size_t)points * sizeof(int32_t)));
-        c->sc_points = points;
-    }
     return ILE_OK;
 }
 
@@ -308,29 +296,16 @@ static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
     const IleSortPlan &sp = c->ssp;
     const size_t nseg = (size_t)sp.n1 * sp.n2;
     const int64_t slot_cap = (((a.n_per_point + 7) & ~(int64_t)7) + 8 * (int64_t)nseg + 31) & ~(int64_t)31;  // groups per point: multiple of 4
-    int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES + 1, a.n_points, st);
+    int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * (sp.ncell + nseg) + ILE_STREAM_MAX_RANGES, st);
     if (r != ILE_OK) return r;
-    const size_t need_slots = (size_t)a.n_points * slot_cap, need_adj = (size_t)a.n_points * nseg, need_g = 2 * (size_t)a.n_points + 2;
-    const size_t need_go = need_slots / 8;
-    if (need_slots > c->ss_slots || need_adj > c->ss_adj || need_g > c->ss_gcum || need_go > c->ss_gorder) {
+    const size_t need_slots = (size_t)a.n_points * slot_cap, need_g = 2 * (size_t)a.n_points + 2;
+    if (need_slots > c->ss_slots || need_g > c->ss_gcum) {
         CK(cudaStreamSynchronize(st));
         if (need_slots > c->ss_slots) {
             cudaFree(c->ss.slots);
             c->ss.slots = nullptr, c->ss_slots = 0;
             CK(cudaMalloc(&c->ss.slots, need_slots * sizeof(int32_t)));
             c->ss_slots = need_slots;
-        }
-        if (need_adj > c->ss_adj) {
-            cudaFree(c->ss.adj);
-            c->ss.adj = nullptr, c->ss_adj = 0;
-            CK(cudaMalloc(&c->ss.adj, need_adj * sizeof(int32_t)));
-            c->ss_adj = need_adj;
-        }
-        if (need_go > c->ss_gorder) {
-            cudaFree(c->ss.gorder);
-            c->ss.gorder = nullptr, c->ss_gorder = 0;
-            CK(cudaMalloc(&c->ss.gorder, need_go * sizeof(int32_t)));
-            c->ss_gorder = need_go;
         }
         if (need_g > c->ss_gcum) {
             cudaFree(c->ss.gcum);

@@ -37,8 +37,10 @@
 #include "ile_kernels.h"
 
 #define ST_FULL 0xffffffffu
-#define ST_TAB 1024
+#ifndef ST_TAB_LOG2
 #define ST_TAB_LOG2 10
+#endif
+#define ST_TAB (1 << ST_TAB_LOG2)
 #ifndef ST_THREADS
 #define ST_THREADS 128
 #endif
@@ -58,8 +60,16 @@ __device__ __forceinline__ void st_dmma(double &c0, double &c1, double a, double
 }
 
 #define ST_MAGIC 6755399441055744.0            /* 1.5 * 2^52: adding it rounds to the nearest integer */
-#define ST_C1 1477.3197218702985               /* 1024 / ln 2 */
-#define ST_C2 6.769015435155716e-04            /* ln 2 / 1024 = 0x1.62e42fefa39efp-11 */
+#define ST_C1 (1.4426950408889634 * ST_TAB)     /* ST_TAB / ln 2 */
+#define ST_C2 (0.6931471805599453 / ST_TAB)     /* ln 2 / ST_TAB (a power-of-two fraction of the double nearest ln 2: exact) */
+// exp(r) - the part the table does not cover: |r| <= ln 2 / (2 ST_TAB)
+#if ST_TAB_LOG2 >= 10
+#define ST_POLY(r) fma(fma(fma(1.0 / 6.0, (r), 0.5), (r), 1.0), (r), 1.0) /* truncation r^4/24 <= 5.5e-16 */
+#elif ST_TAB_LOG2 >= 6
+#define ST_POLY(r) fma(fma(fma(fma(1.0 / 24.0, (r), 1.0 / 6.0), (r), 0.5), (r), 1.0), (r), 1.0) /* r^5/120 <= 4e-14 at 64 entries */
+#else
+#define ST_POLY(r) fma(fma(fma(fma(fma(1.0 / 120.0, (r), 1.0 / 24.0), (r), 1.0 / 6.0), (r), 0.5), (r), 1.0), (r), 1.0) /* r^6/720 <= 1.4e-13 at 16 */
+#endif
 
 // entry i of the table 2^(i/1024) in shared memory (tab = 32-bit shared address of entry 0)
 __device__ __forceinline__ double st_tab(uint32_t tab, int i)
@@ -78,65 +88,14 @@ __device__ __forceinline__ double st_exp_neg(double d, uint32_t tab)
     const double r = fma(kf, -ST_C2, d);
     const int ti = __double2loint(t);
     const double T = st_tab(tab, ti);
-    const double q = fma(fma(fma(1.0 / 6.0, r, 0.5), r, 1.0), r, 1.0);
+    const double q = ST_POLY(r);
     return q * __hiloint2double(__double2hiint(T) + ((ti >> ST_TAB_LOG2) << 20), __double2loint(T));
 }
 
-// Log-sum-exp of one block, first half: d = lin - m for the lane's two columns; a valid element more than 64 above the
-// reference moves the reference up (rare: the only branch of the block).
-//   v0, v1 : the element lies inside the sample's window (PRED only; otherwise every element does)
-template <bool PRED>
-__device__ __forceinline__ void st_lse_pre(double x0, double x1, bool v0, bool v1, double &m0, double &s0, double &m1, double &s1,
-                                           double &d0, double &d1, uint32_t tab)
-{
-    d0 = x0 - m0;
-    d1 = x1 - m1;
-    bool g0 = __double2hiint(d0) > 0x40500000, g1 = __double2hiint(d1) > 0x40500000;  // d > 64, +inf
-    if (PRED) {
-        g0 = g0 && v0;
-        g1 = g1 && v1;
-    }
-    if (g0 | g1) {
-        if (g0) {
-            s0 *= st_exp_neg(m0 - x0, tab);
-            m0 = x0;
-            d0 = 0.0;
-        }
-        if (g1) {
-            s1 *= st_exp_neg(m1 - x1, tab);
-            m1 = x1;
-            d1 = 0.0;
-        }
-    }
-    if (PRED) {  // elements outside the window may carry d = +inf (reference still unset): keep the arithmetic finite
-        d0 = v0 ? d0 : 0.0;
-        d1 = v1 ? d1 : 0.0;
-    }
-}
-
-// second half, branch free: s += exp(d) = 2^k * tab[i] * cubic(r) with d = (1024 k + i) ln2/1024 + r
-template <bool PRED>
-__device__ __forceinline__ void st_lse_main(double d0, double d1, bool v0, bool v1, double &s0, double &s1, uint32_t tab)
-{
-    const double t0 = fma(d0, ST_C1, ST_MAGIC), t1 = fma(d1, ST_C1, ST_MAGIC);
-    const double k0 = t0 - ST_MAGIC, k1 = t1 - ST_MAGIC;
-    const double r0 = fma(k0, -ST_C2, d0), r1 = fma(k1, -ST_C2, d1);
-    const int i0 = __double2loint(t0), i1 = __double2loint(t1);
-    const double T0 = st_tab(tab, i0), T1 = st_tab(tab, i1);
-    bool ok0 = (unsigned)__double2hiint(d0) < 0xC0862000u, ok1 = (unsigned)__double2hiint(d1) < 0xC0862000u;  // d > -708
-    if (PRED) {
-        ok0 = ok0 && v0;
-        ok1 = ok1 && v1;
-    }
-    const int h0 = __double2hiint(T0) + ((i0 >> ST_TAB_LOG2) << 20), h1 = __double2hiint(T1) + ((i1 >> ST_TAB_LOG2) << 20);
-    const double S0 = __hiloint2double(ok0 ? h0 : 0, ok0 ? __double2loint(T0) : 0);
-    const double S1 = __hiloint2double(ok1 ? h1 : 0, ok1 ? __double2loint(T1) : 0);
-    const double q0 = fma(fma(fma(1.0 / 6.0, r0, 0.5), r0, 1.0), r0, 1.0);
-    const double q1 = fma(fma(fma(1.0 / 6.0, r1, 0.5), r1, 1.0), r1, 1.0);
-    s0 = fma(q0, S0, s0);
-    s1 = fma(q1, S1, s1);
-}
-
+// Log-sum-exp of a pair of blocks, in two halves.  First half: d = lin - m for the lane's elements; a valid element more than 64
+// above the reference moves the reference up (rare: the only branch of the step).
+//   v : the element lies inside the sample's window (PRED only; otherwise every element does)
+// Second half, branch free: s += exp(d) = 2^k * tab[i] * poly(r) with d = (ST_TAB k + i) ln2 / ST_TAB + r.
 // Pair version (two blocks b = 0, 1 of the lane's two columns c = 0, 1; x[b][c], column c carries (m[c], s[c])): one branch
 // for the four elements.  The elements of a column are taken in block order, so the rare path redoes the second one
 // against the reference the first one may have moved.
@@ -196,7 +155,7 @@ __device__ __forceinline__ void st_lse_main2(const double (&d)[2][2], const bool
             if (PRED) ok = ok && v[b][c];
             const int h = __double2hiint(T) + ((ti >> ST_TAB_LOG2) << 20);
             S[b][c] = __hiloint2double(ok ? h : 0, ok ? __double2loint(T) : 0);
-            e[b][c] = fma(fma(fma(1.0 / 6.0, r, 0.5), r, 1.0), r, 1.0);
+            e[b][c] = ST_POLY(r);
         }
 #pragma unroll
     for (int c = 0; c < 2; ++c) s[c] = fma(e[1][c], S[1][c], fma(e[0][c], S[0][c], s[c]));
@@ -225,17 +184,15 @@ struct IleStreamKArgs {
     const int32_t *i0;
     const int32_t *slots;
     const int32_t *gcum;
-    const int32_t *gorder;  // [n_points][gcap]: the groups of a point in the order of their detector-0 window start
     uint32_t *rcnt;         // [n_ranges] claim counters, zeroed per launch
     int32_t n_ranges;
-    int64_t gcap;
     double *lnL;
 };
 
 template <int K, int KS, int NC, int MINB>
 __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const __grid_constant__ IleStreamKArgs a)
 {
-    __shared__ double tab[ST_TAB];
+    __shared__ __align__(128) double tab[ST_TAB];
     for (int i = threadIdx.x; i < ST_TAB; i += blockDim.x) tab[i] = exp2((double)i * (1.0 / ST_TAB));
     __syncthreads();
     const uint32_t tab_addr = (uint32_t)__cvta_generic_to_shared(tab);
@@ -290,7 +247,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
             }
             pt = lo;
         }
-        const int g = a.gorder[(size_t)pt * a.gcap + (w - a.gcum[pt])];
+        const int g = w - a.gcum[pt];  // groups in slot order: segment by segment, window starts ascending inside a segment
         const int32_t *__restrict__ slots = a.slots + (size_t)pt * a.slot_cap + 8 * (size_t)g;
         const long long sbase = (long long)pt * a.n_per_point;
 
@@ -556,21 +513,66 @@ cudaError_t ile_launch_pack_q_stream(const IleSizes &sz, const IleStreamPlan &pl
 
 // ------------------------------------------------------------------------------------------------------------
 // counting sort of variant 4: cells = (segment, i0_0 >> g0); every segment's slots are padded to a multiple of 8 so that a
-// group of 8 consecutive slots never mixes two (d1, d2) cells
+// group of 8 consecutive slots never mixes two (d1, d2) cells.  Three kernels: index (keys + histograms), scan (one block per
+// segment: final slot position of every cell), scatter.
 // ------------------------------------------------------------------------------------------------------------
-#define SS_THREADS 1024 /* scan kernel of multi-point launches */
-#define SS_BIG 64       /* a cell with more groups than this is written to the group list by the whole block */
-#define SS_NBIG 256
+#define SS_THREADS 256
 #ifndef IX_THREADS
-#define IX_THREADS 1024
+#define IX_THREADS 256
 #endif
-/* index kernel; its last block does the scan of a single-point launch */
 
-// exclusive scan of v[0..n) in place by the NT threads of a block (v in shared or global memory); returns the total
+// Index pre-pass: step 2 of the hot path for every sample -- window starts i0_k (PAPER.md L62, L88; readings R2, R8, R9),
+// the cell key, the cell histogram and the per-segment counts of the counting sort.
+__global__ void __launch_bounds__(IX_THREADS)
+    ile_stream_index_kernel(const __grid_constant__ IleDevParams P, const __grid_constant__ IleEvalArgs a,
+                            const __grid_constant__ IleSortPlan sp, int32_t *__restrict__ i0_out, int32_t *__restrict__ cell,
+                            uint32_t *__restrict__ hist, uint32_t *__restrict__ segcnt)
+{
+    const long long n_total = a.n_per_point * a.n_points;
+    const int K = P.n_det, nseg = sp.n1 * sp.n2;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n_total; s += (long long)gridDim.x * blockDim.x) {
+        const int pt = (int)(s / a.n_per_point);
+        double dir[3], sl, cl, sd, cd;
+        ile_source_dir(a.ra[s], a.dec[s], P.gmst, dir, &sl, &cl, &sd, &cd);
+        const double t_ref = a.t_ref[s];
+        int bad = 0;
+        int32_t i0[3] = {0, 0, 0};
+        for (int k = 0; k < K; ++k) {
+            const int32_t idx = ile_window_index(P.vertex[k], dir, t_ref, P.t0_q, P.fs, P.n_t);
+            if (k < 3) i0[k] = idx;
+            if (idx < 0 || (long long)idx + P.n_t > P.n_q) bad = 1;
+            i0_out[s * K + k] = idx;
+            if (a.shift_idx) a.shift_idx[s * K + k] = idx;
+        }
+        int32_t c, seg = nseg;
+        if (bad) {  // reading R9: -inf for the sample, sticky counter, never a wrapped or clamped window
+            c = sp.ncell - 1;
+            atomicAdd(a.oob_counter, 1ULL);
+            a.lnL[s] = -CUDART_INF;
+        } else {
+            // segment = (d1, d2) cell of width 2^g, then the i0_0 bin inside the segment
+            seg = 0;
+            if (sp.nd > 1) seg = min(max(i0[1] - i0[0] + sp.dmax[1], 0), 2 * sp.dmax[1]) >> sp.g;
+            if (sp.nd > 2) seg = seg * sp.n2 + (min(max(i0[2] - i0[0] + sp.dmax[2], 0), 2 * sp.dmax[2]) >> sp.g);
+            c = seg * sp.n0 + (i0[0] >> sp.g0);  // 0 <= i0_0 <= n_q - n_t here
+        }
+        cell[s] = c;
+        // warp-aggregated: lanes with the same counter send ONE atomic (late in a run the adaptive sampler's draws
+        // crowd into a handful of cells, L47, L109, and one atomic per sample on the same address serialises in L2)
+        const unsigned long long key = (unsigned long long)pt * sp.ncell + c;
+        const unsigned peers = __match_any_sync(__activemask(), key);
+        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) {
+            atomicAdd(&hist[key], (uint32_t)__popc(peers));
+            if (seg < nseg) atomicAdd(&segcnt[(size_t)pt * nseg + seg], (uint32_t)__popc(peers));
+        }
+    }
+}
+
+// exclusive scan of v[0..n) held in shared memory by the NT threads of a block; returns the total
 template <int NT>
 __device__ uint32_t ss_block_scan(uint32_t *__restrict__ v, int n, uint32_t *wsum)
 {
-    const int per = ((n + NT - 1) / NT) | 1;  // odd: conflict-free when v is in shared memory
+    const int per = ((n + NT - 1) / NT) | 1;  // odd: conflict-free
     const int lo = min((int)threadIdx.x * per, n), hi = min(lo + per, n);
     uint32_t loc = 0;
     for (int i = lo; i < hi; ++i) loc += v[i];
@@ -602,220 +604,55 @@ __device__ uint32_t ss_block_scan(uint32_t *__restrict__ v, int n, uint32_t *wsu
         v[i] = run;
         run += x;
     }
+    __syncthreads();
     return wsum[32];
 }
 
-struct IleScanArgs {
-    int32_t ncell, n0, nseg, n_points;
-    uint32_t *hist;   // [n_points][ncell] counts in, exclusive positions out
-    uint32_t *adj;    // [n_points][nseg]
-    int32_t *ngood;   // [n_points]
-    uint32_t *ngr;    // [n_points]
-    int32_t *gcum;    // [n_points + 1]
-    int32_t *gorder;  // [n_points][gcap]
-    int32_t *slots;   // [n_points][8 gcap]: the scan marks the padding at the end of every segment with -1
-    long long gcap;
-    int32_t stage;    // words of shared memory behind the histogram for assembling the group list (0: none)
-};
-
-// Scan of one point by one block of NT threads; the point's histogram lives in shared memory (h: ncell + 1 + nseg words,
-// followed by `stage` words in which the group list is assembled when it fits; stage = 0: written straight to global).
-//   hist  -> exclusive positions (written back for the scatter kernel)
-//   adj[seg] = padded base of the segment minus its first position;  ngr[pt] = groups of the point (a single point also
-//   gets gcum = {0, groups})
-//   gorder[pt][.] = the point's groups listed by i0_0 bin first, segment second: group ids are positions / 8 in the padded
-//   slot table; a group belongs to the (segment, bin) cell its first slot falls in.
-template <int NT>
-__device__ void ss_scan_point(const IleScanArgs &A, int pt, uint32_t *__restrict__ h, uint32_t *wsum)
+// Scan: block (seg, pt).  Padded base of the segment from the per-segment counts (every block scans all of them: a few
+// hundred words), then the exclusive scan of the segment's own i0_0 bins: hist[cell] becomes the cell's first slot.  The
+// padding at the end of the segment's slots is marked -1; block 0 of a point records its number of groups.
+__global__ void __launch_bounds__(SS_THREADS)
+    ile_stream_scan_kernel(int32_t n0, int32_t nseg, int32_t ncell, long long slot_cap, uint32_t *__restrict__ hist,
+                           const uint32_t *__restrict__ segcnt, int32_t *__restrict__ slots, uint32_t *__restrict__ ngr,
+                           int32_t *__restrict__ gcum, int32_t n_points)
 {
-    const int ncell = A.ncell, n0 = A.n0, nseg = A.nseg;
-    uint32_t *hg = A.hist + (size_t)pt * ncell;
-    uint32_t *adg = A.adj + (size_t)pt * nseg;
-    uint32_t *ad = h + ncell + 1;
-    int32_t *go = A.gorder + (size_t)pt * A.gcap;
-#pragma unroll 8
-    for (int i = threadIdx.x; i < ncell; i += NT) h[i] = __ldcg(hg + i);
-    __syncthreads();
-    const uint32_t n_all = ss_block_scan<NT>(h, ncell, wsum);
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        h[ncell] = n_all;
-        A.ngood[pt] = (int32_t)h[ncell - 1];  // samples before the out-of-range cell
-    }
-    for (int i = threadIdx.x; i < ncell; i += NT) hg[i] = h[i];
-    // padded size of every segment (its end is the next segment's start; the last one ends at the out-of-range cell)
-    for (int s = threadIdx.x; s < nseg; s += NT) ad[s] = (h[(size_t)(s + 1) * n0] - h[(size_t)s * n0] + 7u) & ~7u;
-    __syncthreads();
-    const uint32_t tot = ss_block_scan<NT>(ad, nseg, wsum);
-    __syncthreads();
-    for (int s = threadIdx.x; s < nseg; s += NT) {
-        const uint32_t first = h[(size_t)s * n0], cnt = h[(size_t)(s + 1) * n0] - first;
-        int32_t *sl = A.slots + (size_t)pt * 8 * A.gcap + ad[s];  // ad[s] is still the segment's padded base here
-        for (uint32_t i = cnt; i < ((cnt + 7u) & ~7u); ++i) sl[i] = -1;
-        ad[s] -= first;
-        adg[s] = ad[s];
-    }
-    if (threadIdx.x == 0) {
-        A.ngr[pt] = tot >> 3;
-        if (A.n_points == 1) {
-            A.gcum[0] = 0;
-            A.gcum[1] = (int32_t)(tot >> 3);
-        }
-    }
-    __syncthreads();
-    // traversal q = bin * nseg + seg: groups that start in cell (seg, bin) = multiples of 8 in [p0, p1)
-    const int nq = n0 * nseg;
-    const int per = (nq + NT - 1) / NT;
-    const int qlo = min((int)threadIdx.x * per, nq), qhi = min(qlo + per, nq);
-    uint32_t loc = 0;
-    {
-        int b = qlo / nseg, sgm = qlo - b * nseg;
-        for (int q = qlo; q < qhi; ++q) {
-            const int c = sgm * n0 + b;
-            const uint32_t p0 = h[c] + ad[sgm], p1 = h[c + 1] + ad[sgm];
-            loc += ((p1 + 7u) >> 3) - ((p0 + 7u) >> 3);
-            if (++sgm == nseg) sgm = 0, ++b;
-        }
-    }
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t inc = loc;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const uint32_t x = __shfl_up_sync(ST_FULL, inc, o);
-        if (lane >= o) inc += x;
-    }
-    if (lane == 31) wsum[warp] = inc;
-    __syncthreads();
-    if (warp == 0) {
-        const uint32_t x = lane < NT / 32 ? wsum[lane] : 0u;
-        uint32_t xi = x;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const uint32_t y = __shfl_up_sync(ST_FULL, xi, o);
-            if (lane >= o) xi += y;
-        }
-        wsum[lane] = xi - x;
-    }
-    __syncthreads();
-    __shared__ uint3 big[SS_NBIG];
-    __shared__ uint32_t nbig;
-    if (threadIdx.x == 0) nbig = 0;
-    __syncthreads();
-    // the list is assembled in shared memory when it fits (scattered 4-byte global stores cost a cycle each), then copied out
-    const bool staged = (tot >> 3) <= (uint32_t)A.stage;
-    int32_t *__restrict__ dst = staged ? reinterpret_cast<int32_t *>(h + ((ncell + 1 + nseg + 3) & ~3)) : go;
-    uint32_t run = wsum[warp] + inc - loc;
-    {
-        int b = qlo / nseg, sgm = qlo - b * nseg;
-        for (int q = qlo; q < qhi; ++q) {
-            const int c = sgm * n0 + b;
-            const uint32_t p0 = h[c] + ad[sgm], p1 = h[c + 1] + ad[sgm];
-            const uint32_t g0 = (p0 + 7u) >> 3, g1 = (p1 + 7u) >> 3;
-            if (g1 - g0 > SS_BIG) {  // a crowded cell (concentrated samples): left to the whole block
-                const uint32_t e = atomicAdd(&nbig, 1u);
-                if (e < SS_NBIG) {
-                    big[e] = make_uint3(run, g0, g1 - g0);
-                    run += g1 - g0;
-                    if (++sgm == nseg) sgm = 0, ++b;
-                    continue;
-                }
-            }
-            for (uint32_t g = g0; g < g1; ++g) dst[run++] = (int32_t)g;
-            if (++sgm == nseg) sgm = 0, ++b;
-        }
-    }
-    __syncthreads();
-    for (uint32_t e = 0; e < min(nbig, (uint32_t)SS_NBIG); ++e) {
-        const uint3 w = big[e];
-        for (uint32_t i = threadIdx.x; i < w.z; i += NT) dst[w.x + i] = (int32_t)(w.y + i);
-    }
-    if (staged) {
-        __syncthreads();
-        // 16-byte stores (gorder rows and the staging area are 16-byte aligned; the tail past the list is scratch)
-        const uint32_t n4 = ((tot >> 3) + 3) >> 2;
-        for (uint32_t i = threadIdx.x; i < n4; i += NT) reinterpret_cast<int4 *>(go)[i] = reinterpret_cast<const int4 *>(dst)[i];
-    }
-}
-
-__global__ void __launch_bounds__(SS_THREADS) ile_stream_scan_kernel(const __grid_constant__ IleScanArgs A)
-{
-    extern __shared__ uint32_t ss_h[];
+    extern __shared__ uint32_t ss_v[];  // max(nseg, n0) words
     __shared__ uint32_t wsum[33];
-    ss_scan_point<SS_THREADS>(A, blockIdx.x, ss_h, wsum);
-}
-
-// Index pre-pass: step 2 of the hot path for every sample -- window starts i0_k (PAPER.md L62, L88; readings R2, R8, R9),
-// the cell key and the histogram of the counting sort.  For a single-point launch (FUSED) the block that finishes last
-// goes on to scan the histogram, which saves a launch and a trip through the block scheduler.
-template <bool FUSED>
-__global__ void __launch_bounds__(IX_THREADS)
-    ile_stream_index_kernel(const __grid_constant__ IleDevParams P, const __grid_constant__ IleEvalArgs a,
-                            const __grid_constant__ IleSortPlan sp, int32_t *__restrict__ i0_out, int32_t *__restrict__ cell,
-                            const __grid_constant__ IleScanArgs A, uint32_t *__restrict__ ticket)
-{
-    const long long n_total = a.n_per_point * a.n_points;
-    const int K = P.n_det;
-    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n_total; s += (long long)gridDim.x * blockDim.x) {
-        const int pt = (int)(s / a.n_per_point);
-        double dir[3], sl, cl, sd, cd;
-        ile_source_dir(a.ra[s], a.dec[s], P.gmst, dir, &sl, &cl, &sd, &cd);
-        const double t_ref = a.t_ref[s];
-        int bad = 0;
-        int32_t i0[3] = {0, 0, 0};
-        for (int k = 0; k < K; ++k) {
-            const int32_t idx = ile_window_index(P.vertex[k], dir, t_ref, P.t0_q, P.fs, P.n_t);
-            if (k < 3) i0[k] = idx;
-            if (idx < 0 || (long long)idx + P.n_t > P.n_q) bad = 1;
-            i0_out[s * K + k] = idx;
-            if (a.shift_idx) a.shift_idx[s * K + k] = idx;
-        }
-        int32_t c;
-        if (bad) {  // reading R9: -inf for the sample, sticky counter, never a wrapped or clamped window
-            c = sp.ncell - 1;
-            atomicAdd(a.oob_counter, 1ULL);
-            a.lnL[s] = -CUDART_INF;
-        } else {
-            // segment = (d1, d2) cell of width 2^g, then the i0_0 bin inside the segment
-            int32_t seg = 0;
-            if (sp.nd > 1) seg = min(max(i0[1] - i0[0] + sp.dmax[1], 0), 2 * sp.dmax[1]) >> sp.g;
-            if (sp.nd > 2) seg = seg * sp.n2 + (min(max(i0[2] - i0[0] + sp.dmax[2], 0), 2 * sp.dmax[2]) >> sp.g);
-            c = seg * sp.n0 + (i0[0] >> sp.g0);  // 0 <= i0_0 <= n_q - n_t here
-        }
-        cell[s] = c;
-        // warp-aggregated: lanes with the same counter send ONE atomic (late in a run the adaptive sampler's draws
-        // crowd into a handful of cells, L47, L109, and one atomic per sample on the same address serialises in L2)
-        const unsigned long long key = (unsigned long long)pt * sp.ncell + c;
-        const unsigned peers = __match_any_sync(__activemask(), key);
-        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&A.hist[key], (uint32_t)__popc(peers));
+    const int seg = blockIdx.x, pt = blockIdx.y;
+    for (int i = threadIdx.x; i < nseg; i += SS_THREADS) ss_v[i] = (segcnt[(size_t)pt * nseg + i] + 7u) & ~7u;
+    __syncthreads();
+    const uint32_t cnt = segcnt[(size_t)pt * nseg + seg];
+    const uint32_t tot = ss_block_scan<SS_THREADS>(ss_v, nseg, wsum);
+    const uint32_t base = ss_v[seg];
+    __syncthreads();
+    if (seg == 0 && threadIdx.x == 0) {
+        ngr[pt] = tot >> 3;
+        if (n_points == 1) gcum[0] = 0, gcum[1] = (int32_t)(tot >> 3);
     }
-    if (FUSED) {
-        extern __shared__ uint32_t ss_h[];
-        __shared__ uint32_t wsum[33];
-        __shared__ uint32_t last;
-        __threadfence();
-        __syncthreads();
-        if (threadIdx.x == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
-        __syncthreads();
-        if (!last) return;
-        __threadfence();
-        ss_scan_point<IX_THREADS>(A, 0, ss_h, wsum);
-    }
+    uint32_t *hg = hist + (size_t)pt * ncell + (size_t)seg * n0;
+    for (int i = threadIdx.x; i < n0; i += SS_THREADS) ss_v[i] = hg[i];
+    __syncthreads();
+    ss_block_scan<SS_THREADS>(ss_v, n0, wsum);
+    for (int i = threadIdx.x; i < n0; i += SS_THREADS) hg[i] = base + ss_v[i];
+    int32_t *sl = slots + (size_t)pt * slot_cap + base;
+    for (uint32_t i = cnt + threadIdx.x; i < ((cnt + 7u) & ~7u); i += SS_THREADS) sl[i] = -1;
 }
 
 // exclusive prefix of the points' group counts (multi-point launches)
-__global__ void __launch_bounds__(SS_THREADS) ile_stream_prefix_kernel(int32_t n_points, uint32_t *__restrict__ ngr, int32_t *__restrict__ gcum)
+__global__ void __launch_bounds__(1024) ile_stream_prefix_kernel(int32_t n_points, const uint32_t *__restrict__ ngr, int32_t *__restrict__ gcum)
 {
+    extern __shared__ uint32_t ss_v[];
     __shared__ uint32_t wsum[33];
-    const uint32_t tot = ss_block_scan<SS_THREADS>(ngr, n_points, wsum);
+    for (int p = threadIdx.x; p < n_points; p += 1024) ss_v[p] = ngr[p];
     __syncthreads();
-    for (int p = threadIdx.x; p < n_points; p += SS_THREADS) gcum[p] = (int32_t)ngr[p];
+    const uint32_t tot = ss_block_scan<1024>(ss_v, n_points, wsum);
+    for (int p = threadIdx.x; p < n_points; p += 1024) gcum[p] = (int32_t)ss_v[p];
     if (threadIdx.x == 0) gcum[n_points] = (int32_t)tot;
 }
 
-__global__ void __launch_bounds__(IX_THREADS) ile_stream_scatter_kernel(long long n_per_point, int32_t n_points, int32_t ncell, int32_t n0,
-                                                                 int32_t nseg, long long slot_cap, const int32_t *__restrict__ cell,
-                                                                 uint32_t *__restrict__ offs, const uint32_t *__restrict__ adj,
-                                                                 int32_t *__restrict__ slots)
+__global__ void __launch_bounds__(IX_THREADS) ile_stream_scatter_kernel(long long n_per_point, int32_t n_points, int32_t ncell,
+                                                                        long long slot_cap, const int32_t *__restrict__ cell,
+                                                                        uint32_t *__restrict__ offs, int32_t *__restrict__ slots)
 {
     const long long n_total = n_per_point * n_points;
     for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n_total; s += (long long)gridDim.x * blockDim.x) {
@@ -829,7 +666,7 @@ __global__ void __launch_bounds__(IX_THREADS) ile_stream_scatter_kernel(long lon
         uint32_t first = 0;
         if (lane == leader) first = atomicAdd(&offs[key], (uint32_t)__popc(peers));
         first = __shfl_sync(peers, first, leader);
-        const uint32_t pos = first + (uint32_t)__popc(peers & ((1u << lane) - 1u)) + adj[(size_t)pt * nseg + c / n0];
+        const uint32_t pos = first + (uint32_t)__popc(peers & ((1u << lane) - 1u));
         slots[(size_t)pt * slot_cap + pos] = (int32_t)(s - (long long)pt * n_per_point);
     }
 }
@@ -872,11 +709,12 @@ bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per
     }
     sp.n1 = sp.nd > 1 ? ((2 * sp.dmax[1]) >> sp.g) + 1 : 1;
     sp.n2 = sp.nd > 2 ? ((2 * sp.dmax[2]) >> sp.g) + 1 : 1;
+    if ((long long)sp.n1 * sp.n2 > 12288) return false;  // the scan kernel holds the per-segment counts in shared memory
     int g0 = 3;
-    for (;; ++g0) {
+    for (;; ++g0) {  // i0_0 bins of 8 rows unless the series is so long that a segment's bins (shared memory) or the histogram get too big
         sp.n0 = ((sz.n_q - sz.n_t) >> g0) + 1;
         const long long nc = (long long)sp.n0 * sp.n1 * sp.n2 + 1;
-        if ((nc + 1 + (long long)sp.n1 * sp.n2) * 4 <= (long long)sz.max_smem_optin - 8192 - 64) {  // the scan kernel keeps a point's histogram in shared memory
+        if (sp.n0 <= 12288 && nc <= (1LL << 22)) {
             sp.ncell = (int32_t)nc;
             break;
         }
@@ -931,16 +769,11 @@ static cudaError_t st_launch(const IleSizes &sz, int ks, const IleStreamKArgs *k
     return st_launch_k<3, ST_NC>(sz, ks, ka, mg, per_sm, st);
 }
 
-// Once per context, on the context's device: opt-in shared memory of the scan kernels, carve-out and occupancy of the
-// streaming kernel this context's sizes select.
+// Once per context, on the context's device: carve-out and occupancy of the streaming kernel this context's sizes select.
 cudaError_t ile_stream_prepare(const IleSizes &sz, IleStreamPlan *pl)
 {
-    cudaError_t e = cudaFuncSetAttribute(ile_stream_scan_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 8192);
-    if (e != cudaSuccess) return e;
-    e = cudaFuncSetAttribute(ile_stream_index_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sz.max_smem_optin - 8192);
-    if (e != cudaSuccess) return e;
     int per_sm = 0;
-    e = st_launch(sz, pl->ks, nullptr, 0, &per_sm, 0);
+    cudaError_t e = st_launch(sz, pl->ks, nullptr, 0, &per_sm, 0);
     pl->ctas_per_sm = per_sm;
     return e;
 }
@@ -952,27 +785,12 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     if (a.n_per_point <= 0 || a.n_points <= 0) return cudaSuccess;
     const long long n_total = a.n_per_point * a.n_points;
     const int nseg = sp.n1 * sp.n2;
-    // histogram + claim counters of the streaming kernel (right behind the histograms)
-    cudaError_t e = cudaMemsetAsync(sc.hist, 0, ((size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES + 1) * sizeof(uint32_t), st);
+    // cell histograms, per-segment counts and the claim counters of the streaming kernel, one zeroed block
+    const size_t n_hist = (size_t)a.n_points * sp.ncell, n_segc = (size_t)a.n_points * nseg;
+    cudaError_t e = cudaMemsetAsync(sc.hist, 0, (n_hist + n_segc + ILE_STREAM_MAX_RANGES) * sizeof(uint32_t), st);
     if (e != cudaSuccess) return e;
-    // window starts + histogram on the caller's stream; a single point's scan runs in the index kernel's last block
-    IleScanArgs sa;
-    sa.ncell = sp.ncell, sa.n0 = sp.n0, sa.nseg = nseg, sa.n_points = a.n_points;
-    sa.hist = sc.hist;
-    sa.adj = reinterpret_cast<uint32_t *>(ss.adj);
-    sa.ngood = sc.ngood;
-    sa.ngr = reinterpret_cast<uint32_t *>(ss.gcum) + a.n_points + 1;
-    sa.gcum = ss.gcum;
-    sa.gorder = ss.gorder;
-    sa.slots = ss.slots;
-    sa.gcap = ss.slot_cap / 8;
-    size_t scan_smem = (((size_t)sp.ncell + 1 + nseg + 3) & ~(size_t)3) * sizeof(uint32_t);
-    {
-        const size_t room = (size_t)(sz.max_smem_optin - 8192) - scan_smem, want = (size_t)sa.gcap * sizeof(int32_t);
-        sa.stage = want <= room ? (int32_t)sa.gcap : 0;
-        if (sa.stage) scan_smem += want;
-    }
-    uint32_t *ticket = sc.hist + (size_t)a.n_points * sp.ncell + ILE_STREAM_MAX_RANGES;  // its own word behind the claim counters
+    uint32_t *segcnt = sc.hist + n_hist, *rcnt = segcnt + n_segc;
+    uint32_t *ngr = reinterpret_cast<uint32_t *>(ss.gcum) + a.n_points + 1;
     long long iblocks = (n_total + IX_THREADS - 1) / IX_THREADS;
     const long long cap = (long long)sz.sm_count * 32;
     if (iblocks > cap) iblocks = cap;
@@ -981,12 +799,8 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     e = cudaEventRecord(ss.ev_fork, st);
     if (e != cudaSuccess) return e;
     int nl = 0;
-    if (a.n_points == 1) {
-        ile_stream_index_kernel<true><<<(unsigned)iblocks, IX_THREADS, scan_smem, st>>>(hp, a, sp, sc.i0, sc.cell, sa, ticket);
-        ++nl;
-    } else {
-        ile_stream_index_kernel<false><<<(unsigned)iblocks, IX_THREADS, 0, st>>>(hp, a, sp, sc.i0, sc.cell, sa, ticket);
-    }
+    ile_stream_index_kernel<<<(unsigned)iblocks, IX_THREADS, 0, st>>>(hp, a, sp, sc.i0, sc.cell, sc.hist, segcnt);
+    ++nl;
     e = cudaStreamWaitEvent(ss.aux, ss.ev_fork, 0);
     if (e != cudaSuccess) return e;
     if (ss.ev_late) {  // ile_run_host: those arrays are still being copied on the copy stream
@@ -1002,13 +816,15 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     ++nl;
     e = cudaEventRecord(ss.ev_join, ss.aux);
     if (e != cudaSuccess) return e;
+    const size_t scan_smem = (size_t)(nseg > sp.n0 ? nseg : sp.n0) * sizeof(uint32_t);
+    ile_stream_scan_kernel<<<dim3((unsigned)nseg, (unsigned)a.n_points), SS_THREADS, scan_smem, st>>>(sp.n0, nseg, sp.ncell, ss.slot_cap, sc.hist, segcnt,
+                                                                                                    ss.slots, ngr, ss.gcum, a.n_points);
+    ++nl;
     if (a.n_points > 1) {
-        ile_stream_scan_kernel<<<(unsigned)a.n_points, SS_THREADS, scan_smem, st>>>(sa);
-        ile_stream_prefix_kernel<<<1, SS_THREADS, 0, st>>>(a.n_points, sa.ngr, ss.gcum);
-        nl += 3;
+        ile_stream_prefix_kernel<<<1, 1024, (size_t)a.n_points * sizeof(uint32_t), st>>>(a.n_points, ngr, ss.gcum);
+        ++nl;
     }
-    ile_stream_scatter_kernel<<<(unsigned)iblocks, IX_THREADS, 0, st>>>(a.n_per_point, a.n_points, sp.ncell, sp.n0, nseg, ss.slot_cap, sc.cell,
-                                                                        sc.hist, reinterpret_cast<const uint32_t *>(ss.adj), ss.slots);
+    ile_stream_scatter_kernel<<<(unsigned)iblocks, IX_THREADS, 0, st>>>(a.n_per_point, a.n_points, sp.ncell, ss.slot_cap, sc.cell, sc.hist, ss.slots);
     ++nl;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -1032,10 +848,8 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     ka.i0 = sc.i0;
     ka.slots = ss.slots;
     ka.gcum = ss.gcum;
-    ka.gorder = ss.gorder;
-    ka.rcnt = sc.hist + (size_t)a.n_points * sp.ncell;
+    ka.rcnt = rcnt;
     ka.n_ranges = sz.sm_count < ILE_STREAM_MAX_RANGES ? sz.sm_count : ILE_STREAM_MAX_RANGES;
-    ka.gcap = ss.slot_cap / 8;
     ka.lnL = a.lnL;
     const long long max_groups = (long long)a.n_points * (ss.slot_cap / 8);
     int per_sm = pl.ctas_per_sm;

@@ -63,8 +63,7 @@ struct IleSortScratch {
     double *quad;      // [n]
     int32_t *i0;       // [n][K]
     int32_t *cell;     // [n]
-    uint32_t *hist;    // [n_points][ncell], followed by ILE_STREAM_MAX_RANGES claim counters and the index kernel's ticket
-    int32_t *ngood;    // [n_points]
+    uint32_t *hist;    // [n_points][ncell] cell counts -> first slots, then [n_points][nseg] segment counts, then ILE_STREAM_MAX_RANGES claim counters
     double *qform;     // [n][K][3] quadratic forms from the FP64-MMA kernel, or NULL (the coefficient kernel computes them)
 };
 
@@ -78,14 +77,12 @@ struct IleStreamPlan {
     int32_t ctas_per_sm;  // resident CTAs of the streaming kernel per SM on the context's device (ile_stream_prepare)
 };
 
-#define ILE_STREAM_MAX_RANGES 256 /* claim counters of the streaming kernel, kept right behind the histograms (+ 1 ticket word) */
+#define ILE_STREAM_MAX_RANGES 256 /* claim counters of the streaming kernel, kept right behind the histograms */
 
 struct IleStreamScratch {
     const double *Qs;   // packed Q [P][K][ks][nqp][4]
     int32_t *slots;     // [n_points][slot_cap]: sample index or -1, groups of 8 consecutive slots
-    int32_t *adj;       // [n_points][nseg]: padded segment base minus the segment's first sorted position
     int32_t *gcum;      // [n_points + 1]: exclusive prefix of the group counts, followed by [n_points] group counts
-    int32_t *gorder;    // [n_points][slot_cap / 8]: group ids in the order of their detector-0 window start
     int64_t slot_cap;   // slots per point (multiple of 8)
     cudaStream_t aux;   // side stream: the coefficient kernel runs there while the caller's stream sorts
     cudaEvent_t ev_fork, ev_join;
