@@ -522,14 +522,14 @@ cudaError_t ile_launch_pack_q_stream(const IleSizes &sz, const IleStreamPlan &pl
 #endif
 
 // Index pre-pass: step 2 of the hot path for every sample -- window starts i0_k (readings R2, R8, R9),
-// the cell key, the cell histogram and the per-segment counts of the counting sort.
+// the cell key and the cell histogram of the counting sort.
 __global__ void __launch_bounds__(IX_THREADS)
     ile_stream_index_kernel(const __grid_constant__ IleDevParams P, const __grid_constant__ IleEvalArgs a,
                             const __grid_constant__ IleSortPlan sp, int32_t *__restrict__ i0_out, int32_t *__restrict__ cell,
-                            uint32_t *__restrict__ hist, uint32_t *__restrict__ segcnt)
+                            uint32_t *__restrict__ hist)
 {
     const long long n_total = a.n_per_point * a.n_points;
-    const int K = P.n_det, nseg = sp.n1 * sp.n2;
+    const int K = P.n_det;
     for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n_total; s += (long long)gridDim.x * blockDim.x) {
         const int pt = (int)(s / a.n_per_point);
         double dir[3], sl, cl, sd, cd;
@@ -544,14 +544,14 @@ __global__ void __launch_bounds__(IX_THREADS)
             i0_out[s * K + k] = idx;
             if (a.shift_idx) a.shift_idx[s * K + k] = idx;
         }
-        int32_t c, seg = nseg;
+        int32_t c;
         if (bad) {  // reading R9: -inf for the sample, sticky counter, never a wrapped or clamped window
             c = sp.ncell - 1;
             atomicAdd(a.oob_counter, 1ULL);
             a.lnL[s] = -CUDART_INF;
         } else {
             // segment = (d1, d2) cell of width 2^g, then the i0_0 bin inside the segment
-            seg = 0;
+            int32_t seg = 0;
             if (sp.nd > 1) seg = min(max(i0[1] - i0[0] + sp.dmax[1], 0), 2 * sp.dmax[1]) >> sp.g;
             if (sp.nd > 2) seg = seg * sp.n2 + (min(max(i0[2] - i0[0] + sp.dmax[2], 0), 2 * sp.dmax[2]) >> sp.g);
             c = seg * sp.n0 + (i0[0] >> sp.g0);  // 0 <= i0_0 <= n_q - n_t here
@@ -561,10 +561,7 @@ __global__ void __launch_bounds__(IX_THREADS)
         // crowd into a handful of cells, L47, L109, and one atomic per sample on the same address serialises in L2)
         const unsigned long long key = (unsigned long long)pt * sp.ncell + c;
         const unsigned peers = __match_any_sync(__activemask(), key);
-        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) {
-            atomicAdd(&hist[key], (uint32_t)__popc(peers));
-            if (seg < nseg) atomicAdd(&segcnt[(size_t)pt * nseg + seg], (uint32_t)__popc(peers));
-        }
+        if ((int)(threadIdx.x & 31) == __ffs(peers) - 1) atomicAdd(&hist[key], (uint32_t)__popc(peers));
     }
 }
 
@@ -608,66 +605,75 @@ __device__ uint32_t ss_block_scan(uint32_t *__restrict__ v, int n, uint32_t *wsu
     return wsum[32];
 }
 
-// Scan: block (seg, pt).  Padded base of the segment from the per-segment counts (every block scans all of them: a few
-// hundred words), then the exclusive scan of the segment's own i0_0 bins: hist[cell] becomes the cell's first slot.  The
-// padding at the end of the segment's slots is marked -1; block 0 of a point records its number of groups.
+// Scan: block (seg, pt) turns the counts of the segment's i0_0 bins into exclusive positions inside the segment and
+// records the segment's total.
 __global__ void __launch_bounds__(SS_THREADS)
-    ile_stream_scan_kernel(int32_t n0, int32_t nseg, int32_t ncell, long long slot_cap, uint32_t *__restrict__ hist,
-                           const uint32_t *__restrict__ segcnt, int32_t *__restrict__ slots, uint32_t *__restrict__ ngr,
-                           int32_t *__restrict__ gcum, int32_t n_points)
+    ile_stream_scan_kernel(int32_t n0, int32_t nseg, int32_t ncell, uint32_t *__restrict__ hist, uint32_t *__restrict__ segtot)
 {
-    extern __shared__ uint32_t ss_v[];  // max(nseg, n0) words
+    extern __shared__ uint32_t ss_v[];  // n0 words
     __shared__ uint32_t wsum[33];
     const int seg = blockIdx.x, pt = blockIdx.y;
-    for (int i = threadIdx.x; i < nseg; i += SS_THREADS) ss_v[i] = (segcnt[(size_t)pt * nseg + i] + 7u) & ~7u;
-    __syncthreads();
-    const uint32_t cnt = segcnt[(size_t)pt * nseg + seg];
-    const uint32_t tot = ss_block_scan<SS_THREADS>(ss_v, nseg, wsum);
-    const uint32_t base = ss_v[seg];
-    __syncthreads();
-    if (seg == 0 && threadIdx.x == 0) {
-        ngr[pt] = tot >> 3;
-        if (n_points == 1) gcum[0] = 0, gcum[1] = (int32_t)(tot >> 3);
-    }
     uint32_t *hg = hist + (size_t)pt * ncell + (size_t)seg * n0;
     for (int i = threadIdx.x; i < n0; i += SS_THREADS) ss_v[i] = hg[i];
     __syncthreads();
-    ss_block_scan<SS_THREADS>(ss_v, n0, wsum);
-    for (int i = threadIdx.x; i < n0; i += SS_THREADS) hg[i] = base + ss_v[i];
-    int32_t *sl = slots + (size_t)pt * slot_cap + base;
-    for (uint32_t i = cnt + threadIdx.x; i < ((cnt + 7u) & ~7u); i += SS_THREADS) sl[i] = -1;
+    const uint32_t tot = ss_block_scan<SS_THREADS>(ss_v, n0, wsum);
+    for (int i = threadIdx.x; i < n0; i += SS_THREADS) hg[i] = ss_v[i];
+    if (threadIdx.x == 0) segtot[(size_t)pt * nseg + seg] = tot;
 }
 
 // exclusive prefix of the points' group counts (multi-point launches)
-__global__ void __launch_bounds__(1024) ile_stream_prefix_kernel(int32_t n_points, const uint32_t *__restrict__ ngr, int32_t *__restrict__ gcum)
+__global__ void __launch_bounds__(1024) ile_stream_prefix_kernel(int32_t n_points, int32_t nseg, const uint32_t *__restrict__ segtot,
+                                                                 int32_t *__restrict__ gcum)
 {
     extern __shared__ uint32_t ss_v[];
     __shared__ uint32_t wsum[33];
-    for (int p = threadIdx.x; p < n_points; p += 1024) ss_v[p] = ngr[p];
+    for (int p = threadIdx.x; p < n_points; p += 1024) {
+        uint32_t g = 0;
+        for (int sg = 0; sg < nseg; ++sg) g += (segtot[(size_t)p * nseg + sg] + 7u) >> 3;
+        ss_v[p] = g;
+    }
     __syncthreads();
     const uint32_t tot = ss_block_scan<1024>(ss_v, n_points, wsum);
     for (int p = threadIdx.x; p < n_points; p += 1024) gcum[p] = (int32_t)ss_v[p];
     if (threadIdx.x == 0) gcum[n_points] = (int32_t)tot;
 }
 
-__global__ void __launch_bounds__(IX_THREADS) ile_stream_scatter_kernel(long long n_per_point, int32_t n_points, int32_t ncell,
-                                                                        long long slot_cap, const int32_t *__restrict__ cell,
-                                                                        uint32_t *__restrict__ offs, int32_t *__restrict__ slots)
+// Scatter: blocks (b, pt).  Every block first builds the padded base of every segment of its point in shared memory (an
+// exclusive scan of the segment totals rounded up to 8), then places its samples: slot = base[segment] + position of the
+// cell inside the segment + rank inside the cell.  Block 0 of a point marks the padding at the end of every segment with -1
+// and, for a single-point launch, records the number of groups.
+__global__ void __launch_bounds__(IX_THREADS)
+    ile_stream_scatter_kernel(long long n_per_point, int32_t n_points, int32_t ncell, int32_t n0, int32_t nseg, long long slot_cap,
+                              const int32_t *__restrict__ cell, uint32_t *__restrict__ offs, const uint32_t *__restrict__ segtot,
+                              int32_t *__restrict__ slots, int32_t *__restrict__ gcum)
 {
-    const long long n_total = n_per_point * n_points;
-    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n_total; s += (long long)gridDim.x * blockDim.x) {
-        const int pt = (int)(s / n_per_point);
-        const int c = cell[s];
+    extern __shared__ uint32_t ss_v[];  // nseg words
+    __shared__ uint32_t wsum[33];
+    const int pt = blockIdx.y;
+    const uint32_t *st = segtot + (size_t)pt * nseg;
+    for (int i = threadIdx.x; i < nseg; i += IX_THREADS) ss_v[i] = (st[i] + 7u) & ~7u;
+    __syncthreads();
+    const uint32_t tot = ss_block_scan<IX_THREADS>(ss_v, nseg, wsum);
+    int32_t *sl = slots + (size_t)pt * slot_cap;
+    if (blockIdx.x == 0) {
+        for (int sg = threadIdx.x; sg < nseg; sg += IX_THREADS) {
+            const uint32_t cnt = st[sg];
+            for (uint32_t i = cnt; i < ((cnt + 7u) & ~7u); ++i) sl[ss_v[sg] + i] = -1;
+        }
+        if (threadIdx.x == 0 && n_points == 1) gcum[0] = 0, gcum[1] = (int32_t)(tot >> 3);
+    }
+    const int32_t *cl = cell + (size_t)pt * n_per_point;
+    uint32_t *of = offs + (size_t)pt * ncell;
+    for (long long s = (long long)blockIdx.x * blockDim.x + threadIdx.x; s < n_per_point; s += (long long)gridDim.x * blockDim.x) {
+        const int c = cl[s];
         if (c == ncell - 1) continue;  // out of range: lnL = -inf was written by the index kernel
         // warp-aggregated claim: the first lane of every set of lanes with the same counter takes the whole set's places
-        const unsigned long long key = (unsigned long long)pt * ncell + c;
-        const unsigned peers = __match_any_sync(__activemask(), key);
+        const unsigned peers = __match_any_sync(__activemask(), c);
         const int lane = threadIdx.x & 31, leader = __ffs(peers) - 1;
         uint32_t first = 0;
-        if (lane == leader) first = atomicAdd(&offs[key], (uint32_t)__popc(peers));
+        if (lane == leader) first = atomicAdd(&of[c], (uint32_t)__popc(peers));
         first = __shfl_sync(peers, first, leader);
-        const uint32_t pos = first + (uint32_t)__popc(peers & ((1u << lane) - 1u));
-        slots[(size_t)pt * slot_cap + pos] = (int32_t)(s - (long long)pt * n_per_point);
+        sl[ss_v[c / n0] + first + (uint32_t)__popc(peers & ((1u << lane) - 1u))] = (int32_t)s;
     }
 }
 
@@ -785,12 +791,12 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     if (a.n_per_point <= 0 || a.n_points <= 0) return cudaSuccess;
     const long long n_total = a.n_per_point * a.n_points;
     const int nseg = sp.n1 * sp.n2;
-    // cell histograms, per-segment counts and the claim counters of the streaming kernel, one zeroed block
-    const size_t n_hist = (size_t)a.n_points * sp.ncell, n_segc = (size_t)a.n_points * nseg;
-    cudaError_t e = cudaMemsetAsync(sc.hist, 0, (n_hist + n_segc + ILE_STREAM_MAX_RANGES) * sizeof(uint32_t), st);
+    // cell histograms and the claim counters of the streaming kernel, one zeroed block; the segment totals behind them are
+    // written by the scan kernel
+    const size_t n_hist = (size_t)a.n_points * sp.ncell;
+    cudaError_t e = cudaMemsetAsync(sc.hist, 0, (n_hist + ILE_STREAM_MAX_RANGES) * sizeof(uint32_t), st);
     if (e != cudaSuccess) return e;
-    uint32_t *segcnt = sc.hist + n_hist, *rcnt = segcnt + n_segc;
-    uint32_t *ngr = reinterpret_cast<uint32_t *>(ss.gcum) + a.n_points + 1;
+    uint32_t *rcnt = sc.hist + n_hist, *segtot = rcnt + ILE_STREAM_MAX_RANGES;
     long long iblocks = (n_total + IX_THREADS - 1) / IX_THREADS;
     const long long cap = (long long)sz.sm_count * 32;
     if (iblocks > cap) iblocks = cap;
@@ -799,7 +805,7 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     e = cudaEventRecord(ss.ev_fork, st);
     if (e != cudaSuccess) return e;
     int nl = 0;
-    ile_stream_index_kernel<<<(unsigned)iblocks, IX_THREADS, 0, st>>>(hp, a, sp, sc.i0, sc.cell, sc.hist, segcnt);
+    ile_stream_index_kernel<<<(unsigned)iblocks, IX_THREADS, 0, st>>>(hp, a, sp, sc.i0, sc.cell, sc.hist);
     ++nl;
     e = cudaStreamWaitEvent(ss.aux, ss.ev_fork, 0);
     if (e != cudaSuccess) return e;
@@ -816,15 +822,18 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     ++nl;
     e = cudaEventRecord(ss.ev_join, ss.aux);
     if (e != cudaSuccess) return e;
-    const size_t scan_smem = (size_t)(nseg > sp.n0 ? nseg : sp.n0) * sizeof(uint32_t);
-    ile_stream_scan_kernel<<<dim3((unsigned)nseg, (unsigned)a.n_points), SS_THREADS, scan_smem, st>>>(sp.n0, nseg, sp.ncell, ss.slot_cap, sc.hist, segcnt,
-                                                                                                    ss.slots, ngr, ss.gcum, a.n_points);
+    ile_stream_scan_kernel<<<dim3((unsigned)nseg, (unsigned)a.n_points), SS_THREADS, (size_t)sp.n0 * sizeof(uint32_t), st>>>(sp.n0, nseg, sp.ncell,
+                                                                                                                            sc.hist, segtot);
     ++nl;
     if (a.n_points > 1) {
-        ile_stream_prefix_kernel<<<1, 1024, (size_t)a.n_points * sizeof(uint32_t), st>>>(a.n_points, ngr, ss.gcum);
+        ile_stream_prefix_kernel<<<1, 1024, (size_t)a.n_points * sizeof(uint32_t), st>>>(a.n_points, nseg, segtot, ss.gcum);
         ++nl;
     }
-    ile_stream_scatter_kernel<<<(unsigned)iblocks, IX_THREADS, 0, st>>>(a.n_per_point, a.n_points, sp.ncell, ss.slot_cap, sc.cell, sc.hist, ss.slots);
+    long long sblocks = (a.n_per_point + IX_THREADS - 1) / IX_THREADS;
+    const long long scap = ((long long)sz.sm_count * 8 + a.n_points - 1) / a.n_points;
+    if (sblocks > scap) sblocks = scap;
+    ile_stream_scatter_kernel<<<dim3((unsigned)sblocks, (unsigned)a.n_points), IX_THREADS, (size_t)nseg * sizeof(uint32_t), st>>>(
+        a.n_per_point, a.n_points, sp.ncell, sp.n0, nseg, ss.slot_cap, sc.cell, sc.hist, segtot, ss.slots, ss.gcum);
     ++nl;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;

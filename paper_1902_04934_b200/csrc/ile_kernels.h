@@ -63,7 +63,7 @@ struct IleSortScratch {
     double *quad;      // [n]
     int32_t *i0;       // [n][K]
     int32_t *cell;     // [n]
-    uint32_t *hist;    // [n_points][ncell] cell counts -> first slots, then [n_points][nseg] segment counts, then ILE_STREAM_MAX_RANGES claim counters
+    uint32_t *hist;    // [n_points][ncell] cell counts -> positions inside the segment, then ILE_STREAM_MAX_RANGES claim counters, then [n_points][nseg] segment totals
     double *qform;     // [n][K][3] quadratic forms from the FP64-MMA kernel, or NULL (the coefficient kernel computes them)
 };
 
@@ -82,7 +82,7 @@ struct IleStreamPlan {
 struct IleStreamScratch {
     const double *Qs;   // packed Q [P][K][ks][nqp][4]
     int32_t *slots;     // [n_points][slot_cap]: sample index or -1, groups of 8 consecutive slots
-    int32_t *gcum;      // [n_points + 1]: exclusive prefix of the group counts, followed by [n_points] group counts
+    int32_t *gcum;      // [n_points + 1]: exclusive prefix of the points' group counts
     int64_t slot_cap;   // slots per point (multiple of 8)
     cudaStream_t aux;   // side stream: the coefficient kernel runs there while the caller's stream sorts
     cudaEvent_t ev_fork, ev_join;
