@@ -67,7 +67,7 @@ static int check_device(const ile_ctx *c)
 #define ILE_QUAD_MMA_MIN_MODES 8
 #endif
 #ifndef ILE_STREAM_MIN_SAMPLES
-#define ILE_STREAM_MIN_SAMPLES 16384 /* automatic choice: batches per point from this size on take the streaming variant */
+#define ILE_STREAM_MIN_SAMPLES 10000 /* automatic choice: batches per point from this size on take the streaming variant */
 #endif
 #ifndef ILE_CHUNK_MAX
 #define ILE_CHUNK_MAX 1048576

@@ -64,25 +64,34 @@ __global__ void __launch_bounds__(SMP_THREADS) ile_sampler_uniform_kernel(unsign
     }
 }
 
-// tab: [3][n_bins] densities h, then [3][n_bins + 1] cumulatives C (S4: C[b+1] = C[b] + h[b] / n_bins, sequentially)
-__device__ __forceinline__ void smp_cumulative(const double *__restrict__ h, double *__restrict__ C, int nb)
+// tab: [3][n_bins] densities h, then [3][n_bins + 1] cumulatives C (S4: C[b+1] = C[b] + h[b] / n_bins, sequentially).
+// The divisions are done by all threads into `w` (shared, 3 n_bins doubles); thread j < 3 then runs the additions of
+// dimension j in bin order -- the same roundings as the plain loop.
+__device__ __forceinline__ void smp_cumulatives(const double *__restrict__ h, double *__restrict__ C, double *w, int nb)
 {
-    double run = 0.0;
-    C[0] = 0.0;
     const double dnb = (double)nb;
-    for (int b = 0; b < nb; ++b) {
-        run = __dadd_rn(run, __ddiv_rn(h[b], dnb));
-        C[b + 1] = run;
+    for (int i = threadIdx.x; i < 3 * nb; i += blockDim.x) w[i] = __ddiv_rn(h[i], dnb);
+    __syncthreads();
+    if (threadIdx.x < 3) {
+        const double *wj = w + threadIdx.x * nb;
+        double *Cj = C + threadIdx.x * (nb + 1);
+        double run = 0.0;
+        Cj[0] = 0.0;
+        for (int b = 0; b < nb; ++b) {
+            run = __dadd_rn(run, wj[b]);
+            Cj[b + 1] = run;
+        }
     }
 }
 
-__global__ void ile_sampler_tables_kernel(IleSamplerParams P, double *__restrict__ tab, int set_uniform)
+__global__ void __launch_bounds__(256) ile_sampler_tables_kernel(IleSamplerParams P, double *__restrict__ tab, int set_uniform)
 {
+    extern __shared__ double smp_w[];
     const int nb = P.n_bins;
     if (set_uniform)
         for (int i = threadIdx.x; i < 3 * nb; i += blockDim.x) tab[i] = 1.0;
     __syncthreads();
-    if (threadIdx.x < 3) smp_cumulative(tab + threadIdx.x * nb, tab + 3 * nb + threadIdx.x * (nb + 1), nb);
+    smp_cumulatives(tab, tab + 3 * nb, smp_w, nb);
 }
 
 __global__ void __launch_bounds__(SMP_THREADS)
@@ -135,18 +144,25 @@ __global__ void __launch_bounds__(SMP_THREADS)
     }
 }
 
-// S6: refit from one chunk.  One block; H[3][nb] 64-bit integer histograms in shared memory.
+// S6: refit from one chunk.  One block.  The fixed-point weights q < 2^42 are accumulated as three 14-bit pieces with native
+// 32-bit shared-memory atomics (sums stay below 2^32 for 2^18 samples) and folded exactly into 64-bit totals after every
+// 2^18 samples.
+#define SMP_REFIT_SUB 262144
 __global__ void __launch_bounds__(SMP_REFIT_THREADS)
     ile_sampler_refit_kernel(const __grid_constant__ IleSamplerParams P, double *__restrict__ tab, long long n,
                              const int32_t *__restrict__ bins, const double *__restrict__ lnL, const double *__restrict__ log_w)
 {
-    extern __shared__ unsigned long long smp_H[];  // [3][nb]
+    extern __shared__ __align__(8) unsigned char smp_raw[];
+    const int nb = P.n_bins, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double *w = reinterpret_cast<double *>(smp_raw);                       // [3][nb] bin widths for the cumulatives
+    unsigned long long *H64 = reinterpret_cast<unsigned long long *>(w + 3 * nb);  // [3][nb]
+    uint32_t *H = reinterpret_cast<uint32_t *>(H64 + 3 * nb);              // [3 pieces][3][nb]
     __shared__ double red[SMP_REFIT_THREADS / 32];
     __shared__ unsigned long long redq[3][SMP_REFIT_THREADS / 32];
     __shared__ double M_s;
     __shared__ unsigned long long tot_s[3];
-    const int nb = P.n_bins, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int i = threadIdx.x; i < 3 * nb; i += blockDim.x) smp_H[i] = 0ull;
+    for (int i = threadIdx.x; i < 9 * nb; i += blockDim.x) H[i] = 0u;
+    for (int i = threadIdx.x; i < 3 * nb; i += blockDim.x) H64[i] = 0ull;
     // chunk maximum of e = lnL + ln w
     double mx = -CUDART_INF;
     for (long long i = threadIdx.x; i < n; i += blockDim.x) mx = fmax(mx, lnL[i] + (log_w ? log_w[i] : 0.0));
@@ -161,22 +177,37 @@ __global__ void __launch_bounds__(SMP_REFIT_THREADS)
     __syncthreads();
     const double M = M_s;
     if (!(M > -CUDART_INF)) return;  // no finite sample: the densities are kept
-    for (long long i = threadIdx.x; i < n; i += blockDim.x) {
+    for (long long i0 = 0; i0 < n; i0 += SMP_REFIT_SUB) {
+    const long long i1 = i0 + SMP_REFIT_SUB < n ? i0 + SMP_REFIT_SUB : n;
+    for (long long i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
         const double e = lnL[i] + (log_w ? log_w[i] : 0.0);
         const double W = exp(__dmul_rn(P.temper, __dsub_rn(e, M)));  // exp(-inf) = 0
         const unsigned long long q = (unsigned long long)__double2ll_rn(__dmul_rn(W, 1099511627776.0));
         if (q) {
+            const uint32_t q0 = (uint32_t)(q & 0x3fffu), q1 = (uint32_t)((q >> 14) & 0x3fffu), q2 = (uint32_t)(q >> 28);
 #pragma unroll
             for (int j = 0; j < 3; ++j)
-                if (P.adapt[j]) atomicAdd(&smp_H[j * nb + bins[i * 3 + j]], q);
+                if (P.adapt[j]) {
+                    const int b = bins[i * 3 + j];
+                    if (q0) atomicAdd(&H[j * nb + b], q0);
+                    if (q1) atomicAdd(&H[(3 + j) * nb + b], q1);
+                    if (q2) atomicAdd(&H[(6 + j) * nb + b], q2);
+                }
         }
     }
     __syncthreads();
+    for (int i = threadIdx.x; i < 3 * nb; i += blockDim.x) {
+        H64[i] += (unsigned long long)H[i] + ((unsigned long long)H[3 * nb + i] << 14) + ((unsigned long long)H[6 * nb + i] << 28);
+        H[i] = 0u, H[3 * nb + i] = 0u, H[6 * nb + i] = 0u;
+    }
+    __syncthreads();
+    }
+    auto Hq = [&](int i) { return H64[i]; };
     // totals
     unsigned long long t[3] = {0ull, 0ull, 0ull};
     for (int b = threadIdx.x; b < nb; b += blockDim.x)
 #pragma unroll
-        for (int j = 0; j < 3; ++j) t[j] += smp_H[j * nb + b];
+        for (int j = 0; j < 3; ++j) t[j] += Hq(j * nb + b);
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
 #pragma unroll
@@ -186,7 +217,7 @@ __global__ void __launch_bounds__(SMP_REFIT_THREADS)
     __syncthreads();
     if (threadIdx.x < 3) {
         unsigned long long s = 0ull;
-        for (int w = 0; w < SMP_REFIT_THREADS / 32; ++w) s += redq[threadIdx.x][w];
+        for (int ww = 0; ww < SMP_REFIT_THREADS / 32; ++ww) s += redq[threadIdx.x][ww];
         tot_s[threadIdx.x] = s;
     }
     __syncthreads();
@@ -194,12 +225,10 @@ __global__ void __launch_bounds__(SMP_REFIT_THREADS)
     const double scale = __dmul_rn(__dsub_rn(1.0, P.floor_frac), (double)nb);
     for (int i = threadIdx.x; i < 3 * nb; i += blockDim.x) {
         const int j = i / nb;
-        if (P.adapt[j] && tot_s[j])
-            tab[i] = __dadd_rn(__dmul_rn(scale, __ddiv_rn((double)smp_H[i], (double)tot_s[j])), P.floor_frac);
+        if (P.adapt[j] && tot_s[j]) tab[i] = __dadd_rn(__dmul_rn(scale, __ddiv_rn((double)Hq(i), (double)tot_s[j])), P.floor_frac);
     }
     __syncthreads();
-    if (threadIdx.x < 3 && P.adapt[threadIdx.x] && tot_s[threadIdx.x])
-        smp_cumulative(tab + threadIdx.x * nb, tab + 3 * nb + threadIdx.x * (nb + 1), nb);
+    smp_cumulatives(tab, tab + 3 * nb, w, nb);  // a dimension that was not refit gets the cumulative it already had
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -216,7 +245,7 @@ size_t ile_sampler_table_doubles(int32_t n_bins) { return (size_t)3 * n_bins + (
 
 cudaError_t ile_launch_sampler_tables(const IleSamplerParams &P, double *tab, int set_uniform, cudaStream_t st)
 {
-    ile_sampler_tables_kernel<<<1, 256, 0, st>>>(P, tab, set_uniform);
+    ile_sampler_tables_kernel<<<1, 256, (size_t)3 * P.n_bins * sizeof(double), st>>>(P, tab, set_uniform);
     return cudaGetLastError();
 }
 
@@ -242,6 +271,7 @@ cudaError_t ile_launch_sampler_refit(const IleSamplerParams &P, double *tab, lon
                                      const double *log_w, cudaStream_t st)
 {
     if (n <= 0) return cudaSuccess;
-    ile_sampler_refit_kernel<<<1, SMP_REFIT_THREADS, (size_t)3 * P.n_bins * sizeof(unsigned long long), st>>>(P, tab, n, bins, lnL, log_w);
+    const size_t smem = (size_t)3 * P.n_bins * (sizeof(double) + sizeof(unsigned long long)) + (size_t)9 * P.n_bins * sizeof(uint32_t);
+    ile_sampler_refit_kernel<<<1, SMP_REFIT_THREADS, smem, st>>>(P, tab, n, bins, lnL, log_w);
     return cudaGetLastError();
 }

@@ -261,7 +261,7 @@ def test_edge_all_out_of_range_gives_minus_inf_evidence(gpu_lib, variant):
 
 
 def test_edge_streaming_batch_touching_both_ends_of_Q(gpu_lib):
-    """A production-size batch (>= 16,384 samples: the automatic choice is the streaming kernel) whose windows reach the
+    """A production-size batch (>= 10,000 samples: the automatic choice is the streaming kernel) whose windows reach the
     first and the last stored Q sample -- the kernel then reads the zero padding in front of and behind the packed
     series -- with a few samples just out of range (reading R9: -inf + counter, never wrapped or clamped)."""
     cfg = gi.make_config(1)
@@ -461,7 +461,7 @@ def test_every_variant_matches_the_oracle(gpu_lib, variant):
 
 
 def test_many_modes_quadratic_term_as_mma_with_generic_U_V(gpu_lib):
-    """21 modes through the streaming variant (n >= 16384): the quadratic term runs as the FP64-MMA contraction of
+    """21 modes through the streaming variant (n >= 10000): the quadratic term runs as the FP64-MMA contraction of
     ile_quad_mma.cu.  U deliberately not Hermitian, V not symmetric (reading R15); ragged sample count (not a multiple
     of 8) so the last group of 8 is partial."""
     cfg = gi.make_config(2, n=20_003)
