@@ -128,8 +128,10 @@ cudaError_t ile_launch_sampler_uniforms(const IleSamplerParams &P, int sm_count,
 cudaError_t ile_launch_sampler_draw(const IleSamplerParams &P, int sm_count, const double *tab, long long first, long long n, double *ra,
                                     double *dec, double *t_ref, double *phi_ref, double *psi, double *incl, double *dist, double *log_w,
                                     int32_t *bins, cudaStream_t st);
-cudaError_t ile_launch_sampler_refit(const IleSamplerParams &P, double *tab, long long n, const int32_t *bins, const double *lnL,
-                                     const double *log_w, cudaStream_t st);
+size_t ile_sampler_work_words(int32_t n_bins);  // 64-bit words of refit scratch
+cudaError_t ile_sampler_work_init(const IleSamplerParams &P, unsigned long long *work, cudaStream_t st);
+cudaError_t ile_launch_sampler_refit(const IleSamplerParams &P, int sm_count, double *tab, long long n, const int32_t *bins, const double *lnL,
+                                     const double *log_w, unsigned long long *work, cudaStream_t st);  // 2 kernels
 
 // ---- extrinsic posterior harvesting (ile_harvest.cu; NEXT-3) -------------------------------------------------------------
 cudaError_t ile_launch_harvest(const IleSizes &sz, const IleEvalArgs &a, long long n_sel, const long long *ids, const double *v_uniform,

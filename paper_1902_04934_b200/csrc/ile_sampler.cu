@@ -144,70 +144,86 @@ __global__ void __launch_bounds__(SMP_THREADS)
     }
 }
 
-// S6: refit from one chunk.  One block.  The fixed-point weights q < 2^42 are accumulated as three 14-bit pieces with native
-// 32-bit shared-memory atomics (sums stay below 2^32 for 2^18 samples) and folded exactly into 64-bit totals after every
-// 2^18 samples.
-#define SMP_REFIT_SUB 262144
+// S6: refit from one chunk, two kernels.  (1) chunk maximum of e = lnL + ln w into an order-preserving integer key.
+// (2) every block histograms its slice of the chunk: the fixed-point weights q < 2^42 are accumulated as three 14-bit pieces with
+// native 32-bit shared-memory atomics (a block sees at most 2^18 samples, so the sums stay below 2^32), reassembled exactly and
+// added to the 64-bit global histograms; the block that finishes last (ticket) turns them into the new densities and cumulatives
+// and leaves the scratch (histograms, key, ticket) zeroed for the next call.
+// work: [3 n_bins] 64-bit histograms | key | ticket
+#define SMP_REFIT_SLICE 262144
+__device__ __forceinline__ long long smp_key(double x)
+{
+    const long long b = __double_as_longlong(x);
+    return b >= 0 ? b : b ^ 0x7fffffffffffffffLL;
+}
+__device__ __forceinline__ double smp_unkey(long long k) { return __longlong_as_double(k >= 0 ? k : k ^ 0x7fffffffffffffffLL); }
+#define SMP_KEY_NEG_INF 0x800FFFFFFFFFFFFFLL /* smp_key(-inf) */
+
+__global__ void __launch_bounds__(SMP_THREADS) ile_sampler_refit_max_kernel(long long n, const double *__restrict__ lnL,
+                                                                            const double *__restrict__ log_w, long long *__restrict__ key)
+{
+    double mx = -CUDART_INF;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
+        const double e = lnL[i] + (log_w ? log_w[i] : 0.0);
+        if (e == e) mx = fmax(mx, e);
+    }
+    mx = warp_max(mx);
+    if ((threadIdx.x & 31) == 0 && mx > -CUDART_INF) atomicMax(key, smp_key(mx));
+}
+
 __global__ void __launch_bounds__(SMP_REFIT_THREADS)
     ile_sampler_refit_kernel(const __grid_constant__ IleSamplerParams P, double *__restrict__ tab, long long n,
-                             const int32_t *__restrict__ bins, const double *__restrict__ lnL, const double *__restrict__ log_w)
+                             const int32_t *__restrict__ bins, const double *__restrict__ lnL, const double *__restrict__ log_w,
+                             unsigned long long *__restrict__ work)
 {
     extern __shared__ __align__(8) unsigned char smp_raw[];
     const int nb = P.n_bins, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    double *w = reinterpret_cast<double *>(smp_raw);                       // [3][nb] bin widths for the cumulatives
-    unsigned long long *H64 = reinterpret_cast<unsigned long long *>(w + 3 * nb);  // [3][nb]
-    uint32_t *H = reinterpret_cast<uint32_t *>(H64 + 3 * nb);              // [3 pieces][3][nb]
-    __shared__ double red[SMP_REFIT_THREADS / 32];
+    double *w = reinterpret_cast<double *>(smp_raw);          // [3][nb] bin widths for the cumulatives (last block)
+    uint32_t *H = reinterpret_cast<uint32_t *>(w + 3 * nb);   // [3 pieces][3][nb]
     __shared__ unsigned long long redq[3][SMP_REFIT_THREADS / 32];
-    __shared__ double M_s;
     __shared__ unsigned long long tot_s[3];
-    for (int i = threadIdx.x; i < 9 * nb; i += blockDim.x) H[i] = 0u;
-    for (int i = threadIdx.x; i < 3 * nb; i += blockDim.x) H64[i] = 0ull;
-    // chunk maximum of e = lnL + ln w
-    double mx = -CUDART_INF;
-    for (long long i = threadIdx.x; i < n; i += blockDim.x) mx = fmax(mx, lnL[i] + (log_w ? log_w[i] : 0.0));
-    mx = warp_max(mx);
-    if (lane == 0) red[warp] = mx;
-    __syncthreads();
-    if (warp == 0) {
-        double v = lane < SMP_REFIT_THREADS / 32 ? red[lane] : -CUDART_INF;
-        v = warp_max(v);
-        if (lane == 0) M_s = v;
-    }
-    __syncthreads();
-    const double M = M_s;
-    if (!(M > -CUDART_INF)) return;  // no finite sample: the densities are kept
-    for (long long i0 = 0; i0 < n; i0 += SMP_REFIT_SUB) {
-    const long long i1 = i0 + SMP_REFIT_SUB < n ? i0 + SMP_REFIT_SUB : n;
-    for (long long i = i0 + threadIdx.x; i < i1; i += blockDim.x) {
-        const double e = lnL[i] + (log_w ? log_w[i] : 0.0);
-        const double W = exp(__dmul_rn(P.temper, __dsub_rn(e, M)));  // exp(-inf) = 0
-        const unsigned long long q = (unsigned long long)__double2ll_rn(__dmul_rn(W, 1099511627776.0));
-        if (q) {
-            const uint32_t q0 = (uint32_t)(q & 0x3fffu), q1 = (uint32_t)((q >> 14) & 0x3fffu), q2 = (uint32_t)(q >> 28);
+    __shared__ bool last_s;
+    long long *key = reinterpret_cast<long long *>(work + 3 * nb);
+    unsigned int *ticket = reinterpret_cast<unsigned int *>(work + 3 * nb + 1);
+    const double M = smp_unkey(*key);
+    if (M > -CUDART_INF) {  // otherwise no finite sample: the densities are kept (the last block still cleans up)
+        for (int i = threadIdx.x; i < 9 * nb; i += blockDim.x) H[i] = 0u;
+        __syncthreads();
+        const long long per = (n + gridDim.x - 1) / gridDim.x;  // <= SMP_REFIT_SLICE by the launcher's grid
+        const long long lo = (long long)blockIdx.x * per, hi = lo + per < n ? lo + per : n;
+        for (long long i = lo + threadIdx.x; i < hi; i += blockDim.x) {
+            const double e = lnL[i] + (log_w ? log_w[i] : 0.0);
+            const double W = exp(__dmul_rn(P.temper, __dsub_rn(e, M)));  // exp(-inf) = 0
+            const unsigned long long q = (unsigned long long)__double2ll_rn(__dmul_rn(W, 1099511627776.0));
+            if (q) {
+                const uint32_t q0 = (uint32_t)(q & 0x3fffu), q1 = (uint32_t)((q >> 14) & 0x3fffu), q2 = (uint32_t)(q >> 28);
 #pragma unroll
-            for (int j = 0; j < 3; ++j)
-                if (P.adapt[j]) {
-                    const int b = bins[i * 3 + j];
-                    if (q0) atomicAdd(&H[j * nb + b], q0);
-                    if (q1) atomicAdd(&H[(3 + j) * nb + b], q1);
-                    if (q2) atomicAdd(&H[(6 + j) * nb + b], q2);
-                }
+                for (int j = 0; j < 3; ++j)
+                    if (P.adapt[j]) {
+                        const int b = bins[i * 3 + j];
+                        if (q0) atomicAdd(&H[j * nb + b], q0);
+                        if (q1) atomicAdd(&H[(3 + j) * nb + b], q1);
+                        if (q2) atomicAdd(&H[(6 + j) * nb + b], q2);
+                    }
+            }
+        }
+        __syncthreads();
+        for (int i = threadIdx.x; i < 3 * nb; i += blockDim.x) {
+            const unsigned long long v = (unsigned long long)H[i] + ((unsigned long long)H[3 * nb + i] << 14) + ((unsigned long long)H[6 * nb + i] << 28);
+            if (v) atomicAdd(&work[i], v);
         }
     }
+    __threadfence();
     __syncthreads();
-    for (int i = threadIdx.x; i < 3 * nb; i += blockDim.x) {
-        H64[i] += (unsigned long long)H[i] + ((unsigned long long)H[3 * nb + i] << 14) + ((unsigned long long)H[6 * nb + i] << 28);
-        H[i] = 0u, H[3 * nb + i] = 0u, H[6 * nb + i] = 0u;
-    }
+    if (threadIdx.x == 0) last_s = atomicAdd(ticket, 1u) == gridDim.x - 1;
     __syncthreads();
-    }
-    auto Hq = [&](int i) { return H64[i]; };
-    // totals
+    if (!last_s) return;
+    __threadfence();
+    // ---- the last block: totals, densities, cumulatives; scratch back to zero
     unsigned long long t[3] = {0ull, 0ull, 0ull};
     for (int b = threadIdx.x; b < nb; b += blockDim.x)
 #pragma unroll
-        for (int j = 0; j < 3; ++j) t[j] += Hq(j * nb + b);
+        for (int j = 0; j < 3; ++j) t[j] += __ldcg(&work[j * nb + b]);
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
 #pragma unroll
@@ -225,7 +241,13 @@ __global__ void __launch_bounds__(SMP_REFIT_THREADS)
     const double scale = __dmul_rn(__dsub_rn(1.0, P.floor_frac), (double)nb);
     for (int i = threadIdx.x; i < 3 * nb; i += blockDim.x) {
         const int j = i / nb;
-        if (P.adapt[j] && tot_s[j]) tab[i] = __dadd_rn(__dmul_rn(scale, __ddiv_rn((double)Hq(i), (double)tot_s[j])), P.floor_frac);
+        if (P.adapt[j] && tot_s[j])
+            tab[i] = __dadd_rn(__dmul_rn(scale, __ddiv_rn((double)__ldcg(&work[i]), (double)tot_s[j])), P.floor_frac);
+        work[i] = 0ull;
+    }
+    if (threadIdx.x == 0) {
+        *key = SMP_KEY_NEG_INF;
+        *ticket = 0u;
     }
     __syncthreads();
     smp_cumulatives(tab, tab + 3 * nb, w, nb);  // a dimension that was not refit gets the cumulative it already had
@@ -267,11 +289,26 @@ cudaError_t ile_launch_sampler_draw(const IleSamplerParams &P, int sm_count, con
     return cudaGetLastError();
 }
 
-cudaError_t ile_launch_sampler_refit(const IleSamplerParams &P, double *tab, long long n, const int32_t *bins, const double *lnL,
-                                     const double *log_w, cudaStream_t st)
+size_t ile_sampler_work_words(int32_t n_bins) { return (size_t)3 * n_bins + 2; }  // 64-bit words, zero + key = -inf before the first call
+
+cudaError_t ile_sampler_work_init(const IleSamplerParams &P, unsigned long long *work, cudaStream_t st)
+{
+    cudaError_t e = cudaMemsetAsync(work, 0, ile_sampler_work_words(P.n_bins) * sizeof(unsigned long long), st);
+    if (e != cudaSuccess) return e;
+    const long long k = SMP_KEY_NEG_INF;
+    return cudaMemcpyAsync(work + 3 * P.n_bins, &k, sizeof(k), cudaMemcpyHostToDevice, st);
+}
+
+cudaError_t ile_launch_sampler_refit(const IleSamplerParams &P, int sm_count, double *tab, long long n, const int32_t *bins, const double *lnL,
+                                     const double *log_w, unsigned long long *work, cudaStream_t st)
 {
     if (n <= 0) return cudaSuccess;
-    const size_t smem = (size_t)3 * P.n_bins * (sizeof(double) + sizeof(unsigned long long)) + (size_t)9 * P.n_bins * sizeof(uint32_t);
-    ile_sampler_refit_kernel<<<1, SMP_REFIT_THREADS, smem, st>>>(P, tab, n, bins, lnL, log_w);
+    ile_sampler_refit_max_kernel<<<smp_grid(n, sm_count), SMP_THREADS, 0, st>>>(n, lnL, log_w, reinterpret_cast<long long *>(work + 3 * P.n_bins));
+    long long g = (n + 8191) / 8192;  // 8 samples per thread and block while the grid allows
+    if (g > sm_count) g = sm_count;
+    const long long gmin = (n + SMP_REFIT_SLICE - 1) / SMP_REFIT_SLICE;  // a block's 32-bit piece sums must not overflow
+    if (g < gmin) g = gmin;
+    const size_t smem = (size_t)3 * P.n_bins * sizeof(double) + (size_t)9 * P.n_bins * sizeof(uint32_t);
+    ile_sampler_refit_kernel<<<(unsigned)g, SMP_REFIT_THREADS, smem, st>>>(P, tab, n, bins, lnL, log_w, work);
     return cudaGetLastError();
 }

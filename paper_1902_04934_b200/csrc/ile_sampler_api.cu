@@ -11,6 +11,7 @@ struct ile_sampler {
     int device, sm_count;
     IleSamplerParams P;
     double *d_tab;        // h [3][nb] | C [3][nb + 1]
+    unsigned long long *d_work;  // refit scratch: 64-bit histograms, maximum key, ticket (every refit leaves it clean)
     // scratch of ile_integrate (grown on demand): seven sample arrays, ln w, lnL ([9][cap] doubles), bins [cap][3]
     double *d_buf;
     int32_t *d_bins;
@@ -69,6 +70,8 @@ extern "C" int ile_sampler_create(ile_sampler **out, const ile_sampler_config *c
     P.d3_span = cfg->dist_max_mpc * cfg->dist_max_mpc * cfg->dist_max_mpc - P.dmin3;
     cudaError_t e = cudaMalloc(&s->d_tab, ile_sampler_table_doubles(P.n_bins) * sizeof(double));
     if (e == cudaSuccess) e = cudaMalloc(&s->d_state, 8 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&s->d_work, ile_sampler_work_words(P.n_bins) * sizeof(unsigned long long));
+    if (e == cudaSuccess) e = ile_sampler_work_init(P, s->d_work, 0);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->ev[0], cudaEventDisableTiming);
     if (e == cudaSuccess) e = cudaEventCreateWithFlags(&s->ev[1], cudaEventDisableTiming);
     if (e == cudaSuccess) e = ile_launch_sampler_tables(P, s->d_tab, 1, 0);
@@ -86,6 +89,7 @@ extern "C" void ile_sampler_destroy(ile_sampler *s)
 {
     if (!s) return;
     cudaFree(s->d_tab);
+    cudaFree(s->d_work);
     cudaFree(s->d_buf);
     cudaFree(s->d_bins);
     cudaFree(s->d_state);
@@ -159,8 +163,8 @@ extern "C" int ile_sampler_refit(ile_sampler *s, int64_t n, const int32_t *bin_i
     if (n == 0) return ILE_OK;
     if (!bin_idx || !lnL_margT) return ILE_ERR_BAD_ARGUMENT;
     if (int r = smp_check_device(s)) return r;
-    CK(ile_launch_sampler_refit(s->P, s->d_tab, n, bin_idx, lnL_margT, log_w, (cudaStream_t)cuda_stream));
-    s->launches += 1;
+    CK(ile_launch_sampler_refit(s->P, s->sm_count, s->d_tab, n, bin_idx, lnL_margT, log_w, s->d_work, (cudaStream_t)cuda_stream));
+    s->launches += 2;
     return ILE_OK;
 }
 
