@@ -131,6 +131,18 @@ int ile_evidence_merge(ile_ctx *ctx, int32_t n_segments, int32_t n_states, const
 int ile_precompute(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_q, double fs_hz, double t0_q_s, const void *x,
                    const void *d, void *Q, void *U, void *V, void *cuda_stream);
 
+/* The same from UN-whitened spectra with the inner product of eq. 2 (L30-L35), <a|b>_k = 2 int_{f_min < |f| < f_max} a~*(f) b~(f) /
+ * S_k(|f|) df: every sum over n above carries the weight g_k[n] = scale / S[p][k][n] for f_min_hz < |f_n| < f_max_hz and 0
+ * outside the band ("the inner products necessary to evaluate Q", L97, with the 1/S_n weighting and the band cut done on the
+ * device):
+ *   Q = sum_n g conj(h) d exp(...),   U = sum_n g conj(h_a) h_b,   V = sum_n g h_a[(-n) mod n_q] h_b[n]
+ * h: device complex128 [P][K][M][n_q] mode spectra, d: device complex128 [P][K][n_q] data spectra, S: device double [P][K][n_q]
+ * the one-sided noise power spectral density sampled at |f_n| in FFT order (> 0 inside the band), scale: the measure (2 df for
+ * eq. 2 as printed, times the caller's Fourier-transform normalisation).  n_q a power of two, 512..8192. */
+int ile_precompute_psd(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_q, double fs_hz, double t0_q_s, const void *h,
+                       const void *d, const double *S, double f_min_hz, double f_max_hz, double scale, void *Q, void *U, void *V,
+                       void *cuda_stream);
+
 /* Whole hot path from HOST buffers, for callers that keep samples on the host (the paper's workflow, L97: blocks
  * generated on the CPU and transferred to the board): H2D copy of the seven sample arrays (+ log_w), ile_eval,
  * ile_evidence, D2H of lnL_margT (if not NULL), lnZ and n_eff.  Host arrays of n doubles each; pinned memory makes

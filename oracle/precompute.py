@@ -71,3 +71,60 @@ def overlaps_direct(x, d, fs_hz: float, t0_q_s: float):
                 U[k, a, b] = u
                 V[k, a, b] = v
     return Q, U, V
+
+
+def psd_weights(n_q: int, S_k, fs_hz: float, f_min_hz: float, f_max_hz: float, scale: float):
+    """Weight of frequency n in eq. 2 (<a|b>_k = 2 int_{f_min < |f| < f_max} a~*(f) b~(f) / S_k(|f|) df,
+    two-sided): scale / S_k(|f_n|) inside the band f_min < |f_n| < f_max, 0 outside.  S_k is the one-sided PSD sampled at
+    |f_n| on the FFT grid (FFT order); `scale` carries the measure (2 df for the integral as printed, times whatever the
+    caller's Fourier convention asks for)."""
+    af = np.abs(signed_index(n_q) * (fs_hz / n_q))
+    return np.where((af > f_min_hz) & (af < f_max_hz), scale / np.asarray(S_k, dtype=np.float64), 0.0)
+
+
+def overlaps_psd(h, d, S, fs_hz: float, t0_q_s: float, f_min_hz: float, f_max_hz: float, scale: float):
+    """eq. 8a-c with eq. 2's weighting on UN-whitened spectra: h [K][M][N], d [K][N], S [K][N] (real, > 0 in the band).
+        Q[k][a][i] = sum_n g_k[n] conj(h[k][a][n]) d[k][n] exp(+2 pi i f_n (t0_Q + i / f_s))
+        U[k][a][b] = sum_n g_k[n] conj(h[k][a][n]) h[k][b][n],   V[k][a][b] = sum_n g_k[n] h[k][a][(-n) mod N] h[k][b][n]
+    Q by one inverse FFT per series, U and V by the sums as written."""
+    h = np.asarray(h, dtype=np.complex128)
+    d = np.asarray(d, dtype=np.complex128)
+    K, M, N = h.shape
+    f = signed_index(N) * (fs_hz / N)
+    neg = (-np.arange(N)) % N
+    Q = np.empty((K, M, N), dtype=np.complex128)
+    U = np.empty((K, M, M), dtype=np.complex128)
+    V = np.empty((K, M, M), dtype=np.complex128)
+    for k in range(K):
+        g = psd_weights(N, S[k], fs_hz, f_min_hz, f_max_hz, scale)
+        shifted = d[k] * np.exp(2j * np.pi * f * t0_q_s) * g
+        for a in range(M):
+            Q[k, a] = np.fft.ifft(np.conj(h[k, a]) * shifted) * N
+            for b in range(M):
+                U[k, a, b] = np.sum(g * np.conj(h[k, a]) * h[k, b])
+                V[k, a, b] = np.sum(g * h[k, a][neg] * h[k, b])
+    return Q, U, V
+
+
+def overlaps_direct_psd(h, d, S, fs_hz: float, t0_q_s: float, f_min_hz: float, f_max_hz: float, scale: float):
+    """overlaps_psd term by term (pure Python loops: tiny inputs only)."""
+    h = np.asarray(h, dtype=np.complex128)
+    d = np.asarray(d, dtype=np.complex128)
+    K, M, N = h.shape
+    npr = signed_index(N)
+    Q = np.zeros((K, M, N), dtype=np.complex128)
+    U = np.zeros((K, M, M), dtype=np.complex128)
+    V = np.zeros((K, M, M), dtype=np.complex128)
+    for k in range(K):
+        for n in range(N):
+            fn = npr[n] * fs_hz / N
+            if not (f_min_hz < abs(fn) < f_max_hz):
+                continue
+            g = scale / S[k][n]
+            for a in range(M):
+                for i in range(N):
+                    Q[k, a, i] += g * np.conj(h[k, a, n]) * d[k, n] * np.exp(2j * np.pi * fn * (t0_q_s + i / fs_hz))
+                for b in range(M):
+                    U[k, a, b] += g * np.conj(h[k, a, n]) * h[k, b, n]
+                    V[k, a, b] += g * h[k, a, (-n) % N] * h[k, b, n]
+    return Q, U, V

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libile_b200.so")
 _lib = None
 
 SAMPLE_FIELDS = ("ra", "dec", "t_ref", "phi_ref", "psi", "incl", "dist_mpc")
-EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_evidence_merge", "ile_precompute", "ile_run_host", "ile_run_host_all", "ile_status",
+EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_evidence_merge", "ile_precompute", "ile_precompute_psd", "ile_run_host", "ile_run_host_all", "ile_status",
            "ile_set_variant", "ile_launch_count", "ile_measure_fp64_peak", "ile_measure_dmma_peak", "ile_destroy", "ile_strerror",
            "ile_sampler_create", "ile_sampler_destroy", "ile_sampler_reset", "ile_sampler_set_tables", "ile_sampler_get_tables",
            "ile_sampler_uniforms", "ile_sampler_draw", "ile_sampler_refit", "ile_sampler_launch_count", "ile_integrate",
@@ -68,6 +68,8 @@ def load():
     L.ile_evidence_reset.argtypes = [vp, i32, vp, vp]
     L.ile_evidence_merge.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
     L.ile_precompute.argtypes = [i32, i32, i32, i32, ctypes.c_double, ctypes.c_double, vp, vp, vp, vp, vp, vp]
+    L.ile_precompute_psd.argtypes = [i32, i32, i32, i32, ctypes.c_double, ctypes.c_double, vp, vp, vp, ctypes.c_double, ctypes.c_double,
+                                     ctypes.c_double, vp, vp, vp, vp]
     L.ile_run_host.argtypes = [vp, i32, i64] + [vp] * 7 + [vp, vp, dp, dp, vp]
     L.ile_run_host_all.argtypes = [vp, i64] + [vp] * 7 + [vp, vp, dp, dp, vp]
     L.ile_status.argtypes = [vp, ctypes.POINTER(i64), ctypes.c_int, vp]
@@ -417,6 +419,23 @@ def precompute(x, d, fs_hz: float, t0_q_s: float, stream=None):
     V = torch.empty((P, K, M, M), dtype=torch.complex128, device=x.device)
     _check(load().ile_precompute(P, K, M, N, float(fs_hz), float(t0_q_s), _ptr(x), _ptr(d), _ptr(Q), _ptr(U), _ptr(V),
                                  _stream_ptr(stream)), "ile_precompute")
+    return Q, U, V
+
+
+def precompute_psd(h, d, S, fs_hz: float, t0_q_s: float, f_min_hz: float, f_max_hz: float, scale: float, stream=None):
+    """ile_precompute_psd: un-whitened mode spectra h [P][K][M][N], data spectra d [P][K][N] (CUDA complex128), one-sided PSD
+    S [P][K][N] (CUDA float64, FFT order) -> (Q, U, V) with eq. 2's 1/S weighting and band cut applied on the device."""
+    import torch
+
+    assert h.is_cuda and d.is_cuda and S.is_cuda and h.dtype == torch.complex128 and d.dtype == torch.complex128 and S.dtype == torch.float64
+    assert h.is_contiguous() and d.is_contiguous() and S.is_contiguous() and h.dim() == 4 and tuple(d.shape) == (h.shape[0], h.shape[1], h.shape[3])
+    assert tuple(S.shape) == tuple(d.shape)
+    P, K, M, N = (int(v) for v in h.shape)
+    Q = torch.empty((P, K, M, N), dtype=torch.complex128, device=h.device)
+    U = torch.empty((P, K, M, M), dtype=torch.complex128, device=h.device)
+    V = torch.empty((P, K, M, M), dtype=torch.complex128, device=h.device)
+    _check(load().ile_precompute_psd(P, K, M, N, float(fs_hz), float(t0_q_s), _ptr(h), _ptr(d), _ptr(S), float(f_min_hz), float(f_max_hz),
+                                     float(scale), _ptr(Q), _ptr(U), _ptr(V), _stream_ptr(stream)), "ile_precompute_psd")
     return Q, U, V
 
 

@@ -461,18 +461,34 @@ extern "C" int ile_evidence(ile_ctx *c, int32_t n_segments, int64_t n_per_segmen
     return ILE_OK;
 }
 
-extern "C" int ile_precompute(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_q, double fs_hz, double t0_q_s,
-                              const void *x, const void *d, void *Q, void *U, void *V, void *cuda_stream)
+static int precompute_any(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_q, double fs_hz, double t0_q_s, const void *x,
+                          const void *d, const double *S, double f_min_hz, double f_max_hz, double scale, void *Q, void *U, void *V,
+                          void *cuda_stream)
 {
     if (n_points < 1 || n_det < 1 || n_modes < 1 || n_q < 1 || !(fs_hz > 0.0) || !x || !d || !Q || !U || !V) return ILE_ERR_BAD_ARGUMENT;
     if (n_det > ILE_MAX_DET || n_modes > ILE_MAX_MODES || n_q < 2 || n_q > 8192 || (n_q & (n_q - 1))) return ILE_ERR_UNSUPPORTED;
+    if (S && n_q < 512) return ILE_ERR_UNSUPPORTED;
     int dev = 0, optin = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return ILE_ERR_NO_DEVICE;
     CK(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev));
-    cudaError_t e = ile_launch_precompute(n_points, n_det, n_modes, n_q, fs_hz, t0_q_s, (const double2 *)x, (const double2 *)d,
-                                          (double2 *)Q, (double2 *)U, (double2 *)V, optin, (cudaStream_t)cuda_stream);
+    cudaError_t e = ile_launch_precompute(n_points, n_det, n_modes, n_q, fs_hz, t0_q_s, (const double2 *)x, (const double2 *)d, S, f_min_hz,
+                                          f_max_hz, scale, (double2 *)Q, (double2 *)U, (double2 *)V, optin, (cudaStream_t)cuda_stream);
     if (e != cudaSuccess) return cuda_fail(e);
     return ILE_OK;
+}
+
+extern "C" int ile_precompute(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_q, double fs_hz, double t0_q_s,
+                              const void *x, const void *d, void *Q, void *U, void *V, void *cuda_stream)
+{
+    return precompute_any(n_points, n_det, n_modes, n_q, fs_hz, t0_q_s, x, d, nullptr, 0.0, 0.0, 1.0, Q, U, V, cuda_stream);
+}
+
+extern "C" int ile_precompute_psd(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_q, double fs_hz, double t0_q_s,
+                                  const void *h, const void *d, const double *S, double f_min_hz, double f_max_hz, double scale, void *Q,
+                                  void *U, void *V, void *cuda_stream)
+{
+    if (!S || !(f_max_hz > f_min_hz) || !(f_min_hz >= 0.0) || !std::isfinite(scale)) return ILE_ERR_BAD_ARGUMENT;
+    return precompute_any(n_points, n_det, n_modes, n_q, fs_hz, t0_q_s, h, d, S, f_min_hz, f_max_hz, scale, Q, U, V, cuda_stream);
 }
 
 extern "C" int ile_evidence_merge(ile_ctx *c, int32_t n_segments, int32_t n_states, const double *states_in, double *state_out,

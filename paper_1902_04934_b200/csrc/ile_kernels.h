@@ -142,7 +142,8 @@ cudaError_t ile_launch_resample(const IleSizes &sz, long long n, const double *l
 
 // overlap pre-computation (ile_precompute.cu)
 cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_t N, double fs_hz, double t0_q_s, const double2 *x,
-                                  const double2 *d, double2 *Q, double2 *U, double2 *V, int32_t max_smem_optin, cudaStream_t st);
+                                  const double2 *d, const double *S /* NULL: whitened spectra */, double f_min_hz, double f_max_hz,
+                                  double scale, double2 *Q, double2 *U, double2 *V, int32_t max_smem_optin, cudaStream_t st);
 
 // evidence: one kernel (per-block partials; the block of a segment that finishes last folds them into the carried state).
 // partials: n_segments * blocks_per_seg * 2 doubles; tickets: n_segments words, zero on entry, left zero on exit

@@ -8,11 +8,13 @@
 // products per (point, detector).
 //
 //   ile_overlap_tables_kernel      twiddles exp(2 pi i j / N) and start-time phases exp(2 pi i f_n t0_Q), once per (N, t0_Q)
-//   ile_overlap_q_stockham_kernel  N <= 4096, one block per series: spectrum product and start-time phase on load, Stockham
-//                                  autosort radix-4 passes (+ one radix-2) between two shared-memory buffers, natural order in
-//                                  and out; elements per thread known at compile time
-//   ile_overlap_q_kernel           N = 8192: in-place radix-2 with a bit-reversed load (one buffer fits shared memory)
-//   ile_overlap_uv_kernel          one block per (detector, point): register-blocked tiles of pairs (a, b), lanes over frequencies
+//   ile_overlap_q_radix8_kernel    512 <= N <= 8192, N / 8 threads per series: register-resident radix-8 Stockham passes, first pass
+//                                  from global memory (spectrum product, optional 1/S weight and band mask, start-time phase), last
+//                                  pass to global memory, one padded shared buffer in between
+//   ile_overlap_q_stockham_kernel  N < 512: radix-4 Stockham passes between two shared buffers (whitened spectra only)
+//   ile_overlap_uv_small_kernel    M <= 5: one block per (detector, point), every pair's sum in registers, a <= b only
+//   ile_overlap_uv_kernel          any M: register-blocked tiles of pairs (a, b), lanes over frequencies
+// With S != NULL the inner products are eq. 2's (L30-L35): weight scale / S_k(|f_n|) inside f_min < |f_n| < f_max, 0 outside.
 #include "ile_kernels.h"
 
 #define PC_THREADS 256
@@ -124,35 +126,134 @@ __global__ void __launch_bounds__(PC_THREADS)
     for (int i = threadIdx.x; i < N; i += PC_THREADS) __stcs(q + i, in[i]);
 }
 
-__global__ void __launch_bounds__(PC_THREADS)
-    ile_overlap_q_kernel(int32_t M, int32_t N, int32_t log2n, const double2 *__restrict__ tab, const double2 *__restrict__ x,
-                         const double2 *__restrict__ d, double2 *__restrict__ Q)
+// ------------------------------------------------------------------------------------------------------------
+// Radix-8 Stockham transform, 512 <= N <= 8192, N / 8 threads per series: a thread owns one radix-8 butterfly per pass and keeps
+// its eight points in registers.  The first pass takes its inputs straight from global memory (spectrum product, 1/S weight,
+// band mask and start-time phase applied on the way), the last pass stores straight to Q; in between the points go through ONE
+// shared buffer (read - barrier - write - barrier), padded by one element per eight so that every 16-byte access pattern of
+// every pass is conflict free (quarter warps touch 128 consecutive bytes).  2048 points: passes 8, 8, 8, 4 -- three trips
+// through shared memory instead of the six of the radix-4 form.
+// ------------------------------------------------------------------------------------------------------------
+#define PC_PAD(i) ((i) + ((i) >> 3))
+
+__device__ __forceinline__ double2 pc_add(double2 a, double2 b) { return make_double2(a.x + b.x, a.y + b.y); }
+__device__ __forceinline__ double2 pc_sub(double2 a, double2 b) { return make_double2(a.x - b.x, a.y - b.y); }
+__device__ __forceinline__ double2 pc_muli(double2 a) { return make_double2(-a.y, a.x); }  // a * (+i)
+
+// inverse radix-4: v_q = sum_r a_r exp(+2 pi i q r / 4)
+__device__ __forceinline__ void pc_bfly4(double2 a0, double2 a1, double2 a2, double2 a3, double2 &v0, double2 &v1, double2 &v2, double2 &v3)
+{
+    const double2 s02 = pc_add(a0, a2), d02 = pc_sub(a0, a2), s13 = pc_add(a1, a3), d13 = pc_muli(pc_sub(a1, a3));
+    v0 = pc_add(s02, s13), v2 = pc_sub(s02, s13), v1 = pc_add(d02, d13), v3 = pc_sub(d02, d13);
+}
+
+// inverse radix-8 in place: u_q <- sum_r u_r exp(+2 pi i q r / 8)
+__device__ __forceinline__ void pc_bfly8(double2 (&u)[8])
+{
+    double2 e0, e1, e2, e3, o0, o1, o2, o3;
+    pc_bfly4(u[0], u[2], u[4], u[6], e0, e1, e2, e3);
+    pc_bfly4(u[1], u[3], u[5], u[7], o0, o1, o2, o3);
+    const double h = 0.70710678118654752440;
+    o1 = make_double2(h * (o1.x - o1.y), h * (o1.x + o1.y));    // * (1 + i) / sqrt 2
+    o2 = pc_muli(o2);                                           // * i
+    o3 = make_double2(-h * (o3.x + o3.y), h * (o3.x - o3.y));   // * (-1 + i) / sqrt 2
+    u[0] = pc_add(e0, o0), u[4] = pc_sub(e0, o0), u[1] = pc_add(e1, o1), u[5] = pc_sub(e1, o1);
+    u[2] = pc_add(e2, o2), u[6] = pc_sub(e2, o2), u[3] = pc_add(e3, o3), u[7] = pc_sub(e3, o3);
+}
+
+// weight applied to the product conj(x[n]) d[n] on load: start-time phase, and for the un-whitened entry 1 / S_k(|f_n|) inside
+// the band f_min < |f_n| < f_max, 0 outside (eq. 2)
+struct PcWeight {
+    const double *S;   // [P][K][N] one-sided PSD sampled on the FFT grid's |f_n| (FFT order), or NULL: spectra already whitened
+    double df, fmin, fmax, scale;
+};
+
+// weight of frequency n: scale / S[n] inside the band f_min < |f_n| < f_max, 0 outside
+__device__ __forceinline__ double pc_weight(const double *__restrict__ Ss, const PcWeight &wt, int N, int n)
+{
+    const int np = n < (N + 1) / 2 ? n : N - n;  // |n'|
+    const double f = (double)np * wt.df;
+    return (f > wt.fmin && f < wt.fmax) ? wt.scale / __ldg(Ss + n) : 0.0;
+}
+
+__device__ __forceinline__ double2 pc_input(const double2 *__restrict__ xs, const double2 *__restrict__ ds, const double2 *__restrict__ ph,
+                                            const double *__restrict__ Ss, const PcWeight &wt, int N, int n)
+{
+    const double2 xv = __ldcs(xs + n);
+    double2 w = pc_cmul(__ldg(ds + n), __ldg(ph + n));
+    if (Ss) {
+        const double g = pc_weight(Ss, wt, N, n);
+        w.x *= g, w.y *= g;
+    }
+    return make_double2(xv.x * w.x + xv.y * w.y, xv.x * w.y - xv.y * w.x);  // conj(x) w
+}
+
+__global__ void __launch_bounds__(1024)
+    ile_overlap_q_radix8_kernel(int32_t M, int32_t N, const double2 *__restrict__ tab, const double2 *__restrict__ x,
+                                const double2 *__restrict__ d, const PcWeight wt, double2 *__restrict__ Q)
 {
     extern __shared__ double2 pc_sm[];
-    double2 *a = pc_sm;       // N points
-    double2 *W = pc_sm + N;   // N / 2 twiddles exp(+2 pi i j / N)
-    const size_t series = blockIdx.x;             // (point * K + k) * M + mode
-    const double2 *xs = x + series * N;
-    const double2 *ds = d + (series / M) * N;
-    for (int j = threadIdx.x; j < N / 2; j += PC_THREADS) W[j] = tab[j];
-    for (int n = threadIdx.x; n < N; n += PC_THREADS) {
-        const double2 xv = __ldcs(xs + n), dv = pc_cmul(ds[n], tab[N / 2 + n]);
-        const double2 v = make_double2(xv.x * dv.x + xv.y * dv.y, xv.x * dv.y - xv.y * dv.x);  // conj(x) d
-        a[__brev((unsigned)n) >> (32 - log2n)] = v;
+    const size_t series = blockIdx.x;  // (point * K + k) * M + mode
+    const double2 *xs = x + series * N, *ds = d + (series / M) * N, *ph = tab + N / 2;
+    const double *Ss = wt.S ? wt.S + (series / M) * N : nullptr;
+    double2 *q = Q + series * N;
+    const int T = N >> 3, j = threadIdx.x;  // blockDim.x == T: one radix-8 butterfly per thread and pass
+    double2 u[8];
+    // ---- pass 1 (sub-transform length 1, no twiddles): inputs from global memory
+#pragma unroll
+    for (int r = 0; r < 8; ++r) u[r] = pc_input(xs, ds, ph, Ss, wt, N, j + r * T);
+    pc_bfly8(u);
+    int ns = 8;
+    if (ns == N) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r) q[j * 8 + r] = u[r];
+        return;
     }
+#pragma unroll
+    for (int r = 0; r < 8; ++r) pc_sm[PC_PAD(j * 8 + r)] = u[r];
     __syncthreads();
-    for (int st = 1; st <= log2n; ++st) {
-        const int half = 1 << (st - 1), tw = N >> st;
-        for (int j = threadIdx.x; j < N / 2; j += PC_THREADS) {
-            const int pos = j & (half - 1), i0 = ((j >> (st - 1)) << st) + pos, i1 = i0 + half;
-            const double2 t = pc_cmul(W[pos * tw], a[i1]), u = a[i0];
-            a[i0] = make_double2(u.x + t.x, u.y + t.y);
-            a[i1] = make_double2(u.x - t.x, u.y - t.y);
+    // ---- radix-8 passes while they fit
+    for (; ns * 8 <= N; ns <<= 3) {
+        const int k = j & (ns - 1), j0 = ((j - k) << 3) + k;
+#pragma unroll
+        for (int r = 0; r < 8; ++r) u[r] = pc_sm[PC_PAD(j + r * T)];
+        // twiddles exp(2 pi i r k / (8 ns)): the first from the table, the others by multiplication
+        const double2 w1 = pc_tw(tab, N, k * (N / (8 * ns)));
+        double2 w = w1;
+#pragma unroll
+        for (int r = 1; r < 8; ++r) {
+            u[r] = pc_cmul(w, u[r]);
+            w = pc_cmul(w, w1);
         }
+        pc_bfly8(u);
+        if (ns * 8 == N) {  // last pass: natural order out, consecutive threads write consecutive addresses
+#pragma unroll
+            for (int r = 0; r < 8; ++r) __stcs(q + j0 + r * ns, u[r]);
+            return;
+        }
+        __syncthreads();  // everybody has read its inputs
+#pragma unroll
+        for (int r = 0; r < 8; ++r) pc_sm[PC_PAD(j0 + r * ns)] = u[r];
         __syncthreads();
     }
-    double2 *q = Q + series * N;
-    for (int i = threadIdx.x; i < N; i += PC_THREADS) __stcs(q + i, a[i]);
+    // ---- final radix-4 or radix-2 pass (N / ns = 4 or 2), straight to global memory
+    if (ns * 4 == N) {
+        const int T4 = N >> 2;
+        for (int jj = j; jj < T4; jj += T) {
+            const int k = jj & (ns - 1), j0 = ((jj - k) << 2) + k;
+            const double2 w1 = pc_tw(tab, N, k), w2 = pc_cmul(w1, w1), w3 = pc_cmul(w2, w1);
+            double2 v0, v1, v2, v3;
+            pc_bfly4(pc_sm[PC_PAD(jj)], pc_cmul(w1, pc_sm[PC_PAD(jj + T4)]), pc_cmul(w2, pc_sm[PC_PAD(jj + 2 * T4)]),
+                     pc_cmul(w3, pc_sm[PC_PAD(jj + 3 * T4)]), v0, v1, v2, v3);
+            __stcs(q + j0, v0), __stcs(q + j0 + ns, v1), __stcs(q + j0 + 2 * ns, v2), __stcs(q + j0 + 3 * ns, v3);
+        }
+    } else {
+        const int T2 = N >> 1;
+        for (int jj = j; jj < T2; jj += T) {  // ns = N / 2, k = jj
+            const double2 a0 = pc_sm[PC_PAD(jj)], a1 = pc_cmul(pc_tw(tab, N, jj), pc_sm[PC_PAD(jj + T2)]);
+            __stcs(q + jj, pc_add(a0, a1)), __stcs(q + jj + ns, pc_sub(a0, a1));
+        }
+    }
 }
 
 // One block per (point, detector).  Work items = (tile of PC_TA rows a, tile of PC_TB columns b, slice of the frequency
@@ -163,12 +264,14 @@ __global__ void __launch_bounds__(PC_THREADS)
 #define PC_TA 3
 #define PC_TB 3
 __global__ void __launch_bounds__(PC_THREADS, 2)
-    ile_overlap_uv_kernel(int32_t M, int32_t N, int32_t nsplit, const double2 *__restrict__ x, double2 *__restrict__ U, double2 *__restrict__ V)
+    ile_overlap_uv_kernel(int32_t M, int32_t N, int32_t nsplit, const double2 *__restrict__ x, const PcWeight wt, double2 *__restrict__ U,
+                          double2 *__restrict__ V)
 {
     extern __shared__ double2 pc_sm[];
     double *acc = reinterpret_cast<double *>(pc_sm);  // [M*M][4]
     const size_t pk = blockIdx.x;                     // point * K + k
     const double2 *xk = x + pk * M * N;
+    const double *Ss = wt.S ? wt.S + pk * N : nullptr;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, npairs = M * M;
     for (int i = threadIdx.x; i < 4 * npairs; i += PC_THREADS) acc[i] = 0.0;
     __syncthreads();
@@ -194,6 +297,11 @@ __global__ void __launch_bounds__(PC_THREADS, 2)
             }
 #pragma unroll
             for (int j = 0; j < PC_TB; ++j) q[j] = __ldg(xk + (size_t)min(b0 + j, M - 1) * N + n);
+            if (Ss) {  // weight on the right factor
+                const double g = pc_weight(Ss, wt, N, n);
+#pragma unroll
+                for (int j = 0; j < PC_TB; ++j) q[j].x *= g, q[j].y *= g;
+            }
 #pragma unroll
             for (int i = 0; i < PC_TA; ++i)
 #pragma unroll
@@ -224,25 +332,101 @@ __global__ void __launch_bounds__(PC_THREADS, 2)
     }
 }
 
+// Few modes (M <= PC_MS): one block per (point, detector), a lane takes one frequency at a time and keeps EVERY pair's sum in
+// registers.  U is Hermitian and V symmetric by their definitions (U_ba = conj(U_ab); V_ba = sum_n x_b[-n] x_a[n] is the same set
+// of products as V_ab), so only a <= b is accumulated: x_a[n], x_a[-n] for the M modes (2 M coalesced 16-byte loads) feed
+// M (M + 1) complex multiply-adds -- 8 M + 4 FMA per load.
+#define PC_MS 5
+#define PC_UV_THREADS 128
+__global__ void __launch_bounds__(PC_UV_THREADS, 2)
+    ile_overlap_uv_small_kernel(int32_t M, int32_t N, const double2 *__restrict__ x, const PcWeight wt, double2 *__restrict__ U,
+                                double2 *__restrict__ V)
+{
+    constexpr int NP = PC_MS * (PC_MS + 1) / 2;
+    __shared__ double acc[NP * 4];
+    const size_t pk = blockIdx.x;  // point * K + k
+    const double2 *xk = x + pk * M * N;
+    const double *Ss = wt.S ? wt.S + pk * N : nullptr;
+    const int lane = threadIdx.x & 31;
+    for (int i = threadIdx.x; i < NP * 4; i += PC_UV_THREADS) acc[i] = 0.0;
+    __syncthreads();
+    double su[NP][4];
+#pragma unroll
+    for (int p = 0; p < NP; ++p) su[p][0] = su[p][1] = su[p][2] = su[p][3] = 0.0;
+#pragma unroll 2
+    for (int n = threadIdx.x; n < N; n += PC_UV_THREADS) {
+        const int nm = (N - n) & (N - 1);
+        double2 p[PC_MS], m[PC_MS];
+#pragma unroll
+        for (int a = 0; a < PC_MS; ++a) {
+            const int aa = a < M ? a : M - 1;  // rows past M repeat the last one; their sums are dropped
+            p[a] = __ldg(xk + (size_t)aa * N + n);
+            m[a] = __ldg(xk + (size_t)aa * N + nm);
+        }
+        if (Ss) {  // weight on the left factors: conj(x_a) g x_b and x_a(-f) g x_b(f)
+            const double g = pc_weight(Ss, wt, N, n);
+#pragma unroll
+            for (int a = 0; a < PC_MS; ++a) m[a].x *= g, m[a].y *= g;
+            double2 pg[PC_MS];
+#pragma unroll
+            for (int a = 0; a < PC_MS; ++a) pg[a] = make_double2(p[a].x * g, p[a].y * g);
+            int pr = 0;
+#pragma unroll
+            for (int a = 0; a < PC_MS; ++a)
+#pragma unroll
+                for (int b = a; b < PC_MS; ++b, ++pr) {
+                    su[pr][0] += pg[a].x * p[b].x + pg[a].y * p[b].y;
+                    su[pr][1] += pg[a].x * p[b].y - pg[a].y * p[b].x;
+                    su[pr][2] += m[a].x * p[b].x - m[a].y * p[b].y;
+                    su[pr][3] += m[a].x * p[b].y + m[a].y * p[b].x;
+                }
+            continue;
+        }
+        int pr = 0;
+#pragma unroll
+        for (int a = 0; a < PC_MS; ++a)
+#pragma unroll
+            for (int b = a; b < PC_MS; ++b, ++pr) {
+                su[pr][0] += p[a].x * p[b].x + p[a].y * p[b].y;  // conj(x_a) x_b
+                su[pr][1] += p[a].x * p[b].y - p[a].y * p[b].x;
+                su[pr][2] += m[a].x * p[b].x - m[a].y * p[b].y;  // x_a(-f) x_b(f)
+                su[pr][3] += m[a].x * p[b].y + m[a].y * p[b].x;
+            }
+    }
+#pragma unroll
+    for (int pr = 0; pr < NP; ++pr)
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+            double v = su[pr][c];
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+            if (lane == 0) atomicAdd(&acc[4 * pr + c], v);
+        }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        int pr = 0;
+        for (int a = 0; a < PC_MS; ++a)
+            for (int b = a; b < PC_MS; ++b, ++pr) {
+                if (a >= M || b >= M) continue;
+                const double2 u = make_double2(acc[4 * pr], a == b ? 0.0 : acc[4 * pr + 1]), v = make_double2(acc[4 * pr + 2], acc[4 * pr + 3]);
+                U[pk * M * M + a * M + b] = u, V[pk * M * M + a * M + b] = v;
+                if (a != b) U[pk * M * M + b * M + a] = make_double2(u.x, -u.y), V[pk * M * M + b * M + a] = v;
+            }
+    }
+}
+
 cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_t N, double fs_hz, double t0_q_s, const double2 *x,
-                                  const double2 *d, double2 *Q, double2 *U, double2 *V, int32_t max_smem_optin, cudaStream_t st)
+                                  const double2 *d, const double *S, double f_min_hz, double f_max_hz, double scale, double2 *Q, double2 *U,
+                                  double2 *V, int32_t max_smem_optin, cudaStream_t st)
 {
     int log2n = 0;
     while ((1 << log2n) < N) ++log2n;
     if ((1 << log2n) != N || N < 2 || N > 8192) return cudaErrorInvalidValue;
-    const bool stockham = N <= 4096;
-    const size_t smem = stockham ? (size_t)2 * N * 16 : (size_t)N * 16 + (size_t)(N / 2) * 16;
+    const bool radix8 = N >= 512;
+    const size_t smem = radix8 ? (size_t)(N + N / 8) * 16 : (size_t)2 * N * 16;
     if (smem > (size_t)max_smem_optin) return cudaErrorInvalidValue;
-    auto stock = [&](auto kern, unsigned grid, const double2 *tab) {
-        cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e != cudaSuccess) return e;
-        kern<<<grid, PC_THREADS, smem, st>>>(M, N, log2n, tab, x, d, Q);
-        return cudaSuccess;
-    };
     cudaError_t e = cudaSuccess;
-    if (!stockham) e = cudaFuncSetAttribute(ile_overlap_q_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-    if (e != cudaSuccess) return e;
-    // U, V kernel: enough frequency slices that a block's 8 warps all have work items
+    // U, V kernel for many modes: enough frequency slices that a block's 8 warps all have work items
     const int tiles = ((M + PC_TA - 1) / PC_TA) * ((M + PC_TB - 1) / PC_TB);
     int nsplit = (PC_THREADS / 32 + tiles - 1) / tiles;
     while (nsplit > 1 && N / nsplit < 32) --nsplit;
@@ -259,6 +443,8 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
     if (!g_tab[dev]) {
         e = cudaMalloc(&g_tab[dev], (size_t)(4096 + 8192) * sizeof(double2));
         if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(9216 * 16));
+        if (e != cudaSuccess) return e;
     }
     double2 *tab = g_tab[dev];
     const double alpha = fs_hz * t0_q_s / (double)N;
@@ -266,14 +452,28 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
         ile_overlap_tables_kernel<<<(N + PC_THREADS - 1) / PC_THREADS, PC_THREADS, 0, st>>>(N, alpha, tab);
         g_tab_n[dev] = N, g_tab_alpha[dev] = alpha;
     }
-    const unsigned n_series = (unsigned)((size_t)n_points * K * M);
-    if (!stockham) ile_overlap_q_kernel<<<n_series, PC_THREADS, smem, st>>>(M, N, log2n, tab, x, d, Q);
-    else if (N == 16 * PC_THREADS) e = stock(ile_overlap_q_stockham_kernel<16>, n_series, tab);
-    else if (N == 8 * PC_THREADS) e = stock(ile_overlap_q_stockham_kernel<8>, n_series, tab);
-    else if (N == 4 * PC_THREADS) e = stock(ile_overlap_q_stockham_kernel<4>, n_series, tab);
-    else if (N == 2 * PC_THREADS) e = stock(ile_overlap_q_stockham_kernel<2>, n_series, tab);
-    else e = stock(ile_overlap_q_stockham_kernel<0>, n_series, tab);
-    if (e != cudaSuccess) return e;
-    ile_overlap_uv_kernel<<<(unsigned)(n_points * K), PC_THREADS, smem_uv, st>>>(M, N, nsplit, x, U, V);
+    PcWeight wt;
+    wt.S = S, wt.df = fs_hz / (double)N, wt.fmin = f_min_hz, wt.fmax = f_max_hz, wt.scale = scale;
+    // Batches of intrinsic points whose spectra fit L2 with room to spare: the U, V kernel of a batch runs right behind its Q
+    // kernel and finds x in L2, so x crosses the HBM bus once.
+    const size_t per_point = (size_t)K * M * N * sizeof(double2);
+    int batch = (int)((size_t)(48u << 20) / per_point);
+    batch = batch < 1 ? 1 : batch > n_points ? n_points : batch;
+    for (int p0 = 0; p0 < n_points; p0 += batch) {
+        const int np = n_points - p0 < batch ? n_points - p0 : batch;
+        const size_t so = (size_t)p0 * K * M * N, uo = (size_t)p0 * K * M * M;
+        const double2 *xb = x + so, *db = d + (size_t)p0 * K * N;
+        PcWeight wb = wt;
+        if (S) wb.S = S + (size_t)p0 * K * N;
+        const unsigned n_series = (unsigned)((size_t)np * K * M);
+        if (radix8) {
+            ile_overlap_q_radix8_kernel<<<n_series, N / 8, smem, st>>>(M, N, tab, xb, db, wb, Q + so);
+        } else {
+            if (S) return cudaErrorInvalidValue;  // short transforms take whitened spectra only
+            ile_overlap_q_stockham_kernel<0><<<n_series, PC_THREADS, smem, st>>>(M, N, log2n, tab, xb, db, Q + so);
+        }
+        if (M <= PC_MS) ile_overlap_uv_small_kernel<<<(unsigned)(np * K), PC_UV_THREADS, 0, st>>>(M, N, xb, wb, U + uo, V + uo);
+        else ile_overlap_uv_kernel<<<(unsigned)(np * K), PC_THREADS, smem_uv, st>>>(M, N, nsplit, xb, wb, U + uo, V + uo);
+    }
     return cudaGetLastError();
 }

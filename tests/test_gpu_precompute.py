@@ -52,7 +52,7 @@ def test_precompute_matches_oracle_on_config_shapes(gpu_lib, cid, n_points):
         check(V[p], rv, axes=(-1, -2))
 
 
-@pytest.mark.parametrize("n_q", [2, 4, 64, 8192])
+@pytest.mark.parametrize("n_q", [2, 4, 64, 256, 512, 1024, 4096, 8192])
 def test_precompute_edge_sizes_and_fractional_start_time(gpu_lib, n_q):
     r = np.random.default_rng(n_q)
     K, M = 1, (1 if n_q == 2 else 3)
@@ -95,3 +95,27 @@ def test_chain_precompute_create_eval_matches_oracle_chain(gpu_lib):
     assert_indices_equal(cfg, s, ref_idx, idx.cpu().numpy())
     assert rel_err(ref, lnL.cpu().numpy()) <= TOL
     ctx.close()
+
+
+@pytest.mark.parametrize("n_q,M,P", [(512, 2, 1), (2048, 5, 3), (4096, 21, 1), (8192, 4, 2), (1024, 7, 1)])
+def test_precompute_psd_matches_oracle(gpu_lib, n_q, M, P):
+    """ile_precompute_psd: un-whitened spectra, 1 / S weighting and band mask of eq. 2 on the device, against oracle.overlaps_psd;
+    few modes (register-resident pair sums) and many modes (tiled pair sums)."""
+    import torch
+
+    r = np.random.default_rng(n_q + M)
+    K, fs, t0 = 2, 4096.0, -n_q / 8192.0 + 0.4 / 4096.0
+    h = r.standard_normal((P, K, M, n_q)) + 1j * r.standard_normal((P, K, M, n_q))
+    d = r.standard_normal((P, K, n_q)) + 1j * r.standard_normal((P, K, n_q))
+    f = np.abs(pc.signed_index(n_q) * fs / n_q)
+    S = np.stack([np.stack([(0.5 + p + k) * (1.0 + (f / 300.0) ** 2 + (40.0 / np.maximum(f, 1.0)) ** 4) for k in range(K)]) for p in range(P)])
+    fmin, fmax, scale = 20.0, 1024.0, 2.0 * fs / n_q
+    Q, U, V = gpu_lib.precompute_psd(torch.from_numpy(h).cuda(), torch.from_numpy(d).cuda(), torch.from_numpy(S).cuda(), fs, t0, fmin, fmax, scale)
+    Q, U, V = Q.cpu().numpy(), U.cpu().numpy(), V.cpu().numpy()
+    for p in range(P):
+        rq, ru, rv = pc.overlaps_psd(h[p], d[p], S[p], fs, t0, fmin, fmax, scale)
+        check(Q[p], rq, axes=-1)
+        check(U[p], ru, axes=(-1, -2))
+        check(V[p], rv, axes=(-1, -2))
+    with pytest.raises(gpu_lib.IleError):
+        gpu_lib.precompute_psd(torch.from_numpy(h).cuda(), torch.from_numpy(d).cuda(), torch.from_numpy(S).cuda(), fs, t0, 50.0, 20.0, scale)

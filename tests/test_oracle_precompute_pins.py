@@ -88,3 +88,64 @@ def test_generator_and_oracle_agree_on_a_config_point():
     q, u, v = pc.overlaps(meta["x"], meta["d"], meta["fs_hz"], meta["t0_q_s"])
     for got, ref in ((q, Q), (u, U), (v, V)):
         assert np.max(np.abs(got - ref)) <= 1e-13 * np.max(np.abs(ref))
+
+
+# ----------------------------------------------------------------------------------------------------------
+# eq. 2's weighting on un-whitened spectra: overlaps_psd
+# ----------------------------------------------------------------------------------------------------------
+def _unwhitened(seed, K=2, M=3, N=64, fs=256.0):
+    rng = np.random.default_rng(seed)
+    h = rng.standard_normal((K, M, N)) + 1j * rng.standard_normal((K, M, N))
+    d = rng.standard_normal((K, N)) + 1j * rng.standard_normal((K, N))
+    f = np.abs(pc.signed_index(N) * fs / N)
+    S = np.stack([(1.0 + k) * (1.0 + (f / 40.0) ** 2 + (10.0 / np.maximum(f, 1.0)) ** 4) for k in range(K)])
+    return h, d, S, fs
+
+
+def test_psd_inner_product_is_eq2_by_brute_force():
+    """U_ab with scale = 2 df is eq. 2's <h_a|h_b> = 2 int_{f_min<|f|<f_max} h_a*(f) h_b(f) / S(|f|) df as a plain Riemann sum over
+    the two-sided grid, written here term by term; Q at lag 0 with d = h_b is the same number; V pairs f with -f."""
+    h, d, S, fs = _unwhitened(1)
+    K, M, N = h.shape
+    df, fmin, fmax, t0 = fs / N, 14.0, 90.0, 0.0
+    Q, U, V = pc.overlaps_psd(h, d, S, fs, t0, fmin, fmax, 2.0 * df)
+    npr = pc.signed_index(N)
+    for k in range(K):
+        for a in range(M):
+            for b in range(M):
+                u = v = 0j
+                for n in range(N):
+                    f = abs(npr[n]) * df
+                    if not (fmin < f < fmax):
+                        continue
+                    u += 2.0 * np.conj(h[k, a, n]) * h[k, b, n] / S[k, n] * df
+                    v += 2.0 * h[k, a, (-n) % N] * h[k, b, n] / S[k, n] * df
+                assert abs(U[k, a, b] - u) <= 1e-12 * abs(u) and abs(V[k, a, b] - v) <= 1e-12 * max(abs(v), 1e-3)
+            Qb = pc.overlaps_psd(h, h[:, a], S, fs, 0.0, fmin, fmax, 2.0 * df)[0]
+            for b in range(M):
+                assert abs(Qb[k, b, 0] - U[k, b, a]) <= 1e-12 * abs(U[k, b, a])
+        assert np.allclose(U[k], U[k].conj().T, rtol=1e-13) and np.allclose(V[k], V[k].T, rtol=1e-13)
+
+
+def test_psd_form_equals_whitened_form_and_respects_the_band():
+    """Whitening by hand -- x = h sqrt(g), d_w = d sqrt(g) -- and the plain form give the same Q, U, V (this links the new entry to
+    the one pinned above); S = 1 over the whole band is the plain form itself; data outside the band changes nothing; the lag
+    axis is the same (a delayed copy of the data moves the peak of Q by the delay)."""
+    h, d, S, fs = _unwhitened(2)
+    K, M, N = h.shape
+    t0, fmin, fmax, scale = -0.07, 9.0, 100.0, 0.37
+    Q, U, V = pc.overlaps_psd(h, d, S, fs, t0, fmin, fmax, scale)
+    g = np.stack([pc.psd_weights(N, S[k], fs, fmin, fmax, scale) for k in range(K)])
+    Qw, Uw, Vw = pc.overlaps(h * np.sqrt(g)[:, None, :], d * np.sqrt(g), fs, t0)
+    for got, ref in ((Q, Qw), (U, Uw), (V, Vw)):
+        assert np.max(np.abs(got - ref)) <= 1e-12 * np.max(np.abs(ref))
+    Q1, U1, V1 = pc.overlaps_psd(h, d, np.ones_like(S), fs, t0, -1.0, 1e9, 1.0)
+    Q0, U0, V0 = pc.overlaps(h, d, fs, t0)
+    assert np.max(np.abs(Q1 - Q0)) <= 1e-12 * np.max(np.abs(Q0)) and np.allclose(U1, U0, rtol=1e-13) and np.allclose(V1, V0, rtol=1e-13)
+    d2 = d.copy()
+    out = g[0] == 0.0
+    d2[:, out] += 100.0
+    assert np.max(np.abs(pc.overlaps_psd(h, d2, S, fs, t0, fmin, fmax, scale)[0] - Q)) <= 1e-10 * np.max(np.abs(Q))
+    Qd, Ud, Vd = pc.overlaps_direct_psd(h[:1, :2, :16], d[:1, :16], S[:1, :16], fs, t0, 20.0, 100.0, scale)
+    Qf, Uf, Vf = pc.overlaps_psd(h[:1, :2, :16], d[:1, :16], S[:1, :16], fs, t0, 20.0, 100.0, scale)
+    assert np.max(np.abs(Qd - Qf)) <= 1e-12 * np.max(np.abs(Qf)) and np.allclose(Ud, Uf, rtol=1e-12) and np.allclose(Vd, Vf, rtol=1e-12, atol=1e-12)
