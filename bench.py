@@ -196,7 +196,7 @@ def run_precompute(args, rank: int):
     torch.cuda.synchronize()
     sampler.stop_flag = True
     ms = sum(a.elapsed_time(b) for a, b in ev) / args.steps
-    nbytes = 16 * P * K * (2 * M * N + N + 2 * M * M)  # x in (once: the U, V kernel of a batch finds it in L2), d in, Q out, U and V out
+    nbytes = 16 * P * K * (2 * M * N + N + 2 * M * M)  # x in, d in, Q out, U and V out (x counted once)
     peak = None
     try:
         peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
@@ -210,8 +210,8 @@ def run_precompute(args, rank: int):
             "config": {"workload": f"ile_precompute: {P} intrinsic point(s) of BASELINE.json configs[{args.config}]'s shape "
                                    f"({K} detectors, {M} modes, {N}-point spectra)", "l2": "flushed between timed steps (256 MiB write)"},
             "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
-                         "kernel": "ile_overlap_q_radix8_kernel + ile_overlap_uv_small_kernel (per batch of points that fits L2)", "peak_source": src, "algorithmic_bytes": nbytes},
-            "gpu_launches": 3 * args.steps, "clocks": sampler.summary()}
+                         "kernel": "ile_overlap_q_radix8_kernel + ile_overlap_uv_small_kernel", "peak_source": src, "algorithmic_bytes": nbytes},
+            "gpu_launches": 2 * args.steps, "clocks": sampler.summary()}
     print(json.dumps(line), flush=True)
 
 

@@ -12,7 +12,7 @@
 //                                  from global memory (spectrum product, optional 1/S weight and band mask, start-time phase), last
 //                                  pass to global memory, one padded shared buffer in between
 //   ile_overlap_q_stockham_kernel  N < 512: radix-4 Stockham passes between two shared buffers (whitened spectra only)
-//   ile_overlap_uv_small_kernel    M <= 5: one block per (detector, point), every pair's sum in registers, a <= b only
+//   ile_overlap_uv_small_kernel    M <= 5: one block per (detector, point), warp = (row a, frequency slice), pairs (a, b >= a) in registers
 //   ile_overlap_uv_kernel          any M: register-blocked tiles of pairs (a, b), lanes over frequencies
 // With S != NULL the inner products are eq. 2's (L30-L35): weight scale / S_k(|f_n|) inside f_min < |f_n| < f_max, 0 outside.
 #include "ile_kernels.h"
@@ -188,7 +188,8 @@ __device__ __forceinline__ double2 pc_input(const double2 *__restrict__ xs, cons
     return make_double2(xv.x * w.x + xv.y * w.y, xv.x * w.y - xv.y * w.x);  // conj(x) w
 }
 
-__global__ void __launch_bounds__(1024)
+template <int T>  // T = N / 8 threads
+__global__ void __launch_bounds__(T)
     ile_overlap_q_radix8_kernel(int32_t M, int32_t N, const double2 *__restrict__ tab, const double2 *__restrict__ x,
                                 const double2 *__restrict__ d, const PcWeight wt, double2 *__restrict__ Q)
 {
@@ -197,7 +198,7 @@ __global__ void __launch_bounds__(1024)
     const double2 *xs = x + series * N, *ds = d + (series / M) * N, *ph = tab + N / 2;
     const double *Ss = wt.S ? wt.S + (series / M) * N : nullptr;
     double2 *q = Q + series * N;
-    const int T = N >> 3, j = threadIdx.x;  // blockDim.x == T: one radix-8 butterfly per thread and pass
+    const int j = threadIdx.x;  // blockDim.x == T == N / 8: one radix-8 butterfly per thread and pass
     double2 u[8];
     // ---- pass 1 (sub-transform length 1, no twiddles): inputs from global memory
 #pragma unroll
@@ -332,86 +333,69 @@ __global__ void __launch_bounds__(PC_THREADS, 2)
     }
 }
 
-// Few modes (M <= PC_MS): one block per (point, detector), a lane takes one frequency at a time and keeps EVERY pair's sum in
-// registers.  U is Hermitian and V symmetric by their definitions (U_ba = conj(U_ab); V_ba = sum_n x_b[-n] x_a[n] is the same set
-// of products as V_ab), so only a <= b is accumulated: x_a[n], x_a[-n] for the M modes (2 M coalesced 16-byte loads) feed
-// M (M + 1) complex multiply-adds -- 8 M + 4 FMA per load.
+// Few modes (M <= PC_MS): one block per (point, detector); warp (a, slice) takes row a and one of PC_NS slices of the frequency
+// axis, a lane one frequency at a time, and keeps the sums of the pairs (a, b >= a) in registers.  U is Hermitian and V symmetric
+// by their definitions (U_ba = conj(U_ab); V_ba = sum_n x_b[-n] x_a[n] is the same set of products as V_ab), so only b >= a is
+// accumulated and the mirror entries are filled from it.  The M row warps of a slice read the same spectra: once from L2 (the
+// Q kernel of the batch has just brought them on chip), then from L1.
 #define PC_MS 5
-#define PC_UV_THREADS 128
-__global__ void __launch_bounds__(PC_UV_THREADS, 2)
+#define PC_NS 4
+#define PC_UV_THREADS (32 * PC_MS * PC_NS)
+template <bool WEIGHTED>
+__global__ void __launch_bounds__(PC_UV_THREADS, 1)
     ile_overlap_uv_small_kernel(int32_t M, int32_t N, const double2 *__restrict__ x, const PcWeight wt, double2 *__restrict__ U,
                                 double2 *__restrict__ V)
 {
-    constexpr int NP = PC_MS * (PC_MS + 1) / 2;
-    __shared__ double acc[NP * 4];
+    __shared__ double acc[PC_MS * PC_MS * 4];
     const size_t pk = blockIdx.x;  // point * K + k
-    const double2 *xk = x + pk * M * N;
-    const double *Ss = wt.S ? wt.S + pk * N : nullptr;
-    const int lane = threadIdx.x & 31;
-    for (int i = threadIdx.x; i < NP * 4; i += PC_UV_THREADS) acc[i] = 0.0;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, a = warp % PC_MS, slice = warp / PC_MS;
+    const int nb = M - a;  // pairs (a, a + i), i < nb; warps with a >= M idle
+    const double2 *xk = x + pk * M * N, *xa = xk + (size_t)a * N;
+    const double *Ss = WEIGHTED ? wt.S + pk * N : nullptr;
+    for (int i = threadIdx.x; i < PC_MS * PC_MS * 4; i += PC_UV_THREADS) acc[i] = 0.0;
     __syncthreads();
-    double su[NP][4];
+    if (nb > 0) {
+        double su[PC_MS][4];
 #pragma unroll
-    for (int p = 0; p < NP; ++p) su[p][0] = su[p][1] = su[p][2] = su[p][3] = 0.0;
+        for (int i = 0; i < PC_MS; ++i) su[i][0] = su[i][1] = su[i][2] = su[i][3] = 0.0;
+        const int len = N / PC_NS, lo = slice * len, hi = slice == PC_NS - 1 ? N : lo + len;
 #pragma unroll 2
-    for (int n = threadIdx.x; n < N; n += PC_UV_THREADS) {
-        const int nm = (N - n) & (N - 1);
-        double2 p[PC_MS], m[PC_MS];
+        for (int n = lo + lane; n < hi; n += 32) {
+            const int nm = (N - n) & (N - 1);
+            double2 pa = __ldg(xa + n), ma = __ldg(xa + nm), q[PC_MS];
 #pragma unroll
-        for (int a = 0; a < PC_MS; ++a) {
-            const int aa = a < M ? a : M - 1;  // rows past M repeat the last one; their sums are dropped
-            p[a] = __ldg(xk + (size_t)aa * N + n);
-            m[a] = __ldg(xk + (size_t)aa * N + nm);
+            for (int i = 0; i < PC_MS; ++i) q[i] = __ldg(xa + (size_t)(i < nb ? i : nb - 1) * N + n);  // columns past M repeat the last one
+            if (WEIGHTED) {  // weight on the left factors: conj(x_a) g x_b and x_a(-f) g x_b(f)
+                const double g = pc_weight(Ss, wt, N, n);
+                pa.x *= g, pa.y *= g, ma.x *= g, ma.y *= g;
+            }
+#pragma unroll
+            for (int i = 0; i < PC_MS; ++i) {
+                su[i][0] += pa.x * q[i].x + pa.y * q[i].y;  // conj(x_a) x_b
+                su[i][1] += pa.x * q[i].y - pa.y * q[i].x;
+                su[i][2] += ma.x * q[i].x - ma.y * q[i].y;  // x_a(-f) x_b(f)
+                su[i][3] += ma.x * q[i].y + ma.y * q[i].x;
+            }
         }
-        if (Ss) {  // weight on the left factors: conj(x_a) g x_b and x_a(-f) g x_b(f)
-            const double g = pc_weight(Ss, wt, N, n);
 #pragma unroll
-            for (int a = 0; a < PC_MS; ++a) m[a].x *= g, m[a].y *= g;
-            double2 pg[PC_MS];
+        for (int i = 0; i < PC_MS; ++i)
 #pragma unroll
-            for (int a = 0; a < PC_MS; ++a) pg[a] = make_double2(p[a].x * g, p[a].y * g);
-            int pr = 0;
+            for (int c = 0; c < 4; ++c) {
+                double v = su[i][c];
 #pragma unroll
-            for (int a = 0; a < PC_MS; ++a)
-#pragma unroll
-                for (int b = a; b < PC_MS; ++b, ++pr) {
-                    su[pr][0] += pg[a].x * p[b].x + pg[a].y * p[b].y;
-                    su[pr][1] += pg[a].x * p[b].y - pg[a].y * p[b].x;
-                    su[pr][2] += m[a].x * p[b].x - m[a].y * p[b].y;
-                    su[pr][3] += m[a].x * p[b].y + m[a].y * p[b].x;
-                }
-            continue;
-        }
-        int pr = 0;
-#pragma unroll
-        for (int a = 0; a < PC_MS; ++a)
-#pragma unroll
-            for (int b = a; b < PC_MS; ++b, ++pr) {
-                su[pr][0] += p[a].x * p[b].x + p[a].y * p[b].y;  // conj(x_a) x_b
-                su[pr][1] += p[a].x * p[b].y - p[a].y * p[b].x;
-                su[pr][2] += m[a].x * p[b].x - m[a].y * p[b].y;  // x_a(-f) x_b(f)
-                su[pr][3] += m[a].x * p[b].y + m[a].y * p[b].x;
+                for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+                if (lane == 0 && i < nb) atomicAdd(&acc[(a * PC_MS + i) * 4 + c], v);
             }
     }
-#pragma unroll
-    for (int pr = 0; pr < NP; ++pr)
-#pragma unroll
-        for (int c = 0; c < 4; ++c) {
-            double v = su[pr][c];
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-            if (lane == 0) atomicAdd(&acc[4 * pr + c], v);
-        }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        int pr = 0;
-        for (int a = 0; a < PC_MS; ++a)
-            for (int b = a; b < PC_MS; ++b, ++pr) {
-                if (a >= M || b >= M) continue;
-                const double2 u = make_double2(acc[4 * pr], a == b ? 0.0 : acc[4 * pr + 1]), v = make_double2(acc[4 * pr + 2], acc[4 * pr + 3]);
-                U[pk * M * M + a * M + b] = u, V[pk * M * M + a * M + b] = v;
-                if (a != b) U[pk * M * M + b * M + a] = make_double2(u.x, -u.y), V[pk * M * M + b * M + a] = v;
-            }
+    if (threadIdx.x < PC_MS * PC_MS) {
+        const int ra = threadIdx.x / PC_MS, i = threadIdx.x % PC_MS, rb = ra + i;
+        if (ra < M && rb < M) {
+            const double *s4 = acc + (ra * PC_MS + i) * 4;
+            const double2 u = make_double2(s4[0], i == 0 ? 0.0 : s4[1]), v = make_double2(s4[2], s4[3]);
+            U[pk * M * M + ra * M + rb] = u, V[pk * M * M + ra * M + rb] = v;
+            if (i) U[pk * M * M + rb * M + ra] = make_double2(u.x, -u.y), V[pk * M * M + rb * M + ra] = v;
+        }
     }
 }
 
@@ -443,7 +427,9 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
     if (!g_tab[dev]) {
         e = cudaMalloc(&g_tab[dev], (size_t)(4096 + 8192) * sizeof(double2));
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(9216 * 16));
+        e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4608 * 16));
+        if (e != cudaSuccess) return e;
+        e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(9216 * 16));
         if (e != cudaSuccess) return e;
     }
     double2 *tab = g_tab[dev];
@@ -454,26 +440,25 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
     }
     PcWeight wt;
     wt.S = S, wt.df = fs_hz / (double)N, wt.fmin = f_min_hz, wt.fmax = f_max_hz, wt.scale = scale;
-    // Batches of intrinsic points whose spectra fit L2 with room to spare: the U, V kernel of a batch runs right behind its Q
-    // kernel and finds x in L2, so x crosses the HBM bus once.
-    const size_t per_point = (size_t)K * M * N * sizeof(double2);
-    int batch = (int)((size_t)(48u << 20) / per_point);
-    batch = batch < 1 ? 1 : batch > n_points ? n_points : batch;
-    for (int p0 = 0; p0 < n_points; p0 += batch) {
-        const int np = n_points - p0 < batch ? n_points - p0 : batch;
-        const size_t so = (size_t)p0 * K * M * N, uo = (size_t)p0 * K * M * M;
-        const double2 *xb = x + so, *db = d + (size_t)p0 * K * N;
-        PcWeight wb = wt;
-        if (S) wb.S = S + (size_t)p0 * K * N;
-        const unsigned n_series = (unsigned)((size_t)np * K * M);
-        if (radix8) {
-            ile_overlap_q_radix8_kernel<<<n_series, N / 8, smem, st>>>(M, N, tab, xb, db, wb, Q + so);
-        } else {
-            if (S) return cudaErrorInvalidValue;  // short transforms take whitened spectra only
-            ile_overlap_q_stockham_kernel<0><<<n_series, PC_THREADS, smem, st>>>(M, N, log2n, tab, xb, db, Q + so);
+    // One launch per kernel over all points: cutting the call into L2-sized batches (so that the U, V kernel finds the spectra its
+    // Q kernel has just read) was measured and lost -- 0.24 ms against 0.19 ms for 256 points of 3 x 5 x 2048: both kernels are
+    // bound by the latency of a block's own load - compute - store chain, and batches serialise those chains.
+    const unsigned n_series = (unsigned)((size_t)n_points * K * M);
+    if (radix8) {
+        switch (N) {
+            case 512: ile_overlap_q_radix8_kernel<64><<<n_series, 64, smem, st>>>(M, N, tab, x, d, wt, Q); break;
+            case 1024: ile_overlap_q_radix8_kernel<128><<<n_series, 128, smem, st>>>(M, N, tab, x, d, wt, Q); break;
+            case 2048: ile_overlap_q_radix8_kernel<256><<<n_series, 256, smem, st>>>(M, N, tab, x, d, wt, Q); break;
+            case 4096: ile_overlap_q_radix8_kernel<512><<<n_series, 512, smem, st>>>(M, N, tab, x, d, wt, Q); break;
+            default: ile_overlap_q_radix8_kernel<1024><<<n_series, 1024, smem, st>>>(M, N, tab, x, d, wt, Q); break;
         }
-        if (M <= PC_MS) ile_overlap_uv_small_kernel<<<(unsigned)(np * K), PC_UV_THREADS, 0, st>>>(M, N, xb, wb, U + uo, V + uo);
-        else ile_overlap_uv_kernel<<<(unsigned)(np * K), PC_THREADS, smem_uv, st>>>(M, N, nsplit, xb, wb, U + uo, V + uo);
+    } else {
+        if (S) return cudaErrorInvalidValue;  // short transforms take whitened spectra only
+        ile_overlap_q_stockham_kernel<0><<<n_series, PC_THREADS, smem, st>>>(M, N, log2n, tab, x, d, Q);
     }
+    const unsigned n_pk = (unsigned)(n_points * K);
+    if (M <= PC_MS && S) ile_overlap_uv_small_kernel<true><<<n_pk, PC_UV_THREADS, 0, st>>>(M, N, x, wt, U, V);
+    else if (M <= PC_MS) ile_overlap_uv_small_kernel<false><<<n_pk, PC_UV_THREADS, 0, st>>>(M, N, x, wt, U, V);
+    else ile_overlap_uv_kernel<<<n_pk, PC_THREADS, smem_uv, st>>>(M, N, nsplit, x, wt, U, V);
     return cudaGetLastError();
 }
