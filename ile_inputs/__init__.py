@@ -49,6 +49,22 @@ DETECTORS = {
 }
 
 
+def _site(lat_deg: float, lon_deg: float, x_arm_azimuth_deg: float, psd_scale: float):
+    """A site on a spherical Earth (R = 6.371e6 m) with orthogonal horizontal arms, the x arm at the given azimuth east of north."""
+    lat, lon, az = np.radians(lat_deg), np.radians(lon_deg), np.radians(x_arm_azimuth_deg)
+    up = np.array([np.cos(lat) * np.cos(lon), np.cos(lat) * np.sin(lon), np.sin(lat)])
+    east = np.array([-np.sin(lon), np.cos(lon), 0.0])
+    north = np.cross(up, east)
+    ax = np.cos(az) * north + np.sin(az) * east
+    ay = np.cos(az + 0.5 * np.pi) * north + np.sin(az + 0.5 * np.pi) * east
+    return dict(vertex_m=tuple(6.371e6 * up), arm_x=tuple(ax), arm_y=tuple(ay), psd_scale=psd_scale)
+
+
+# A fourth site for four-detector networks (PAPER.md L79 treats F as (detectors) x (extrinsic) without a limit of three): a
+# detector at KAGRA's approximate geodetic position.  An input like the others, parity-neutral.
+DETECTORS["K1"] = _site(36.41, 137.31, 60.4, 3.0)
+
+
 def modes_up_to(l_max: int, l_min: int = 2):
     """All (l, m) with l_min <= l <= l_max, m = -l..l, in that order."""
     return [(l, m) for l in range(l_min, l_max + 1) for m in range(-l, l + 1)]

@@ -294,7 +294,7 @@ static int ensure_scratch(ile_ctx *c, size_t samples, size_t hist_words, cudaStr
 static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
 {
     const IleSortPlan &sp = c->ssp;
-    const size_t nseg = (size_t)sp.n1 * sp.n2;
+    const size_t nseg = (size_t)sp.nseg;
     const int64_t slot_cap = (((a.n_per_point + 7) & ~(int64_t)7) + 8 * (int64_t)nseg + 31) & ~(int64_t)31;  // groups per point: multiple of 4
     int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * (sp.ncell + nseg) + ILE_STREAM_MAX_RANGES, st);
     if (r != ILE_OK) return r;

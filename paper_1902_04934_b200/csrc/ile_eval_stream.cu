@@ -324,7 +324,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
             pk[k] += NC * 32;
         }
         // fragments in registers one step ahead while they fit (PIPE); otherwise loaded where they are used
-        constexpr bool PIPE = KS <= ST_PIPE_MAXKS;
+        constexpr bool PIPE = KS <= ST_PIPE_MAXKS && K <= 3;  // four detectors: fragments per chain (register budget)
         double af[K][2][PIPE ? KS : 1];  // [k][block of the pair][k-step]; k = 0 is detector 0
         // too many k-steps for that: two chain-sized buffers, the fragments of chain i + 1 are loaded while chain i runs.
         // Chains of a step in order: (k = 1, bb = 0), (1, 1), ..., (K - 1, 1), (0, 0), (0, 1); 2K of them, so buffer parity
@@ -536,10 +536,10 @@ __global__ void __launch_bounds__(IX_THREADS)
         ile_source_dir(a.ra[s], a.dec[s], P.gmst, dir, &sl, &cl, &sd, &cd);
         const double t_ref = a.t_ref[s];
         int bad = 0;
-        int32_t i0[3] = {0, 0, 0};
+        int32_t i0[4] = {0, 0, 0, 0};
         for (int k = 0; k < K; ++k) {
             const int32_t idx = ile_window_index(P.vertex[k], dir, t_ref, P.t0_q, P.fs, P.n_t);
-            if (k < 3) i0[k] = idx;
+            if (k < 4) i0[k] = idx;
             if (idx < 0 || (long long)idx + P.n_t > P.n_q) bad = 1;
             i0_out[s * K + k] = idx;
             if (a.shift_idx) a.shift_idx[s * K + k] = idx;
@@ -554,6 +554,7 @@ __global__ void __launch_bounds__(IX_THREADS)
             int32_t seg = 0;
             if (sp.nd > 1) seg = min(max(i0[1] - i0[0] + sp.dmax[1], 0), 2 * sp.dmax[1]) >> sp.g;
             if (sp.nd > 2) seg = seg * sp.n2 + (min(max(i0[2] - i0[0] + sp.dmax[2], 0), 2 * sp.dmax[2]) >> sp.g);
+            if (sp.nd > 3) seg = seg * sp.n3 + (min(max(i0[3] - i0[0] + sp.dmax[3], 0), 2 * sp.dmax[3]) >> sp.g);
             c = seg * sp.n0 + (i0[0] >> sp.g0);  // 0 <= i0_0 <= n_q - n_t here
         }
         cell[s] = c;
@@ -692,7 +693,7 @@ static int st_round_ks(int ks)
 // sizes do not fit this variant (more than 3 detectors, too many cells).
 bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point, IleStreamPlan *out, IleSortPlan *spo)
 {
-    if (sz.n_det > 3) return false;
+    if (sz.n_det > 4) return false;  // a lane looks after one (sample, detector) pair of its group: 8 samples x 4 detectors
     IleStreamPlan pl;
     pl.ks = st_round_ks((2 * sz.n_modes + 3) / 4);
     if (!pl.ks) return false;
@@ -704,7 +705,7 @@ bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per
     sp.nd = sz.n_det;
     sp.g = pl.nc == 2 ? 4 : 3;
     sp.dmax[0] = 0;
-    for (int d = 1; d < 3; ++d) {
+    for (int d = 1; d < 4; ++d) {
         sp.dmax[d] = 0;
         if (d < sp.nd) {
             const double dx = hp.vertex[d][0] - hp.vertex[0][0], dy = hp.vertex[d][1] - hp.vertex[0][1], dz = hp.vertex[d][2] - hp.vertex[0][2];
@@ -715,11 +716,13 @@ bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per
     }
     sp.n1 = sp.nd > 1 ? ((2 * sp.dmax[1]) >> sp.g) + 1 : 1;
     sp.n2 = sp.nd > 2 ? ((2 * sp.dmax[2]) >> sp.g) + 1 : 1;
-    if ((long long)sp.n1 * sp.n2 > 12288) return false;  // the scan kernel holds the per-segment counts in shared memory
+    sp.n3 = sp.nd > 3 ? ((2 * sp.dmax[3]) >> sp.g) + 1 : 1;
+    if ((long long)sp.n1 * sp.n2 * sp.n3 > 12288) return false;  // the scatter kernel holds the per-segment bases in shared memory
+    sp.nseg = sp.n1 * sp.n2 * sp.n3;
     int g0 = 3;
     for (;; ++g0) {  // i0_0 bins of 8 rows unless the series is so long that a segment's bins (shared memory) or the histogram get too big
         sp.n0 = ((sz.n_q - sz.n_t) >> g0) + 1;
-        const long long nc = (long long)sp.n0 * sp.n1 * sp.n2 + 1;
+        const long long nc = (long long)sp.n0 * sp.nseg + 1;
         if (sp.n0 <= 12288 && nc <= (1LL << 22)) {
             sp.ncell = (int32_t)nc;
             break;
@@ -772,7 +775,8 @@ static cudaError_t st_launch(const IleSizes &sz, int ks, const IleStreamKArgs *k
 {
     if (sz.n_det == 1) return st_launch_k<1, ST_NC>(sz, ks, ka, mg, per_sm, st);
     if (sz.n_det == 2) return st_launch_k<2, ST_NC>(sz, ks, ka, mg, per_sm, st);
-    return st_launch_k<3, ST_NC>(sz, ks, ka, mg, per_sm, st);
+    if (sz.n_det == 3) return st_launch_k<3, ST_NC>(sz, ks, ka, mg, per_sm, st);
+    return st_launch_k<4, ST_NC>(sz, ks, ka, mg, per_sm, st);
 }
 
 // Once per context, on the context's device: carve-out and occupancy of the streaming kernel this context's sizes select.
@@ -790,7 +794,7 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
 {
     if (a.n_per_point <= 0 || a.n_points <= 0) return cudaSuccess;
     const long long n_total = a.n_per_point * a.n_points;
-    const int nseg = sp.n1 * sp.n2;
+    const int nseg = sp.nseg;
     // cell histograms and the claim counters of the streaming kernel, one zeroed block; the segment totals behind them are
     // written by the scan kernel
     const size_t n_hist = (size_t)a.n_points * sp.ncell;

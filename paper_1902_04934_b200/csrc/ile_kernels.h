@@ -47,14 +47,15 @@ cudaError_t ile_launch_eval_tiled(const IleSizes &sz, const IleDevParams &hp, co
                                   int *n_launches);
 
 // ---- counting sort of the streaming path (variant 4) -----------------------------------------------------------------
-// Cell grid: segments = (i0_1 - i0_0, i0_2 - i0_0) cells of width 2^g, inside a segment bins of i0_0 of width 2^g0.
+// Cell grid: segments = (i0_1 - i0_0, i0_2 - i0_0[, i0_3 - i0_0]) cells of width 2^g, inside a segment bins of i0_0 of width 2^g0.
 struct IleSortPlan {
     int32_t g;        // log2 of the (d1, d2) cell width in samples
     int32_t g0;       // log2 of the i0_0 bin width inside a segment
-    int32_t nd;       // detectors that take part in the key (<= 3)
-    int32_t n0, n1, n2;
-    int32_t ncell;    // n0*n1*n2 + 1; the last cell collects out-of-range samples
-    int32_t dmax[3];  // bound on |i0_d - i0_0| from the light travel time between the sites
+    int32_t nd;       // detectors that take part in the key (<= 4)
+    int32_t n0, n1, n2, n3;
+    int32_t nseg;     // n1*n2*n3 segments
+    int32_t ncell;    // n0*nseg + 1; the last cell collects out-of-range samples
+    int32_t dmax[4];  // bound on |i0_d - i0_0| from the light travel time between the sites
 };
 
 // Device scratch of the sorted path (owned by the context).

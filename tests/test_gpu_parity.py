@@ -535,3 +535,22 @@ def test_paper_window_concentrated_batch_16384_Hz(gpu_lib):
     cfg = gi.make_config(8, n=20_000)
     s = gi.make_concentrated_samples(5150, 20_000)
     full_compare(gpu_lib, cfg, s, log_w=gi.make_log_weights(2, 20_000))
+
+
+# ---------------------------------------------------------------------------------------------- four detectors on the streaming path
+@pytest.mark.parametrize("modes,n", [("l2", 20_000), ("l2", 1_003), ("l4", 10_000)])
+def test_four_detector_network_on_the_streaming_kernel(gpu_lib, modes, n):
+    """H1, L1, V1 and a fourth site (F is (detectors) x (extrinsic), no limit of three): the K = 4 instantiation of the
+    streaming kernel -- sort cells over (d1, d2, d3), three realigned detectors per group -- with 5 and with 21 modes."""
+    dets = ("H1", "L1", "V1", "K1")
+    ml = gi.modes_up_to(2) if modes == "l2" else gi.modes_up_to(4)
+    n_q = 2048 if modes == "l2" else 4096
+    Q, U, V, meta = gi.make_point(4004, dets, ml, n_q, 22.0, admix=0.0 if modes == "l2" else 0.1)
+    v, ax, ay = gi.detector_arrays(dets)
+    cfg = dict(config_id=1, dets=dets, modes=ml, Q=Q[None], U=U[None], V=V[None], l=np.array([x[0] for x in ml], dtype=np.int32),
+               m=np.array([x[1] for x in ml], dtype=np.int32), n_points=1, n_det=4, n_modes=len(ml), n_q=n_q, n_t=410, fs_hz=gi.FS_HZ,
+               t0_q_s=meta["t0_q_s"], gmst_rad=gi.GMST_RAD, d_ref_mpc=gi.D_REF_MPC, vertex_m=v, arm_x=ax, arm_y=ay, n=n)
+    s = gi.make_samples(4005, n)
+    full_compare(gpu_lib, cfg, s, variant=4)
+    if n == 20_000:
+        full_compare(gpu_lib, cfg, s)          # the automatic choice takes the same path
