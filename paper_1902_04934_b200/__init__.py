@@ -48,7 +48,8 @@ class _Config(ctypes.Structure):
     _fields_ = [("n_points", ctypes.c_int32), ("n_det", ctypes.c_int32), ("n_modes", ctypes.c_int32),
                 ("l", ctypes.POINTER(ctypes.c_int32)), ("m", ctypes.POINTER(ctypes.c_int32)),
                 ("n_q", ctypes.c_int32), ("n_t", ctypes.c_int32), ("fs_hz", ctypes.c_double), ("t0_q_s", ctypes.c_double),
-                ("gmst_rad", ctypes.c_double), ("d_ref_mpc", ctypes.c_double), ("det", ctypes.POINTER(_Detector))]
+                ("gmst_rad", ctypes.c_double), ("d_ref_mpc", ctypes.c_double), ("det", ctypes.POINTER(_Detector)),
+                ("shift_mode", ctypes.c_int32)]
 
 
 def load():
@@ -155,7 +156,7 @@ class Context:
                 det[k].arm_y[e] = float(cfg["arm_y"][k][e])
         c = _Config(self.n_points, K, M, l.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)),
                     m.ctypes.data_as(ctypes.POINTER(ctypes.c_int32)), self.n_q, self.n_t, float(cfg["fs_hz"]),
-                    float(cfg["t0_q_s"]), float(cfg["gmst_rad"]), float(cfg["d_ref_mpc"]), det)
+                    float(cfg["t0_q_s"]), float(cfg["gmst_rad"]), float(cfg["d_ref_mpc"]), det, int(cfg.get("shift_mode", 0)))
         Q = np.ascontiguousarray(cfg["Q"], dtype=np.complex128)
         U = np.ascontiguousarray(cfg["U"], dtype=np.complex128)
         V = np.ascontiguousarray(cfg["V"], dtype=np.complex128)

@@ -116,6 +116,7 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     if (!(cfg->fs_hz > 0.0) || !(cfg->d_ref_mpc > 0.0) || !std::isfinite(cfg->t0_q_s) || !std::isfinite(cfg->gmst_rad))
         return ILE_ERR_BAD_ARGUMENT;
     if (cfg->n_det > ILE_MAX_DET || cfg->n_modes > ILE_MAX_MODES) return ILE_ERR_UNSUPPORTED;
+    if (cfg->shift_mode != 0 && cfg->shift_mode != 1) return ILE_ERR_BAD_ARGUMENT;
     for (int j = 0; j < cfg->n_modes; ++j) {
         if (cfg->l[j] < 2 || std::abs(cfg->m[j]) > cfg->l[j]) return ILE_ERR_BAD_ARGUMENT;
         if (cfg->l[j] > ILE_MAX_L) return ILE_ERR_UNSUPPORTED;
@@ -137,6 +138,7 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     c->sz.n_modes = cfg->n_modes;
     c->sz.n_q = cfg->n_q;
     c->sz.n_t = cfg->n_t;
+    c->sz.interp = cfg->shift_mode;
     c->sz.sm_count = prop.multiProcessorCount;
     c->sz.max_smem_optin = (int32_t)prop.sharedMemPerBlockOptin;
     c->sz.smem_per_sm = (int32_t)prop.sharedMemPerMultiprocessor;
@@ -148,6 +150,7 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     P.n_modes = cfg->n_modes;
     P.n_q = cfg->n_q;
     P.n_t = cfg->n_t;
+    P.interp = cfg->shift_mode;
     P.fs = cfg->fs_hz;
     P.t0_q = cfg->t0_q_s;
     P.gmst = cfg->gmst_rad;
@@ -188,7 +191,7 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     CKC(cudaMemcpy(c->dU, U, nU * sizeof(double2), cudaMemcpyDefault));
     CKC(cudaMemcpy(c->dV, V, nU * sizeof(double2), cudaMemcpyDefault));
     CKC(cudaMemset(c->d_oob, 0, sizeof(unsigned long long)));
-    c->stream_ok = ile_stream_plan(c->sz, c->hparams, 0, &c->spl, &c->ssp);
+    c->stream_ok = !c->sz.interp && ile_stream_plan(c->sz, c->hparams, 0, &c->spl, &c->ssp);
     if (c->stream_ok) {
         CKC(ile_stream_prepare(c->sz, &c->spl));
         if (cfg->n_modes >= ILE_QUAD_MMA_MIN_MODES) {
@@ -389,7 +392,7 @@ static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n
     }
     int nl = 0;
     IleTiledLayout L;
-    const bool tiled = c->variant == 2 || (c->variant == 0 && ile_tiled_plan(c->sz, (long long)n * n_points, &L));
+    const bool tiled = !c->sz.interp && (c->variant == 2 || (c->variant == 0 && ile_tiled_plan(c->sz, (long long)n * n_points, &L)));
     cudaError_t e = tiled ? ile_launch_eval_tiled(c->sz, c->hparams, a, st, &nl) : ile_launch_eval_direct(c->sz, a, st, &nl);
     c->launches += nl;
     if (e != cudaSuccess) return cuda_fail(e);
@@ -617,6 +620,7 @@ extern "C" int ile_harvest(ile_ctx *c, int32_t point, int64_t n, const double *r
     if (!ra || !dec || !t_ref || !phi_ref || !psi || !incl || !dist_mpc || !argmax_bin || !lnL_max) return ILE_ERR_BAD_ARGUMENT;
     if (drawn_bin && !v_uniform) return ILE_ERR_BAD_ARGUMENT;
     if (!ids && n_sel > n) return ILE_ERR_BAD_ARGUMENT;
+    if (c->sz.interp) return ILE_ERR_UNSUPPORTED;  // harvesting reads the nearest-sample series
     if (int r = check_device(c)) return r;
     IleEvalArgs a;
     a.params = c->dparams;
@@ -650,6 +654,7 @@ extern "C" int ile_set_variant(ile_ctx *c, int32_t variant)
     if (variant > 4) return ILE_ERR_UNSUPPORTED;
     if (variant == 3) return ILE_ERR_UNSUPPORTED;  // retired (superseded by variant 4)
     if (variant == 4 && !c->stream_ok) return ILE_ERR_UNSUPPORTED;
+    if (c->sz.interp && variant > 1) return ILE_ERR_UNSUPPORTED;  // interpolated shifts: direct kernel only
     if (variant == 2) {
         IleTiledLayout L;
         if (!ile_tiled_plan(c->sz, 1LL << 40, &L)) return ILE_ERR_UNSUPPORTED;

@@ -13,6 +13,7 @@
 
 struct IleDevParams {
     int32_t n_points, n_det, n_modes, n_q, n_t;
+    int32_t interp;  // 1: linear interpolation of Q between samples (reading R8')
     double fs, t0_q, gmst, d_ref;
     double det_tensor[ILE_MAX_DET][6];  // D = (x x^T - y y^T)/2, symmetric: xx, xy, xz, yy, yz, zz
     double vertex[ILE_MAX_DET][3];      // metres
@@ -97,6 +98,18 @@ __device__ __forceinline__ int32_t ile_window_index(const double *__restrict__ v
     return __double2int_rn(x) - n_t / 2;
 }
 
+// The same expression floored instead of rounded, with the fractional part (reading R8': linear interpolation between samples).
+__device__ __forceinline__ int32_t ile_window_floor(const double *__restrict__ v, const double *__restrict__ s, double t_ref,
+                                                    double t0_q, double fs, int32_t n_t, double *phi)
+{
+    double dot = __dadd_rn(__dadd_rn(__dmul_rn(v[0], s[0]), __dmul_rn(v[1], s[1])), __dmul_rn(v[2], s[2]));
+    double dt = __ddiv_rn(-dot, ILE_C_SI);
+    double x = __dmul_rn(__dsub_rn(__dadd_rn(t_ref, dt), t0_q), fs);
+    double fl = floor(x);
+    *phi = __dsub_rn(x, fl);
+    return (int32_t)fl - n_t / 2;
+}
+
 // Y_lm(iota, -phi_ref) = [sum_t coef_t c^pc_t s^ps_t] e^{-i m phi_ref}, c = cos(iota/2), s = sin(iota/2)  (R4, R5)
 __device__ __forceinline__ double2 ile_ylm(const IleDevParams *__restrict__ P, int mode, double ch, double sh,
                                            double phi_ref)
@@ -124,7 +137,7 @@ __device__ __forceinline__ double2 ile_cmul(double2 a, double2 b)
 __device__ __forceinline__ double ile_setup_sample(const IleDevParams *__restrict__ P, const double2 *__restrict__ U,
                                                    const double2 *__restrict__ V, double ra, double dec, double t_ref,
                                                    double phi_ref, double psi, double incl, double dist, double2 *A,
-                                                   int ldA, int32_t *i0, int *bad)
+                                                   int ldA, int32_t *i0, int *bad, double *phi = nullptr)
 {
     const int K = P->n_det, M = P->n_modes;
     IleSky g = ile_sky(ra, dec, psi, P->gmst);
@@ -159,9 +172,15 @@ __device__ __forceinline__ double ile_setup_sample(const IleDevParams *__restric
         double F2 = F.x * F.x + F.y * F.y;
         double2 FF = ile_cmul(F, F);
         tot += F2 * yuy + (FF.x * yvy.x - FF.y * yvy.y);
-        int32_t idx = ile_window_index(P->vertex[k], g.s, t_ref, P->t0_q, P->fs, P->n_t);
+        int32_t idx;
+        if (phi) {  // interpolated shifts: one sample more is read
+            idx = ile_window_floor(P->vertex[k], g.s, t_ref, P->t0_q, P->fs, P->n_t, phi + k);
+            if (idx < 0 || (long long)idx + P->n_t + 1 > P->n_q) oob = 1;
+        } else {
+            idx = ile_window_index(P->vertex[k], g.s, t_ref, P->t0_q, P->fs, P->n_t);
+            if (idx < 0 || (long long)idx + P->n_t > P->n_q) oob = 1;
+        }
         i0[k] = idx;
-        if (idx < 0 || (long long)idx + P->n_t > P->n_q) oob = 1;
     }
     for (int k = K - 1; k >= 0; --k) {  // k = 0 last: it overwrites the parked Y_m in place
         double2 F = ile_antenna(P->det_tensor[k], g);

@@ -17,6 +17,7 @@
 #define DIRECT_WARPS 8
 #define DIRECT_RB 4
 
+template <bool INTERP>
 __global__ void __launch_bounds__(DIRECT_WARPS * 32) ile_eval_direct_kernel(IleEvalArgs a, int G)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -25,12 +26,14 @@ __global__ void __launch_bounds__(DIRECT_WARPS * 32) ile_eval_direct_kernel(IleE
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
 
     // per-warp carve-up
-    const size_t per_warp = (size_t)G * KM * sizeof(double2) + (size_t)G * sizeof(double) + (size_t)G * K * sizeof(int32_t) + (size_t)G * sizeof(int32_t);
+    const size_t per_warp = (size_t)G * KM * sizeof(double2) + (size_t)G * sizeof(double) + (size_t)G * K * sizeof(double) +
+                            (size_t)G * K * sizeof(int32_t) + (size_t)G * sizeof(int32_t);
     const size_t per_warp_al = (per_warp + 15) & ~(size_t)15;
     unsigned char *wbase = smem_raw + warp * per_warp_al;
     double2 *A = reinterpret_cast<double2 *>(wbase);
     double *quadS = reinterpret_cast<double *>(A + (size_t)G * KM);
-    int32_t *i0S = reinterpret_cast<int32_t *>(quadS + G);
+    double *phiS = quadS + G;  // [G][K] fractional parts of the arrival times (INTERP)
+    int32_t *i0S = reinterpret_cast<int32_t *>(phiS + (size_t)G * K);
     int32_t *badS = i0S + (size_t)G * K;
 
     const long long groups_per_point = (a.n_per_point + G - 1) / G;
@@ -50,7 +53,7 @@ __global__ void __launch_bounds__(DIRECT_WARPS * 32) ile_eval_direct_kernel(IleE
             int bad;
             double q = ile_setup_sample(P, a.U + pglob * (size_t)KM * M, a.V + pglob * (size_t)KM * M, a.ra[s], a.dec[s],
                                         a.t_ref[s], a.phi_ref[s], a.psi[s], a.incl[s], a.dist[s], A + (size_t)lane * KM, M,
-                                        i0S + lane * K, &bad);
+                                        i0S + lane * K, &bad, INTERP ? phiS + lane * K : nullptr);
             quadS[lane] = q;
             badS[lane] = bad;
             if (a.shift_idx)
@@ -76,12 +79,17 @@ __global__ void __launch_bounds__(DIRECT_WARPS * 32) ile_eval_direct_kernel(IleE
                 }
                 for (int k = 0; k < K; ++k) {
                     const double2 *Qk = Qp + (size_t)k * M * n_q + i0S[g * K + k];
+                    const double ph = INTERP ? phiS[g * K + k] : 0.0, om = 1.0 - ph;
                     for (int m = 0; m < M; ++m) {
                         const double2 c = Ag[k * M + m];
                         const double2 *Qkm = Qk + (size_t)m * n_q;
 #pragma unroll
                         for (int r = 0; r < DIRECT_RB; ++r) {
                             double2 q = __ldg(Qkm + jj[r]);
+                            if (INTERP) {  // (1 - phi) Q[i] + phi Q[i + 1]  (reading R8')
+                                const double2 q1 = __ldg(Qkm + jj[r] + 1);
+                                q.x = om * q.x + ph * q1.x, q.y = om * q.y + ph * q1.y;
+                            }
                             acc[r] = fma(c.x, q.x, fma(c.y, q.y, acc[r]));  // Re(conj(A) Q)
                         }
                     }
@@ -113,31 +121,38 @@ __global__ void __launch_bounds__(DIRECT_WARPS * 32) ile_eval_direct_kernel(IleE
 static size_t direct_smem_bytes(const IleSizes &sz, int G)
 {
     size_t KM = (size_t)sz.n_det * sz.n_modes;
-    size_t per_warp = (size_t)G * KM * sizeof(double2) + (size_t)G * sizeof(double) + (size_t)G * sz.n_det * sizeof(int32_t) + (size_t)G * sizeof(int32_t);
+    size_t per_warp = (size_t)G * KM * sizeof(double2) + (size_t)G * sizeof(double) + (size_t)G * sz.n_det * sizeof(double) +
+                      (size_t)G * sz.n_det * sizeof(int32_t) + (size_t)G * sizeof(int32_t);
     per_warp = (per_warp + 15) & ~(size_t)15;
     return per_warp * DIRECT_WARPS;
 }
 
-cudaError_t ile_launch_eval_direct(const IleSizes &sz, const IleEvalArgs &a, cudaStream_t st, int *n_launches)
+template <bool INTERP>
+static cudaError_t direct_launch_t(const IleSizes &sz, const IleEvalArgs &a, cudaStream_t st, int *n_launches)
 {
     if (a.n_per_point <= 0 || a.n_points <= 0) return cudaSuccess;
     int G = 32;
     while (G > 1 && direct_smem_bytes(sz, G) > 96 * 1024) G >>= 1;
     size_t smem = direct_smem_bytes(sz, G);
     if (smem > (size_t)sz.max_smem_optin) return cudaErrorInvalidValue;
-    cudaError_t e = cudaFuncSetAttribute(ile_eval_direct_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(ile_eval_direct_kernel<INTERP>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     int per_sm = 0;
-    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ile_eval_direct_kernel, DIRECT_WARPS * 32, smem);
+    e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ile_eval_direct_kernel<INTERP>, DIRECT_WARPS * 32, smem);
     if (e != cudaSuccess) return e;
     if (per_sm < 1) per_sm = 1;
     long long groups = ((a.n_per_point + G - 1) / G) * a.n_points;
     long long blocks_needed = (groups + DIRECT_WARPS - 1) / DIRECT_WARPS;
     long long grid = (long long)sz.sm_count * per_sm;
     if (blocks_needed < grid) grid = blocks_needed;
-    ile_eval_direct_kernel<<<(unsigned)grid, DIRECT_WARPS * 32, smem, st>>>(a, G);
+    ile_eval_direct_kernel<INTERP><<<(unsigned)grid, DIRECT_WARPS * 32, smem, st>>>(a, G);
     if (n_launches) *n_launches += 1;
     return cudaGetLastError();
+}
+
+cudaError_t ile_launch_eval_direct(const IleSizes &sz, const IleEvalArgs &a, cudaStream_t st, int *n_launches)
+{
+    return sz.interp ? direct_launch_t<true>(sz, a, st, n_launches) : direct_launch_t<false>(sz, a, st, n_launches);
 }
 
 // ------------------------------------------------------------------------------------------------------------

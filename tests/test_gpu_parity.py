@@ -554,3 +554,24 @@ def test_four_detector_network_on_the_streaming_kernel(gpu_lib, modes, n):
     full_compare(gpu_lib, cfg, s, variant=4)
     if n == 20_000:
         full_compare(gpu_lib, cfg, s)          # the automatic choice takes the same path
+
+
+# ---------------------------------------------------------------------------------------------- NEXT-4: interpolated (sub-sample) shifts
+@pytest.mark.parametrize("cid,n", [(0, 1_000), (1, 3_001), (5, 400)])
+def test_linear_interpolated_shifts_match_the_oracle(gpu_lib, cid, n):
+    """shift_mode = 1 (reading R8'): per-detector linear interpolation of Q between samples, against oracle/subsample.py; the floor
+    indices bit-exact, lnL_margT within TOL; windows that need the sample beyond the series are out of range."""
+    from oracle import subsample as osub
+
+    cfg = gi.make_config(cid, n=n)
+    cfg["shift_mode"] = 1
+    s = gi.make_samples(cfg["sample_seeds"][0] + 9, n)
+    s["t_ref"][3] = 0.9
+    ctx, lnL, idx, n_bad = run_gpu(gpu_lib, cfg, s)
+    ref, ref_idx, ref_bad = osub.eval_batch_lin(cfg, s)
+    assert n_bad == ref_bad >= 1
+    assert_indices_equal(cfg, s, ref_idx, idx.cpu().numpy())
+    assert rel_err(ref, lnL.cpu().numpy()) <= TOL
+    with pytest.raises(gpu_lib.IleError):
+        ctx.set_variant(4)
+    ctx.close()
