@@ -220,7 +220,9 @@ def run_integrate(args, rank: int):
     ile_integrate -- Philox draws, sampling-prior refits, ile_eval and the evidence all on the device; per chunk two
     doubles cross the bus.  Workload: BASELINE.json configs[--config], chunks of --n samples (default 10,000: the paper's
     block size, L97 / n_chunk L119), --chunks chunks per step (default 200: N_it = 2e6, L119), adapting in RA, dec and
-    distance after every chunk, no early stop (n_eff threshold = inf) so that every step does the same work."""
+    distance after each of the first --adapt-chunks chunks (default 10; L125: "only adapt until a marginalized likelihood evaluation
+    returns significant lnL_marg"), no early stop (n_eff threshold = inf) so that every step does the same work.  With frozen
+    densities the remaining chunks are drawn and evaluated about 2^20 samples at a time; results are those of the chunk-by-chunk loop."""
     if rank != 0:
         return
     import numpy as np
@@ -242,7 +244,7 @@ def run_integrate(args, rank: int):
         ctx.set_variant(args.variant)
     smp = ile.Sampler(scfg)
     for _ in range(max(args.warmup, 3)):
-        ile.integrate(ctx, smp, n_chunk, min(chunks, 10), chunks, float("inf"))
+        ile.integrate(ctx, smp, n_chunk, chunks, min(chunks, args.adapt_chunks), float("inf"))
     torch.cuda.synchronize()
     sampler = ClockSampler(0)
     l0, s0 = ctx.launch_count, smp.launch_count
@@ -251,7 +253,7 @@ def run_integrate(args, rank: int):
     t0 = time.perf_counter()
     e0.record()
     for _ in range(args.steps):
-        r = ile.integrate(ctx, smp, n_chunk, chunks, chunks, float("inf"))
+        r = ile.integrate(ctx, smp, n_chunk, chunks, min(chunks, args.adapt_chunks), float("inf"))
     e1.record()
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
@@ -267,8 +269,9 @@ def run_integrate(args, rank: int):
             "unit": UNIT, "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
             "config": {"workload": f"ile_integrate on BASELINE.json configs[{args.config}] ({K} detectors, {M} modes, {n_t} bins): {chunks} chunks "
-                                   f"of {n_chunk} Philox-drawn samples per step, refit of the (RA, dec, distance) sampling prior after every chunk",
-                       "n_chunk": n_chunk, "chunks_per_step": chunks, "variant": args.variant},
+                                   f"of {n_chunk} Philox-drawn samples per step, refit of the (RA, dec, distance) sampling prior after each of the first "
+                                   f"{min(chunks, args.adapt_chunks)} chunks",
+                       "n_chunk": n_chunk, "chunks_per_step": chunks, "adapt_chunks": min(chunks, args.adapt_chunks), "variant": args.variant},
             "roofline": {"bound": "alu", "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
                          "kernel": "whole loop (draw, index/sort, coefficients, contraction + marginalisation, evidence, refit)",
                          "dfma_equiv_per_sample": w},
@@ -283,7 +286,7 @@ def run_integrate(args, rank: int):
         cores = os.cpu_count() or 1
         nchk = 3
         t0 = time.perf_counter()
-        osm.integrate(scfg, lambda sd: oracle.eval_batch(cfg, sd, n_threads=cores)[0], n_chunk, nchk, nchk, float("inf"))
+        osm.integrate(scfg, lambda sd: oracle.eval_batch(cfg, sd, n_threads=cores)[0], n_chunk, nchk, min(nchk, args.adapt_chunks), float("inf"))
         dt = time.perf_counter() - t0
         line["cpu_baseline"] = {"value": n_chunk * nchk / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"the first {nchk} chunks of the same run: oracle/sampler.py (numpy) around oracle.eval_batch (OpenMP)"}
@@ -323,6 +326,8 @@ def main():
                     help="precompute: time ile_precompute (eq. 8: Q, U, V of --points intrinsic points); integrate: time ile_integrate "
                          "(the adaptive Monte Carlo loop with on-device sampling) instead of the hot path")
     ap.add_argument("--chunks", type=int, default=200, help="--stage integrate: chunks per step")
+    ap.add_argument("--adapt-chunks", type=int, default=10,
+                    help="--stage integrate: chunks after which the sampling prior is frozen (PAPER.md L125: adapt only early in the run)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 

@@ -297,6 +297,29 @@ __global__ void ile_evidence_merge_kernel(int32_t n_segments, int32_t n_states, 
     if (n_eff) n_eff[seg] = ok ? sm : 0.0;
 }
 
+// Running evidence over a sequence of chunks: states [n_chunks][3] of disjoint chunks in order, `run` [3] the carried state
+// (in/out); hist [n_chunks][2] = (lnZ, n_eff) of everything up to and including each chunk.  One thread: n_chunks is small.
+__global__ void ile_evidence_prefix_kernel(int32_t n_chunks, const double *__restrict__ states, double *__restrict__ run,
+                                           double *__restrict__ hist)
+{
+    if (blockIdx.x || threadIdx.x) return;
+    double m = run[0], sm = run[1], cnt = run[2];
+    for (int c = 0; c < n_chunks; ++c) {
+        ev_merge(m, sm, states[3 * c], states[3 * c + 1]);
+        cnt += states[3 * c + 2];
+        const bool ok = m > -CUDART_INF;
+        hist[2 * c] = ok ? m + log(sm) - log(cnt) : -CUDART_INF;
+        hist[2 * c + 1] = ok ? sm : 0.0;
+    }
+    run[0] = m, run[1] = sm, run[2] = cnt;
+}
+
+cudaError_t ile_launch_evidence_prefix(int32_t n_chunks, const double *states, double *run, double *hist, cudaStream_t st)
+{
+    ile_evidence_prefix_kernel<<<1, 32, 0, st>>>(n_chunks, states, run, hist);
+    return cudaGetLastError();
+}
+
 cudaError_t ile_launch_evidence_merge(int32_t n_segments, int32_t n_states, const double *states_in, double *state_out,
                                       double *lnZ, double *n_eff, cudaStream_t st, int *n_launches)
 {

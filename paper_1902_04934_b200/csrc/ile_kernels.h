@@ -155,6 +155,7 @@ cudaError_t ile_launch_evidence(int32_t n_segments, int64_t n_per_segment, const
 int32_t ile_evidence_blocks_per_segment(int32_t n_segments, int64_t n_per_segment, int32_t sm_count);
 cudaError_t ile_launch_evidence_merge(int32_t n_segments, int32_t n_states, const double *states_in, double *state_out,
                                       double *lnZ, double *n_eff, cudaStream_t st, int *n_launches);
+cudaError_t ile_launch_evidence_prefix(int32_t n_chunks, const double *states, double *run, double *hist, cudaStream_t st);
 cudaError_t ile_launch_evidence_reset(int32_t n_segments, double *state, cudaStream_t st, int *n_launches);
 
 // calibration kernels: dmma = 0 register-resident DFMA chains, 1 = DMMA.8x8x4 chains; 8 blocks of 256 threads per SM

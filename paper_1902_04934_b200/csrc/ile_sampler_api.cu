@@ -17,6 +17,8 @@ struct ile_sampler {
     int32_t *d_bins;
     int64_t cap;
     double *d_state;      // evidence state [3] + (lnZ, n_eff) per chunk slot [2][2]
+    double *d_multi;      // frozen-density phase: per-chunk states [B][3], scratch lnZ / n_eff [2 B], history [B][2]
+    int64_t multi_cap;    // B
     double *h_hist;       // pinned [max_chunks][2]
     int64_t hist_cap;
     cudaEvent_t ev[2];
@@ -93,6 +95,7 @@ extern "C" void ile_sampler_destroy(ile_sampler *s)
     cudaFree(s->d_buf);
     cudaFree(s->d_bins);
     cudaFree(s->d_state);
+    cudaFree(s->d_multi);
     if (s->h_hist) cudaFreeHost(s->h_hist);
     if (s->ev[0]) cudaEventDestroy(s->ev[0]);
     if (s->ev[1]) cudaEventDestroy(s->ev[1]);
@@ -173,15 +176,15 @@ extern "C" int64_t ile_sampler_launch_count(const ile_sampler *s) { return s ? (
 // ------------------------------------------------------------------------------------------------------------
 // the adaptive Monte Carlo loop (S7-S8) with every array resident on the device
 // ------------------------------------------------------------------------------------------------------------
-static int smp_ensure(ile_sampler *s, int64_t n_chunk, int32_t max_chunks, cudaStream_t st)
+static int smp_ensure(ile_sampler *s, int64_t n_samples, int32_t max_chunks, int64_t multi, cudaStream_t st)
 {
-    if (n_chunk > s->cap) {
+    if (n_samples > s->cap) {
         CK(cudaStreamSynchronize(st));
         cudaFree(s->d_buf), cudaFree(s->d_bins);
         s->d_buf = nullptr, s->d_bins = nullptr, s->cap = 0;
-        CK(cudaMalloc(&s->d_buf, (size_t)9 * n_chunk * sizeof(double)));
-        CK(cudaMalloc(&s->d_bins, (size_t)3 * n_chunk * sizeof(int32_t)));
-        s->cap = n_chunk;
+        CK(cudaMalloc(&s->d_buf, (size_t)9 * n_samples * sizeof(double)));
+        CK(cudaMalloc(&s->d_bins, (size_t)3 * n_samples * sizeof(int32_t)));
+        s->cap = n_samples;
     }
     if (max_chunks > s->hist_cap) {
         CK(cudaStreamSynchronize(st));
@@ -189,6 +192,13 @@ static int smp_ensure(ile_sampler *s, int64_t n_chunk, int32_t max_chunks, cudaS
         s->h_hist = nullptr, s->hist_cap = 0;
         CK(cudaMallocHost(&s->h_hist, (size_t)2 * max_chunks * sizeof(double)));
         s->hist_cap = max_chunks;
+    }
+    if (multi > s->multi_cap) {
+        CK(cudaStreamSynchronize(st));
+        cudaFree(s->d_multi);
+        s->d_multi = nullptr, s->multi_cap = 0;
+        CK(cudaMalloc(&s->d_multi, (size_t)7 * multi * sizeof(double)));
+        s->multi_cap = multi;
     }
     return ILE_OK;
 }
@@ -199,7 +209,12 @@ extern "C" int ile_integrate(ile_ctx *ctx, ile_sampler *s, int32_t point, int64_
     if (!ctx || !s || n_chunk < 1 || max_chunks < 1 || n_adapt_chunks < 0 || !lnZ) return ILE_ERR_BAD_ARGUMENT;
     if (int r = smp_check_device(s)) return r;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    int r = smp_ensure(s, n_chunk, max_chunks, st);
+    // Once the densities are frozen (c >= n_adapt_chunks) chunks no longer depend on one another: they are drawn and evaluated
+    // `multi` at a time (about 2^20 samples per ile_eval) and only the evidence is still accumulated chunk by chunk.
+    const int32_t frozen = max_chunks > n_adapt_chunks ? max_chunks - n_adapt_chunks : 0;
+    int64_t multi = frozen ? ((int64_t)1 << 20) / n_chunk : 0;
+    multi = multi < 1 ? (frozen ? 1 : 0) : multi > frozen ? frozen : multi;
+    int r = smp_ensure(s, n_chunk * (multi > 1 ? multi : 1), max_chunks, multi, st);
     if (r != ILE_OK) return r;
     r = ile_sampler_reset(s, cuda_stream);  // S9: the first chunk is drawn from the prior
     if (r != ILE_OK) return r;
@@ -214,7 +229,8 @@ extern "C" int ile_integrate(ile_ctx *ctx, ile_sampler *s, int32_t point, int64_
     // and accumulated, so the GPU never idles on the stopping rule.  A chunk that turns out to lie beyond the stop is never
     // refit from and its numbers are never reported: results, densities and sample count are those of the strict rule S8.
     int32_t stop = -1, done = 0;
-    for (int32_t c = 0; c < max_chunks && stop < 0; ++c) {
+    const int32_t n_seq = multi > 1 ? (n_adapt_chunks < max_chunks ? n_adapt_chunks : max_chunks) : max_chunks;  // chunks taken one by one
+    for (int32_t c = 0; c < n_seq && stop < 0; ++c) {
         r = ile_sampler_draw(s, (int64_t)c * n, n, ra, dec, t_ref, phi, psi, incl, dist, log_w, s->d_bins, cuda_stream);
         if (r == ILE_OK) r = ile_eval(ctx, point, n, ra, dec, t_ref, phi, psi, incl, dist, lnL, nullptr, cuda_stream);
         if (r == ILE_OK) r = ile_evidence(ctx, 1, n, lnL, log_w, state, res + 2 * (c & 1), res + 2 * (c & 1) + 1, cuda_stream);
@@ -230,6 +246,30 @@ extern "C" int ile_integrate(ile_ctx *ctx, ile_sampler *s, int32_t point, int64_
             r = ile_sampler_refit(s, n, s->d_bins, lnL, log_w, cuda_stream);
             if (r != ILE_OK) return r;
         }
+    }
+    if (stop < 0 && done > 0 && done < max_chunks) {  // the last adaptive chunk decides whether the frozen phase starts at all
+        CK(cudaEventSynchronize(s->ev[(done - 1) & 1]));
+        if (s->h_hist[2 * (size_t)(done - 1) + 1] >= n_eff_min) stop = done - 1;
+    }
+    // ---- frozen densities: `cnt` chunks per draw / ile_eval, evidence per chunk (segmented reduction, then a running merge)
+    while (stop < 0 && done < max_chunks) {
+        const int32_t cnt = (int32_t)(max_chunks - done < multi ? max_chunks - done : multi);
+        const int64_t tot = (int64_t)cnt * n;
+        double *ra2 = b, *dec2 = b + tot, *t2 = b + 2 * tot, *phi2 = b + 3 * tot, *psi2 = b + 4 * tot, *incl2 = b + 5 * tot, *dist2 = b + 6 * tot;
+        double *lw2 = b + 7 * tot, *lnL2 = b + 8 * tot;
+        double *cst = s->d_multi, *ctmp = cst + 3 * (size_t)multi, *chist = ctmp + 2 * (size_t)multi;
+        r = ile_sampler_draw(s, (int64_t)done * n, tot, ra2, dec2, t2, phi2, psi2, incl2, dist2, lw2, nullptr, cuda_stream);
+        if (r == ILE_OK) r = ile_eval(ctx, point, tot, ra2, dec2, t2, phi2, psi2, incl2, dist2, lnL2, nullptr, cuda_stream);
+        if (r == ILE_OK) r = ile_evidence_reset(ctx, cnt, cst, cuda_stream);
+        if (r == ILE_OK) r = ile_evidence(ctx, cnt, n, lnL2, lw2, cst, ctmp, ctmp + cnt, cuda_stream);
+        if (r != ILE_OK) return r;
+        CK(ile_launch_evidence_prefix(cnt, cst, state, chist, st));
+        ile_ctx_add_launches(ctx, 1);
+        CK(cudaMemcpyAsync(s->h_hist + 2 * (size_t)done, chist, 2 * (size_t)cnt * sizeof(double), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        for (int32_t c = 0; c < cnt && stop < 0; ++c)
+            if (s->h_hist[2 * (size_t)(done + c) + 1] >= n_eff_min) stop = done + c;
+        done += cnt;
     }
     CK(cudaStreamSynchronize(st));
     if (stop < 0) stop = done - 1;  // the last chunk: threshold reached there, or max_chunks exhausted
