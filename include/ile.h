@@ -130,7 +130,8 @@ int ile_evidence_merge(ile_ctx *ctx, int32_t n_segments, int32_t n_states, const
  *   Q[p][k][m][i] = sum_n conj(x[p][k][m][n]) d[p][k][n] exp(+2 pi i f_n (t0_q_s + i / fs_hz))   (one inverse FFT per series)
  *   U[p][k][a][b] = sum_n conj(x[p][k][a][n]) x[p][k][b][n],   V[p][k][a][b] = sum_n x[p][k][a][(-n) mod n_q] x[p][k][b][n]
  * x: device complex128 [P][K][M][n_q]; d: device complex128 [P][K][n_q]; Q, U, V: device outputs, caller-owned, shapes as
- * ile_create reads them.  n_q must be a power of two, 2..8192 (else ILE_ERR_UNSUPPORTED).  Asynchronous on cuda_stream;
+ * ile_create reads them.  n_q must be a power of two, 2..65536 (else ILE_ERR_UNSUPPORTED; above 8192 a two-level
+ * transform through a library-owned scratch buffer).  Asynchronous on cuda_stream;
  * needs no context. */
 int ile_precompute(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_q, double fs_hz, double t0_q_s, const void *x,
                    const void *d, void *Q, void *U, void *V, void *cuda_stream);
@@ -142,7 +143,7 @@ int ile_precompute(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_q
  *   Q = sum_n g conj(h) d exp(...),   U = sum_n g conj(h_a) h_b,   V = sum_n g h_a[(-n) mod n_q] h_b[n]
  * h: device complex128 [P][K][M][n_q] mode spectra, d: device complex128 [P][K][n_q] data spectra, S: device double [P][K][n_q]
  * the one-sided noise power spectral density sampled at |f_n| in FFT order (> 0 inside the band), scale: the measure (2 df for
- * eq. 2 as printed, times the caller's Fourier-transform normalisation).  n_q a power of two, 512..8192. */
+ * eq. 2 as printed, times the caller's Fourier-transform normalisation).  n_q a power of two, 512..65536. */
 int ile_precompute_psd(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_q, double fs_hz, double t0_q_s, const void *h,
                        const void *d, const double *S, double f_min_hz, double f_max_hz, double scale, void *Q, void *U, void *V,
                        void *cuda_stream);

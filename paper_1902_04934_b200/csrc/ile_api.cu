@@ -469,7 +469,7 @@ static int precompute_any(int32_t n_points, int32_t n_det, int32_t n_modes, int3
                           void *cuda_stream)
 {
     if (n_points < 1 || n_det < 1 || n_modes < 1 || n_q < 1 || !(fs_hz > 0.0) || !x || !d || !Q || !U || !V) return ILE_ERR_BAD_ARGUMENT;
-    if (n_det > ILE_MAX_DET || n_modes > ILE_MAX_MODES || n_q < 2 || n_q > 8192 || (n_q & (n_q - 1))) return ILE_ERR_UNSUPPORTED;
+    if (n_det > ILE_MAX_DET || n_modes > ILE_MAX_MODES || n_q < 2 || n_q > 65536 || (n_q & (n_q - 1))) return ILE_ERR_UNSUPPORTED;
     if (S && n_q < 512) return ILE_ERR_UNSUPPORTED;
     int dev = 0, optin = 0;
     if (cudaGetDevice(&dev) != cudaSuccess) return ILE_ERR_NO_DEVICE;

@@ -188,26 +188,30 @@ __device__ __forceinline__ double2 pc_input(const double2 *__restrict__ xs, cons
     return make_double2(xv.x * w.x + xv.y * w.y, xv.x * w.y - xv.y * w.x);  // conj(x) w
 }
 
-template <int T>  // T = N / 8 threads
+// STRIDE = 1: the whole transform of a series.  STRIDE = 8: the second level of a two-level transform of length 8 N -- block
+// (series, i1) transforms row i1 of the first level's output (plain loads from `x`) and writes X[i1 + 8 i2]; `tab` is then the
+// table of the LONG transform, whose every eighth twiddle is the short one's.
+template <int T, int STRIDE>  // T = N / 8 threads
 __global__ void __launch_bounds__(T)
     ile_overlap_q_radix8_kernel(int32_t M, int32_t N, const double2 *__restrict__ tab, const double2 *__restrict__ x,
                                 const double2 *__restrict__ d, const PcWeight wt, double2 *__restrict__ Q)
 {
     extern __shared__ double2 pc_sm[];
-    const size_t series = blockIdx.x;  // (point * K + k) * M + mode
+    const size_t series = blockIdx.x;  // (point * K + k) * M + mode; STRIDE = 8: that times 8 + i1
     const double2 *xs = x + series * N, *ds = d + (series / M) * N, *ph = tab + N / 2;
     const double *Ss = wt.S ? wt.S + (series / M) * N : nullptr;
-    double2 *q = Q + series * N;
+    double2 *q = STRIDE == 1 ? Q + series * N : Q + (series / STRIDE) * ((size_t)N * STRIDE) + (series % STRIDE);
+    const int NB = N * STRIDE;  // length the table was built for
     const int j = threadIdx.x;  // blockDim.x == T == N / 8: one radix-8 butterfly per thread and pass
     double2 u[8];
     // ---- pass 1 (sub-transform length 1, no twiddles): inputs from global memory
 #pragma unroll
-    for (int r = 0; r < 8; ++r) u[r] = pc_input(xs, ds, ph, Ss, wt, N, j + r * T);
+    for (int r = 0; r < 8; ++r) u[r] = STRIDE == 1 ? pc_input(xs, ds, ph, Ss, wt, N, j + r * T) : __ldcs(xs + j + r * T);
     pc_bfly8(u);
     int ns = 8;
     if (ns == N) {
 #pragma unroll
-        for (int r = 0; r < 8; ++r) q[j * 8 + r] = u[r];
+        for (int r = 0; r < 8; ++r) q[(size_t)(j * 8 + r) * STRIDE] = u[r];
         return;
     }
 #pragma unroll
@@ -219,7 +223,7 @@ __global__ void __launch_bounds__(T)
 #pragma unroll
         for (int r = 0; r < 8; ++r) u[r] = pc_sm[PC_PAD(j + r * T)];
         // twiddles exp(2 pi i r k / (8 ns)): the first from the table, the others by multiplication
-        const double2 w1 = pc_tw(tab, N, k * (N / (8 * ns)));
+        const double2 w1 = pc_tw(tab, NB, STRIDE * k * (N / (8 * ns)));
         double2 w = w1;
 #pragma unroll
         for (int r = 1; r < 8; ++r) {
@@ -229,7 +233,7 @@ __global__ void __launch_bounds__(T)
         pc_bfly8(u);
         if (ns * 8 == N) {  // last pass: natural order out, consecutive threads write consecutive addresses
 #pragma unroll
-            for (int r = 0; r < 8; ++r) __stcs(q + j0 + r * ns, u[r]);
+            for (int r = 0; r < 8; ++r) __stcs(q + (size_t)(j0 + r * ns) * STRIDE, u[r]);
             return;
         }
         __syncthreads();  // everybody has read its inputs
@@ -242,17 +246,18 @@ __global__ void __launch_bounds__(T)
         const int T4 = N >> 2;
         for (int jj = j; jj < T4; jj += T) {
             const int k = jj & (ns - 1), j0 = ((jj - k) << 2) + k;
-            const double2 w1 = pc_tw(tab, N, k), w2 = pc_cmul(w1, w1), w3 = pc_cmul(w2, w1);
+            const double2 w1 = pc_tw(tab, NB, STRIDE * k), w2 = pc_cmul(w1, w1), w3 = pc_cmul(w2, w1);
             double2 v0, v1, v2, v3;
             pc_bfly4(pc_sm[PC_PAD(jj)], pc_cmul(w1, pc_sm[PC_PAD(jj + T4)]), pc_cmul(w2, pc_sm[PC_PAD(jj + 2 * T4)]),
                      pc_cmul(w3, pc_sm[PC_PAD(jj + 3 * T4)]), v0, v1, v2, v3);
-            __stcs(q + j0, v0), __stcs(q + j0 + ns, v1), __stcs(q + j0 + 2 * ns, v2), __stcs(q + j0 + 3 * ns, v3);
+            __stcs(q + (size_t)j0 * STRIDE, v0), __stcs(q + (size_t)(j0 + ns) * STRIDE, v1);
+            __stcs(q + (size_t)(j0 + 2 * ns) * STRIDE, v2), __stcs(q + (size_t)(j0 + 3 * ns) * STRIDE, v3);
         }
     } else {
         const int T2 = N >> 1;
         for (int jj = j; jj < T2; jj += T) {  // ns = N / 2, k = jj
-            const double2 a0 = pc_sm[PC_PAD(jj)], a1 = pc_cmul(pc_tw(tab, N, jj), pc_sm[PC_PAD(jj + T2)]);
-            __stcs(q + jj, pc_add(a0, a1)), __stcs(q + jj + ns, pc_sub(a0, a1));
+            const double2 a0 = pc_sm[PC_PAD(jj)], a1 = pc_cmul(pc_tw(tab, NB, STRIDE * jj), pc_sm[PC_PAD(jj + T2)]);
+            __stcs(q + (size_t)jj * STRIDE, pc_add(a0, a1)), __stcs(q + (size_t)(jj + ns) * STRIDE, pc_sub(a0, a1));
         }
     }
 }
@@ -333,6 +338,34 @@ __global__ void __launch_bounds__(PC_THREADS, 2)
     }
 }
 
+// First level of the two-level transform, N = 8 N2 (16384 ... 65536 points): with n = n2 + N2 n1 and i = i1 + 8 i2,
+//   X[i1 + 8 i2] = sum_{n2} W_{N2}^{n2 i2} [ W_N^{n2 i1} sum_{n1} c[n2 + N2 n1] W_8^{n1 i1} ].
+// Thread n2 does the bracket -- eight inputs at stride N2 (coalesced across threads), one radix-8 butterfly, the twiddles -- and
+// writes row i1 of Z[series][8][N2]; the second level is the radix-8 kernel with STRIDE = 8 on every row.
+__global__ void __launch_bounds__(PC_THREADS)
+    ile_overlap_q_split8_kernel(int32_t M, int32_t N, const double2 *__restrict__ tab, const double2 *__restrict__ x,
+                                const double2 *__restrict__ d, const PcWeight wt, double2 *__restrict__ Z)
+{
+    const size_t series = blockIdx.y;
+    const int N2 = N >> 3, n2 = blockIdx.x * blockDim.x + threadIdx.x;
+    if (n2 >= N2) return;
+    const double2 *xs = x + series * N, *ds = d + (series / M) * N, *ph = tab + N / 2;
+    const double *Ss = wt.S ? wt.S + (series / M) * N : nullptr;
+    double2 u[8];
+#pragma unroll
+    for (int r = 0; r < 8; ++r) u[r] = pc_input(xs, ds, ph, Ss, wt, N, n2 + r * N2);
+    pc_bfly8(u);
+    const double2 w1 = pc_tw(tab, N, n2);
+    double2 w = w1;
+    double2 *z = Z + series * N + n2;
+    z[0] = u[0];
+#pragma unroll
+    for (int r = 1; r < 8; ++r) {
+        z[(size_t)r * N2] = pc_cmul(w, u[r]);
+        w = pc_cmul(w, w1);
+    }
+}
+
 // Few modes (M <= PC_MS): one block per (point, detector); warp (a, slice) takes row a and one of PC_NS slices of the frequency
 // axis, a lane one frequency at a time, and keeps the sums of the pairs (a, b >= a) in registers.  U is Hermitian and V symmetric
 // by their definitions (U_ba = conj(U_ab); V_ba = sum_n x_b[-n] x_a[n] is the same set of products as V_ab), so only b >= a is
@@ -405,9 +438,10 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
 {
     int log2n = 0;
     while ((1 << log2n) < N) ++log2n;
-    if ((1 << log2n) != N || N < 2 || N > 8192) return cudaErrorInvalidValue;
-    const bool radix8 = N >= 512;
-    const size_t smem = radix8 ? (size_t)(N + N / 8) * 16 : (size_t)2 * N * 16;
+    if ((1 << log2n) != N || N < 2 || N > 65536) return cudaErrorInvalidValue;
+    const bool radix8 = N >= 512, two_level = N > 8192;
+    const int NS = two_level ? N / 8 : N;  // length of the shared-memory transform
+    const size_t smem = radix8 ? (size_t)(NS + NS / 8) * 16 : (size_t)2 * N * 16;
     if (smem > (size_t)max_smem_optin) return cudaErrorInvalidValue;
     cudaError_t e = cudaSuccess;
     // U, V kernel for many modes: enough frequency slices that a block's 8 warps all have work items
@@ -420,16 +454,19 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
     static double2 *g_tab[64] = {nullptr};
     static int g_tab_n[64] = {0};
     static double g_tab_alpha[64] = {0.0};
+    static double2 *g_z[64] = {nullptr};  // first-level output of the two-level transform, grown on demand
+    static size_t g_z_cap[64] = {0};
     int dev = 0;
     e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return e;
     if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
     if (!g_tab[dev]) {
-        e = cudaMalloc(&g_tab[dev], (size_t)(4096 + 8192) * sizeof(double2));
+        e = cudaMalloc(&g_tab[dev], (size_t)(32768 + 65536) * sizeof(double2));
         if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4608 * 16));
-        if (e != cudaSuccess) return e;
-        e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(9216 * 16));
+        e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel<512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4608 * 16));
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel<1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(9216 * 16));
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel<512, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4608 * 16));
+        if (e == cudaSuccess) e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel<1024, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(9216 * 16));
         if (e != cudaSuccess) return e;
     }
     double2 *tab = g_tab[dev];
@@ -444,13 +481,31 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
     // Q kernel has just read) was measured and lost -- 0.24 ms against 0.19 ms for 256 points of 3 x 5 x 2048: both kernels are
     // bound by the latency of a block's own load - compute - store chain, and batches serialise those chains.
     const unsigned n_series = (unsigned)((size_t)n_points * K * M);
-    if (radix8) {
+    if (two_level) {
+        const size_t need = (size_t)n_series * N;
+        if (need > g_z_cap[dev]) {
+            e = cudaStreamSynchronize(st);
+            if (e != cudaSuccess) return e;
+            cudaFree(g_z[dev]);
+            g_z[dev] = nullptr, g_z_cap[dev] = 0;
+            e = cudaMalloc(&g_z[dev], need * sizeof(double2));
+            if (e != cudaSuccess) return e;
+            g_z_cap[dev] = need;
+        }
+        double2 *Z = g_z[dev];
+        ile_overlap_q_split8_kernel<<<dim3((unsigned)(NS / PC_THREADS), n_series), PC_THREADS, 0, st>>>(M, N, tab, x, d, wt, Z);
+        switch (NS) {  // rows of the first level: plain loads, output stride 8, every eighth twiddle of the long table
+            case 2048: ile_overlap_q_radix8_kernel<256, 8><<<n_series * 8, 256, smem, st>>>(M, NS, tab, Z, d, wt, Q); break;
+            case 4096: ile_overlap_q_radix8_kernel<512, 8><<<n_series * 8, 512, smem, st>>>(M, NS, tab, Z, d, wt, Q); break;
+            default: ile_overlap_q_radix8_kernel<1024, 8><<<n_series * 8, 1024, smem, st>>>(M, NS, tab, Z, d, wt, Q); break;
+        }
+    } else if (radix8) {
         switch (N) {
-            case 512: ile_overlap_q_radix8_kernel<64><<<n_series, 64, smem, st>>>(M, N, tab, x, d, wt, Q); break;
-            case 1024: ile_overlap_q_radix8_kernel<128><<<n_series, 128, smem, st>>>(M, N, tab, x, d, wt, Q); break;
-            case 2048: ile_overlap_q_radix8_kernel<256><<<n_series, 256, smem, st>>>(M, N, tab, x, d, wt, Q); break;
-            case 4096: ile_overlap_q_radix8_kernel<512><<<n_series, 512, smem, st>>>(M, N, tab, x, d, wt, Q); break;
-            default: ile_overlap_q_radix8_kernel<1024><<<n_series, 1024, smem, st>>>(M, N, tab, x, d, wt, Q); break;
+            case 512: ile_overlap_q_radix8_kernel<64, 1><<<n_series, 64, smem, st>>>(M, N, tab, x, d, wt, Q); break;
+            case 1024: ile_overlap_q_radix8_kernel<128, 1><<<n_series, 128, smem, st>>>(M, N, tab, x, d, wt, Q); break;
+            case 2048: ile_overlap_q_radix8_kernel<256, 1><<<n_series, 256, smem, st>>>(M, N, tab, x, d, wt, Q); break;
+            case 4096: ile_overlap_q_radix8_kernel<512, 1><<<n_series, 512, smem, st>>>(M, N, tab, x, d, wt, Q); break;
+            default: ile_overlap_q_radix8_kernel<1024, 1><<<n_series, 1024, smem, st>>>(M, N, tab, x, d, wt, Q); break;
         }
     } else {
         if (S) return cudaErrorInvalidValue;  // short transforms take whitened spectra only

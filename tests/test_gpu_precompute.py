@@ -52,7 +52,7 @@ def test_precompute_matches_oracle_on_config_shapes(gpu_lib, cid, n_points):
         check(V[p], rv, axes=(-1, -2))
 
 
-@pytest.mark.parametrize("n_q", [2, 4, 64, 256, 512, 1024, 4096, 8192])
+@pytest.mark.parametrize("n_q", [2, 4, 64, 256, 512, 1024, 4096, 8192, 16384, 32768, 65536])
 def test_precompute_edge_sizes_and_fractional_start_time(gpu_lib, n_q):
     r = np.random.default_rng(n_q)
     K, M = 1, (1 if n_q == 2 else 3)
@@ -97,7 +97,7 @@ def test_chain_precompute_create_eval_matches_oracle_chain(gpu_lib):
     ctx.close()
 
 
-@pytest.mark.parametrize("n_q,M,P", [(512, 2, 1), (2048, 5, 3), (4096, 21, 1), (8192, 4, 2), (1024, 7, 1)])
+@pytest.mark.parametrize("n_q,M,P", [(512, 2, 1), (2048, 5, 3), (4096, 21, 1), (8192, 4, 2), (1024, 7, 1), (16384, 2, 2), (32768, 4, 1)])
 def test_precompute_psd_matches_oracle(gpu_lib, n_q, M, P):
     """ile_precompute_psd: un-whitened spectra, 1 / S weighting and band mask of eq. 2 on the device, against oracle.overlaps_psd;
     few modes (register-resident pair sums) and many modes (tiled pair sums)."""
