@@ -24,10 +24,11 @@
 // Per 8-row block and warp: K*KS DMMA (16 pipe cycles each), 2 x 9 FP64 operations of log-sum-exp, K*KS coalesced 256-byte
 // fragment loads that hit L1 (consecutive groups use the same rows), 4 (K-1) SHFL.
 //
-// Q is repacked once per context as Qs[point][k][s][row][4]: the A fragment of (detector k, k-step s, rows base..base+7) is
-// 32 consecutive doubles starting at any row -- one coalesced 256-byte load per DMMA at an arbitrary 32-byte offset.  The
-// series are zero padded in front and behind so that rows outside [0, N_Q), which only ever feed elements outside every
-// window, read as zeros.
+// Q is repacked once per context as Qs[point][k][row / 8][s][row % 8][4]: the A fragment of (detector k, k-step s, rows
+// base..base+7) is two contiguous runs of 32-byte rows (one if base is a multiple of 8) -- a 256-byte load per DMMA that touches
+// 2-3 lines -- and the fragments of the other k-steps and of the following 8-row blocks lie at compile-time offsets from it, so
+// a lane keeps ONE pointer per detector.  The series are zero padded in front and behind so that rows outside [0, N_Q), which only
+// ever feed elements outside every window, read as zeros.
 #include <cstdio>
 #include <limits.h>
 #include <math_constants.h>
@@ -201,7 +202,6 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
     const int n_t = a.n_t;
     const double log_nt = log((double)n_t);
     const int total = a.gcum[a.n_points];
-    const size_t nqp4 = (size_t)a.nqp * 4;
 
     // Work distribution: the group list (all points, each in window-start order) is cut into n_ranges contiguous ranges and
     // an SM works through the range of its own id, so that the warps of one SM stream the same few hundred rows of Q and the
@@ -300,11 +300,15 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
 #pragma unroll
                 for (int s = 0; s < KS; ++s) bf[k][s] = has ? ST_STREAM_LD(rp + k * a.cp + 4 * s) : 0.0;
         }
-        // ---- A fragment pointers: pk[k] = this lane's element of the next block to load of detector k
+        // ---- A fragment pointers: pk[k] = this lane's element (row base_k + r, channel cc) of k-step 0 of detector k.  The packed
+        // series is blocked by 8 rows with a block's KS k-steps side by side, so the other k-steps and the next 8-row blocks of the
+        // lane are at compile-time offsets: (blocks * KS + s) * 32 doubles.
         const double *pk[K];
 #pragma unroll
-        for (int k = 0; k < K; ++k)
-            pk[k] = a.Qs + ((size_t)((a.point0 + pt) * K + k) * KS * a.nqp + (size_t)(a.padf + base[k])) * 4 + lane;
+        for (int k = 0; k < K; ++k) {
+            const int row = a.padf + base[k] + r;
+            pk[k] = a.Qs + (size_t)((a.point0 + pt) * K + k) * KS * a.nqp * 4 + (size_t)(row >> 3) * (KS * 32) + (row & 7) * 4 + cc;
+        }
 
         const int nblk = ((dspread + n_t + 7) >> 3) + 1 & ~1;  // even: the stream advances two blocks per step
         const int t_lo = (dspread + 7) >> 3, t_hi = n_t >> 3;  // blocks [t_lo, t_hi) lie inside every window of the group
@@ -317,11 +321,11 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
             for (int u = 0; u < NC; ++u) {
                 double c0 = 0.0, c1 = 0.0;
 #pragma unroll
-                for (int s = 0; s < KS; ++s) st_dmma(c0, c1, __ldg(pk[k] + s * nqp4 + (size_t)u * 32), bf[k][s]);
+                for (int s = 0; s < KS; ++s) st_dmma(c0, c1, __ldg(pk[k] + (u * KS + s) * 32), bf[k][s]);
                 ring[k - 1][u][0] = c0;
                 ring[k - 1][u][1] = c1;
             }
-            pk[k] += NC * 32;
+            pk[k] += NC * KS * 32;
         }
         // fragments in registers one step ahead while they fit (PIPE); otherwise loaded where they are used
         constexpr bool PIPE = KS <= ST_PIPE_MAXKS && K <= 3;  // four detectors: fragments per chain (register budget)
@@ -333,7 +337,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
         auto ldchain = [&](auto BUF, int k, int bb) {
             constexpr int B = decltype(BUF)::value;
 #pragma unroll
-            for (int s = 0; s < KS; ++s) fa[B][PIPE ? 0 : s] = __ldg(pk[k] + s * nqp4 + bb * 32);
+            for (int s = 0; s < KS; ++s) fa[B][PIPE ? 0 : s] = __ldg(pk[k] + (bb * KS + s) * 32);
         };
         if (PIPE) {
 #pragma unroll
@@ -341,8 +345,8 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
 #pragma unroll
                 for (int bb = 0; bb < 2; ++bb)
 #pragma unroll
-                    for (int s = 0; s < KS; ++s) af[k][bb][PIPE ? s : 0] = __ldg(pk[k] + s * nqp4 + bb * 32);
-                pk[k] += 64;
+                    for (int s = 0; s < KS; ++s) af[k][bb][PIPE ? s : 0] = __ldg(pk[k] + (bb * KS + s) * 32);
+                pk[k] += 64 * KS;
             }
         } else {
             ldchain(std::integral_constant<int, 0>(), K > 1 ? 1 : 0, 0);
@@ -387,8 +391,8 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
 #pragma unroll
                     for (int bb = 0; bb < 2; ++bb)
 #pragma unroll
-                        for (int s = 0; s < KS; ++s) af[k][bb][PIPE ? s : 0] = __ldg(pk[k] + s * nqp4 + bb * 32);
-                    pk[k] += 64;
+                        for (int s = 0; s < KS; ++s) af[k][bb][PIPE ? s : 0] = __ldg(pk[k] + (bb * KS + s) * 32);
+                    pk[k] += 64 * KS;
                 }
             }
             st_lse_main2<PRED>(d, v, sm, tab_addr);
@@ -414,7 +418,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
                         ldchain(std::integral_constant<int, 1>(), 0, 1);
                     } else {  // the step is over for the pointers: the next chain is the next step's first
 #pragma unroll
-                        for (int k = 0; k < K; ++k) pk[k] += 64;
+                        for (int k = 0; k < K; ++k) pk[k] += 64 * KS;
                         ldchain(std::integral_constant<int, 0>(), K > 1 ? 1 : 0, 0);
                     }
                 }
@@ -427,8 +431,8 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
 #pragma unroll
                 for (int bb = 0; bb < 2; ++bb)
 #pragma unroll
-                    for (int s = 0; s < KS; ++s) af[0][bb][PIPE ? s : 0] = __ldg(pk[0] + s * nqp4 + bb * 32);
-                pk[0] += 64;
+                    for (int s = 0; s < KS; ++s) af[0][bb][PIPE ? s : 0] = __ldg(pk[0] + (bb * KS + s) * 32);
+                pk[0] += 64 * KS;
             }
         };
 #define ST_STEP(PP)                                                                                         \
@@ -478,20 +482,21 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
 }
 
 // ------------------------------------------------------------------------------------------------------------
-// Q repacking (once per context): Q [P][K][M][n_q] complex128 -> Qs [P][K][ks][nqp][4] doubles, channel 2m = Re, 2m+1 = Im
+// Q repacking (once per context): Q [P][K][M][n_q] complex128 -> Qs [P][K][nqp / 8][ks][8][4] doubles, channel 2m = Re, 2m+1 = Im
 // ------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) ile_pack_q_stream_kernel(int32_t n_series, int32_t M, int32_t n_q, int32_t ks, int32_t nqp,
                                                                 int32_t padf, const double2 *__restrict__ Q, double *__restrict__ Qs)
 {
     const long long total = (long long)n_series * ks * nqp * 4;
     for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < total; o += (long long)gridDim.x * blockDim.x) {
-        const int c4 = (int)(o & 3);
-        long long q = o >> 2;
-        const int row = (int)(q % nqp);
-        q /= nqp;
+        // o = (((series * (nqp / 8) + block) * ks + s) * 8 + row in block) * 4 + channel in k-step
+        const int c4 = (int)(o & 3), rr = (int)((o >> 2) & 7);
+        long long q = o >> 5;
         const int s = (int)(q % ks);
-        q /= ks;  // = p * K + k
-        const int ch = 4 * s + c4, m = ch >> 1, i = row - padf;
+        q /= ks;
+        const int blk = (int)(q % (nqp >> 3));
+        q /= (nqp >> 3);  // = p * K + k
+        const int ch = 4 * s + c4, m = ch >> 1, i = blk * 8 + rr - padf;
         double v = 0.0;
         if (m < M && i >= 0 && i < n_q) {
             const double2 z = Q[((size_t)q * M + m) * n_q + i];
@@ -699,8 +704,8 @@ bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per
     if (!pl.ks) return false;
     pl.cp = 4 * pl.ks;
     pl.nc = ST_NC;
-    pl.padf = sz.n_q - sz.n_t + 32;
-    pl.nqp = pl.padf + sz.n_q + (sz.n_q - sz.n_t) + 64;
+    pl.padf = (sz.n_q - sz.n_t + 32 + 7) & ~7;                               // multiples of the 8-row blocking
+    pl.nqp = (pl.padf + sz.n_q + (sz.n_q - sz.n_t) + 64 + 7) & ~7;
     IleSortPlan sp;
     sp.nd = sz.n_det;
     sp.g = pl.nc == 2 ? 4 : 3;
