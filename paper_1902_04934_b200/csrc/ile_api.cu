@@ -13,6 +13,7 @@ struct ile_ctx {
     IleDevParams hparams;
     IleDevParams *dparams;
     double2 *dQ, *dU, *dV;
+    double2 *hU, *hV;  // host mirrors of U, V (coefficient kernel: kernel-parameter path)
     unsigned long long *d_oob;
     double *d_partials;
     size_t partials_cap;  // doubles
@@ -191,28 +192,30 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     CKC(cudaMemcpy(c->dU, U, nU * sizeof(double2), cudaMemcpyDefault));
     CKC(cudaMemcpy(c->dV, V, nU * sizeof(double2), cudaMemcpyDefault));
     CKC(cudaMemset(c->d_oob, 0, sizeof(unsigned long long)));
+    c->hU = new (std::nothrow) double2[nU];
+    c->hV = new (std::nothrow) double2[nU];
+    if (!c->hU || !c->hV) {
+        ile_destroy(c);
+        return ILE_ERR_BAD_ARGUMENT;
+    }
+    CKC(cudaMemcpy(c->hU, c->dU, nU * sizeof(double2), cudaMemcpyDeviceToHost));
+    CKC(cudaMemcpy(c->hV, c->dV, nU * sizeof(double2), cudaMemcpyDeviceToHost));
     c->stream_ok = !c->sz.interp && ile_stream_plan(c->sz, c->hparams, 0, &c->spl, &c->ssp);
     if (c->stream_ok) {
         CKC(ile_stream_prepare(c->sz, &c->spl));
         if (cfg->n_modes >= ILE_QUAD_MMA_MIN_MODES) {
             const size_t nd = ile_quad_pack_doubles(cfg->n_points, cfg->n_det, cfg->n_modes);
             double *hm = new (std::nothrow) double[nd];
-            double2 *hU = new (std::nothrow) double2[nU], *hV = new (std::nothrow) double2[nU];
-            if (!hm || !hU || !hV) {
-                delete[] hm, delete[] hU, delete[] hV;
+            if (!hm) {
                 ile_destroy(c);
                 return ILE_ERR_CUDA;
             }
-            cudaError_t e1 = cudaMemcpy(hU, c->dU, nU * sizeof(double2), cudaMemcpyDeviceToHost);
-            cudaError_t e2 = cudaMemcpy(hV, c->dV, nU * sizeof(double2), cudaMemcpyDeviceToHost);
             cudaError_t e3 = cudaMalloc(&c->d_quad_mats, nd * sizeof(double));
-            if (e1 == cudaSuccess && e2 == cudaSuccess && e3 == cudaSuccess) {
-                ile_quad_pack_host(cfg->n_points, cfg->n_det, cfg->n_modes, hU, hV, hm);
+            if (e3 == cudaSuccess) {
+                ile_quad_pack_host(cfg->n_points, cfg->n_det, cfg->n_modes, c->hU, c->hV, hm);
                 e3 = cudaMemcpy(c->d_quad_mats, hm, nd * sizeof(double), cudaMemcpyHostToDevice);
             }
-            delete[] hm, delete[] hU, delete[] hV;
-            CKC(e1);
-            CKC(e2);
+            delete[] hm;
             CKC(e3);
         }
         CKC(cudaStreamCreateWithFlags(&c->ss.aux, cudaStreamNonBlocking));
@@ -264,6 +267,8 @@ extern "C" void ile_destroy(ile_ctx *c)
     if (c->ev_copy_go) cudaEventDestroy(c->ev_copy_go);
     if (c->ev_copy_done) cudaEventDestroy(c->ev_copy_done);
     if (c->h_small) cudaFreeHost(c->h_small);
+    delete[] c->hU;
+    delete[] c->hV;
     delete c;
 }
 
@@ -318,6 +323,7 @@ static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
         }
     }
     c->ss.Qs = c->dQs;
+    c->ss.hU = c->hU, c->ss.hV = c->hV;
     c->ss.slot_cap = slot_cap;
     // many modes: the quadratic forms run as an FP64-MMA contraction in front of the coefficient kernel (side stream)
     const bool quad_mma = c->d_quad_mats && (a.n_points == 1 || (a.n_per_point & 7) == 0);

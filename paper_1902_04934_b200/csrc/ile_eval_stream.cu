@@ -827,8 +827,7 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
         if (e != cudaSuccess) return e;
         ++nl;
     }
-    ile_launch_setup_coef(sz, hp, a, pl.cp, sc, ss.aux);
-    ++nl;
+    nl += ile_launch_setup_coef(sz, hp, a, pl.cp, sc, ss.hU, ss.hV, ss.aux);
     e = cudaEventRecord(ss.ev_join, ss.aux);
     if (e != cudaSuccess) return e;
     ile_stream_scan_kernel<<<dim3((unsigned)nseg, (unsigned)a.n_points), SS_THREADS, (size_t)sp.n0 * sizeof(uint32_t), st>>>(sp.n0, nseg, sp.ncell,

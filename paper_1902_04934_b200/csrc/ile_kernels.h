@@ -90,6 +90,7 @@ struct IleStreamScratch {
     cudaEvent_t ev_fork, ev_join;
     const double *quad_mats;  // packed U, V for ile_launch_quad_mma, or NULL
     cudaEvent_t ev_late;  // if not NULL: the arrays the coefficient kernel reads (phi_ref, psi, incl, dist) arrive with this event
+    const double2 *hU, *hV;  // host mirrors of U, V [P][K][M][M] (kernel-parameter path of the coefficient kernel), or NULL
 };
 
 bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point, IleStreamPlan *out, IleSortPlan *sp);
@@ -101,8 +102,9 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
                                    const IleSortPlan &sp, const IleSortScratch &sc, const IleStreamScratch &ss,
                                    cudaStream_t st, int *n_launches);
 // variant 4: coefficients a F_k Y_lm and quadratic term of every sample (steps 1, 3, 4), no sorting work
-void ile_launch_setup_coef(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, int32_t cp, const IleSortScratch &sc,
-                           cudaStream_t st);
+// (hU, hV: host mirrors of the context's U, V, or NULL; returns the number of kernels launched)
+int ile_launch_setup_coef(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, int32_t cp, const IleSortScratch &sc,
+                          const double2 *hU, const double2 *hV, cudaStream_t st);
 
 // step 4 for many modes (ile_quad_mma.cu): packed real representations of U, V and the batched quadratic forms
 size_t ile_quad_pack_doubles(int32_t n_points, int32_t K, int32_t M);
