@@ -1,6 +1,7 @@
 // ile_api.cu -- the C ABI of include/ile.h: context management, argument checking, kernel dispatch.
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 
@@ -203,6 +204,7 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     c->stream_ok = !c->sz.interp && ile_stream_plan(c->sz, c->hparams, 0, &c->spl, &c->ssp);
     if (c->stream_ok) {
         CKC(ile_stream_prepare(c->sz, &c->spl));
+        CKC(ile_stream_alloc_tables(&c->ss));
         if (cfg->n_modes >= ILE_QUAD_MMA_MIN_MODES) {
             const size_t nd = ile_quad_pack_doubles(cfg->n_points, cfg->n_det, cfg->n_modes);
             double *hm = new (std::nothrow) double[nd];
@@ -257,6 +259,7 @@ extern "C" void ile_destroy(ile_ctx *c)
     cudaFree(c->dQs);
     cudaFree(c->ss.slots);
     cudaFree(c->ss.gcum);
+    cudaFree(c->ss.tabs);
     cudaFree(c->d_quad_mats);
     cudaFree(c->d_qform);
     cudaFree(c->d_resample);

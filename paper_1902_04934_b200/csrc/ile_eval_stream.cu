@@ -7,8 +7,7 @@
 // [4 channels x 8 samples], C = lin [8 time rows x 8 samples].  On B200 DMMA and DFMA share the FP64 units (measured: their
 // times add), so DMMA buys no arithmetic; it buys issue slots and operand delivery: one instruction does 8 DFMA per lane.
 //
-// What differs from variant 3 (ile_eval_mma.cu): nothing of lin ever goes through shared memory and no block-level barrier
-// exists.  A warp owns 8 samples for the whole window and streams over 8-row time blocks:
+// Nothing of lin ever goes through shared memory and no block-level barrier exists.  A warp owns 8 samples for the whole window and streams over 8-row time blocks:
 //   * rows are absolute time rows of detector 0 (row rho <-> Q_0 row G0 + rho, G0 = the group's smallest window start); a
 //     sample's own window start inside the group, delta0 = i0_0 - G0, only decides WHICH rows enter its log-sum-exp;
 //   * detector k >= 1 is evaluated on rows base_k + rho with base_k = G0 + min over the group of d_k = i0_k - i0_0; the
@@ -17,11 +16,12 @@
 //     among the NC + 1 live blocks of that detector, the one its destination lane needs and one 64-bit warp shuffle moves
 //     it to row (r' - eps) mod 8.  The shifted partial sums are the C input of detector 0's MMA, so the detector sum costs
 //     K - 2 additions per element;
-//   * the time marginalisation (eq. 9) is an online max-free log-sum-exp per lane: running reference m (one of
-//     the lane's own lin values) and s = sum exp(lin - m); a new element more than 64 above m rescales s (rare: lin(t) is
-//     smooth on the scale of a block).  exp is a 1024-entry table of 2^(i/1024) in shared memory times a cubic in the
-//     remainder (|r| <= ln2/2048, truncation 5.5e-16): 7 FP64 operations per element plus the subtraction of m.
-// Per 8-row block and warp: K*KS DMMA (16 pipe cycles each), 2 x 9 FP64 operations of log-sum-exp, K*KS coalesced 256-byte
+//   * the time marginalisation (eq. 9) is an online log-sum-exp per lane: a running reference of a whole number of
+//     octaves and s = sum exp(lin) 2^-ref; an element more than 192 octaves above the reference moves it (rare: lin(t) is
+//     smooth on the scale of a block).  exp runs in fixed point (see ST_MAGIC below): one FMA puts lin / ln 2 - ref into the
+//     mantissa, a 2048-entry table of 2^(i/2048) in shared memory and a quadratic in the remaining 32 fraction bits do the rest --
+//     4 FP64 instructions per element (round 1-2a: 9), relative error 2.4e-13.
+// Per 8-row block and warp: K*KS DMMA (16 pipe cycles each), 2 x 4 FP64 operations of log-sum-exp, K*KS coalesced 256-byte
 // fragment loads that hit L1 (consecutive groups use the same rows), 4 (K-1) SHFL.
 //
 // Q is repacked once per context as Qs[point][k][row / 8][s][row % 8][4]: the A fragment of (detector k, k-step s, rows
@@ -39,7 +39,7 @@
 
 #define ST_FULL 0xffffffffu
 #ifndef ST_TAB_LOG2
-#define ST_TAB_LOG2 10
+#define ST_TAB_LOG2 11
 #endif
 #define ST_TAB (1 << ST_TAB_LOG2)
 #ifndef ST_THREADS
@@ -60,57 +60,75 @@ __device__ __forceinline__ void st_dmma(double &c0, double &c1, double a, double
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-#define ST_MAGIC 6755399441055744.0            /* 1.5 * 2^52: adding it rounds to the nearest integer */
-#define ST_C1 (1.4426950408889634 * ST_TAB)     /* ST_TAB / ln 2 */
-#define ST_C2 (0.6931471805599453 / ST_TAB)     /* ln 2 / ST_TAB (a power-of-two fraction of the double nearest ln 2: exact) */
-// exp(r) - the part the table does not cover: |r| <= ln 2 / (2 ST_TAB)
-#if ST_TAB_LOG2 >= 10
-#define ST_POLY(r) fma(fma(fma(1.0 / 6.0, (r), 0.5), (r), 1.0), (r), 1.0) /* truncation r^4/24 <= 5.5e-16 */
-#elif ST_TAB_LOG2 >= 6
-#define ST_POLY(r) fma(fma(fma(fma(1.0 / 24.0, (r), 1.0 / 6.0), (r), 0.5), (r), 1.0), (r), 1.0) /* r^5/120 <= 4e-14 at 64 entries */
+// ---- exp for the time marginalisation (eq. 9), in fixed point.  For an element x and a column reference of n octaves
+//   t = fma(x, ST_C1, mg),  mg = ST_MAGIC - n * ST_TAB,  ST_C1 = ST_TAB / ln 2,  ST_MAGIC = 1.5 * 2^20
+// is ONE rounding of  ST_MAGIC + y,  y = (x / ln 2 - n) * ST_TAB  (x - n ln 2 in table steps), to ulp(t) = 2^-32 as long as
+// |y| < 2^19: the low word of t is the fraction f of y (32 bits, floor semantics), the 20 mantissa bits of the high word are
+// [k + ST_KOFF | i] with y = ST_TAB k + i + f 2^-32.  Then
+//   exp(x - n ln 2) = 2^k * 2^(i / ST_TAB) * exp(ln 2 / ST_TAB * f 2^-32) = 2^(k + ST_KOFF) * tab[i] * p(g)
+// with tab[i] = 2^(i / ST_TAB - ST_KOFF) in shared memory, g = 1 + f 2^-32 assembled from the bits of f, and p the minimax quadratic
+// of exp(ln 2 / ST_TAB (g - 1)) on [1, 2) (error 2.0e-13 at 2048 entries; the rounding of y adds 4e-14): four FP64 instructions per
+// element -- the fma above, two for p, one to accumulate -- and the bit work on the integer pipes.  An element more than
+// ST_UP_OCT octaves above the reference (or NaN, +inf) shows as a high word above ST_HI_UP and takes the rare path, which moves
+// the reference; elements below -ST_KOFF + 6 octaves are clamped there (2^-250 of an element the sum already holds).
+#define ST_MAGIC 1572864.0                       /* 1.5 * 2^20 */
+#define ST_C1 (1.4426950408889634 * ST_TAB)      /* ST_TAB / ln 2 */
+#define ST_KOFF (1 << (19 - ST_TAB_LOG2))        /* offset of the octave field; the table carries 2^-ST_KOFF */
+#define ST_IDX_MASK (ST_TAB - 1)
+#define ST_K_MASK (0xFFFFF & ~ST_IDX_MASK)
+#define ST_UP_OCT (3 * ST_KOFF / 4)
+#define ST_HI_UP (0x41300000 + ((ST_KOFF + ST_UP_OCT) << ST_TAB_LOG2))
+#define ST_HI_FLOOR (0x41300000 + (6 << ST_TAB_LOG2))
+#if ST_TAB_LOG2 == 11
+#define ST_A0 0x1.ffd3a5661bac7p-1
+#define ST_A1 0x1.62c56e9ca3a21p-12
+#define ST_A2 0x1.ec1130cd9fbd5p-25
+#elif ST_TAB_LOG2 == 10
+#define ST_A0 0x1.ffa74ea4e1a54p-1  /* error 1.6e-12 */
+#define ST_A1 0x1.62a6aa1f75becp-11
+#define ST_A2 0x1.ec2682c0c27c1p-23
 #else
-#define ST_POLY(r) fma(fma(fma(fma(fma(1.0 / 120.0, (r), 1.0 / 24.0), (r), 1.0 / 6.0), (r), 0.5), (r), 1.0), (r), 1.0) /* r^6/720 <= 1.4e-13 at 16 */
+#error "ST_TAB_LOG2: 10 or 11"
 #endif
+#define ST_MG_UNSET (ST_MAGIC + 1073741824.0 * ST_TAB) /* reference at -2^30 octaves: the first valid element takes the rare path */
 
-// entry i of the table 2^(i/1024) in shared memory (tab = 32-bit shared address of entry 0)
-__device__ __forceinline__ double st_tab(uint32_t tab, int i)
+// 2^d for an integer-valued d <= 0; 0 below -1000
+__device__ __forceinline__ double st_pow2_neg(double d)
 {
-    double v;
-    asm("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(tab + ((uint32_t)(i & (ST_TAB - 1)) << 3)));
-    return v;
+    return d > -1000.0 ? __hiloint2double((1023 + (int)d) << 20, 0) : 0.0;
 }
 
-// exp(d) for d <= 0 (also -inf; NaN propagates), full result.  Used on the rare paths only.
-__device__ __forceinline__ double st_exp_neg(double d, uint32_t tab)
+// octaves of the reference held in mg
+__device__ __forceinline__ double st_ref_oct(double mg) { return (ST_MAGIC - mg) * (1.0 / ST_TAB); }
+
+// rare path: element x becomes the reference of its column
+__device__ __forceinline__ void st_reref(double x, double &mg, double &s)
 {
-    if (!(d > -708.0)) return d != d ? d : 0.0;
-    const double t = fma(d, ST_C1, ST_MAGIC);
-    const double kf = t - ST_MAGIC;
-    const double r = fma(kf, -ST_C2, d);
-    const int ti = __double2loint(t);
-    const double T = st_tab(tab, ti);
-    const double q = ST_POLY(r);
-    return q * __hiloint2double(__double2hiint(T) + ((ti >> ST_TAB_LOG2) << 20), __double2loint(T));
+    if (!(fabs(x) < 1.0e15)) {  // NaN, +inf: poison the sum (the reference stays, so every later element comes here too)
+        s = CUDART_NAN;
+        return;
+    }
+    const double n_new = rint(x * 1.4426950408889634);
+    s *= st_pow2_neg(st_ref_oct(mg) - n_new);
+    mg = ST_MAGIC - n_new * ST_TAB;
 }
 
-// Log-sum-exp of a pair of blocks, in two halves.  First half: d = lin - m for the lane's elements; a valid element more than 64
-// above the reference moves the reference up (rare: the only branch of the step).
+// Log-sum-exp of a pair of blocks (b = 0, 1) of the lane's two columns (c = 0, 1; column c carries (mg[c], s[c])), in two halves.
+// First half: t for the lane's four elements; one branch for the four (rare: lin(t) is smooth on the scale of a block).  The
+// elements of a column are taken in block order and all of them redone against the final reference (none has been added yet).
 //   v : the element lies inside the sample's window (PRED only; otherwise every element does)
-// Second half, branch free: s += exp(d) = 2^k * tab[i] * poly(r) with d = (ST_TAB k + i) ln2 / ST_TAB + r.
-// Pair version (two blocks b = 0, 1 of the lane's two columns c = 0, 1; x[b][c], column c carries (m[c], s[c])): one branch
-// for the four elements.  The elements of a column are taken in block order, so the rare path redoes the second one
-// against the reference the first one may have moved.
+// Second half, branch free: s += 2^(k + ST_KOFF) tab[i] p(g).
 template <bool PRED>
-__device__ __forceinline__ void st_lse_pre2(const double (&x)[2][2], const bool (&v)[2][2], double (&m)[2], double (&s)[2],
-                                            double (&d)[2][2], uint32_t tab)
+__device__ __forceinline__ void st_lse_pre2(const double (&x)[2][2], const bool (&v)[2][2], double (&mg)[2], double (&s)[2],
+                                            double (&t)[2][2])
 {
     bool any = false;
 #pragma unroll
     for (int b = 0; b < 2; ++b)
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
-            d[b][c] = x[b][c] - m[c];
-            bool g = __double2hiint(d[b][c]) > 0x40500000;  // d > 64, +inf
+            t[b][c] = fma(x[b][c], ST_C1, mg[c]);
+            bool g = __double2hiint(t[b][c]) > ST_HI_UP;
             if (PRED) g = g && v[b][c];
             any = any || g;
         }
@@ -119,44 +137,37 @@ __device__ __forceinline__ void st_lse_pre2(const double (&x)[2][2], const bool 
         for (int c = 0; c < 2; ++c) {
 #pragma unroll
             for (int b = 0; b < 2; ++b) {
-                bool g = __double2hiint(x[b][c] - m[c]) > 0x40500000;
+                bool g = __double2hiint(fma(x[b][c], ST_C1, mg[c])) > ST_HI_UP;
                 if (PRED) g = g && v[b][c];
-                if (g) {
-                    s[c] *= st_exp_neg(m[c] - x[b][c], tab);
-                    m[c] = x[b][c];
-                }
+                if (g) st_reref(x[b][c], mg[c], s[c]);
             }
-            // every element of the column against the final reference (none of them has been added to s yet)
-            d[0][c] = x[0][c] - m[c];
-            d[1][c] = x[1][c] - m[c];
+            t[0][c] = fma(x[0][c], ST_C1, mg[c]);
+            t[1][c] = fma(x[1][c], ST_C1, mg[c]);
         }
-    }
-    if (PRED) {  // elements outside the window may carry d = +inf (reference still unset): keep the arithmetic finite
-#pragma unroll
-        for (int b = 0; b < 2; ++b)
-#pragma unroll
-            for (int c = 0; c < 2; ++c) d[b][c] = v[b][c] ? d[b][c] : 0.0;
     }
 }
 
 template <bool PRED>
-__device__ __forceinline__ void st_lse_main2(const double (&d)[2][2], const bool (&v)[2][2], double (&s)[2], uint32_t tab)
+__device__ __forceinline__ void st_lse_main2(const double (&t)[2][2], const bool (&v)[2][2], double (&s)[2], uint32_t tab)
 {
     double e[2][2], S[2][2];
 #pragma unroll
     for (int b = 0; b < 2; ++b)
 #pragma unroll
         for (int c = 0; c < 2; ++c) {
-            const double t = fma(d[b][c], ST_C1, ST_MAGIC);
-            const double kf = t - ST_MAGIC;
-            const double r = fma(kf, -ST_C2, d[b][c]);
-            const int ti = __double2loint(t);
-            const double T = st_tab(tab, ti);
-            bool ok = (unsigned)__double2hiint(d[b][c]) < 0xC0862000u;  // d > -708
-            if (PRED) ok = ok && v[b][c];
-            const int h = __double2hiint(T) + ((ti >> ST_TAB_LOG2) << 20);
-            S[b][c] = __hiloint2double(ok ? h : 0, ok ? __double2loint(T) : 0);
-            e[b][c] = ST_POLY(r);
+            const int lo = __double2loint(t[b][c]);
+            const int hi = max(__double2hiint(t[b][c]), ST_HI_FLOOR);
+            double T;
+            asm("ld.shared.f64 %0, [%1];" : "=d"(T) : "r"(tab + ((uint32_t)(hi & ST_IDX_MASK) << 3)));
+            int Sh = __double2hiint(T) + ((hi & ST_K_MASK) << (20 - ST_TAB_LOG2));
+            int Sl = __double2loint(T);
+            if (PRED) {
+                Sh = v[b][c] ? Sh : 0;
+                Sl = v[b][c] ? Sl : 0;
+            }
+            S[b][c] = __hiloint2double(Sh, Sl);
+            const double g = __hiloint2double((int)__funnelshift_r((unsigned)lo, 0x3FFu, 12), lo << 20);
+            e[b][c] = fma(fma(ST_A2, g, ST_A1), g, ST_A0);
         }
 #pragma unroll
     for (int c = 0; c < 2; ++c) s[c] = fma(e[1][c], S[1][c], fma(e[0][c], S[0][c], s[c]));
@@ -169,11 +180,30 @@ __device__ __forceinline__ void st_lse_main2(const double (&d)[2][2], const bool
 
 __device__ __forceinline__ double st_shfl(double v, int src) { return __shfl_sync(ST_FULL, v, src); }
 
+
 // m ? b : a for an all-ones / all-zeros mask m: two LOP3, no predicate
 __device__ __forceinline__ double st_bsel(double a, double b, int m)
 {
     const int al = __double2loint(a), ah = __double2hiint(a), bl = __double2loint(b), bh = __double2hiint(b);
     return __hiloint2double(ah ^ ((ah ^ bh) & m), al ^ ((al ^ bl) & m));
+}
+
+// ln S + n ln 2 for a finite S > 0 (else through log()): S = 2^e m, m in [1, 2); with c the table centre next to m,
+// r = m / c - 1 (one rounding, |r| <= 2^-8) and ln m = ln c + (r - r^2/2 + ... - r^6/6), truncation 2e-18.  A dozen FP64
+// instructions where log() issues several dozen -- behind the other warps' DMMAs each of them waits for the pipe.
+__device__ __forceinline__ double st_log_plus(double S, double n, const double2 *__restrict__ ltab)
+{
+    const int hi = __double2hiint(S);
+    if ((unsigned)(hi - 0x00100000) >= 0x7fe00000u) return fma(n, 0.6931471805599453, log(S));  // 0, subnormal, inf, NaN, negative
+    const double m = __hiloint2double((hi & 0x000fffff) | 0x3ff00000, __double2loint(S));
+    const double2 t = ltab[(hi >> 13) & 127];
+    const double r = fma(m, t.x, -1.0);
+    double q = fma(r, -1.0 / 6.0, 0.2);
+    q = fma(q, r, -0.25);
+    q = fma(q, r, 1.0 / 3.0);
+    q = fma(q, r, -0.5);
+    q = fma(q * r, r, r);
+    return fma(n + (double)((hi >> 20) - 1023), 0.6931471805599453, t.y + q);
 }
 
 struct IleStreamKArgs {
@@ -188,13 +218,16 @@ struct IleStreamKArgs {
     uint32_t *rcnt;         // [n_ranges] claim counters, zeroed per launch
     int32_t n_ranges;
     double *lnL;
+    const double *tabs;     // [ST_TAB] exp table, then [128][2] log table (ile_stream_tab_kernel, once per context)
 };
 
 template <int K, int KS, int NC, int MINB>
 __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const __grid_constant__ IleStreamKArgs a)
 {
     __shared__ __align__(128) double tab[ST_TAB];
-    for (int i = threadIdx.x; i < ST_TAB; i += blockDim.x) tab[i] = exp2((double)i * (1.0 / ST_TAB));
+    __shared__ __align__(16) double2 ltab[128];  // (1 / c_i rounded, -ln of that) for c_i = 1 + (i + 1/2) / 128: st_log
+    for (int i = threadIdx.x; i < ST_TAB; i += blockDim.x) tab[i] = a.tabs[i];
+    for (int i = threadIdx.x; i < 128; i += blockDim.x) ltab[i] = make_double2(a.tabs[ST_TAB + 2 * i], a.tabs[ST_TAB + 2 * i + 1]);
     __syncthreads();
     const uint32_t tab_addr = (uint32_t)__cvta_generic_to_shared(tab);
 
@@ -203,40 +236,50 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
     const double log_nt = log((double)n_t);
     const int total = a.gcum[a.n_points];
 
-    // Work distribution: the group list (all points, each in window-start order) is cut into n_ranges contiguous ranges and
-    // an SM works through the range of its own id, so that the warps of one SM stream the same few hundred rows of Q and the
-    // fragments stay in its L1.  A warp whose range is used up moves on to the next range for good (ranges only shrink).
+    // Work distribution: the group list (all points, each in window-start order) is cut into n_ranges contiguous ranges of rq groups
+    // and an SM works through the range of its own id, so that the warps of one SM stream the same few hundred rows of Q and the
+    // fragments stay in its L1.  A warp whose range is used up moves on to another range for good (ranges only shrink).  Small
+    // launches have ONE range (a plain global counter).
     unsigned smid;
     asm("mov.u32 %0, %%smid;" : "=r"(smid));
-    int rg = (int)(smid % (unsigned)a.n_ranges);
     const int nr = a.n_ranges;
+    const int rq = (total + nr - 1) / nr;
+    int rg = (int)(smid % (unsigned)nr);
+    // the claim of a group is issued while the previous one is streamed (tn: lane 0's ticket in range rg)
+    unsigned tn = 0;
+    if (lane == 0) tn = atomicAdd(a.rcnt + rg, 1u);
     for (;;) {
         int w = -1;
         for (;;) {
-            const long long lo = (long long)total * rg / nr, hi = (long long)total * (rg + 1) / nr;
-            unsigned t = 0;
-            if (lane == 0) t = atomicAdd(a.rcnt + rg, 1u);
-            t = __shfl_sync(ST_FULL, t, 0);
-            if (lo + (long long)t < hi) {
-                w = (int)(lo + t);
+            const int lo = rg * rq, hi = min(lo + rq, total);
+            const unsigned t = __shfl_sync(ST_FULL, tn, 0);
+            if (t < (unsigned)max(hi - lo, 0)) {
+                w = lo + (int)t;
                 break;
             }
             // own range used up: the lanes look at 32 other ranges at a time for one with groups left
             int found = -1;
             for (int base = 1; base < nr && found < 0; base += 32) {
-                const int off = base + lane, cand = (rg + off) % nr;
+                const int off = base + lane;
+                int cand = rg + off;
+                if (cand >= nr) cand -= nr;
                 bool left = false;
                 if (off < nr) {
-                    const long long clo = (long long)total * cand / nr, chi = (long long)total * (cand + 1) / nr;
-                    left = clo + (long long)*((volatile uint32_t *)a.rcnt + cand) < chi;
+                    const int clo = cand * rq, chi = min(clo + rq, total);
+                    left = *((volatile uint32_t *)a.rcnt + cand) < (unsigned)max(chi - clo, 0);
                 }
                 const unsigned mk = __ballot_sync(ST_FULL, left);
-                if (mk) found = (rg + base + __ffs(mk) - 1) % nr;
+                if (mk) {
+                    found = rg + base + __ffs(mk) - 1;
+                    if (found >= nr) found -= nr;
+                }
             }
             if (found < 0) break;
             rg = found;
+            if (lane == 0) tn = atomicAdd(a.rcnt + rg, 1u);
         }
         if (w < 0) break;
+        if (lane == 0) tn = atomicAdd(a.rcnt + rg, 1u);  // the next group's ticket
         int pt = 0;
         if (a.n_points > 1) {
             int lo = 0, hi = a.n_points;
@@ -291,6 +334,9 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
         }
         const int jc[2] = {jA, jB};
 
+        const int nblk = ((dspread + n_t + 7) >> 3) + 1 & ~1;  // even: the stream advances two blocks per step
+        const int t_lo = (dspread + 7) >> 3, t_hi = n_t >> 3;  // blocks [t_lo, t_hi) lie inside every window of the group
+
         // ---- B fragments: coefficients a F_k Y_lm of sample r, channels 4s + cc
         double bf[K][KS];
         {
@@ -309,9 +355,6 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
             const int row = a.padf + base[k] + r;
             pk[k] = a.Qs + (size_t)((a.point0 + pt) * K + k) * KS * a.nqp * 4 + (size_t)(row >> 3) * (KS * 32) + (row & 7) * 4 + cc;
         }
-
-        const int nblk = ((dspread + n_t + 7) >> 3) + 1 & ~1;  // even: the stream advances two blocks per step
-        const int t_lo = (dspread + 7) >> 3, t_hi = n_t >> 3;  // blocks [t_lo, t_hi) lie inside every window of the group
 
         // ---- prologue: blocks 0 .. NC-1 of the shifted detectors into the ring (slot of block b = b % 4); first fragments
         double ring[K > 1 ? K - 1 : 1][4][2];
@@ -356,7 +399,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
         // (2 (K-1) independent chains), the log-sum-exp of the PREVIOUS pair (independent of everything else in the step),
         // the realignment, detector 0's MMAs (2 chains).  Fragments are loaded one step ahead into the registers the
         // chains have just released.
-        double m[2] = {-CUDART_INF, -CUDART_INF}, sm[2] = {0.0, 0.0}, lin[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
+        double mg[2] = {ST_MG_UNSET, ST_MG_UNSET}, sm[2] = {0.0, 0.0}, lin[2][2] = {{0.0, 0.0}, {0.0, 0.0}};
         auto step = [&](auto PC, auto PREDC, const int t0) {
             constexpr int P = decltype(PC)::value;  // t0 % 4 == 2 P
             constexpr bool PRED = decltype(PREDC)::value;
@@ -368,7 +411,7 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
                     for (int c = 0; c < 2; ++c) v[bb][c] = (unsigned)(jc[c] + 8 * (t0 - 2 + bb)) < (unsigned)n_t;
             }
             double d[2][2];
-            st_lse_pre2<PRED>(lin, v, m, sm, d, tab_addr);
+            st_lse_pre2<PRED>(lin, v, mg, sm, d);
             // shifted detectors: blocks t0 + NC + bb into ring slots (2 P + NC + bb) % 4
 #pragma unroll
             for (int k = 1; k < K; ++k) {
@@ -448,6 +491,10 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
             ST_STEP(1)
         }
 #undef ST_STEP
+        // lanes of row 0 finish column A, lanes of row 1 column B: their sample's quad is fetched now, behind the last log-sum-exp
+        const int s_fin = (r & 1) ? sB : sA;
+        double quad_fin = 0.0;
+        if (r < 2 && s_fin >= 0) quad_fin = ST_STREAM_LD(a.quad + sbase + s_fin);
         {  // the last pair's log-sum-exp
             bool v[2][2];
 #pragma unroll
@@ -455,30 +502,47 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
 #pragma unroll
                 for (int c = 0; c < 2; ++c) v[bb][c] = (unsigned)(jc[c] + 8 * (nblk - 2 + bb)) < (unsigned)n_t;
             double d[2][2];
-            st_lse_pre2<true>(lin, v, m, sm, d, tab_addr);
+            st_lse_pre2<true>(lin, v, mg, sm, d);
             st_lse_main2<true>(d, v, sm, tab_addr);
         }
-        const double mA = m[0], mB = m[1], sumA = sm[0], sumB = sm[1];
-
         // ---- merge the 8 row lanes of each column, write lnL_margT = LSE - ln N_t - quad  (eq. 9 with the rectangle rule)
-        double MA = mA, MB = mB;
+        const double nA = st_ref_oct(mg[0]), nB = st_ref_oct(mg[1]);  // references in octaves (-2^30: the lane saw no element)
+        double NA = nA, NB = nB;
 #pragma unroll
         for (int o = 4; o < 32; o <<= 1) {
-            MA = fmax(MA, st_shfl(MA, lane ^ o));
-            MB = fmax(MB, st_shfl(MB, lane ^ o));
+            NA = fmax(NA, st_shfl(NA, lane ^ o));
+            NB = fmax(NB, st_shfl(NB, lane ^ o));
         }
-        double SA = mA > -CUDART_INF ? sumA * st_exp_neg(mA - MA, tab_addr) : 0.0;
-        double SB = mB > -CUDART_INF ? sumB * st_exp_neg(mB - MB, tab_addr) : 0.0;
+        double SA = sm[0] * st_pow2_neg(nA - NA), SB = sm[1] * st_pow2_neg(nB - NB);
 #pragma unroll
         for (int o = 4; o < 32; o <<= 1) {
             SA += st_shfl(SA, lane ^ o);
             SB += st_shfl(SB, lane ^ o);
         }
-        if (r == 0) {
-            if (sA >= 0) a.lnL[sbase + sA] = MA + log(SA) - log_nt - a.quad[sbase + sA];
-            if (sB >= 0) a.lnL[sbase + sB] = MB + log(SB) - log_nt - a.quad[sbase + sB];
-        }
+        if (r < 2 && s_fin >= 0) a.lnL[sbase + s_fin] = st_log_plus((r & 1) ? SB : SA, (r & 1) ? NB : NA, ltab) - log_nt - quad_fin;
     }
+}
+
+// exp and log tables of the streaming kernel (once per context)
+__global__ void ile_stream_tab_kernel(double *__restrict__ t)
+{
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < ST_TAB) t[i] = exp2((double)i * (1.0 / ST_TAB) - (double)ST_KOFF);
+    if (i < 128) {
+        const double rc = 1.0 / (1.0 + ((double)i + 0.5) * (1.0 / 128.0));
+        t[ST_TAB + 2 * i] = rc;
+        t[ST_TAB + 2 * i + 1] = -log(rc);
+    }
+}
+
+cudaError_t ile_stream_alloc_tables(IleStreamScratch *ss)
+{
+    cudaError_t e = cudaMalloc(&ss->tabs, (ST_TAB + 256) * sizeof(double));
+    if (e != cudaSuccess) return e;
+    ile_stream_tab_kernel<<<(ST_TAB + 255) / 256, 256>>>(ss->tabs);
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    return cudaSuccess;
 }
 
 // ------------------------------------------------------------------------------------------------------------
@@ -747,7 +811,8 @@ template <int K, int KS, int NC, int MINB>
 static cudaError_t st_launch_t(const IleSizes &sz, const IleStreamKArgs *ka, long long max_groups, int *per_sm, cudaStream_t st)
 {
     if (!ka) {
-        cudaError_t e = cudaFuncSetAttribute(ile_eval_stream_kernel<K, KS, NC, MINB>, cudaFuncAttributePreferredSharedMemoryCarveout, 8);
+        cudaError_t e = cudaFuncSetAttribute(ile_eval_stream_kernel<K, KS, NC, MINB>, cudaFuncAttributePreferredSharedMemoryCarveout,
+                                             (MINB * (ST_TAB * 8 + 1024) * 100 + 228 * 1024 - 1) / (228 * 1024));
         if (e != cudaSuccess) return e;
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(per_sm, ile_eval_stream_kernel<K, KS, NC, MINB>, ST_THREADS, 0);
         if (e != cudaSuccess) return e;
@@ -866,10 +931,14 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     ka.slots = ss.slots;
     ka.gcum = ss.gcum;
     ka.rcnt = rcnt;
-    ka.n_ranges = sz.sm_count < ILE_STREAM_MAX_RANGES ? sz.sm_count : ILE_STREAM_MAX_RANGES;
     ka.lnL = a.lnL;
+    ka.tabs = ss.tabs;
     const long long max_groups = (long long)a.n_points * (ss.slot_cap / 8);
     int per_sm = pl.ctas_per_sm;
+    // per-SM ranges pay off from a few groups per SM (measured: 66 vs 72 us at 10,000 samples, 65 vs 59 us at 1,000); below
+    // that one global counter
+    const int nr_sm = sz.sm_count < ILE_STREAM_MAX_RANGES ? sz.sm_count : ILE_STREAM_MAX_RANGES;
+    ka.n_ranges = max_groups < 4LL * nr_sm ? 1 : nr_sm;
     e = st_launch(sz, pl.ks, &ka, max_groups, &per_sm, st);
     ++nl;
     if (e == cudaSuccess && n_launches) *n_launches += nl;

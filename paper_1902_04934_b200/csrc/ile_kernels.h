@@ -91,7 +91,10 @@ struct IleStreamScratch {
     const double *quad_mats;  // packed U, V for ile_launch_quad_mma, or NULL
     cudaEvent_t ev_late;  // if not NULL: the arrays the coefficient kernel reads (phi_ref, psi, incl, dist) arrive with this event
     const double2 *hU, *hV;  // host mirrors of U, V [P][K][M][M] (kernel-parameter path of the coefficient kernel), or NULL
+    double *tabs;        // exp and log tables of the streaming kernel (ile_stream_alloc_tables)
 };
+
+cudaError_t ile_stream_alloc_tables(IleStreamScratch *ss);
 
 bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point, IleStreamPlan *out, IleSortPlan *sp);
 cudaError_t ile_stream_prepare(const IleSizes &sz, IleStreamPlan *pl);  // per context: function attributes + occupancy on its device
