@@ -210,7 +210,7 @@ def run_precompute(args, rank: int):
             "config": {"workload": f"ile_precompute: {P} intrinsic point(s) of BASELINE.json configs[{args.config}]'s shape "
                                    f"({K} detectors, {M} modes, {N}-point spectra)", "l2": "flushed between timed steps (256 MiB write)"},
             "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
-                         "kernel": "ile_overlap_q_radix8_kernel + ile_overlap_uv_small_kernel", "peak_source": src, "algorithmic_bytes": nbytes},
+                         "kernel": "ile_overlap_q_radix8_kernel + ile_overlap_uv_bulk_kernel", "peak_source": src, "algorithmic_bytes": nbytes},
             "gpu_launches": 2 * args.steps, "clocks": sampler.summary()}
     print(json.dumps(line), flush=True)
 

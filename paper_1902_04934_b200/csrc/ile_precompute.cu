@@ -432,6 +432,234 @@ __global__ void __launch_bounds__(PC_UV_THREADS, 1)
     }
 }
 
+// ------------------------------------------------------------------------------------------------------------
+// U, V for few modes (M <= PC_MS) and N >= 512: persistent blocks fed by bulk copies (cp.async.bulk + mbarrier), so the bytes in
+// flight do not depend on registers or occupancy -- round 2a's warp-per-row kernel was bound by the latency of its own loads
+// (1.4 TB/s).  A work unit is (point-detector pk, chunk c): the PC_CH frequency pairs (n, N - n), n = c PC_CH + 1 + t, of all M
+// modes, i.e. per mode one contiguous run x[n ..] and one contiguous run of mirrors x[N - (c + 1) PC_CH ..] -- 2 M bulk copies of 4 KB
+// into one of PC_STG stage buffers.  Thread t owns pair t: both frequencies' terms of U_ab and V_ab, b >= a, are local (U Hermitian, V
+// symmetric by their definitions), 16 FMA per pair (a, b), sums in registers across the chunks of a pk.  n = 0 and n = N / 2 pair
+// with themselves and are added by the threads that flush.  Units are dealt to the blocks in contiguous
+// ranges, so a pk is finished by one block or split between two neighbours: partial sums go to global memory with atomic adds onto
+// zeros (two commuting addends: the result does not depend on their order).
+// ------------------------------------------------------------------------------------------------------------
+#define PC_CH 256
+#define PC_STG 4
+
+__device__ __forceinline__ void pc_mbar_init(uint32_t bar, uint32_t count) { asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count)); }
+__device__ __forceinline__ void pc_mbar_expect(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void pc_mbar_wait(uint32_t bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n.reg .pred p;\nPC_WAIT:\nmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n@p bra PC_DONE;\nbra PC_WAIT;\nPC_DONE:\n}" ::"r"(bar),
+        "r"(parity)
+        : "memory");
+}
+__device__ __forceinline__ void pc_bulk_load(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst), "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+
+// Sums of NV (a power of two <= 32) values over the 32 lanes of a warp by recursive halving: in a round a lane keeps half of its
+// values and sends the other half across (lane ^ w), so 32 values cost 31 shuffles and not 160.  Returns the index of the value whose
+// total ends up in v[0] of this lane (lanes that agree in the bits used hold the same total).
+template <int NV>
+__device__ __forceinline__ int pc_warp_sums(double (&v)[NV], int lane)
+{
+    int idx = 0, bit = 1, cnt = NV;
+#pragma unroll
+    for (int w = 16; w >= 1; w >>= 1) {
+        if (cnt > 1) {
+            const bool up = (lane & w) != 0;
+#pragma unroll
+            for (int i = 0; i < NV / 2; ++i)
+                if (i < cnt / 2) {
+                    const double keep = up ? v[2 * i + 1] : v[2 * i], send = up ? v[2 * i] : v[2 * i + 1];
+                    v[i] = keep + __shfl_xor_sync(0xffffffffu, send, w);
+                }
+            if (up) idx |= bit;
+            bit <<= 1, cnt >>= 1;
+        } else {
+            v[0] += __shfl_xor_sync(0xffffffffu, v[0], w);
+        }
+    }
+    return idx;
+}
+
+// Threads 0 .. PC_CH-1 accumulate U, threads PC_CH .. 2 PC_CH-1 accumulate V of the same PC_CH frequency pairs (half the sums per
+// thread: 16 warps of <= 128 registers per SM instead of 8 warps of 250).
+template <int MM, bool WEIGHTED>
+__global__ void __launch_bounds__(2 * PC_CH, 1)
+    ile_overlap_uv_bulk_kernel(int32_t N, int32_t n_pk, const double2 *__restrict__ x, const PcWeight wt, double *__restrict__ U, double *__restrict__ V)
+{
+    constexpr int NPAIR = MM * (MM + 1) / 2;
+    constexpr int NV = 2 * NPAIR <= 2 ? 2 : 2 * NPAIR <= 8 ? 8 : 2 * NPAIR <= 16 ? 16 : 32;
+    constexpr uint32_t X_BYTES = PC_CH * 16, S_LEFT = (PC_CH + 2) * 8, S_MIRR = PC_CH * 8;
+    constexpr uint32_t DC_OFF = MM * 2 * X_BYTES + (WEIGHTED ? S_LEFT + S_MIRR : 0);  // x_a[0] of the pk, with chunk 0 only
+    constexpr uint32_t STAGE = DC_OFF + 128;
+    extern __shared__ __align__(128) unsigned char pc_raw[];
+    __shared__ __align__(8) uint64_t full[PC_STG];
+    __shared__ double red[2][PC_CH / 32][NV];
+    __shared__ double2 self0[MM], selfN[MM];  // x_a[0], x_a[N / 2] of the pk under way: the two frequencies that are their own mirrors
+    __shared__ double wself[2];               // and their weights
+    const uint32_t sm0 = (uint32_t)__cvta_generic_to_shared(pc_raw), bar0 = (uint32_t)__cvta_generic_to_shared(full);
+    const int half = threadIdx.x / PC_CH, t = threadIdx.x % PC_CH, lane = t & 31, warp = t >> 5;
+    const int nch = (N / 2) / PC_CH;
+    const long long units = (long long)n_pk * nch;
+    const long long u_lo = units * blockIdx.x / gridDim.x, u_hi = units * (blockIdx.x + 1) / gridDim.x;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < PC_STG; ++s) pc_mbar_init(bar0 + 8 * s, 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    auto issue = [&](long long u) {  // thread 0: the copies of unit u into stage (u - u_lo) % PC_STG
+        const int s = (int)((u - u_lo) % PC_STG);
+        const size_t pk = (size_t)(u / nch);
+        const int c = (int)(u % nch);
+        const uint32_t bar = bar0 + 8 * s, dst = sm0 + s * STAGE;
+        pc_mbar_expect(bar, DC_OFF + (c == 0 ? MM * 16 : 0));
+#pragma unroll
+        for (int a = 0; a < MM; ++a) {
+            const double2 *xa = x + (pk * MM + a) * N;
+            if (c == 0) pc_bulk_load(dst + DC_OFF + a * 16, xa, 16, bar);
+            pc_bulk_load(dst + (2 * a) * X_BYTES, xa + c * PC_CH + 1, X_BYTES, bar);
+            pc_bulk_load(dst + (2 * a + 1) * X_BYTES, xa + N - (c + 1) * PC_CH, X_BYTES, bar);
+        }
+        if (WEIGHTED) {
+            const double *Ss = wt.S + pk * N;
+            pc_bulk_load(dst + 2 * MM * X_BYTES, Ss + c * PC_CH, S_LEFT, bar);  // from the even index below n
+            pc_bulk_load(dst + 2 * MM * X_BYTES + S_LEFT, Ss + N - (c + 1) * PC_CH, S_MIRR, bar);
+        }
+    };
+    if (threadIdx.x == 0)
+        for (long long u = u_lo; u < u_hi && u < u_lo + PC_STG; ++u) issue(u);
+
+    bool dc_due = false, ny_due = false;
+    double acc[NV];  // pair p: (re, im) at 2 p, 2 p + 1
+#pragma unroll
+    for (int i = 0; i < NV; ++i) acc[i] = 0.0;
+
+    for (long long u = u_lo; u < u_hi; ++u) {
+        const int s = (int)((u - u_lo) % PC_STG);
+        const size_t pk = (size_t)(u / nch);
+        const int c = (int)(u % nch);
+        pc_mbar_wait(bar0 + 8 * s, (uint32_t)(((u - u_lo) / PC_STG) & 1));
+        const unsigned char *st = pc_raw + (size_t)s * STAGE;
+        const int n = c * PC_CH + 1 + t;  // n = N / 2 (its own mirror) is counted twice here: the flush takes one copy back
+        double wl = 1.0, wm = 1.0;
+        if (WEIGHTED) {
+            const double f = (double)n * wt.df;
+            const bool in = f > wt.fmin && f < wt.fmax;
+            const double *sl = reinterpret_cast<const double *>(st + 2 * MM * X_BYTES);
+            wl = in ? wt.scale / sl[t + 1] : 0.0;
+            wm = in ? wt.scale / sl[PC_CH + 2 + PC_CH - 1 - t] : 0.0;
+        }
+        // left factors of the two terms of a pair: U_ab = conj(x_a[n]) g[n] x_b[n] + conj(x_a[-n]) g[-n] x_b[-n]  (threads of half 0),
+        // V_ab = x_a[-n] g[n] x_b[n] + x_a[n] g[-n] x_b[-n]  (half 1); the right factors x_b[n], x_b[-n] carry the weights
+        double2 X1[MM], X2[MM], L[MM], R[MM];
+#pragma unroll
+        for (int a = 0; a < MM; ++a) {
+            L[a] = reinterpret_cast<const double2 *>(st + (2 * a) * X_BYTES)[t];
+            R[a] = reinterpret_cast<const double2 *>(st + (2 * a + 1) * X_BYTES)[PC_CH - 1 - t];
+            if (c == nch - 1 && threadIdx.x == PC_CH - 1) selfN[a] = L[a];  // n = N / 2: this thread counts it twice, the flush takes one back
+            if (c == 0 && threadIdx.x == 0) self0[a] = reinterpret_cast<const double2 *>(st + DC_OFF)[a];
+            X1[a] = half ? R[a] : make_double2(L[a].x, -L[a].y);
+            X2[a] = half ? L[a] : make_double2(R[a].x, -R[a].y);
+            if (WEIGHTED) L[a].x *= wl, L[a].y *= wl, R[a].x *= wm, R[a].y *= wm;
+        }
+        if (c == nch - 1 && threadIdx.x == PC_CH - 1) wself[1] = wl;
+        if (c == 0 && threadIdx.x == 0) {
+            double w0 = 1.0;
+            if (WEIGHTED) w0 = (0.0 > wt.fmin && 0.0 < wt.fmax) ? wt.scale / reinterpret_cast<const double *>(st + 2 * MM * X_BYTES)[0] : 0.0;
+            wself[0] = w0;
+        }
+        {
+            int p = 0;
+#pragma unroll
+            for (int a = 0; a < MM; ++a)
+#pragma unroll
+                for (int b = a; b < MM; ++b, ++p) {
+                    acc[2 * p] += X1[a].x * L[b].x - X1[a].y * L[b].y + X2[a].x * R[b].x - X2[a].y * R[b].y;
+                    acc[2 * p + 1] += X1[a].x * L[b].y + X1[a].y * L[b].x + X2[a].x * R[b].y + X2[a].y * R[b].x;
+                }
+        }
+        dc_due = dc_due || c == 0;
+        ny_due = ny_due || c == nch - 1;
+        const bool flush = u + 1 == u_hi || (u + 1) % nch == 0;  // the block's last unit, or the pk's
+        __syncthreads();  // every thread has read stage s (an mbarrier per stage that lets the warps drift apart was measured: 64 vs 51 us)
+        if (threadIdx.x == 0 && u + PC_STG < u_hi) issue(u + PC_STG);
+        if (flush) {
+            const int idx = pc_warp_sums<NV>(acc, lane);
+            red[half][warp][idx] = acc[0];  // lanes that hold the same total write the same value
+#pragma unroll
+            for (int i = 0; i < NV; ++i) acc[i] = 0.0;
+            __syncthreads();
+            if (t < NPAIR) {
+                int a = 0, b = t;  // pair index -> (a, b)
+                while (b >= MM - a) b -= MM - a, ++a;
+                b += a;
+                double re = 0.0, im = 0.0;
+#pragma unroll
+                for (int w = 0; w < PC_CH / 32; ++w) re += red[half][w][2 * t], im += red[half][w][2 * t + 1];
+                // the two frequencies that are their own mirrors: + n = 0 (came with chunk 0), - one of the two copies of n = N / 2 that
+                // the last chunk's last thread has added
+#pragma unroll
+                for (int e = 0; e < 2; ++e) {
+                    if (e == 0 ? dc_due : ny_due) {
+                        const double2 xa = e == 0 ? self0[a] : selfN[a], xb = e == 0 ? self0[b] : selfN[b];
+                        const double w0 = e == 0 ? wself[0] : -wself[1];
+                        const double2 xw = make_double2(w0 * xb.x, w0 * xb.y);
+                        if (half == 0) re += xa.x * xw.x + xa.y * xw.y, im += xa.x * xw.y - xa.y * xw.x;
+                        else re += xa.x * xw.x - xa.y * xw.y, im += xa.x * xw.y + xa.y * xw.x;
+                    }
+                }
+                double *Mk = (half == 0 ? U : V) + 2 * pk * MM * MM;
+                const double ims = half == 0 ? -im : im;  // U_ba = conj(U_ab), V_ba = V_ab; the diagonal of U is real
+                atomicAdd(Mk + 2 * (a * MM + b), re);
+                if (a != b || half == 1) atomicAdd(Mk + 2 * (a * MM + b) + 1, im);
+                if (a != b) atomicAdd(Mk + 2 * (b * MM + a), re), atomicAdd(Mk + 2 * (b * MM + a) + 1, ims);
+            }
+            __syncthreads();  // red is free again
+            dc_due = ny_due = false;
+        }
+    }
+}
+
+__global__ void __launch_bounds__(256) ile_overlap_zero_kernel(double2 *__restrict__ U, double2 *__restrict__ V, long long n)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x)
+        U[i] = make_double2(0.0, 0.0), V[i] = make_double2(0.0, 0.0);
+}
+
+template <int MM>
+static cudaError_t pc_launch_uv_bulk(int32_t N, int32_t n_pk, const double2 *x, const PcWeight &wt, double2 *U, double2 *V, int sm_count,
+                                     cudaStream_t st)
+{
+    const long long n_uv = (long long)n_pk * MM * MM;
+    ile_overlap_zero_kernel<<<(unsigned)((n_uv + 255) / 256 < 1024 ? (n_uv + 255) / 256 : 1024), 256, 0, st>>>(U, V, n_uv);
+    cudaError_t e = cudaGetLastError();
+    if (e != cudaSuccess) return e;
+    const long long units = (long long)n_pk * ((N / 2) / PC_CH);
+    const unsigned grid = (unsigned)(units < sm_count ? units : sm_count);
+    if (wt.S) {
+        const size_t smem = (size_t)PC_STG * (MM * 2 * PC_CH * 16 + (PC_CH + 2) * 8 + PC_CH * 8 + 128);
+        e = cudaFuncSetAttribute(ile_overlap_uv_bulk_kernel<MM, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        ile_overlap_uv_bulk_kernel<MM, true><<<grid, 2 * PC_CH, smem, st>>>(N, n_pk, x, wt, (double *)U, (double *)V);
+    } else {
+        const size_t smem = (size_t)PC_STG * (MM * 2 * PC_CH * 16 + 128);
+        e = cudaFuncSetAttribute(ile_overlap_uv_bulk_kernel<MM, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+        ile_overlap_uv_bulk_kernel<MM, false><<<grid, 2 * PC_CH, smem, st>>>(N, n_pk, x, wt, (double *)U, (double *)V);
+    }
+    return cudaGetLastError();
+}
+
 cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_t N, double fs_hz, double t0_q_s, const double2 *x,
                                   const double2 *d, const double *S, double f_min_hz, double f_max_hz, double scale, double2 *Q, double2 *U,
                                   double2 *V, int32_t max_smem_optin, cudaStream_t st)
@@ -512,6 +740,18 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
         ile_overlap_q_stockham_kernel<0><<<n_series, PC_THREADS, smem, st>>>(M, N, log2n, tab, x, d, Q);
     }
     const unsigned n_pk = (unsigned)(n_points * K);
+    if (M <= PC_MS && N >= 2 * PC_CH && ((uintptr_t)S & 15) == 0) {  // bulk copies need 16-byte aligned sources (x is double2)
+        int sms = 0;
+        e = cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return e;
+        switch (M) {
+            case 1: return pc_launch_uv_bulk<1>(N, (int32_t)n_pk, x, wt, U, V, sms, st);
+            case 2: return pc_launch_uv_bulk<2>(N, (int32_t)n_pk, x, wt, U, V, sms, st);
+            case 3: return pc_launch_uv_bulk<3>(N, (int32_t)n_pk, x, wt, U, V, sms, st);
+            case 4: return pc_launch_uv_bulk<4>(N, (int32_t)n_pk, x, wt, U, V, sms, st);
+            default: return pc_launch_uv_bulk<5>(N, (int32_t)n_pk, x, wt, U, V, sms, st);
+        }
+    }
     if (M <= PC_MS && S) ile_overlap_uv_small_kernel<true><<<n_pk, PC_UV_THREADS, 0, st>>>(M, N, x, wt, U, V);
     else if (M <= PC_MS) ile_overlap_uv_small_kernel<false><<<n_pk, PC_UV_THREADS, 0, st>>>(M, N, x, wt, U, V);
     else ile_overlap_uv_kernel<<<n_pk, PC_THREADS, smem_uv, st>>>(M, N, nsplit, x, wt, U, V);
