@@ -451,6 +451,17 @@ def test_evidence_merge_of_split_batch_equals_whole(gpu_lib):
     ctx.close()
 
 
+def test_streaming_kernel_extreme_amplitudes(gpu_lib):
+    """The streaming kernel's fixed-point exp keeps lin / ln 2 - reference in a 2^19-step window around a running reference of a
+    whole number of octaves: samples whose linear term runs to 1e3 ... 1e8 (sources at 1 kpc ... 30 Mpc, a = D_ref / D up to 1e5, where
+    quad ~ a^2 dwarfs everything) or to 1e-7 (D = 1e9 Mpc) must come out like the oracle's within TOL of |lnL|, next to ordinary ones."""
+    cfg = gi.make_config(1, n=20_000)
+    s = gi.make_samples(cfg["sample_seeds"][0], cfg["n"])
+    m = len(s["dist_mpc"][::7])
+    s["dist_mpc"][::7] = np.tile(np.array([1e-3, 5e-2, 1.0, 3.0, 10.0, 30.0, 1e9]), m // 7 + 1)[:m]
+    full_compare(gpu_lib, cfg, s, variant=4)
+
+
 @pytest.mark.parametrize("variant", [1, 2, 4])
 def test_every_variant_matches_the_oracle(gpu_lib, variant):
     """ile_set_variant: each evaluation kernel family on the same 20,000 samples of config 1 (indices bit-exact, values
