@@ -32,8 +32,9 @@ struct ile_ctx {
     size_t sc_samples, sc_hist;  // capacities (samples, histogram words)
     int32_t sc_recg;             // doubles per record the scratch was sized for
     bool stream_ok;
-    IleStreamPlan spl;
-    IleSortPlan ssp;
+    IleStreamPlan spl, spl1;  // sort cells of 16 rows (nc = 2) and of 8 rows (nc = 1, big batches)
+    IleSortPlan ssp, ssp1;
+    bool nc1_ok;
     double *dQs;
     IleStreamScratch ss;
     size_t ss_slots, ss_gcum;  // capacities in words
@@ -201,9 +202,11 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     }
     CKC(cudaMemcpy(c->hU, c->dU, nU * sizeof(double2), cudaMemcpyDeviceToHost));
     CKC(cudaMemcpy(c->hV, c->dV, nU * sizeof(double2), cudaMemcpyDeviceToHost));
-    c->stream_ok = !c->sz.interp && ile_stream_plan(c->sz, c->hparams, 0, &c->spl, &c->ssp);
+    c->stream_ok = !c->sz.interp && ile_stream_plan(c->sz, c->hparams, 2, &c->spl, &c->ssp);
+    c->nc1_ok = c->stream_ok && ile_stream_plan(c->sz, c->hparams, 1, &c->spl1, &c->ssp1);
     if (c->stream_ok) {
         CKC(ile_stream_prepare(c->sz, &c->spl));
+        if (c->nc1_ok) CKC(ile_stream_prepare(c->sz, &c->spl1));
         CKC(ile_stream_alloc_tables(&c->ss));
         if (cfg->n_modes >= ILE_QUAD_MMA_MIN_MODES) {
             const size_t nd = ile_quad_pack_doubles(cfg->n_points, cfg->n_det, cfg->n_modes);
@@ -304,7 +307,8 @@ static int ensure_scratch(ile_ctx *c, size_t samples, size_t hist_words, cudaStr
 // variant 4 for one launch group: setup + sort into padded segments + streaming kernel
 static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
 {
-    const IleSortPlan &sp = c->ssp;
+    const bool nc1 = c->nc1_ok && a.n_per_point >= (int64_t)ILE_STREAM_NC1_MIN_PER_SEGMENT * c->ssp1.nseg;
+    const IleSortPlan &sp = nc1 ? c->ssp1 : c->ssp;
     const size_t nseg = (size_t)sp.nseg;
     const int64_t slot_cap = (((a.n_per_point + 7) & ~(int64_t)7) + 8 * (int64_t)nseg + 31) & ~(int64_t)31;  // groups per point: multiple of 4
     int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * (sp.ncell + nseg) + ILE_STREAM_MAX_RANGES, st);
@@ -343,7 +347,7 @@ static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
     c->sc.qform = quad_mma ? c->d_qform : nullptr;
     c->ss.quad_mats = quad_mma ? c->d_quad_mats : nullptr;
     int nl = 0;
-    cudaError_t e = ile_launch_eval_stream(c->sz, c->hparams, a, c->spl, sp, c->sc, c->ss, st, &nl);
+    cudaError_t e = ile_launch_eval_stream(c->sz, c->hparams, a, nc1 ? c->spl1 : c->spl, sp, c->sc, c->ss, st, &nl);
     c->launches += nl;
     if (e != cudaSuccess) return cuda_fail(e);
     return ILE_OK;

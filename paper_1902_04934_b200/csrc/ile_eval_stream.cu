@@ -48,9 +48,6 @@
 #ifndef ST_MINB3
 #define ST_MINB3 3
 #endif
-#ifndef ST_NC
-#define ST_NC 2 /* (d1, d2) cells are 8 ST_NC rows wide */
-#endif
 #ifndef ST_PIPE_MAXKS
 #define ST_PIPE_MAXKS 4
 #endif
@@ -83,12 +80,8 @@ __device__ __forceinline__ void st_dmma(double &c0, double &c1, double a, double
 #define ST_A0 0x1.ffd3a5661bac7p-1
 #define ST_A1 0x1.62c56e9ca3a21p-12
 #define ST_A2 0x1.ec1130cd9fbd5p-25
-#elif ST_TAB_LOG2 == 10
-#define ST_A0 0x1.ffa74ea4e1a54p-1  /* error 1.6e-12 */
-#define ST_A1 0x1.62a6aa1f75becp-11
-#define ST_A2 0x1.ec2682c0c27c1p-23
 #else
-#error "ST_TAB_LOG2: 10 or 11"
+#error "ST_TAB_LOG2: 11 (the minimax coefficients below belong to the 2048-entry table)"
 #endif
 #define ST_MG_UNSET (ST_MAGIC + 1073741824.0 * ST_TAB) /* reference at -2^30 octaves: the first valid element takes the rare path */
 
@@ -760,14 +753,14 @@ static int st_round_ks(int ks)
 
 // Plan for one launch of n_per_point samples per point: cell widths and the padded Q geometry.  Returns false when the
 // sizes do not fit this variant (more than 3 detectors, too many cells).
-bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point, IleStreamPlan *out, IleSortPlan *spo)
+bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, int nc, IleStreamPlan *out, IleSortPlan *spo)
 {
     if (sz.n_det > 4) return false;  // a lane looks after one (sample, detector) pair of its group: 8 samples x 4 detectors
     IleStreamPlan pl;
     pl.ks = st_round_ks((2 * sz.n_modes + 3) / 4);
     if (!pl.ks) return false;
     pl.cp = 4 * pl.ks;
-    pl.nc = ST_NC;
+    pl.nc = nc;
     pl.padf = (sz.n_q - sz.n_t + 32 + 7) & ~7;                               // multiples of the 8-row blocking
     pl.nqp = (pl.padf + sz.n_q + (sz.n_q - sz.n_t) + 64 + 7) & ~7;
     IleSortPlan sp;
@@ -799,7 +792,6 @@ bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per
         if (g0 >= 30) return false;
     }
     sp.g0 = g0;
-    (void)n_per_point;
     *out = pl;
     *spo = sp;
     return true;
@@ -841,19 +833,25 @@ static cudaError_t st_launch_k(const IleSizes &sz, int ks, const IleStreamKArgs 
     }
 }
 
-static cudaError_t st_launch(const IleSizes &sz, int ks, const IleStreamKArgs *ka, long long mg, int *per_sm, cudaStream_t st)
+static cudaError_t st_launch(const IleSizes &sz, int ks, int nc, const IleStreamKArgs *ka, long long mg, int *per_sm, cudaStream_t st)
 {
-    if (sz.n_det == 1) return st_launch_k<1, ST_NC>(sz, ks, ka, mg, per_sm, st);
-    if (sz.n_det == 2) return st_launch_k<2, ST_NC>(sz, ks, ka, mg, per_sm, st);
-    if (sz.n_det == 3) return st_launch_k<3, ST_NC>(sz, ks, ka, mg, per_sm, st);
-    return st_launch_k<4, ST_NC>(sz, ks, ka, mg, per_sm, st);
+    if (nc == 1) {
+        if (sz.n_det == 1) return st_launch_k<1, 1>(sz, ks, ka, mg, per_sm, st);
+        if (sz.n_det == 2) return st_launch_k<2, 1>(sz, ks, ka, mg, per_sm, st);
+        if (sz.n_det == 3) return st_launch_k<3, 1>(sz, ks, ka, mg, per_sm, st);
+        return st_launch_k<4, 1>(sz, ks, ka, mg, per_sm, st);
+    }
+    if (sz.n_det == 1) return st_launch_k<1, 2>(sz, ks, ka, mg, per_sm, st);
+    if (sz.n_det == 2) return st_launch_k<2, 2>(sz, ks, ka, mg, per_sm, st);
+    if (sz.n_det == 3) return st_launch_k<3, 2>(sz, ks, ka, mg, per_sm, st);
+    return st_launch_k<4, 2>(sz, ks, ka, mg, per_sm, st);
 }
 
 // Once per context, on the context's device: carve-out and occupancy of the streaming kernel this context's sizes select.
 cudaError_t ile_stream_prepare(const IleSizes &sz, IleStreamPlan *pl)
 {
     int per_sm = 0;
-    cudaError_t e = st_launch(sz, pl->ks, nullptr, 0, &per_sm, 0);
+    cudaError_t e = st_launch(sz, pl->ks, pl->nc, nullptr, 0, &per_sm, 0);
     pl->ctas_per_sm = per_sm;
     return e;
 }
@@ -939,7 +937,7 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     // that one global counter
     const int nr_sm = sz.sm_count < ILE_STREAM_MAX_RANGES ? sz.sm_count : ILE_STREAM_MAX_RANGES;
     ka.n_ranges = max_groups < 4LL * nr_sm ? 1 : nr_sm;
-    e = st_launch(sz, pl.ks, &ka, max_groups, &per_sm, st);
+    e = st_launch(sz, pl.ks, pl.nc, &ka, max_groups, &per_sm, st);
     ++nl;
     if (e == cudaSuccess && n_launches) *n_launches += nl;
     return e;

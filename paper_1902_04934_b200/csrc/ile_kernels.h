@@ -96,7 +96,11 @@ struct IleStreamScratch {
 
 cudaError_t ile_stream_alloc_tables(IleStreamScratch *ss);
 
-bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, long long n_per_point, IleStreamPlan *out, IleSortPlan *sp);
+// nc = 1, 2: (d1, d2) sort cells of 8 nc rows -- narrow cells need one select per realigned element instead of two but four times the
+// segments (padding and shorter runs of equal rows); measured: nc = 1 wins by 2-6 % once a segment holds a thousand samples or more
+// (three detectors: 280 segments, 1e6 samples; two: 21 segments, 1e5), nc = 2 below (6 % at 30,000 samples, three detectors)
+bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, int nc, IleStreamPlan *out, IleSortPlan *sp);
+#define ILE_STREAM_NC1_MIN_PER_SEGMENT 1024
 cudaError_t ile_stream_prepare(const IleSizes &sz, IleStreamPlan *pl);  // per context: function attributes + occupancy on its device
 cudaError_t ile_launch_pack_q_stream(const IleSizes &sz, const IleStreamPlan &pl, int32_t n_points, const double2 *Q,
                                      double *Qs, cudaStream_t st);
