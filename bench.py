@@ -36,11 +36,11 @@ EXP_DFMA = 20.0      # "Total DFMA-equivalents with exp ~ 20" 
 NOMINAL_FP64_TFLOPS = 37.2  # 148 SMs x 64 FP64 lanes x 2 flop x 1.965 GHz
 
 
-def dfma_per_sample(K: int, M: int, n_t: int, exp_cost: float = EXP_DFMA) -> float:
+def dfma_per_sample(K: int, M: int, n_t: int, exp_cost: float = EXP_DFMA, interp: bool = False) -> float:
     """config 1 -> 12,300 + 720 + 8,200 + 400 = 21,620 DFMA-equivalents per sample.
     `exp_cost` = FP64-pipe instructions per time bin of step 6: 20 is the survey's convention; the kernel's own count
     (from the committed ncu SASS mix) gives the "measured exp" accounting of SURVEY.md §8(d)."""
-    linear = 2.0 * K * M * n_t                      # step 5: Re sum conj(A) Q, 2 DFMA per complex element
+    linear = 2.0 * K * M * n_t * (2 if interp else 1)  # step 5: Re sum conj(A) Q, 2 DFMA per complex element (two rows when interpolating)
     quad = 2.0 * K * (4.0 * M * M + 4.0 * M)        # step 4: Y^dagger U Y and Y^T V Y per detector
     lse = n_t * exp_cost                            # step 6
     geom = 250.0 + 30.0 * M                         # steps 1-3: five sincos, F_k, dt_k, Y_lm, K*M coefficient products
@@ -320,6 +320,8 @@ def main():
     ap.add_argument("--variant", type=int, default=0)
     ap.add_argument("--points", type=int, default=1, help="intrinsic points evaluated concurrently per step (config 4: 256), ile_eval_all")
     ap.add_argument("--samples", default="prior", choices=["prior", "concentrated"])
+    ap.add_argument("--shift-mode", type=int, default=0, choices=[0, 1],
+                    help="1: linear interpolation of Q between samples (NEXT-4, reading R8'); hot-path stage only, no cpu_baseline leg")
     ap.add_argument("--ref-samples-per-step", type=int, default=100_000)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--stage", default="hotpath", choices=["hotpath", "precompute", "integrate"],
@@ -365,6 +367,9 @@ def main():
     # ---- workload: one intrinsic point and one batch per rank (independent workers)
     P = max(1, args.points)
     base = gi.make_config(args.config, n_points=P)
+    if args.shift_mode:
+        base["shift_mode"] = 1
+        args.no_cpu_baseline = True
     n = args.n if args.n is not None else base["n"]
     if rank > 0:  # a different seeded intrinsic point per rank, same recipe
         c = gi.CONFIGS[args.config]
@@ -458,7 +463,7 @@ def main():
 
     if rank == 0:
         K, M, n_t = base["n_det"], base["n_modes"], base["n_t"]
-        w = dfma_per_sample(K, M, n_t)
+        w = dfma_per_sample(K, M, n_t, interp=bool(args.shift_mode))
         value = world * P * n * args.steps / (step_ms * 1e-3)
         eval_avg_ms = eval_ms / args.steps
         achieved = 2.0 * w * P * n / (eval_avg_ms * 1e-3) * 1e-12
@@ -469,13 +474,13 @@ def main():
         exp_meas = frac_meas = frac_pipe = None
         if sc_:
             exp_meas = sc_["fp64_other_inst"] * 32.0 / (sc_["samples"] * sc_["n_t"])
-            frac_meas = 2.0 * dfma_per_sample(K, M, n_t, exp_meas) * P * n / (eval_avg_ms * 1e-3) * 1e-12 / peak_tflops
+            frac_meas = 2.0 * dfma_per_sample(K, M, n_t, exp_meas, bool(args.shift_mode)) * P * n / (eval_avg_ms * 1e-3) * 1e-12 / peak_tflops
             frac_pipe = (16.0 * sc_["dmma_inst"] + 2.0 * sc_["fp64_other_inst"]) / (sc_["cycles_elapsed_max"] * 4.0 * 148.0)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": step_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": workload_config(base, n, args, extra={"variant": args.variant, "samples": args.samples}),
+            "config": workload_config(base, n, args, extra={"variant": args.variant, "samples": args.samples, "shift_mode": args.shift_mode}),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
                          "traffic": int(sc_["dram_bytes_read"] + sc_["dram_bytes_write"]) if sc_ else None,
                          "kernel": "ile_eval (steps 1-6)", "kernel_ms": eval_avg_ms, "dfma_equiv_per_sample": w,

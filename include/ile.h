@@ -78,7 +78,8 @@ typedef struct {
     int32_t shift_mode; /* 0: nearest-sample window shifts (reading R8, the hot path); 1: linear interpolation between the two
                            neighbouring samples of every detector's Q (NEXT-4, reading R8'): i0_k = floor(x_k) - floor(N_t/2),
                            lnL_j uses (1 - phi_k) Q[i0_k + j] + phi_k Q[i0_k + j + 1], phi_k = x_k - floor(x_k); the window then
-                           needs i0_k + N_t + 1 <= N_Q; evaluated by the direct kernel (variant 1) only */
+                           needs i0_k + N_t + 1 <= N_Q; evaluated by the direct kernel (variant 1) and, with
+                           twice the channels (Q[i] weighted 1 - phi, Q[i + 1] weighted phi), by the streaming kernel (variant 4) */
 } ile_config;
 
 /* Create a context on the current CUDA device: validates cfg, copies Q, U, V (host or device pointers) to the

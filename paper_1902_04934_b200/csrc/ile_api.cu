@@ -202,7 +202,7 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     }
     CKC(cudaMemcpy(c->hU, c->dU, nU * sizeof(double2), cudaMemcpyDeviceToHost));
     CKC(cudaMemcpy(c->hV, c->dV, nU * sizeof(double2), cudaMemcpyDeviceToHost));
-    c->stream_ok = !c->sz.interp && ile_stream_plan(c->sz, c->hparams, 2, &c->spl, &c->ssp);
+    c->stream_ok = ile_stream_plan(c->sz, c->hparams, 2, &c->spl, &c->ssp);
     c->nc1_ok = c->stream_ok && ile_stream_plan(c->sz, c->hparams, 1, &c->spl1, &c->ssp1);
     if (c->stream_ok) {
         CKC(ile_stream_prepare(c->sz, &c->spl));
@@ -667,7 +667,7 @@ extern "C" int ile_set_variant(ile_ctx *c, int32_t variant)
     if (variant > 4) return ILE_ERR_UNSUPPORTED;
     if (variant == 3) return ILE_ERR_UNSUPPORTED;  // retired (superseded by variant 4)
     if (variant == 4 && !c->stream_ok) return ILE_ERR_UNSUPPORTED;
-    if (c->sz.interp && variant > 1) return ILE_ERR_UNSUPPORTED;  // interpolated shifts: direct kernel only
+    if (c->sz.interp && (variant == 2 || variant == 3)) return ILE_ERR_UNSUPPORTED;  // interpolated shifts: direct and streaming kernels
     if (variant == 2) {
         IleTiledLayout L;
         if (!ile_tiled_plan(c->sz, 1LL << 40, &L)) return ILE_ERR_UNSUPPORTED;

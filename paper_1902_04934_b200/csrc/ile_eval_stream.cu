@@ -542,7 +542,8 @@ cudaError_t ile_stream_alloc_tables(IleStreamScratch *ss)
 // Q repacking (once per context): Q [P][K][M][n_q] complex128 -> Qs [P][K][nqp / 8][ks][8][4] doubles, channel 2m = Re, 2m+1 = Im
 // ------------------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256) ile_pack_q_stream_kernel(int32_t n_series, int32_t M, int32_t n_q, int32_t ks, int32_t nqp,
-                                                                int32_t padf, const double2 *__restrict__ Q, double *__restrict__ Qs)
+                                                                int32_t padf, int32_t interp, const double2 *__restrict__ Q,
+                                                                double *__restrict__ Qs)
 {
     const long long total = (long long)n_series * ks * nqp * 4;
     for (long long o = (long long)blockIdx.x * blockDim.x + threadIdx.x; o < total; o += (long long)gridDim.x * blockDim.x) {
@@ -553,7 +554,11 @@ __global__ void __launch_bounds__(256) ile_pack_q_stream_kernel(int32_t n_series
         q /= ks;
         const int blk = (int)(q % (nqp >> 3));
         q /= (nqp >> 3);  // = p * K + k
-        const int ch = 4 * s + c4, m = ch >> 1, i = blk * 8 + rr - padf;
+        // interpolated shifts (reading R8'): channels [2M, 4M) are the series one sample later, so that
+        // (1 - phi) Q[i] + phi Q[i + 1] is ONE contraction over 4M channels with coefficients (1 - phi) A and phi A
+        int ch = 4 * s + c4, i = blk * 8 + rr - padf;
+        if (interp && ch >= 2 * M) ch -= 2 * M, ++i;  // (channels from 4M on stay beyond the modes: zero)
+        const int m = ch >> 1;
         double v = 0.0;
         if (m < M && i >= 0 && i < n_q) {
             const double2 z = Q[((size_t)q * M + m) * n_q + i];
@@ -569,7 +574,7 @@ cudaError_t ile_launch_pack_q_stream(const IleSizes &sz, const IleStreamPlan &pl
     const long long total = (long long)n_points * sz.n_det * pl.ks * pl.nqp * 4;
     long long blocks = (total + 255) / 256;
     if (blocks > (long long)sz.sm_count * 32) blocks = (long long)sz.sm_count * 32;
-    ile_pack_q_stream_kernel<<<(unsigned)blocks, 256, 0, st>>>(n_points * sz.n_det, sz.n_modes, sz.n_q, pl.ks, pl.nqp, pl.padf, Q, Qs);
+    ile_pack_q_stream_kernel<<<(unsigned)blocks, 256, 0, st>>>(n_points * sz.n_det, sz.n_modes, sz.n_q, pl.ks, pl.nqp, pl.padf, sz.interp, Q, Qs);
     return cudaGetLastError();
 }
 
@@ -600,9 +605,11 @@ __global__ void __launch_bounds__(IX_THREADS)
         int bad = 0;
         int32_t i0[4] = {0, 0, 0, 0};
         for (int k = 0; k < K; ++k) {
-            const int32_t idx = ile_window_index(P.vertex[k], dir, t_ref, P.t0_q, P.fs, P.n_t);
+            double phi;
+            const int32_t idx = P.interp ? ile_window_floor(P.vertex[k], dir, t_ref, P.t0_q, P.fs, P.n_t, &phi)
+                                         : ile_window_index(P.vertex[k], dir, t_ref, P.t0_q, P.fs, P.n_t);
             if (k < 4) i0[k] = idx;
-            if (idx < 0 || (long long)idx + P.n_t > P.n_q) bad = 1;
+            if (idx < 0 || (long long)idx + P.n_t + (P.interp ? 1 : 0) > P.n_q) bad = 1;  // interpolation reads one sample more
             i0_out[s * K + k] = idx;
             if (a.shift_idx) a.shift_idx[s * K + k] = idx;
         }
@@ -745,7 +752,7 @@ __global__ void __launch_bounds__(IX_THREADS)
 // ------------------------------------------------------------------------------------------------------------
 static int st_round_ks(int ks)
 {
-    const int avail[] = {1, 2, 3, 4, 6, 8, 11, 16};
+    const int avail[] = {1, 2, 3, 4, 5, 6, 8, 11, 16};
     for (int v : avail)
         if (ks <= v) return v;
     return 0;
@@ -757,7 +764,7 @@ bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, int nc, IleStre
 {
     if (sz.n_det > 4) return false;  // a lane looks after one (sample, detector) pair of its group: 8 samples x 4 detectors
     IleStreamPlan pl;
-    pl.ks = st_round_ks((2 * sz.n_modes + 3) / 4);
+    pl.ks = st_round_ks(((sz.interp ? 4 : 2) * sz.n_modes + 3) / 4);  // interpolated shifts: twice the channels
     if (!pl.ks) return false;
     pl.cp = 4 * pl.ks;
     pl.nc = nc;
@@ -825,6 +832,7 @@ static cudaError_t st_launch_k(const IleSizes &sz, int ks, const IleStreamKArgs 
         case 2: return st_launch_t<K, 2, NC, 4>(sz, ka, mg, per_sm, st);
         case 3: return st_launch_t<K, 3, NC, ST_MINB3>(sz, ka, mg, per_sm, st);
         case 4: return st_launch_t<K, 4, NC, 3>(sz, ka, mg, per_sm, st);
+        case 5: return st_launch_t<K, 5, NC, 2>(sz, ka, mg, per_sm, st);
         case 6: return st_launch_t<K, 6, NC, 2>(sz, ka, mg, per_sm, st);
         case 8: return st_launch_t<K, 8, NC, 2>(sz, ka, mg, per_sm, st);
         case 11: return st_launch_t<K, 11, NC, 2>(sz, ka, mg, per_sm, st);

@@ -21,7 +21,7 @@ struct IleEvalArgs {
 // Host copy of the sizes every launcher needs.
 struct IleSizes {
     int32_t n_det, n_modes, n_q, n_t;
-    int32_t interp;          // 1: linear interpolation of Q between samples (direct kernel only)
+    int32_t interp;          // 1: linear interpolation of Q between samples (direct kernel; streaming kernel with doubled channels)
     int32_t sm_count;
     int32_t max_smem_optin;  // largest dynamic shared memory one block may ask for
     int32_t smem_per_sm;     // shared memory of one SM

@@ -116,10 +116,24 @@ __device__ __forceinline__ void ile_setup_one(const IleDevParams &P, const IleEv
 
         const double2 aF = make_double2(amp_a * F.x, amp_a * F.y);
         double2 *__restrict__ rk = reinterpret_cast<double2 *>(rec + (size_t)k * cp);
+        if (P.interp) {  // reading R8': channels [0, 2M) weigh Q[i] by 1 - phi_k, channels [2M, 4M) weigh Q[i + 1] by phi_k
+            double phi;
+            ile_window_floor(P.vertex[k], g.s, a.t_ref[s], P.t0_q, P.fs, P.n_t, &phi);
+            const double om = 1.0 - phi;
 #pragma unroll
-        for (int m = 0; m < MMAX; ++m)
-            if (m < M) rk[m] = ile_cmul(aF, Y[m]);
-        for (int m = M; m < cp / 2; ++m) rk[m] = make_double2(0.0, 0.0);
+            for (int m = 0; m < MMAX; ++m)
+                if (m < M) {
+                    const double2 c = ile_cmul(aF, Y[m]);
+                    rk[m] = make_double2(om * c.x, om * c.y);
+                    rk[M + m] = make_double2(phi * c.x, phi * c.y);
+                }
+            for (int m = 2 * M; m < cp / 2; ++m) rk[m] = make_double2(0.0, 0.0);
+        } else {
+#pragma unroll
+            for (int m = 0; m < MMAX; ++m)
+                if (m < M) rk[m] = ile_cmul(aF, Y[m]);
+            for (int m = M; m < cp / 2; ++m) rk[m] = make_double2(0.0, 0.0);
+        }
     };
     if constexpr (UVP) {
         detector(0, std::integral_constant<int, 0>());

@@ -584,5 +584,33 @@ def test_linear_interpolated_shifts_match_the_oracle(gpu_lib, cid, n):
     assert_indices_equal(cfg, s, ref_idx, idx.cpu().numpy())
     assert rel_err(ref, lnL.cpu().numpy()) <= TOL
     with pytest.raises(gpu_lib.IleError):
+        ctx.set_variant(2)
+    ctx.close()
+
+
+@pytest.mark.parametrize("cid,n", [(1, 20_011), (5, 12_000), (6, 3_000), (0, 2_500)])
+def test_linear_interpolated_shifts_streaming_kernel(gpu_lib, cid, n):
+    """shift_mode = 1 through the streaming FP64-MMA kernel: the packed Q carries every series twice (row i and row i + 1), the
+    coefficient records (1 - phi_k) a F_k Y_lm and phi_k a F_k Y_lm, and the contraction is the nearest-sample one over 4M channels.
+    Automatic choice from 10,000 samples, variant 4 forced below; floor indices bit-exact, values within TOL, evidence included."""
+    from oracle import subsample as osub
+
+    cfg = gi.make_config(cid, n=n)
+    cfg["shift_mode"] = 1
+    s = gi.make_samples(cfg["sample_seeds"][0] + 11, n)
+    s["t_ref"][5] = 0.9
+    s["t_ref"][6] = -0.9
+    ctx = gpu_lib.Context(cfg)
+    if n < 10_000:
         ctx.set_variant(4)
+    lnL, idx = ctx.eval(to_dev(s))
+    n_bad, _ = ctx.status()
+    ref, ref_idx, ref_bad = osub.eval_batch_lin(cfg, s)
+    assert n_bad == ref_bad >= 2
+    assert_indices_equal(cfg, s, ref_idx, idx.cpu().numpy())
+    assert rel_err(ref, lnL.cpu().numpy()) <= TOL
+    assert ctx.launch_count >= 5  # index, scan, scatter, coefficient, streaming kernels
+    lnZ, neff = ctx.evidence(lnL)
+    rZ, rN = oracle.evidence(ref)
+    assert rel_err([rZ], lnZ.cpu().numpy()) <= TOL and rel_err([rN], neff.cpu().numpy()) <= TOL
     ctx.close()
