@@ -759,7 +759,7 @@ static int st_round_ks(int ks)
 }
 
 // Plan for one launch of n_per_point samples per point: cell widths and the padded Q geometry.  Returns false when the
-// sizes do not fit this variant (more than 3 detectors, too many cells).
+// sizes do not fit this variant (more than 4 detectors, too many cells).
 bool ile_stream_plan(const IleSizes &sz, const IleDevParams &hp, int nc, IleStreamPlan *out, IleSortPlan *spo)
 {
     if (sz.n_det > 4) return false;  // a lane looks after one (sample, detector) pair of its group: 8 samples x 4 detectors
