@@ -202,12 +202,12 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     }
     CKC(cudaMemcpy(c->hU, c->dU, nU * sizeof(double2), cudaMemcpyDeviceToHost));
     CKC(cudaMemcpy(c->hV, c->dV, nU * sizeof(double2), cudaMemcpyDeviceToHost));
+    CKC(ile_stream_alloc_tables(&c->ss));  // exp / log tables of the streaming and tiled kernels
     c->stream_ok = ile_stream_plan(c->sz, c->hparams, 2, &c->spl, &c->ssp);
     c->nc1_ok = c->stream_ok && ile_stream_plan(c->sz, c->hparams, 1, &c->spl1, &c->ssp1);
     if (c->stream_ok) {
         CKC(ile_stream_prepare(c->sz, &c->spl));
         if (c->nc1_ok) CKC(ile_stream_prepare(c->sz, &c->spl1));
-        CKC(ile_stream_alloc_tables(&c->ss));
         if (cfg->n_modes >= ILE_QUAD_MMA_MIN_MODES) {
             const size_t nd = ile_quad_pack_doubles(cfg->n_points, cfg->n_det, cfg->n_modes);
             double *hm = new (std::nothrow) double[nd];
@@ -369,6 +369,7 @@ static int eval_dispatch(ile_ctx *c, int32_t point0, int32_t n_points, int64_t n
     a.lnL = lnL;
     a.shift_idx = shift_idx;
     a.oob_counter = c->d_oob;
+    a.exp_tab = c->ss.tabs;
     const bool use_stream = c->variant == 4 || (c->variant == 0 && c->stream_ok && n >= ILE_STREAM_MIN_SAMPLES);
     if (use_stream) {
         // launch groups of at most chunk_samples samples: whole points while they fit, else slices of one point
@@ -640,7 +641,7 @@ extern "C" int ile_harvest(ile_ctx *c, int32_t point, int64_t n, const double *r
     a.Q = c->dQ, a.U = c->dU, a.V = c->dV;
     a.point0 = point, a.n_points = 1, a.n_per_point = n;
     a.ra = ra, a.dec = dec, a.t_ref = t_ref, a.phi_ref = phi_ref, a.psi = psi, a.incl = incl, a.dist = dist_mpc;
-    a.lnL = nullptr, a.shift_idx = nullptr, a.oob_counter = c->d_oob;
+    a.lnL = nullptr, a.shift_idx = nullptr, a.oob_counter = c->d_oob, a.exp_tab = c->ss.tabs;
     cudaError_t e = ile_launch_harvest(c->sz, a, n_sel, reinterpret_cast<const long long *>(ids), v_uniform, argmax_bin, lnL_max, drawn_bin,
                                        (cudaStream_t)cuda_stream);
     c->launches += 1;

@@ -38,10 +38,6 @@
 #include "ile_kernels.h"
 
 #define ST_FULL 0xffffffffu
-#ifndef ST_TAB_LOG2
-#define ST_TAB_LOG2 11
-#endif
-#define ST_TAB (1 << ST_TAB_LOG2)
 #ifndef ST_THREADS
 #define ST_THREADS 128
 #endif
@@ -57,32 +53,7 @@ __device__ __forceinline__ void st_dmma(double &c0, double &c1, double a, double
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};" : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-// ---- exp for the time marginalisation (eq. 9), in fixed point.  For an element x and a column reference of n octaves
-//   t = fma(x, ST_C1, mg),  mg = ST_MAGIC - n * ST_TAB,  ST_C1 = ST_TAB / ln 2,  ST_MAGIC = 1.5 * 2^20
-// is ONE rounding of  ST_MAGIC + y,  y = (x / ln 2 - n) * ST_TAB  (x - n ln 2 in table steps), to ulp(t) = 2^-32 as long as
-// |y| < 2^19: the low word of t is the fraction f of y (32 bits, floor semantics), the 20 mantissa bits of the high word are
-// [k + ST_KOFF | i] with y = ST_TAB k + i + f 2^-32.  Then
-//   exp(x - n ln 2) = 2^k * 2^(i / ST_TAB) * exp(ln 2 / ST_TAB * f 2^-32) = 2^(k + ST_KOFF) * tab[i] * p(g)
-// with tab[i] = 2^(i / ST_TAB - ST_KOFF) in shared memory, g = 1 + f 2^-32 assembled from the bits of f, and p the minimax quadratic
-// of exp(ln 2 / ST_TAB (g - 1)) on [1, 2) (error 2.0e-13 at 2048 entries; the rounding of y adds 4e-14): four FP64 instructions per
-// element -- the fma above, two for p, one to accumulate -- and the bit work on the integer pipes.  An element more than
-// ST_UP_OCT octaves above the reference (or NaN, +inf) shows as a high word above ST_HI_UP and takes the rare path, which moves
-// the reference; elements below -ST_KOFF + 6 octaves are clamped there (2^-250 of an element the sum already holds).
-#define ST_MAGIC 1572864.0                       /* 1.5 * 2^20 */
-#define ST_C1 (1.4426950408889634 * ST_TAB)      /* ST_TAB / ln 2 */
-#define ST_KOFF (1 << (19 - ST_TAB_LOG2))        /* offset of the octave field; the table carries 2^-ST_KOFF */
-#define ST_IDX_MASK (ST_TAB - 1)
-#define ST_K_MASK (0xFFFFF & ~ST_IDX_MASK)
-#define ST_UP_OCT (3 * ST_KOFF / 4)
-#define ST_HI_UP (0x41300000 + ((ST_KOFF + ST_UP_OCT) << ST_TAB_LOG2))
-#define ST_HI_FLOOR (0x41300000 + (6 << ST_TAB_LOG2))
-#if ST_TAB_LOG2 == 11
-#define ST_A0 0x1.ffd3a5661bac7p-1
-#define ST_A1 0x1.62c56e9ca3a21p-12
-#define ST_A2 0x1.ec1130cd9fbd5p-25
-#else
-#error "ST_TAB_LOG2: 11 (the minimax coefficients below belong to the 2048-entry table)"
-#endif
+#include "ile_fixexp.cuh"
 #define ST_MG_UNSET (ST_MAGIC + 1073741824.0 * ST_TAB) /* reference at -2^30 octaves: the first valid element takes the rare path */
 
 // 2^d for an integer-valued d <= 0; 0 below -1000

@@ -18,37 +18,12 @@
 #include <math_constants.h>
 
 #include "ile_kernels.h"
+#include "ile_fixexp.cuh"
 
 #define TILED_CWARPS 8                         /* consumer warps: accumulation phases and the LSE pass */
 #define TILED_THREADS ((TILED_CWARPS + 1) * 32) /* + one producer warp: per-sample setup of the next tile */
 #define TILED_CHUNK 64
 
-// exp(x) for x <= 0 (max-subtracted arguments): Cody-Waite reduction x = k ln2 + r, |r| <= ln2/2, degree-11
-// near-minimax polynomial (Chebyshev-node interpolant, relative error 1.7e-17 before rounding), exponent patched in
-// as an integer add.  Arguments below -708 (result < 3.4e-308) return 0; NaN propagates.
-__device__ __forceinline__ double ile_exp_nonpos(double x)
-{
-    const double MAGIC = 6755399441055744.0;  // 1.5 * 2^52: adding it rounds to the nearest integer
-    const double t = fma(x, 1.4426950408889634, MAGIC);
-    const double kf = t - MAGIC;
-    double r = fma(kf, -6.93147180369123816490e-01, x);
-    r = fma(kf, -1.90821492927058770002e-10, r);
-    double p = 2.5110037605963777e-08;
-    p = fma(p, r, 2.763263963904103e-07);
-    p = fma(p, r, 2.755724091857897e-06);
-    p = fma(p, r, 2.4801485482328494e-05);
-    p = fma(p, r, 0.00019841269890047113);
-    p = fma(p, r, 0.0013888888952314775);
-    p = fma(p, r, 0.008333333333319601);
-    p = fma(p, r, 0.0416666666664881);
-    p = fma(p, r, 0.1666666666666668);
-    p = fma(p, r, 0.5000000000000019);
-    p = fma(p, r, 1.0);
-    p = fma(p, r, 1.0);
-    const int k = __double2loint(t);
-    const double res = __hiloint2double(__double2hiint(p) + (k << 20), __double2loint(p));
-    return x < -708.0 ? 0.0 : res;
-}
 
 // ------------------------------------------------------------------------------------------------------------
 // named barriers (PTX bar.sync / bar.arrive): producer warp <-> consumer warps hand-off of the per-tile setup
@@ -331,12 +306,12 @@ __global__ void __launch_bounds__(TILED_THREADS, 2)
             j = 0;
             for (; j + 96 < nl; j += 128) {
                 const double x0 = row[j] - mx, x1 = row[j + 32] - mx, x2 = row[j + 64] - mx, x3 = row[j + 96] - mx;
-                e0 += ile_exp_nonpos(x0);
-                e1 += ile_exp_nonpos(x1);
-                e2 += ile_exp_nonpos(x2);
-                e3 += ile_exp_nonpos(x3);
+                e0 += ile_fixexp_nonpos(x0, a.exp_tab);
+                e1 += ile_fixexp_nonpos(x1, a.exp_tab);
+                e2 += ile_fixexp_nonpos(x2, a.exp_tab);
+                e3 += ile_fixexp_nonpos(x3, a.exp_tab);
             }
-            for (; j < nl; j += 32) e0 += ile_exp_nonpos(row[j] - mx);
+            for (; j < nl; j += 32) e0 += ile_fixexp_nonpos(row[j] - mx, a.exp_tab);
             const double sm = warp_sum((e0 + e1) + (e2 + e3));
             if (lane == 0) a.lnL[flat0 + al] = mx + log(sm) - log_nt - quadS[al];
         }

@@ -16,6 +16,7 @@ struct IleEvalArgs {
     double *lnL;
     int32_t *shift_idx;                 // may be NULL
     unsigned long long *oob_counter;    // device, sticky
+    const double *exp_tab;              // device: 2^(i/2048 - 256), i < 2048 (ile_fixexp.cuh; made once per context)
 };
 
 // Host copy of the sizes every launcher needs.
