@@ -299,7 +299,9 @@ static int ensure_scratch(ile_ctx *c, size_t samples, size_t hist_words, cudaStr
         c->sc.hist = nullptr;
         c->sc_hist = 0;
         CK(cudaMalloc(&c->sc.hist, hist_words * sizeof(uint32_t)));
+        CK(cudaMemsetAsync(c->sc.hist, 0, hist_words * sizeof(uint32_t), st));
         c->sc_hist = hist_words;
+        c->ss.hist_clean = true;
     }
     return ILE_OK;
 }
@@ -311,7 +313,7 @@ static int eval_stream_group(ile_ctx *c, IleEvalArgs a, cudaStream_t st)
     const IleSortPlan &sp = nc1 ? c->ssp1 : c->ssp;
     const size_t nseg = (size_t)sp.nseg;
     const int64_t slot_cap = (((a.n_per_point + 7) & ~(int64_t)7) + 8 * (int64_t)nseg + 31) & ~(int64_t)31;  // groups per point: multiple of 4
-    int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * (sp.ncell + nseg) + ILE_STREAM_MAX_RANGES, st);
+    int r = ensure_scratch(c, (size_t)a.n_per_point * a.n_points, (size_t)a.n_points * (sp.ncell + nseg) + 2 * ILE_STREAM_MAX_RANGES, st);
     if (r != ILE_OK) return r;
     const size_t need_slots = (size_t)a.n_points * slot_cap, need_g = 2 * (size_t)a.n_points + 2;
     if (need_slots > c->ss_slots || need_g > c->ss_gcum) {

@@ -179,7 +179,10 @@ struct IleStreamKArgs {
     const int32_t *i0;
     const int32_t *slots;
     const int32_t *gcum;
-    uint32_t *rcnt;         // [n_ranges] claim counters, zeroed per launch
+    uint32_t *rcnt;         // [n_ranges] claim counters, zero at launch (the previous launch cleaned them: rcnt_next)
+    uint32_t *rcnt_next;    // the claim counters of the NEXT launch, and
+    uint32_t *zero_ptr;     // the sort's histograms and segment totals (not needed any more): zeroed here, so that no memset
+    long long zero_n;       // stands in front of the next launch's index kernel
     int32_t n_ranges;
     double *lnL;
     const double *tabs;     // [ST_TAB] exp table, then [128][2] log table (ile_stream_tab_kernel, once per context)
@@ -194,6 +197,9 @@ __global__ void __launch_bounds__(ST_THREADS, MINB) ile_eval_stream_kernel(const
     for (int i = threadIdx.x; i < 128; i += blockDim.x) ltab[i] = make_double2(a.tabs[ST_TAB + 2 * i], a.tabs[ST_TAB + 2 * i + 1]);
     __syncthreads();
     const uint32_t tab_addr = (uint32_t)__cvta_generic_to_shared(tab);
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < a.zero_n; i += (long long)gridDim.x * blockDim.x) a.zero_ptr[i] = 0u;
+    if (blockIdx.x == 0)
+        for (int i = threadIdx.x; i < ILE_STREAM_MAX_RANGES; i += blockDim.x) a.rcnt_next[i] = 0u;
 
     const int lane = threadIdx.x & 31, r = lane >> 2, cc = lane & 3;
     const int n_t = a.n_t;
@@ -836,18 +842,25 @@ cudaError_t ile_stream_prepare(const IleSizes &sz, IleStreamPlan *pl)
 }
 
 cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleStreamPlan &pl,
-                                   const IleSortPlan &sp, const IleSortScratch &sc, const IleStreamScratch &ss, cudaStream_t st,
+                                   const IleSortPlan &sp, const IleSortScratch &sc, IleStreamScratch &ss, cudaStream_t st,
                                    int *n_launches)
 {
     if (a.n_per_point <= 0 || a.n_points <= 0) return cudaSuccess;
     const long long n_total = a.n_per_point * a.n_points;
     const int nseg = sp.nseg;
-    // cell histograms and the claim counters of the streaming kernel, one zeroed block; the segment totals behind them are
-    // written by the scan kernel
-    const size_t n_hist = (size_t)a.n_points * sp.ncell;
-    cudaError_t e = cudaMemsetAsync(sc.hist, 0, (n_hist + ILE_STREAM_MAX_RANGES) * sizeof(uint32_t), st);
-    if (e != cudaSuccess) return e;
-    uint32_t *rcnt = sc.hist + n_hist, *segtot = rcnt + ILE_STREAM_MAX_RANGES;
+    // sc.hist = [claim counters A][claim counters B][cell histograms][segment totals].  Everything in it is zero between launches: the
+    // streaming kernel of a launch zeroes the histograms and totals (the sort is done with them by then) and the claim counters the NEXT
+    // launch will use (A and B alternate), so no memset stands in front of the index kernel.  After a failed launch (hist_clean false)
+    // the whole block is zeroed the plain way.
+    const size_t n_hist = (size_t)a.n_points * sp.ncell, n_used = n_hist + (size_t)a.n_points * nseg;
+    uint32_t *rcnt = sc.hist + ILE_STREAM_MAX_RANGES * (ss.launch_no & 1u), *rcnt_next = sc.hist + ILE_STREAM_MAX_RANGES * ((ss.launch_no + 1u) & 1u);
+    uint32_t *hist = sc.hist + 2 * ILE_STREAM_MAX_RANGES, *segtot = hist + n_hist;
+    cudaError_t e = cudaSuccess;
+    if (!ss.hist_clean) {
+        e = cudaMemsetAsync(sc.hist, 0, (2 * ILE_STREAM_MAX_RANGES + n_used) * sizeof(uint32_t), st);
+        if (e != cudaSuccess) return e;
+    }
+    ss.hist_clean = false;
     long long iblocks = (n_total + IX_THREADS - 1) / IX_THREADS;
     const long long cap = (long long)sz.sm_count * 32;
     if (iblocks > cap) iblocks = cap;
@@ -856,7 +869,7 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     e = cudaEventRecord(ss.ev_fork, st);
     if (e != cudaSuccess) return e;
     int nl = 0;
-    ile_stream_index_kernel<<<(unsigned)iblocks, IX_THREADS, 0, st>>>(hp, a, sp, sc.i0, sc.cell, sc.hist);
+    ile_stream_index_kernel<<<(unsigned)iblocks, IX_THREADS, 0, st>>>(hp, a, sp, sc.i0, sc.cell, hist);
     ++nl;
     e = cudaStreamWaitEvent(ss.aux, ss.ev_fork, 0);
     if (e != cudaSuccess) return e;
@@ -873,7 +886,7 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     e = cudaEventRecord(ss.ev_join, ss.aux);
     if (e != cudaSuccess) return e;
     ile_stream_scan_kernel<<<dim3((unsigned)nseg, (unsigned)a.n_points), SS_THREADS, (size_t)sp.n0 * sizeof(uint32_t), st>>>(sp.n0, nseg, sp.ncell,
-                                                                                                                            sc.hist, segtot);
+                                                                                                                            hist, segtot);
     ++nl;
     if (a.n_points > 1) {
         ile_stream_prefix_kernel<<<1, 1024, (size_t)a.n_points * sizeof(uint32_t), st>>>(a.n_points, nseg, segtot, ss.gcum);
@@ -883,7 +896,7 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     const long long scap = ((long long)sz.sm_count * 8 + a.n_points - 1) / a.n_points;
     if (sblocks > scap) sblocks = scap;
     ile_stream_scatter_kernel<<<dim3((unsigned)sblocks, (unsigned)a.n_points), IX_THREADS, (size_t)nseg * sizeof(uint32_t), st>>>(
-        a.n_per_point, a.n_points, sp.ncell, sp.n0, nseg, ss.slot_cap, sc.cell, sc.hist, segtot, ss.slots, ss.gcum);
+        a.n_per_point, a.n_points, sp.ncell, sp.n0, nseg, ss.slot_cap, sc.cell, hist, segtot, ss.slots, ss.gcum);
     ++nl;
     e = cudaGetLastError();
     if (e != cudaSuccess) return e;
@@ -908,6 +921,9 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     ka.slots = ss.slots;
     ka.gcum = ss.gcum;
     ka.rcnt = rcnt;
+    ka.rcnt_next = rcnt_next;
+    ka.zero_ptr = hist;
+    ka.zero_n = (long long)n_used;
     ka.lnL = a.lnL;
     ka.tabs = ss.tabs;
     const long long max_groups = (long long)a.n_points * (ss.slot_cap / 8);
@@ -918,6 +934,7 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     ka.n_ranges = max_groups < 4LL * nr_sm ? 1 : nr_sm;
     e = st_launch(sz, pl.ks, pl.nc, &ka, max_groups, &per_sm, st);
     ++nl;
+    if (e == cudaSuccess) ss.hist_clean = true, ++ss.launch_no;
     if (e == cudaSuccess && n_launches) *n_launches += nl;
     return e;
 }

@@ -66,7 +66,7 @@ struct IleSortScratch {
     double *quad;      // [n]
     int32_t *i0;       // [n][K]
     int32_t *cell;     // [n]
-    uint32_t *hist;    // [n_points][ncell] cell counts -> positions inside the segment, then ILE_STREAM_MAX_RANGES claim counters, then [n_points][nseg] segment totals
+    uint32_t *hist;    // 2 x ILE_STREAM_MAX_RANGES claim counters, [n_points][ncell] cell counts -> positions inside the segment, [n_points][nseg] segment totals; zero between launches
     double *qform;     // [n][K][3] quadratic forms from the FP64-MMA kernel, or NULL (the coefficient kernel computes them)
 };
 
@@ -93,6 +93,8 @@ struct IleStreamScratch {
     cudaEvent_t ev_late;  // if not NULL: the arrays the coefficient kernel reads (phi_ref, psi, incl, dist) arrive with this event
     const double2 *hU, *hV;  // host mirrors of U, V [P][K][M][M] (kernel-parameter path of the coefficient kernel), or NULL
     double *tabs;        // exp and log tables of the streaming kernel (ile_stream_alloc_tables)
+    uint32_t launch_no;  // parity picks the claim counters of a launch
+    bool hist_clean;     // sc.hist is all zero (set when it is allocated and by every successful launch)
 };
 
 cudaError_t ile_stream_alloc_tables(IleStreamScratch *ss);
@@ -107,7 +109,7 @@ cudaError_t ile_launch_pack_q_stream(const IleSizes &sz, const IleStreamPlan &pl
                                      double *Qs, cudaStream_t st);
 // setup + sort of variant 4 (memsets + setup + scan + scatter), then the streaming kernel
 cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, const IleEvalArgs &a, const IleStreamPlan &pl,
-                                   const IleSortPlan &sp, const IleSortScratch &sc, const IleStreamScratch &ss,
+                                   const IleSortPlan &sp, const IleSortScratch &sc, IleStreamScratch &ss,
                                    cudaStream_t st, int *n_launches);
 // variant 4: coefficients a F_k Y_lm and quadratic term of every sample (steps 1, 3, 4), no sorting work
 // (hU, hV: host mirrors of the context's U, V, or NULL; returns the number of kernels launched)
