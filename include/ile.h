@@ -125,6 +125,34 @@ int ile_evidence_reset(ile_ctx *ctx, int32_t n_segments, double *state, void *cu
 int ile_evidence_merge(ile_ctx *ctx, int32_t n_segments, int32_t n_states, const double *states_in, double *state_out,
                        double *lnZ, double *n_eff, void *cuda_stream);
 
+/* ile_evidence without a context and without a single device allocation (eq. 4; n_eff L101): same inputs, same
+ * outputs, same arithmetic as ile_evidence above.
+ *
+ * Why it exists: everything else in this library works out of an ile_ctx, and a context is built from cudaMalloc calls
+ * (at ile_create, and later whenever its scratch has to grow).  That rules the library out for callers who may not
+ * allocate on the device: code living inside a memory pool it does not own (a framework's caching allocator, a fixed
+ * slab handed to a batch job -- a raw cudaMalloc goes around the pool, may fail while the pool still has room, and
+ * stalls every stream of the device), real-time loops and plug-ins whose host forbids driver allocations after
+ * start-up, or a worker that only wants to fold lnL_margT values it already has into lnZ.  Here the kernel's scratch
+ * (per-block partial sums and one ticket word per segment) is a fixed array inside the library's device image, and the
+ * call uses no cudaMalloc, cudaFree or allocating library routine.
+ *
+ * Limits and rules that come with that:
+ *  - n_segments <= ILE_EVIDENCE_STATIC_MAX_SEGMENTS, else ILE_ERR_UNSUPPORTED ("size or variant not supported by this
+ *    build") and nothing is launched; n_per_segment is not limited.  Devices with an ordinal >= 64 are refused likewise.
+ *  - The array (ILE_EVIDENCE_STATIC_SCRATCH_BYTES) is held on every GPU that loads the library, until the process ends.
+ *  - The first call made on a device looks up the array's device address (cudaGetSymbolAddress, once per device, with
+ *    that device current) and the SM count.  Make that first call during start-up, before any stream capture begins.
+ *  - One array per device, shared by all callers and threads, keeping whatever the last call left: each call clears the
+ *    ticket words it needs on cuda_stream before its kernel.  Calls that can overlap on the GPU (two streams with no event
+ *    between them) race on the array and give wrong results; calls on one stream, or ordered by events, are safe.
+ *  - lnL_margT, log_w (may be NULL), state (IN/OUT, may be NULL), lnZ, n_eff (may be NULL): device memory of the current
+ *    device, caller-owned, shapes as for ile_evidence.  Asynchronous on cuda_stream. */
+#define ILE_EVIDENCE_STATIC_MAX_SEGMENTS 1024
+#define ILE_EVIDENCE_STATIC_SCRATCH_BYTES 69632 /* 68 KiB: 1024 ticket words + 4096 (max, sum) pairs */
+int ile_evidence_static(int32_t n_segments, int64_t n_per_segment, const double *lnL_margT, const double *log_w,
+                        double *state, double *lnZ, double *n_eff, void *cuda_stream);
+
 /* Overlap pre-computation of n_points intrinsic points (eq. 8a-c: Q_{k,lm}(t) = <h_lm|d_k>(t), U_k = <h_lm|h_l'm'>,
  * V_k = <h_lm^*|h_l'm'>) -- what ile_create takes as input, made on the GPU.  Discrete two-sided setting: n_q samples at
  * fs_hz, FFT-order frequency grid f_n = n' fs_hz / n_q (n' the signed index), whitened spectra, <a|b> = sum_n conj(a[n]) b[n]:

@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libile_b200.so")
 _lib = None
 
 SAMPLE_FIELDS = ("ra", "dec", "t_ref", "phi_ref", "psi", "incl", "dist_mpc")
-EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_evidence_merge", "ile_precompute", "ile_precompute_psd", "ile_run_host", "ile_run_host_all", "ile_status",
+EXPORTS = ("ile_create", "ile_eval", "ile_eval_all", "ile_evidence", "ile_evidence_reset", "ile_evidence_merge", "ile_evidence_static", "ile_precompute", "ile_precompute_psd", "ile_run_host", "ile_run_host_all", "ile_status",
            "ile_set_variant", "ile_launch_count", "ile_measure_fp64_peak", "ile_measure_dmma_peak", "ile_destroy", "ile_strerror",
            "ile_sampler_create", "ile_sampler_destroy", "ile_sampler_reset", "ile_sampler_set_tables", "ile_sampler_get_tables",
            "ile_sampler_uniforms", "ile_sampler_draw", "ile_sampler_refit", "ile_sampler_launch_count", "ile_integrate",
@@ -67,6 +67,7 @@ def load():
     L.ile_eval_all.argtypes = [vp, i64] + [vp] * 7 + [vp, vp, vp]
     L.ile_evidence.argtypes = [vp, i32, i64, vp, vp, vp, vp, vp, vp]
     L.ile_evidence_reset.argtypes = [vp, i32, vp, vp]
+    L.ile_evidence_static.argtypes = [i32, i64, vp, vp, vp, vp, vp, vp]
     L.ile_evidence_merge.argtypes = [vp, i32, i32, vp, vp, vp, vp, vp]
     L.ile_precompute.argtypes = [i32, i32, i32, i32, ctypes.c_double, ctypes.c_double, vp, vp, vp, vp, vp, vp]
     L.ile_precompute_psd.argtypes = [i32, i32, i32, i32, ctypes.c_double, ctypes.c_double, vp, vp, vp, ctypes.c_double, ctypes.c_double,
@@ -405,6 +406,31 @@ def integrate(ctx: "Context", sampler: "Sampler", n_chunk: int, max_chunks: int,
                                 _stream_ptr(stream)), "ile_integrate")
     nc = int(ns.value) // int(n_chunk)
     return dict(lnZ=lnZ.value, n_eff=neff.value, n_samples=int(ns.value), n_chunks=nc, history=hist[:nc])
+
+
+def evidence_static(lnL, log_w=None, state=None, n_segments: int = 1, out=None, stream=None):
+    """ile_evidence_static: the evidence reduction for callers that may not allocate device memory -- no Context (whose
+    creation is a series of cudaMalloc calls) is needed; the kernel's scratch is a fixed 68 KiB array inside the library
+    (see include/ile.h for who needs this and for the rules: at most ILE_EVIDENCE_STATIC_MAX_SEGMENTS = 1024 segments, one
+    shared array per device, so calls that may overlap on the GPU race; first call on a device before any stream capture).
+    lnL [n_segments][n_per_segment] CUDA float64 -> (lnZ, n_eff) CUDA tensors [n_segments].  Pass `out=(lnZ, n_eff)`
+    (preallocated) if even PyTorch's allocator must stay untouched; `state` [n_segments][3] must start as (-inf, 0, 0)."""
+    import torch
+
+    assert lnL.is_cuda and lnL.dtype == torch.float64 and lnL.is_contiguous()
+    n = lnL.numel()
+    assert n % n_segments == 0
+    if log_w is not None:
+        assert log_w.is_cuda and log_w.dtype == torch.float64 and log_w.is_contiguous() and log_w.numel() == n
+    if out is None:
+        out = (torch.empty(n_segments, dtype=torch.float64, device=lnL.device),
+               torch.empty(n_segments, dtype=torch.float64, device=lnL.device))
+    lnZ, neff = out
+    assert lnZ.numel() == n_segments and neff.numel() == n_segments
+    with torch.cuda.device(lnL.device):
+        _check(load().ile_evidence_static(int(n_segments), n // n_segments, _ptr(lnL), _ptr(log_w), _ptr(state), _ptr(lnZ),
+                                          _ptr(neff), _stream_ptr(stream)), "ile_evidence_static")
+    return lnZ, neff
 
 
 def precompute(x, d, fs_hz: float, t0_q_s: float, stream=None):
