@@ -239,8 +239,43 @@ def test_O3_higher_l_closed_forms():
         assert abs(oracle.sYlm(3, -3, th, ph) - y3m3) < 5e-15
 
 
+def test_O3_highest_weight_closed_form_to_l8():
+    """m = l has a one-term closed form for every l (Goldberg et al. 1967 eq. 3.1 with s = -2):
+    -2Y_ll = (-1)^l sqrt((2l+1)/4pi) sqrt((2l)! / ((l+2)! (l-2)!)) cos^(l+2)(theta/2) sin^(l-2)(theta/2) e^{i l phi};
+    l = 5 is the literature's -sqrt(330/pi) cos^7 sin^3 e^{5 i phi}.  Pins the factorial bounds of O3 up to ILE_MAX_L = 8
+    (eq. 5-6)."""
+    from math import factorial as f
+    for _ in range(50):
+        th, ph = np.arccos(RNG.uniform(-1, 1)), RNG.uniform(0, 2 * np.pi)
+        ch, sh = np.cos(th / 2), np.sin(th / 2)
+        assert abs(oracle.sYlm(5, 5, th, ph) + np.sqrt(330.0 / np.pi) * ch ** 7 * sh ** 3 * np.exp(5j * ph)) < 5e-15
+        for l in range(2, 9):
+            v = (-1) ** l * np.sqrt((2 * l + 1) / (4 * np.pi)) * np.sqrt(f(2 * l) / (f(l + 2) * f(l - 2))) * ch ** (l + 2) * sh ** (l - 2) * np.exp(1j * l * ph)
+            assert abs(oracle.sYlm(l, l, th, ph) - v) < 1e-14, l
+
+
+def test_O3_wigner_d_is_the_rotation_matrix_to_l8():
+    """A definition that shares nothing with the finite sum: d^l_{m',m}(beta) = <l m'| exp(-i beta J_y) |l m>, J_y from the ladder
+    operators J+-|l m> = sqrt(l(l+1) - m(m+-1)) |l m+-1>, exponentiated by a library routine.  -2Y_lm = sqrt((2l+1)/4pi) d^l_{m,2}(theta)
+    e^{i m phi} (reading R5) for EVERY (l, m), l = 2..8: a wrong factorial bound, sign or exponent in any term fails here."""
+    import scipy.linalg as sl
+
+    for l in range(2, 9):
+        ms = list(range(l, -l - 1, -1))
+        Jp = np.zeros((2 * l + 1, 2 * l + 1))
+        for i, m in enumerate(ms):
+            if m < l:
+                Jp[i - 1, i] = np.sqrt(l * (l + 1) - m * (m + 1))
+        Jy = (Jp - Jp.T) / 2j
+        for th in (0.0, 0.3, 1.1, np.pi / 2, 2.9, np.pi):
+            D = sl.expm(-1j * th * Jy)
+            for i, m in enumerate(ms):
+                ref = np.sqrt((2 * l + 1) / (4 * np.pi)) * D[i, ms.index(2)] * np.exp(1j * m * 0.7)
+                assert abs(oracle.sYlm(l, m, th, 0.7) - ref) < 2e-14, (l, m, th)
+
+
 def test_O3_pole_values_and_sum_rule():
-    for l in (2, 3, 4):
+    for l in range(2, 9):
         for m in range(-l, l + 1):
             v = oracle.sYlm(l, m, 0.0, 0.7)
             if m == 2:
@@ -253,9 +288,9 @@ def test_O3_pole_values_and_sum_rule():
 
 
 def test_O3_orthonormality_by_quadrature():
-    mu, w = np.polynomial.legendre.leggauss(12)      # exact for the degree <= 8 polynomials in cos(theta)
-    n_phi = 16
-    modes = gi.modes_up_to(4)
+    mu, w = np.polynomial.legendre.leggauss(20)      # exact to degree 39 >= 16 = 2 ILE_MAX_L in cos(theta)
+    n_phi = 24                                       # the trapezoid in phi is exact while |m - m'| <= 16 < n_phi
+    modes = gi.modes_up_to(8)
     vals = np.zeros((len(modes), len(mu), n_phi), dtype=complex)
     for a, (l, m) in enumerate(modes):
         for i, x in enumerate(mu):
