@@ -109,7 +109,7 @@ int ile_eval_all(ile_ctx *ctx, int64_t n_per_point, const double *ra, const doub
  *        be fed in chunks from one stream (config 3); initialise with ile_evidence_reset or to (-inf, 0, 0).
  *        May be NULL: then the call is self-contained.
  * lnZ, n_eff: device, n_segments doubles out; n_eff may be NULL.  A segment with no finite sample gives
- * lnZ = -inf, n_eff = 0. */
+ * lnZ = -inf, n_eff = 0.  n_segments <= 65535 (else ILE_ERR_UNSUPPORTED). */
 int ile_evidence(ile_ctx *ctx, int32_t n_segments, int64_t n_per_segment, const double *lnL_margT,
                  const double *log_w, double *state, double *lnZ, double *n_eff, void *cuda_stream);
 
@@ -160,8 +160,9 @@ int ile_evidence_static(int32_t n_segments, int64_t n_per_segment, const double 
  *   U[p][k][a][b] = sum_n conj(x[p][k][a][n]) x[p][k][b][n],   V[p][k][a][b] = sum_n x[p][k][a][(-n) mod n_q] x[p][k][b][n]
  * x: device complex128 [P][K][M][n_q]; d: device complex128 [P][K][n_q]; Q, U, V: device outputs, caller-owned, shapes as
  * ile_create reads them.  n_q must be a power of two, 2..65536 (else ILE_ERR_UNSUPPORTED; above 8192 a two-level
- * transform through a library-owned scratch buffer).  Asynchronous on cuda_stream;
- * needs no context. */
+ * transform through a library-owned scratch buffer).  Asynchronous on cuda_stream; needs no context.  The twiddle table and
+ * that scratch buffer are library-owned, one set per device (never freed): calls are thread-safe, and calls on one device are
+ * serialised on the GPU -- each waits for the kernels of the previous call, whichever stream that was issued on. */
 int ile_precompute(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t n_q, double fs_hz, double t0_q_s, const void *x,
                    const void *d, void *Q, void *U, void *V, void *cuda_stream);
 

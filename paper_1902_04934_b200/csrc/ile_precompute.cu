@@ -15,6 +15,8 @@
 //   ile_overlap_uv_small_kernel    M <= 5: one block per (detector, point), warp = (row a, frequency slice), pairs (a, b >= a) in registers
 //   ile_overlap_uv_kernel          any M: register-blocked tiles of pairs (a, b), lanes over frequencies
 // With S != NULL the inner products are eq. 2's (L30-L35): weight scale / S_k(|f_n|) inside f_min < |f_n| < f_max, 0 outside.
+#include <mutex>
+
 #include "ile_kernels.h"
 
 #define PC_THREADS 256
@@ -660,9 +662,53 @@ static cudaError_t pc_launch_uv_bulk(int32_t N, int32_t n_pk, const double2 *x, 
     return cudaGetLastError();
 }
 
+// Library-owned state of the pre-computation, one per device: the twiddle / start-time phase table (rebuilt in stream order when
+// the grid or the start time changes) and the first-level output Z of the two-level transform (grown on demand).  Both are
+// shared by every call on the device, so calls are serialised: g_pc_mutex covers the host side (the bookkeeping below and the
+// launches of one call), and every call waits on the event recorded at the end of the previous one, so that a call on another
+// stream neither reads a half-written table nor overwrites table / Z under kernels that still use them.  Never freed.
+struct PcDevice {
+    double2 *tab;
+    int tab_n;
+    double tab_alpha;
+    double2 *z;
+    size_t z_cap;
+    cudaEvent_t done;  // end of the most recent call's work on this device
+    bool have_done;
+};
+static PcDevice g_pc[64];
+static std::mutex g_pc_mutex;
+
+static cudaError_t pc_launch_locked(PcDevice &pd, int dev, int32_t n_points, int32_t K, int32_t M, int32_t N, double fs_hz, double t0_q_s,
+                                    const double2 *x, const double2 *d, const double *S, double f_min_hz, double f_max_hz, double scale,
+                                    double2 *Q, double2 *U, double2 *V, int32_t max_smem_optin, cudaStream_t st);
+
 cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_t N, double fs_hz, double t0_q_s, const double2 *x,
                                   const double2 *d, const double *S, double f_min_hz, double f_max_hz, double scale, double2 *Q, double2 *U,
                                   double2 *V, int32_t max_smem_optin, cudaStream_t st)
+{
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(g_pc_mutex);
+    PcDevice &pd = g_pc[dev];
+    if (!pd.have_done) {
+        e = cudaEventCreateWithFlags(&pd.done, cudaEventDisableTiming);
+        if (e != cudaSuccess) return e;
+        pd.have_done = true;
+    } else {
+        e = cudaStreamWaitEvent(st, pd.done, 0);  // no-op when the previous call was made on this stream
+        if (e != cudaSuccess) return e;
+    }
+    e = pc_launch_locked(pd, dev, n_points, K, M, N, fs_hz, t0_q_s, x, d, S, f_min_hz, f_max_hz, scale, Q, U, V, max_smem_optin, st);
+    const cudaError_t er = cudaEventRecord(pd.done, st);  // also after an error: part of the call may be in flight
+    return e != cudaSuccess ? e : er;
+}
+
+static cudaError_t pc_launch_locked(PcDevice &pd, int dev, int32_t n_points, int32_t K, int32_t M, int32_t N, double fs_hz, double t0_q_s,
+                                    const double2 *x, const double2 *d, const double *S, double f_min_hz, double f_max_hz, double scale,
+                                    double2 *Q, double2 *U, double2 *V, int32_t max_smem_optin, cudaStream_t st)
 {
     int log2n = 0;
     while ((1 << log2n) < N) ++log2n;
@@ -677,31 +723,28 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
     int nsplit = (PC_THREADS / 32 + tiles - 1) / tiles;
     while (nsplit > 1 && N / nsplit < 32) --nsplit;
     const size_t smem_uv = (size_t)M * M * 32;
-    // twiddles and start-time phases: one table per device, recomputed (in stream order) when the grid or the start time
-    // changes.  Calls for DIFFERENT (n_q, fs t0) must not run concurrently on two streams of one device.
-    static double2 *g_tab[64] = {nullptr};
-    static int g_tab_n[64] = {0};
-    static double g_tab_alpha[64] = {0.0};
-    static double2 *g_z[64] = {nullptr};  // first-level output of the two-level transform, grown on demand
-    static size_t g_z_cap[64] = {0};
-    int dev = 0;
-    e = cudaGetDevice(&dev);
-    if (e != cudaSuccess) return e;
-    if (dev < 0 || dev >= 64) return cudaErrorInvalidDevice;
-    if (!g_tab[dev]) {
-        e = cudaMalloc(&g_tab[dev], (size_t)(32768 + 65536) * sizeof(double2));
+    if (!pd.tab) {
+        double2 *t = nullptr;
+        e = cudaMalloc(&t, (size_t)(32768 + 65536) * sizeof(double2));
         if (e != cudaSuccess) return e;
         e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel<512, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4608 * 16));
         if (e == cudaSuccess) e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel<1024, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(9216 * 16));
         if (e == cudaSuccess) e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel<512, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(4608 * 16));
         if (e == cudaSuccess) e = cudaFuncSetAttribute(ile_overlap_q_radix8_kernel<1024, 8>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(9216 * 16));
-        if (e != cudaSuccess) return e;
+        if (e != cudaSuccess) {
+            cudaFree(t);
+            return e;
+        }
+        pd.tab = t, pd.tab_n = 0;
     }
-    double2 *tab = g_tab[dev];
+    double2 *tab = pd.tab;
     const double alpha = fs_hz * t0_q_s / (double)N;
-    if (g_tab_n[dev] != N || g_tab_alpha[dev] != alpha) {
+    if (pd.tab_n != N || pd.tab_alpha != alpha) {
+        pd.tab_n = 0;  // the table belongs to no grid until its kernel has been launched
         ile_overlap_tables_kernel<<<(N + PC_THREADS - 1) / PC_THREADS, PC_THREADS, 0, st>>>(N, alpha, tab);
-        g_tab_n[dev] = N, g_tab_alpha[dev] = alpha;
+        e = cudaGetLastError();
+        if (e != cudaSuccess) return e;
+        pd.tab_n = N, pd.tab_alpha = alpha;
     }
     PcWeight wt;
     wt.S = S, wt.df = fs_hz / (double)N, wt.fmin = f_min_hz, wt.fmax = f_max_hz, wt.scale = scale;
@@ -711,16 +754,16 @@ cudaError_t ile_launch_precompute(int32_t n_points, int32_t K, int32_t M, int32_
     const unsigned n_series = (unsigned)((size_t)n_points * K * M);
     if (two_level) {
         const size_t need = (size_t)n_series * N;
-        if (need > g_z_cap[dev]) {
-            e = cudaStreamSynchronize(st);
+        if (need > pd.z_cap) {
+            e = cudaStreamSynchronize(st);  // st has waited for the previous call, whichever stream it ran on
             if (e != cudaSuccess) return e;
-            cudaFree(g_z[dev]);
-            g_z[dev] = nullptr, g_z_cap[dev] = 0;
-            e = cudaMalloc(&g_z[dev], need * sizeof(double2));
+            cudaFree(pd.z);
+            pd.z = nullptr, pd.z_cap = 0;
+            e = cudaMalloc(&pd.z, need * sizeof(double2));
             if (e != cudaSuccess) return e;
-            g_z_cap[dev] = need;
+            pd.z_cap = need;
         }
-        double2 *Z = g_z[dev];
+        double2 *Z = pd.z;
         ile_overlap_q_split8_kernel<<<dim3((unsigned)(NS / PC_THREADS), n_series), PC_THREADS, 0, st>>>(M, N, tab, x, d, wt, Z);
         switch (NS) {  // rows of the first level: plain loads, output stride 8, every eighth twiddle of the long table
             case 2048: ile_overlap_q_radix8_kernel<256, 8><<<n_series * 8, 256, smem, st>>>(M, NS, tab, Z, d, wt, Q); break;

@@ -119,3 +119,32 @@ def test_precompute_psd_matches_oracle(gpu_lib, n_q, M, P):
         check(V[p], rv, axes=(-1, -2))
     with pytest.raises(gpu_lib.IleError):
         gpu_lib.precompute_psd(torch.from_numpy(h).cuda(), torch.from_numpy(d).cuda(), torch.from_numpy(S).cuda(), fs, t0, 50.0, 20.0, scale)
+
+
+def test_precompute_calls_on_two_streams_share_the_library_tables_safely(gpu_lib):
+    """The twiddle / phase table and the two-level scratch are library-owned, one set per device.  Calls with DIFFERENT
+    (n_q, start time) issued back to back on two non-blocking streams, with no event between them, must each see their
+    own table: every call waits on the device for the previous call (include/ile.h, ile_precompute).  Repeated so that a
+    missing order would show as a wrong Q in at least one round."""
+    import torch
+
+    r = np.random.default_rng(77)
+    cases = []
+    for n_q, t0 in [(2048, 3.25 / 4096.0), (16384, -1.5 / 4096.0), (1024, 0.0), (2048, 7.75 / 4096.0)]:
+        x = r.standard_normal((4, 2, 3, n_q)) + 1j * r.standard_normal((4, 2, 3, n_q))
+        d = r.standard_normal((4, 2, n_q)) + 1j * r.standard_normal((4, 2, n_q))
+        cases.append((torch.from_numpy(x).cuda(), torch.from_numpy(d).cuda(), t0, [pc.overlaps(x[p], d[p], 4096.0, t0) for p in range(4)]))
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    torch.cuda.synchronize()
+    for rnd in range(3):
+        outs = []
+        for i, (xd, dd, t0, _) in enumerate(cases):
+            st = streams[(i + rnd) & 1]
+            with torch.cuda.stream(st):
+                outs.append(gpu_lib.precompute(xd, dd, 4096.0, t0, stream=st))
+        torch.cuda.synchronize()
+        for (Q, U, V), (_, _, _, ref) in zip(outs, cases):
+            for p in range(4):
+                check(Q[p].cpu().numpy(), ref[p][0], axes=-1)
+                check(U[p].cpu().numpy(), ref[p][1], axes=(-1, -2))
+                check(V[p].cpu().numpy(), ref[p][2], axes=(-1, -2))
