@@ -203,11 +203,19 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
     CKC(cudaMemcpy(c->hU, c->dU, nU * sizeof(double2), cudaMemcpyDeviceToHost));
     CKC(cudaMemcpy(c->hV, c->dV, nU * sizeof(double2), cudaMemcpyDeviceToHost));
     CKC(ile_stream_alloc_tables(&c->ss));  // exp / log tables of the streaming and tiled kernels
+    CKC(cudaStreamSynchronize(0));         // their kernel runs on the legacy default stream: done before ile_create returns, whatever follows
     c->stream_ok = ile_stream_plan(c->sz, c->hparams, 2, &c->spl, &c->ssp);
+    // a streaming plan the device cannot host (no resident block) is a refused plan, not a failed create: variants 2 / 1 serve it
+    if (c->stream_ok && ile_stream_prepare(c->sz, &c->spl) != cudaSuccess) {
+        cudaGetLastError();
+        c->stream_ok = false;
+    }
     c->nc1_ok = c->stream_ok && ile_stream_plan(c->sz, c->hparams, 1, &c->spl1, &c->ssp1);
+    if (c->nc1_ok && ile_stream_prepare(c->sz, &c->spl1) != cudaSuccess) {
+        cudaGetLastError();
+        c->nc1_ok = false;
+    }
     if (c->stream_ok) {
-        CKC(ile_stream_prepare(c->sz, &c->spl));
-        if (c->nc1_ok) CKC(ile_stream_prepare(c->sz, &c->spl1));
         if (cfg->n_modes >= ILE_QUAD_MMA_MIN_MODES) {
             const size_t nd = ile_quad_pack_doubles(cfg->n_points, cfg->n_det, cfg->n_modes);
             double *hm = new (std::nothrow) double[nd];
@@ -301,6 +309,7 @@ static int ensure_scratch(ile_ctx *c, size_t samples, size_t hist_words, cudaStr
         CK(cudaMalloc(&c->sc.hist, hist_words * sizeof(uint32_t)));
         CK(cudaMemsetAsync(c->sc.hist, 0, hist_words * sizeof(uint32_t), st));
         c->sc_hist = hist_words;
+        c->ss.hist_words = hist_words;
         c->ss.hist_clean = true;
     }
     return ILE_OK;
@@ -466,6 +475,7 @@ extern "C" int ile_evidence(ile_ctx *c, int32_t n_segments, int64_t n_per_segmen
 {
     if (!c || n_segments < 1 || n_per_segment < 0 || !lnZ) return ILE_ERR_BAD_ARGUMENT;
     if (n_per_segment > 0 && !lnL_margT) return ILE_ERR_BAD_ARGUMENT;
+    if (n_segments > 65535) return ILE_ERR_UNSUPPORTED;  // segments are the y dimension of the grid
     int r = check_device(c);
     if (r != ILE_OK) return r;
     const int32_t B = ile_evidence_blocks_per_segment(n_segments, n_per_segment, c->sz.sm_count);

@@ -856,8 +856,9 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     uint32_t *rcnt = sc.hist + ILE_STREAM_MAX_RANGES * (ss.launch_no & 1u), *rcnt_next = sc.hist + ILE_STREAM_MAX_RANGES * ((ss.launch_no + 1u) & 1u);
     uint32_t *hist = sc.hist + 2 * ILE_STREAM_MAX_RANGES, *segtot = hist + n_hist;
     cudaError_t e = cudaSuccess;
-    if (!ss.hist_clean) {
-        e = cudaMemsetAsync(sc.hist, 0, (2 * ILE_STREAM_MAX_RANGES + n_used) * sizeof(uint32_t), st);
+    if (!ss.hist_clean) {  // the failed launch may have been a larger one (more points or cells): clear everything that is allocated
+        const size_t words = ss.hist_words > 2 * ILE_STREAM_MAX_RANGES + n_used ? ss.hist_words : 2 * ILE_STREAM_MAX_RANGES + n_used;
+        e = cudaMemsetAsync(sc.hist, 0, words * sizeof(uint32_t), st);
         if (e != cudaSuccess) return e;
     }
     ss.hist_clean = false;
@@ -873,18 +874,24 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
     ++nl;
     e = cudaStreamWaitEvent(ss.aux, ss.ev_fork, 0);
     if (e != cudaSuccess) return e;
+    // from here on work may sit on the side stream: an error return first makes the caller's stream wait for it, so that the caller
+    // never frees or reuses buffers under a kernel it cannot see
+    auto fail = [&](cudaError_t err) {
+        if (cudaEventRecord(ss.ev_join, ss.aux) == cudaSuccess) cudaStreamWaitEvent(st, ss.ev_join, 0);
+        return err;
+    };
     if (ss.ev_late) {  // ile_run_host: those arrays are still being copied on the copy stream
         e = cudaStreamWaitEvent(ss.aux, ss.ev_late, 0);
-        if (e != cudaSuccess) return e;
+        if (e != cudaSuccess) return fail(e);
     }
     if (ss.quad_mats && sc.qform) {
         e = ile_launch_quad_mma(sz, hp, a, ss.quad_mats, sc.qform, ss.aux);
-        if (e != cudaSuccess) return e;
+        if (e != cudaSuccess) return fail(e);
         ++nl;
     }
     nl += ile_launch_setup_coef(sz, hp, a, pl.cp, sc, ss.hU, ss.hV, ss.aux);
     e = cudaEventRecord(ss.ev_join, ss.aux);
-    if (e != cudaSuccess) return e;
+    if (e != cudaSuccess) return fail(e);
     ile_stream_scan_kernel<<<dim3((unsigned)nseg, (unsigned)a.n_points), SS_THREADS, (size_t)sp.n0 * sizeof(uint32_t), st>>>(sp.n0, nseg, sp.ncell,
                                                                                                                             hist, segtot);
     ++nl;
@@ -899,7 +906,7 @@ cudaError_t ile_launch_eval_stream(const IleSizes &sz, const IleDevParams &hp, c
         a.n_per_point, a.n_points, sp.ncell, sp.n0, nseg, ss.slot_cap, sc.cell, hist, segtot, ss.slots, ss.gcum);
     ++nl;
     e = cudaGetLastError();
-    if (e != cudaSuccess) return e;
+    if (e != cudaSuccess) return fail(e);
 
     e = cudaStreamWaitEvent(st, ss.ev_join, 0);  // join
     if (e != cudaSuccess) return e;

@@ -95,6 +95,7 @@ struct IleStreamScratch {
     double *tabs;        // exp and log tables of the streaming kernel (ile_stream_alloc_tables)
     uint32_t launch_no;  // parity picks the claim counters of a launch
     bool hist_clean;     // sc.hist is all zero (set when it is allocated and by every successful launch)
+    size_t hist_words;   // allocated words of sc.hist: what a launch after a failed one clears
 };
 
 cudaError_t ile_stream_alloc_tables(IleStreamScratch *ss);

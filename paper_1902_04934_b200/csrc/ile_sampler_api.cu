@@ -214,6 +214,7 @@ extern "C" int ile_integrate(ile_ctx *ctx, ile_sampler *s, int32_t point, int64_
     const int32_t frozen = max_chunks > n_adapt_chunks ? max_chunks - n_adapt_chunks : 0;
     int64_t multi = frozen ? ((int64_t)1 << 20) / n_chunk : 0;
     multi = multi < 1 ? (frozen ? 1 : 0) : multi > frozen ? frozen : multi;
+    if (multi > 4096) multi = 4096;  // chunks of a batch are segments of one ile_evidence launch (grid.y) and steps of a one-thread prefix
     int r = smp_ensure(s, n_chunk * (multi > 1 ? multi : 1), max_chunks, multi, st);
     if (r != ILE_OK) return r;
     r = ile_sampler_reset(s, cuda_stream);  // S9: the first chunk is drawn from the prior
