@@ -141,6 +141,35 @@ def test_config3_1e7_chunked_from_one_stream_every_sample(gpu_lib):
     ctx.close()
 
 
+def test_one_call_above_the_launch_group_size_every_sample(gpu_lib):
+    """ONE ile_eval call and ONE ile_run_host call with n = 2,500,000 on config 3's shape: more than the 1,048,576 samples
+    of a launch group, so the library itself cuts the call into three groups with shifted pointers, the last one ragged
+    (the paths bench.py --config 3 --n 10000000 takes).  EVERY lnL_margT, EVERY shift index, lnZ and n_eff against the
+    oracle (eq. 7, 9: L64-L67, L81-L86; eq. 4: L42-L47)."""
+    import torch
+
+    n = 2_500_000
+    cfg = gi.make_config(3, n=n)
+    s = gi.make_samples(cfg["sample_seeds"][0], n)
+    lw = gi.make_log_weights(9, n)
+    ref, ref_idx, ref_bad = oracle.eval_batch(cfg, s, n_threads=ORACLE_THREADS)
+    rZ, rN = oracle.evidence(ref, lw)
+    ctx = gpu_lib.Context(cfg)
+    lnL, idx = ctx.eval(to_dev(s), want_idx=True)                      # one call, three launch groups
+    n_bad, _ = ctx.status()
+    assert n_bad == ref_bad == 0
+    assert_indices_equal(cfg, s, ref_idx, idx.cpu().numpy())
+    assert rel_err(ref, lnL.cpu().numpy()) <= TOL
+    lnZ, neff = ctx.evidence(lnL, torch.from_numpy(lw).cuda())
+    assert rel_err([rZ], lnZ.cpu().numpy()) <= TOL and rel_err([rN], neff.cpu().numpy()) <= TOL
+    del lnL, idx
+    host = {k: torch.from_numpy(v).pin_memory() for k, v in s.items()}
+    out, lnZh, neffh = ctx.run_host(host, torch.from_numpy(lw).pin_memory())   # one call from host buffers
+    assert rel_err(ref, out.numpy()) <= TOL
+    assert rel_err([rZ], [lnZh]) <= TOL and rel_err([rN], [neffh]) <= TOL
+    ctx.close()
+
+
 # ---------------------------------------------------------------------------------------------- config 4 (many points)
 def test_config4_small_all_points_elementwise(gpu_lib):
     import torch

@@ -114,6 +114,14 @@ def test_draw_eval_evidence_chain_on_device_equals_oracle_chain(gpu_lib):
 
 @pytest.mark.parametrize("case", ["config0_adaptive", "config1_streaming", "stop_rule", "prior_only"])
 def test_integrate_matches_the_oracle_loop(gpu_lib, case):
+    """Tolerances in north_star's terms (lnL and log-evidence within 1e-10 relative, fp64): a run that never refits
+    (prior_only) and the FIRST chunk of every run, which is drawn from the prior, are held to TOL = 1e-10.  Later chunks of
+    an adaptive run are held to 1e-9, ten times looser than north_star, and this is the only place in the suite where that
+    happens: the refit turns the GPU's own lnL (within 1e-10 of the oracle's, not bit-equal) into INTEGER histogram counts
+    rint(W 2^40) (reading S6), whose roundings differ on a few samples per chunk, so the two sides draw later chunks from
+    densities that agree to ~1e-10, not exactly; a sample within that distance of a bin edge changes bin, and its ln w with
+    it.  The refit densities themselves are compared at 1e-8 below for the same reason, and the sampler's
+    own pieces (draws, bins, weights, one refit from identical inputs) are bit-exact / 1e-10 in the tests above."""
     if case == "config1_streaming":      # chunks of 20,000: every ile_eval takes the sorted streaming path
         cfg_ile, n_chunk, max_chunks, n_adapt, thr, scfg = gi.make_config(1, n=1), 20_000, 5, 5, 1e30, dict(CFG, temper=0.5)
     elif case == "config0_adaptive":     # the paper's block size (L97, L119)
@@ -134,6 +142,7 @@ def test_integrate_matches_the_oracle_loop(gpu_lib, case):
     assert g["n_chunks"] == r["n_chunks"] and g["n_samples"] == r["n_samples"]
     rh = np.array(r["history"])
     tol = 1e-9 if n_adapt else TOL
+    assert np.max(np.abs(g["history"][0] - rh[0]) / np.maximum(np.abs(rh[0]), 1.0)) <= TOL   # chunk 0: prior draws, north_star's bar
     assert np.max(np.abs(g["history"][:, 0] - rh[:, 0]) / np.maximum(np.abs(rh[:, 0]), 1.0)) <= tol
     assert np.max(np.abs(g["history"][:, 1] - rh[:, 1]) / np.maximum(np.abs(rh[:, 1]), 1.0)) <= tol
     assert abs(g["lnZ"] - r["lnZ"]) <= tol * max(abs(r["lnZ"]), 1.0)
