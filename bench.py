@@ -40,7 +40,9 @@ def dfma_per_sample(K: int, M: int, n_t: int, exp_cost: float = EXP_DFMA, interp
     """config 1 -> 12,300 + 720 + 8,200 + 400 = 21,620 DFMA-equivalents per sample.
     `exp_cost` = FP64-pipe instructions per time bin of step 6: 20 is the survey's convention; the kernel's own count
     (from the committed ncu SASS mix) gives the "measured exp" accounting of SURVEY.md §8(d)."""
-    linear = 2.0 * K * M * n_t * (2 if interp else 1)  # step 5: Re sum conj(A) Q, 2 DFMA per complex element (two rows when interpolating)
+    # step 5: Re sum conj(A) Q, 2 DFMA per complex element.  Interpolated shifts (R8'): the contraction at n_t + 1 rows, then one
+    # (1 - phi) T_j + phi T_{j+1} per detector and bin -- that the streaming kernel runs it as twice the channels is its own choice
+    linear = 2.0 * K * M * (n_t + 1) + 2.0 * K * n_t if interp else 2.0 * K * M * n_t
     quad = 2.0 * K * (4.0 * M * M + 4.0 * M)        # step 4: Y^dagger U Y and Y^T V Y per detector
     lse = n_t * exp_cost                            # step 6
     geom = 250.0 + 30.0 * M                         # steps 1-3: five sincos, F_k, dt_k, Y_lm, K*M coefficient products
@@ -71,11 +73,12 @@ def max_over_ranks(values, device):
 class ClockSampler(threading.Thread):
     """Samples SM clock and throttle reasons through NVML while the timed region runs."""
 
-    def __init__(self, index: int, period_s: float = 0.005):
+    def __init__(self, index: int, period_s: float = 0.0005):
         super().__init__(daemon=True)
         self.index, self.period = index, period_s
         self.samples, self.reasons, self.stop_flag = [], set(), False
         self.max_mhz = None
+        self.edge = {}  # one reading taken by the launching thread right before and right after the event loop
         try:
             import pynvml
 
@@ -86,29 +89,45 @@ class ClockSampler(threading.Thread):
         except Exception:
             self.nv = None
 
-    def run(self):
-        if self.nv is None:
-            return
+    def _read(self):
         nv = self.nv
         names = {nv.nvmlClocksThrottleReasonHwSlowdown: "hw_slowdown", nv.nvmlClocksThrottleReasonHwThermalSlowdown: "hw_thermal_slowdown",
                  nv.nvmlClocksThrottleReasonSwThermalSlowdown: "sw_thermal_slowdown", nv.nvmlClocksThrottleReasonSwPowerCap: "sw_power_cap",
                  nv.nvmlClocksThrottleReasonHwPowerBrakeSlowdown: "hw_power_brake"}
+        mhz = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+        r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+        return mhz, [nm for bit, nm in names.items() if r & bit]
+
+    def read_edge(self, which: str):
+        """One reading by the calling thread (`which` = "before" / "after" the event loop): a timed region of a few
+        milliseconds may end before the polling thread has run once."""
+        if self.nv is None:
+            return
+        try:
+            mhz, rs = self._read()
+            self.edge[which] = mhz
+            self.reasons.update(rs)
+        except Exception:
+            pass
+
+    def run(self):
+        if self.nv is None:
+            return
         while not self.stop_flag:
             try:
-                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
-                r = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
-                for bit, nm in names.items():
-                    if r & bit:
-                        self.reasons.add(nm)
+                mhz, rs = self._read()
+                self.samples.append(mhz)
+                self.reasons.update(rs)
             except Exception:
                 pass
             time.sleep(self.period)
 
     def summary(self):
-        if not self.samples:
-            return {"sm_mhz": None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "n_samples": 0}
-        s = sorted(self.samples)
-        return {"sm_mhz": s[len(s) // 2], "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons), "n_samples": len(s)}
+        allv = sorted(self.samples + list(self.edge.values()))
+        out = {"sm_mhz": allv[len(allv) // 2] if allv else None, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+               "n_samples": len(self.samples), "poll_ms": self.period * 1e3}
+        out.update({"sm_mhz_" + k: v for k, v in self.edge.items()})
+        return out
 
 
 def read_stream_counters():
@@ -121,9 +140,16 @@ def read_stream_counters():
         import csv
 
         row = [r for r in csv.DictReader(open(p))][-1]
-        return {k: (v if k in ("capture", "kernel", "source") else float(v)) for k, v in row.items()}
+        return {k: (v if k in ("capture", "kernel", "source", "commit") else float(v)) for k, v in row.items()}
     except Exception:
         return None
+
+
+def counters_describe_run(sc_, cfg, n, P, variant, shift_mode) -> bool:
+    """The committed ncu row is ONE launch of the streaming kernel on config 1: its traffic, pipe fraction and per-bin exp
+    cost are attached to a run only if that run launches the same kernel on the same sizes."""
+    return bool(sc_) and cfg["config_id"] == 1 and P == 1 and n == int(sc_["samples"]) and cfg["n_t"] == int(sc_["n_t"]) \
+        and variant in (0, 4) and not shift_mode
 
 
 # ------------------------------------------------------------------------------------------------------------------
@@ -162,7 +188,7 @@ def run_precompute(args, rank: int):
     """SURVEY.md §8(f) NEXT-1, single GPU: ile_precompute over --points intrinsic points of --config's shape per step.
     HBM-bound by construction (every spectrum is read once, every Q written once); roofline against MEASURED_PEAKS.json."""
     if rank != 0:
-        return
+        return None
     import numpy as np
     import torch
 
@@ -188,12 +214,14 @@ def run_precompute(args, rank: int):
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     sampler = ClockSampler(0)
     sampler.start()
+    sampler.read_edge("before")
     for i in range(args.steps):
         flush.fill_(i & 1)
         ev[i][0].record()
         ile.precompute(x, d, meta["fs_hz"], meta["t0_q_s"])
         ev[i][1].record()
     torch.cuda.synchronize()
+    sampler.read_edge("after")
     sampler.stop_flag = True
     ms = sum(a.elapsed_time(b) for a, b in ev) / args.steps
     nbytes = 16 * P * K * (2 * M * N + N + 2 * M * M)  # x in, d in, Q out, U and V out (x counted once)
@@ -212,7 +240,7 @@ def run_precompute(args, rank: int):
             "roofline": {"bound": "hbm", "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak, "traffic": None,
                          "kernel": "ile_overlap_q_radix8_kernel + ile_overlap_uv_bulk_kernel", "peak_source": src, "algorithmic_bytes": nbytes},
             "gpu_launches": 2 * args.steps, "clocks": sampler.summary()}
-    print(json.dumps(line), flush=True)
+    return line
 
 
 def run_integrate(args, rank: int):
@@ -224,7 +252,7 @@ def run_integrate(args, rank: int):
     returns significant lnL_marg"), no early stop (n_eff threshold = inf) so that every step does the same work.  With frozen
     densities the remaining chunks are drawn and evaluated about 2^20 samples at a time; results are those of the chunk-by-chunk loop."""
     if rank != 0:
-        return
+        return None
     import numpy as np
     import torch
 
@@ -249,6 +277,7 @@ def run_integrate(args, rank: int):
     sampler = ClockSampler(0)
     l0, s0 = ctx.launch_count, smp.launch_count
     sampler.start()
+    sampler.read_edge("before")
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     t0 = time.perf_counter()
     e0.record()
@@ -257,6 +286,7 @@ def run_integrate(args, rank: int):
     e1.record()
     torch.cuda.synchronize()
     wall = time.perf_counter() - t0
+    sampler.read_edge("after")
     sampler.stop_flag = True
     ms = max(e0.elapsed_time(e1), wall * 1e3) / args.steps      # the call synchronises: device and wall time agree
     launches = (ctx.launch_count - l0) + (smp.launch_count - s0)
@@ -290,9 +320,127 @@ def run_integrate(args, rank: int):
         dt = time.perf_counter() - t0
         line["cpu_baseline"] = {"value": n_chunk * nchk / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
                                 "sample": f"the first {nchk} chunks of the same run: oracle/sampler.py (numpy) around oracle.eval_batch (OpenMP)"}
-    print(json.dumps(line), flush=True)
     ctx.close()
     smp.close()
+    return line
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# sweep: every other workload of BASELINE.json / SURVEY.md 8(f), short runs attached to the headline's JSON line
+# ------------------------------------------------------------------------------------------------------------------
+SWEEP_HOTPATH = [  # (config, samples per point, points): configs 0, 2, 3 at every batch size (1e7 as ONE call), 4, the paper's windows 5-8
+    (0, None, 1), (2, 1_000_000, 1), (3, 1_000, 1), (3, 10_000, 1), (3, 100_000, 1), (3, 1_000_000, 1), (3, 10_000_000, 1),
+    (4, 100_000, 256), (5, 100_000, 1), (6, 100_000, 1), (7, 100_000, 1), (8, 100_000, 1)]
+ORACLE_BUDGET = 3.0e10  # detector x mode x bin x sample products the oracle is asked for per entry (about 10 s on 16 cores)
+
+
+def sweep_hotpath_entry(cid, n, P, steps, peak_tflops, exp_meas, with_oracle, local_rank=0):
+    """One hot-path workload, timed like the headline: warm-up 3, `steps` steps with an L2 flush in front of each, CUDA events
+    on the launching stream around ile_eval + ile_evidence, NVML polled at 0.5 ms and read before / after the loop."""
+    import numpy as np
+    import torch
+
+    import ile_inputs as gi
+    import paper_1902_04934_b200 as ile
+
+    cfg = gi.make_config(cid, n_points=P)
+    n = cfg["n"] if n is None else n
+    if P == 1:
+        s_np = gi.make_samples(cfg["sample_seeds"][0], n)
+    else:
+        parts = [gi.make_samples(cfg["sample_seeds"][p], n) for p in range(P)]
+        s_np = {k: np.ascontiguousarray(np.concatenate([q[k] for q in parts])) for k in parts[0]}
+        del parts
+    ctx = ile.Context(cfg)
+    dev = ile.samples_to_device(s_np)
+    lnL = torch.empty(P * n, dtype=torch.float64, device="cuda")
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    stream = torch.cuda.current_stream()
+
+    def do_eval():
+        if P == 1:
+            ctx.eval(dev, want_idx=False, out=lnL)       # ONE call whatever n (above 2^20 samples the library cuts it into launch groups)
+        else:
+            ctx.eval_all(dev, want_idx=False, out=lnL.view(P, n))
+
+    for _ in range(3):
+        flush.fill_(1)
+        do_eval()
+        ctx.evidence(lnL, n_segments=P)
+    torch.cuda.synchronize()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    sampler = ClockSampler(local_rank)
+    l0 = ctx.launch_count
+    sampler.start()
+    sampler.read_edge("before")
+    for i in range(steps):
+        flush.fill_(i & 1)
+        ev[i][0].record(stream)
+        do_eval()
+        ev[i][1].record(stream)
+        lnZ, neff = ctx.evidence(lnL, n_segments=P)
+        ev[i][2].record(stream)
+    torch.cuda.synchronize()
+    sampler.read_edge("after")
+    sampler.stop_flag = True
+    launches = ctx.launch_count - l0
+    step_ms = sum(a.elapsed_time(c) for a, _, c in ev) / steps
+    eval_ms = sum(a.elapsed_time(b) for a, b, _ in ev) / steps
+    n_bad, _ = ctx.status()
+    K, M, n_t = cfg["n_det"], cfg["n_modes"], cfg["n_t"]
+    w = dfma_per_sample(K, M, n_t)
+    e = {"stage": "hotpath", "config": cid, "samples_per_point": n, "points": P, "steps": steps,
+         "workload": workload_config(cfg, n, argparse.Namespace(gpus=1))["workload"],
+         "value": P * n / (step_ms * 1e-3), "unit": UNIT, "ms_per_step": step_ms, "ile_eval_ms": eval_ms,
+         "frac": 2.0 * w * P * n / (eval_ms * 1e-3) * 1e-12 / peak_tflops,
+         "frac_model_measured_exp": (2.0 * dfma_per_sample(K, M, n_t, exp_meas) * P * n / (eval_ms * 1e-3) * 1e-12 / peak_tflops) if exp_meas else None,
+         "gpu_launches": int(launches), "n_out_of_range": int(n_bad), "clocks": sampler.summary(),
+         "lnZ": float(lnZ[0].item()), "n_eff": float(neff[0].item()), "lnZ_oracle": None}
+    if with_oracle and float(K) * M * n_t * n <= ORACLE_BUDGET:  # intrinsic point 0, every sample of it
+        import oracle  # cpu_baseline leg
+
+        pb = dict(cfg)
+        if P > 1:
+            pb["Q"], pb["U"], pb["V"], pb["n_points"] = cfg["Q"][:1], cfg["U"][:1], cfg["V"][:1], 1
+        ref, _, _ = oracle.eval_batch(pb, {k: v[:n] for k, v in s_np.items()}, n_threads=os.cpu_count() or 1)
+        rZ, rN = oracle.evidence(ref)
+        e["lnZ_oracle"], e["n_eff_oracle"] = rZ, rN
+        e["lnZ_rel_err"] = abs(e["lnZ"] - rZ) / max(abs(rZ), 1.0)
+    ctx.close()
+    del dev, lnL, flush
+    torch.cuda.empty_cache()
+    return e
+
+
+def run_sweep(args, peak_tflops, exp_meas):
+    """Short runs of every workload the headline does not cover.  Entries are independent: one that fails is reported as
+    {"error": ...} and the sweep goes on."""
+    out = []
+    steps = max(3, min(args.steps, 10))
+    with_oracle = not args.no_cpu_baseline
+    for cid, n, P in SWEEP_HOTPATH:
+        try:
+            k = 3 if (n or 0) * P >= 5_000_000 else steps
+            out.append(sweep_hotpath_entry(cid, n, P, k, peak_tflops, exp_meas, with_oracle))
+        except Exception as ex:  # noqa: BLE001
+            out.append({"stage": "hotpath", "config": cid, "samples_per_point": n, "points": P, "error": repr(ex)})
+    keep = ("metric", "value", "unit", "ms_per_step", "steps", "clocks", "gpu_launches", "lnZ", "n_eff", "us_per_chunk")
+    for stage, kw in [("precompute", dict(config=4, points=256)), ("precompute", dict(config=2, points=16)),
+                      ("integrate", dict(config=1, n=10_000, chunks=200, adapt_chunks=10)),      # densities frozen after 10 chunks (L125)
+                      ("integrate", dict(config=1, n=10_000, chunks=200, adapt_chunks=200))]:    # refit after every chunk
+        a = argparse.Namespace(**vars(args))
+        for k_, v_ in kw.items():
+            setattr(a, k_, v_)
+        a.steps, a.warmup, a.variant, a.no_cpu_baseline = (steps if stage == "precompute" else 3), 3, 0, True
+        try:
+            line = run_precompute(a, 0) if stage == "precompute" else run_integrate(a, 0)
+            e = {"stage": stage, **kw, **{k_: line[k_] for k_ in keep if k_ in line}, "workload": line["config"]["workload"],
+                 "frac": line["roofline"]["frac"], "bound": line["roofline"]["bound"]}
+        except Exception as ex:  # noqa: BLE001
+            e = {"stage": stage, **kw, "error": repr(ex)}
+        out.append(e)
+    return out
+
 
 
 def workload_config(cfg, n, args, extra=None):
@@ -328,6 +476,7 @@ def main():
                     help="precompute: time ile_precompute (eq. 8: Q, U, V of --points intrinsic points); integrate: time ile_integrate "
                          "(the adaptive Monte Carlo loop with on-device sampling) instead of the hot path")
     ap.add_argument("--chunks", type=int, default=200, help="--stage integrate: chunks per step")
+    ap.add_argument("--no-sweep", action="store_true", help="skip the sweep over the other workloads (the default N = 1 run attaches it as \"sweep\")")
     ap.add_argument("--adapt-chunks", type=int, default=10,
                     help="--stage integrate: chunks after which the sampling prior is frozen (PAPER.md L125: adapt only early in the run)")
     args = ap.parse_args()
@@ -342,12 +491,16 @@ def main():
         run_reference(args, rank)
         return
     if args.stage == "precompute":
-        run_precompute(args, rank)
+        line = run_precompute(args, rank)
+        if line:
+            print(json.dumps(line), flush=True)
         return
     if args.stage == "integrate":
         if args.steps > 20:
             args.steps = 20
-        run_integrate(args, rank)
+        line = run_integrate(args, rank)
+        if line:
+            print(json.dumps(line), flush=True)
         return
 
     import numpy as np
@@ -428,6 +581,7 @@ def main():
     torch.cuda.synchronize()
     launches0 = ctx.launch_count
     sampler.start()
+    sampler.read_edge("before")
     wall0 = time.perf_counter()
     for i in range(args.steps):
         flush.fill_(i & 1)                      # L2 flush, outside the event pair
@@ -438,6 +592,7 @@ def main():
         ev[i][2].record(stream)
     torch.cuda.synchronize()
     wall = time.perf_counter() - wall0
+    sampler.read_edge("after")
     sampler.stop_flag = True
     launches = ctx.launch_count - launches0
     if world > 1:
@@ -471,24 +626,31 @@ def main():
         # committed ncu SASS mix) and the FP64 pipe's busy fraction in that capture (DMMA 16 cycles, DFMA/DADD/DMUL 2 cycles
         # per warp instruction and SMSP): SURVEY.md §8(d) "model fraction" and "pipe fraction"
         sc_ = read_stream_counters()
+        if not counters_describe_run(sc_, base, n, P, args.variant, args.shift_mode):
+            sc_ = None  # another config, variant or shift mode: the capture says nothing about this run
         exp_meas = frac_meas = frac_pipe = None
         if sc_:
+            sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
             exp_meas = sc_["fp64_other_inst"] * 32.0 / (sc_["samples"] * sc_["n_t"])
             frac_meas = 2.0 * dfma_per_sample(K, M, n_t, exp_meas, bool(args.shift_mode)) * P * n / (eval_avg_ms * 1e-3) * 1e-12 / peak_tflops
-            frac_pipe = (16.0 * sc_["dmma_inst"] + 2.0 * sc_["fp64_other_inst"]) / (sc_["cycles_elapsed_max"] * 4.0 * 148.0)
+            frac_pipe = (16.0 * sc_["dmma_inst"] + 2.0 * sc_["fp64_other_inst"]) / (sc_["cycles_elapsed_max"] * 4.0 * sms)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": step_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": workload_config(base, n, args, extra={"variant": args.variant, "samples": args.samples, "shift_mode": args.shift_mode}),
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s", "frac": achieved / peak_tflops,
+                         "frac_model_measured_exp": frac_meas,
+                         "fractions": "two accountings of the SAME measured time, to be read side by side: `frac` credits 20 DFMA-equivalents "
+                                      "per exp (SURVEY.md 8(d)'s table, comparable across rounds); `frac_model_measured_exp` credits what the "
+                                      "shipped table exp costs (8(d)'s 'model fraction'), the stricter of the two",
                          "traffic": int(sc_["dram_bytes_read"] + sc_["dram_bytes_write"]) if sc_ else None,
                          "kernel": "ile_eval (steps 1-6)", "kernel_ms": eval_avg_ms, "dfma_equiv_per_sample": w,
                          "peak_dfma": peak_dfma, "peak_dmma": peak_dmma, "peak_nominal": NOMINAL_FP64_TFLOPS,
                          "frac_vs_nominal": achieved / NOMINAL_FP64_TFLOPS,
-                         "exp_fp64_inst_per_bin_measured": exp_meas, "frac_model_measured_exp": frac_meas,
+                         "exp_fp64_inst_per_bin_measured": exp_meas,
                          "frac_pipe": frac_pipe, "pipe_fp64_pct_ncu": sc_["pipe_fp64_pct"] if sc_ else None,
-                         "counters_capture": sc_["capture"] if sc_ else None,
+                         "counters_capture": sc_["capture"] if sc_ else None, "counters_commit": sc_.get("commit") if sc_ else None,
                          "peak_source": "max(ile_measure_fp64_peak: register-resident DFMA chains, ile_measure_dmma_peak: DMMA.8x8x4 chains), "
                          "both measured in this run; frac counts exp at 20 DFMA-equivalents per bin (SURVEY.md 8(d)), "
                          "frac_model_measured_exp at the kernel's own FP64 instruction count per bin, frac_pipe is the FP64 pipe's "
@@ -527,6 +689,16 @@ def main():
                                     "sample": f"{passes} passes over the first {n_cpu} samples of the same batch (eval + evidence), OpenMP over samples",
                                     "value_1thread": n_one / dt1, "sample_1thread": f"one pass over the first {n_one} samples, 1 thread",
                                     "lnZ_oracle": rZ if n_cpu == n else None}
+        default_run = (world == 1 and args.config == 1 and P == 1 and args.n is None and not args.variant and not args.shift_mode
+                       and args.samples == "prior")
+        if default_run and not args.no_sweep:
+            ctx.close()
+            del dev, lnL, flush
+            torch.cuda.empty_cache()
+            line["sweep_note"] = ("the other workloads, each timed like the headline (L2 flush, CUDA events, NVML at 0.5 ms) over fewer steps; "
+                                  "frac counts exp at 20 DFMA-equivalents, frac_model_measured_exp at the per-bin cost of the committed capture "
+                                  "of the same streaming kernel; lnZ_oracle is the CPU oracle on intrinsic point 0 where it fits in about 10 s")
+            line["sweep"] = run_sweep(args, peak_tflops, exp_meas)
         print(json.dumps(line), flush=True)
     ctx.close()
     if world > 1:

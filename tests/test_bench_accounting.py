@@ -15,8 +15,9 @@ def test_work_per_sample_is_the_survey_figure():
     assert bench.dfma_per_sample(3, 21, 410) == 71828.0
     # the kernel's own exp cost replaces the 20 per bin, nothing else
     assert bench.dfma_per_sample(3, 5, 410, 6.0) == 21620.0 - 14.0 * 410
-    # interpolated shifts read two rows per element: the linear term doubles, the rest stays
-    assert bench.dfma_per_sample(3, 5, 410, interp=True) == 21620.0 + 12300.0
+    # interpolated shifts (R8'): the contraction at n_t + 1 rows plus one blend per detector and bin -- NOT twice the contraction,
+    # which is how the streaming kernel happens to run it
+    assert bench.dfma_per_sample(3, 5, 410, interp=True) == 21620.0 + 2 * 3 * 5 + 2 * 3 * 410
 
 
 def test_committed_stream_counters_parse_and_are_consistent():
