@@ -48,7 +48,10 @@ typedef enum {
     ILE_ERR_OUT_OF_RANGE = -5  /* returned by ile_status(): at least one sample's window left the stored Q */
 } ile_error;
 
-#define ILE_MAX_DET 8    /* K */
+#define ILE_MAX_DET 8    /* K.  The fast path (sorted streaming FP64-MMA kernel, variant 4) serves K <= 4; contexts with 5..8 detectors are
+                            evaluated by the tiled DFMA kernel (variant 2: about twice the time per sample, 0.40 ms against 0.20 ms per
+                            1e5 samples at K = 3) or, where its tile does not fit shared memory, by the direct kernel (variant 1, slower
+                            still).  Results are the same within rounding.  The paper's own runs use two detectors (L109). */
 #define ILE_MAX_MODES 32 /* M */
 #define ILE_MAX_L 8      /* largest l of a mode */
 #define ILE_SAMPLER_MAX_BINS 512 /* histogram bins per adaptive dimension */
@@ -226,6 +229,9 @@ int ile_measure_dmma_peak(int32_t iters, double *tflops, double *ms);
  * H1 ile_resample: equal-weight posterior samples of the Monte Carlo parameters by SYSTEMATIC resampling of n draws with weights
  * W_a = exp(lnL_margT[a] + log_w[a]) (eq. 4's integrand): output i (i = 0..n_out-1) is the smallest a whose inclusive cumulative
  * weight, accumulated in sample order and normalised, exceeds (i + v0) / n_out; v0 in [0, 1) is the caller's single uniform.
+ * The cumulative is a parallel prefix sum in binary64: it equals the sequential sum to a few ulp, not bit for bit, so where a
+ * threshold (i + v0) / n_out falls within that distance of a cumulative value the returned id may be the neighbouring sample
+ * (both are valid draws; tests/test_gpu_harvest.py accepts either and checks the rest exactly).
  * lnL_margT, log_w (may be NULL): device, n doubles; ids_out: device int64 [n_out], non-decreasing; every entry -1 when no
  * sample has a finite weight. */
 int ile_resample(ile_ctx *ctx, int64_t n, const double *lnL_margT, const double *log_w, int64_t n_out, double v0,

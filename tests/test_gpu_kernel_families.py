@@ -1,19 +1,17 @@
-"""Workload for compute-sanitizer (SURVEY.md §5 "race detection / sanitizers"); not collected by pytest.
+"""Every kernel family of the library on reduced sizes, in one process, each result checked against the oracle: configs 0 and 1
+through variants 1, 2 and 4 (with one out-of-range window), a multi-point launch, segmented / chunked / merged evidence,
+ile_run_host / ile_run_host_all, the 21-mode path with the FP64-MMA quadratic term, and ile_precompute.
 
-    compute-sanitizer --tool memcheck  python tests/sanitizer_run.py
-    compute-sanitizer --tool racecheck python tests/sanitizer_run.py
-    compute-sanitizer --tool initcheck python tests/sanitizer_run.py
-    compute-sanitizer --tool synccheck python tests/sanitizer_run.py
+Collected by pytest (-m gpu).  The same file is the workload for compute-sanitizer (SURVEY.md 5 "race detection / sanitizers"),
+sized for its 10-100x slowdown, where that tool is available (it is closed on this pool: profiles/r02_sanitizer.md):
 
-Every kernel family of the library on reduced sizes (the sanitizers slow kernels down 10-100x): configs 0 and 1 through
-variants 1, 2 and 4, a multi-point launch, the 21-mode path with the FP64-MMA quadratic term, chunked and segmented
-evidence, evidence merge, ile_run_host / ile_run_host_all, ile_precompute, and the NEXT-2 / NEXT-3 entries when present.
-Results are compared loosely with the oracle so that a sanitizer-induced scheduling change that exposes a race shows up as
-a wrong number too.  Summaries of the runs are kept under profiles/."""
+    for t in memcheck racecheck initcheck synccheck; do compute-sanitizer --tool $t python tests/test_gpu_kernel_families.py; done
+"""
 import os
 import sys
 
 import numpy as np
+import pytest
 import torch
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
@@ -103,13 +101,13 @@ def main():
         g = b.cpu().numpy()[0]
         assert np.max(np.abs(g - a)) <= 1e-10 * np.max(np.abs(a)), nm
     print("  ok ile_precompute", flush=True)
-    extra = os.path.join(os.path.dirname(os.path.abspath(__file__)), "sanitizer_extra.py")
-    if os.path.exists(extra):
-        import runpy
-
-        runpy.run_path(extra, run_name="__main__")
     torch.cuda.synchronize()
-    print("sanitizer workload finished", flush=True)
+    print("kernel-family workload finished", flush=True)
+
+
+@pytest.mark.gpu
+def test_every_kernel_family_on_reduced_sizes(gpu_lib):
+    main()
 
 
 if __name__ == "__main__":
