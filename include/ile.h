@@ -244,7 +244,8 @@ int ile_resample(ile_ctx *ctx, int64_t n, const double *lnL_margT, const double 
  *   drawn_bin[i]   (may be NULL) the smallest bin whose inclusive cumulative of exp(lnL_j) reaches v_uniform[i] times the total:
  *                  a draw of the arrival time from eq. 9's normalised integrand; v_uniform: device, n_sel doubles in (0, 1)
  * Bin j of a sample means the geocentric time t_ref + (j - floor(N_t/2)) / f_s.  A sample whose window leaves the stored Q
- * (reading R9) or an id outside [0, n) gives -1, -inf, -1.  All outputs device, n_sel entries. */
+ * (reading R9) or an id outside [0, n) gives -1, -inf, -1.  All outputs device, n_sel entries.  With shift_mode = 1 the series is
+ * the interpolated one of reading R8' (bin j then means t_ref + (j - floor(N_t/2)) / f_s exactly, not to the nearest sample). */
 int ile_harvest(ile_ctx *ctx, int32_t point, int64_t n, const double *ra, const double *dec, const double *t_ref,
                 const double *phi_ref, const double *psi, const double *incl, const double *dist_mpc, int64_t n_sel,
                 const int64_t *ids, const double *v_uniform, int32_t *argmax_bin, double *lnL_max, int32_t *drawn_bin,

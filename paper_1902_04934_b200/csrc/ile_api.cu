@@ -646,7 +646,6 @@ extern "C" int ile_harvest(ile_ctx *c, int32_t point, int64_t n, const double *r
     if (!ra || !dec || !t_ref || !phi_ref || !psi || !incl || !dist_mpc || !argmax_bin || !lnL_max) return ILE_ERR_BAD_ARGUMENT;
     if (drawn_bin && !v_uniform) return ILE_ERR_BAD_ARGUMENT;
     if (!ids && n_sel > n) return ILE_ERR_BAD_ARGUMENT;
-    if (c->sz.interp) return ILE_ERR_UNSUPPORTED;  // harvesting reads the nearest-sample series
     if (int r = check_device(c)) return r;
     IleEvalArgs a;
     a.params = c->dparams;

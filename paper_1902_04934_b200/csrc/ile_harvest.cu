@@ -20,6 +20,7 @@
 // ------------------------------------------------------------------------------------------------------------
 // H2 + H3: one warp per harvested sample
 // ------------------------------------------------------------------------------------------------------------
+template <bool INTERP>
 __global__ void __launch_bounds__(HV_WARPS * 32) ile_harvest_kernel(IleEvalArgs a, long long n_sel, const long long *__restrict__ ids,
                                                                     const double *__restrict__ v_uniform, int32_t *__restrict__ argmax_bin,
                                                                     double *__restrict__ lnL_max, int32_t *__restrict__ drawn_bin)
@@ -28,9 +29,10 @@ __global__ void __launch_bounds__(HV_WARPS * 32) ile_harvest_kernel(IleEvalArgs 
     const IleDevParams *__restrict__ P = a.params;
     const int K = P->n_det, M = P->n_modes, KM = K * M, n_q = P->n_q, n_t = P->n_t;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const size_t per_warp = (((size_t)KM * sizeof(double2) + (size_t)K * sizeof(int32_t)) + 15) & ~(size_t)15;
+    const size_t per_warp = (((size_t)KM * sizeof(double2) + (size_t)K * (sizeof(double) + sizeof(int32_t))) + 15) & ~(size_t)15;
     double2 *A = reinterpret_cast<double2 *>(hv_smem + warp * per_warp);
-    int32_t *i0S = reinterpret_cast<int32_t *>(A + KM);
+    double *phiS = reinterpret_cast<double *>(A + KM);  // [K] fractional parts of the arrival times (INTERP; reading R8')
+    int32_t *i0S = reinterpret_cast<int32_t *>(phiS + K);
     const size_t pglob = (size_t)a.point0;
     const double2 *__restrict__ Qp = a.Q + pglob * (size_t)KM * n_q;
 
@@ -40,7 +42,7 @@ __global__ void __launch_bounds__(HV_WARPS * 32) ile_harvest_kernel(IleEvalArgs 
         int bad = s < 0 || s >= a.n_per_point;
         if (lane == 0 && !bad)
             quad = ile_setup_sample(P, a.U + pglob * (size_t)KM * M, a.V + pglob * (size_t)KM * M, a.ra[s], a.dec[s], a.t_ref[s],
-                                    a.phi_ref[s], a.psi[s], a.incl[s], a.dist[s], A, M, i0S, &bad);
+                                    a.phi_ref[s], a.psi[s], a.incl[s], a.dist[s], A, M, i0S, &bad, INTERP ? phiS : nullptr);
         __syncwarp();
         bad = __shfl_sync(0xffffffffu, bad, 0);
         quad = __shfl_sync(0xffffffffu, quad, 0);
@@ -57,8 +59,14 @@ __global__ void __launch_bounds__(HV_WARPS * 32) ile_harvest_kernel(IleEvalArgs 
             double acc = 0.0;
             for (int k = 0; k < K; ++k) {
                 const double2 *Qk = Qp + (size_t)k * M * n_q + i0S[k] + j;
+                const double ph = INTERP ? phiS[k] : 0.0, om = 1.0 - ph;
                 for (int m = 0; m < M; ++m) {
-                    const double2 c = A[k * M + m], q = __ldg(Qk + (size_t)m * n_q);
+                    const double2 c = A[k * M + m];
+                    double2 q = __ldg(Qk + (size_t)m * n_q);
+                    if (INTERP) {  // (1 - phi) Q[i] + phi Q[i + 1], as the direct kernel forms it
+                        const double2 q1 = __ldg(Qk + (size_t)m * n_q + 1);
+                        q.x = om * q.x + ph * q1.x, q.y = om * q.y + ph * q1.y;
+                    }
                     acc = fma(c.x, q.x, fma(c.y, q.y, acc));
                 }
             }
@@ -118,11 +126,15 @@ cudaError_t ile_launch_harvest(const IleSizes &sz, const IleEvalArgs &a, long lo
                                int32_t *argmax_bin, double *lnL_max, int32_t *drawn_bin, cudaStream_t st)
 {
     if (n_sel <= 0) return cudaSuccess;
-    const size_t per_warp = (((size_t)sz.n_det * sz.n_modes * sizeof(double2) + (size_t)sz.n_det * sizeof(int32_t)) + 15) & ~(size_t)15;
+    const size_t per_warp =
+        (((size_t)sz.n_det * sz.n_modes * sizeof(double2) + (size_t)sz.n_det * (sizeof(double) + sizeof(int32_t))) + 15) & ~(size_t)15;
     long long blocks = (n_sel + HV_WARPS - 1) / HV_WARPS;
     const long long cap = (long long)sz.sm_count * 16;
     if (blocks > cap) blocks = cap;
-    ile_harvest_kernel<<<(unsigned)blocks, HV_WARPS * 32, per_warp * HV_WARPS, st>>>(a, n_sel, ids, v_uniform, argmax_bin, lnL_max, drawn_bin);
+    if (sz.interp)
+        ile_harvest_kernel<true><<<(unsigned)blocks, HV_WARPS * 32, per_warp * HV_WARPS, st>>>(a, n_sel, ids, v_uniform, argmax_bin, lnL_max, drawn_bin);
+    else
+        ile_harvest_kernel<false><<<(unsigned)blocks, HV_WARPS * 32, per_warp * HV_WARPS, st>>>(a, n_sel, ids, v_uniform, argmax_bin, lnL_max, drawn_bin);
     return cudaGetLastError();
 }
 

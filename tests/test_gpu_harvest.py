@@ -53,12 +53,24 @@ def test_resample_matches_the_oracle(gpu_lib, n, n_out):
     ctx.close()
 
 
-@pytest.mark.parametrize("cid", [0, 1, 2])
-def test_harvest_matches_the_oracle_series(gpu_lib, cid):
+@pytest.mark.parametrize("cid,shift_mode", [(0, 0), (1, 0), (2, 0), (0, 1), (1, 1)])
+def test_harvest_matches_the_oracle_series(gpu_lib, cid, shift_mode):
+    """shift_mode 1: the harvested series is the linearly interpolated one of reading R8' (oracle/subsample.py), so that the
+    interpolated variant of the path (NEXT-4) has its arg-max and time draw too."""
     import torch
+
+    from oracle import subsample as osub
 
     n = 600 if cid < 2 else 150
     cfg = gi.make_config(cid, n=n)
+    cfg["shift_mode"] = shift_mode
+
+    def series_of(sample):
+        if shift_mode:
+            r = osub.sample_series_lin(cfg, sample)
+            return r[0], None, None, r[4]
+        return oracle.sample_series(cfg, sample)
+
     s = gi.make_samples(cfg["sample_seeds"][0] + 3, n)
     s["t_ref"][11] = 0.9                                   # out of range: -1 / -inf / -1
     rng = np.random.default_rng(cid)
@@ -68,7 +80,7 @@ def test_harvest_matches_the_oracle_series(gpu_lib, cid):
     amax, lmax, drawn = amax.cpu().numpy(), lmax.cpu().numpy(), drawn.cpu().numpy()
     n_amb = 0
     for a in range(n):
-        series, _, _, oob = oracle.sample_series(cfg, {k: s[k][a] for k in s})
+        series, _, _, oob = series_of({k: s[k][a] for k in s})
         if oob:
             assert amax[a] == -1 and drawn[a] == -1 and lmax[a] == -np.inf
             continue
@@ -85,7 +97,7 @@ def test_harvest_matches_the_oracle_series(gpu_lib, cid):
             assert np.all(np.abs(cdf[lo:hi] - v[a]) <= 1e-10), (a, drawn[a], jd)
             n_amb += 1
     assert n_amb <= 2
-    assert oracle.sample_series(cfg, {k: s[k][11] for k in s})[3]
+    assert series_of({k: s[k][11] for k in s})[3]
     ctx.close()
 
 
