@@ -185,7 +185,9 @@ int ile_precompute_psd(int32_t n_points, int32_t n_det, int32_t n_modes, int32_t
  * generated on the CPU and transferred to the board): H2D copy of the seven sample arrays (+ log_w), ile_eval,
  * ile_evidence, D2H of lnL_margT (if not NULL), lnZ and n_eff.  Host arrays of n doubles each; pinned memory makes
  * the copies asynchronous.  Synchronises the stream before returning.  Staging buffers are owned by the context
- * and grow on demand. */
+ * and grow on demand.  From 200,000 samples on (streaming kernel) the batch is cut into 2-4 slices, or one per launch group above 2^20 samples: slice i + 1
+ * is uploaded and slice i - 1 downloaded on the context's own copy streams while slice i computes, the evidence state carried on
+ * the device; results are those of the unsliced call within rounding. */
 int ile_run_host(ile_ctx *ctx, int32_t point, int64_t n, const double *ra, const double *dec, const double *t_ref,
                  const double *phi_ref, const double *psi, const double *incl, const double *dist_mpc,
                  const double *log_w /* may be NULL */, double *lnL_margT /* host out, may be NULL */,

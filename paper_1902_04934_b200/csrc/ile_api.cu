@@ -7,6 +7,11 @@
 
 #include "ile_kernels.h"
 
+#define ILE_PIPE_MAX_SLICES 16
+#ifndef ILE_PIPE_MIN_SLICE
+#define ILE_PIPE_MIN_SLICE 100000 /* samples per slice of a pipelined ile_run_host: at 50,000 the host needs as long to issue two slices as the copies take (measured: 0.369 against 0.374 ms at 1e5 samples), from 2 x 100,000 on the overlap wins (1e6 samples: 2.82 -> 2.16 ms) */
+#endif
+
 struct ile_ctx {
     int device;
     IleSizes sz;
@@ -45,6 +50,11 @@ struct ile_ctx {
     size_t resample_cap;  // doubles
     cudaStream_t copy_stream;  // ile_run_host: second H2D queue
     cudaEvent_t ev_copy_go, ev_copy_done;
+    // ile_run_host, sliced: uploads of slice i + 1 and the download of slice i - 1 run beside the kernels of slice i
+    cudaStream_t d2h_stream;
+    cudaEvent_t ev_pipe[3 * ILE_PIPE_MAX_SLICES];  // per slice: sort inputs arrived, other inputs arrived, lnL_margT ready
+    cudaEvent_t ev_d2h_done;
+    double *d_pipe_state;  // evidence state (max, sum, count) carried over the slices
 };
 
 static thread_local char g_cuda_msg[256] = "no CUDA error recorded";
@@ -237,6 +247,10 @@ extern "C" int ile_create(ile_ctx **out, const ile_config *cfg, const void *Q, c
         CKC(cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
         CKC(cudaEventCreateWithFlags(&c->ev_copy_go, cudaEventDisableTiming));
         CKC(cudaEventCreateWithFlags(&c->ev_copy_done, cudaEventDisableTiming));
+        CKC(cudaStreamCreateWithFlags(&c->d2h_stream, cudaStreamNonBlocking));
+        for (int i = 0; i < 3 * ILE_PIPE_MAX_SLICES; ++i) CKC(cudaEventCreateWithFlags(&c->ev_pipe[i], cudaEventDisableTiming));
+        CKC(cudaEventCreateWithFlags(&c->ev_d2h_done, cudaEventDisableTiming));
+        CKC(cudaMalloc(&c->d_pipe_state, 3 * sizeof(double)));
         const size_t nQs = (size_t)cfg->n_points * cfg->n_det * c->spl.ks * c->spl.nqp * 4;
         CKC(cudaMalloc(&c->dQs, nQs * sizeof(double)));
         CKC(ile_launch_pack_q_stream(c->sz, c->spl, cfg->n_points, c->dQ, c->dQs, 0));
@@ -280,6 +294,11 @@ extern "C" void ile_destroy(ile_ctx *c)
     if (c->copy_stream) cudaStreamDestroy(c->copy_stream);
     if (c->ev_copy_go) cudaEventDestroy(c->ev_copy_go);
     if (c->ev_copy_done) cudaEventDestroy(c->ev_copy_done);
+    if (c->d2h_stream) cudaStreamDestroy(c->d2h_stream);
+    for (int i = 0; i < 3 * ILE_PIPE_MAX_SLICES; ++i)
+        if (c->ev_pipe[i]) cudaEventDestroy(c->ev_pipe[i]);
+    if (c->ev_d2h_done) cudaEventDestroy(c->ev_d2h_done);
+    cudaFree(c->d_pipe_state);
     if (c->h_small) cudaFreeHost(c->h_small);
     delete[] c->hU;
     delete[] c->hV;
@@ -558,6 +577,59 @@ static int run_host(ile_ctx *c, int32_t point0, int32_t np, int64_t n, const dou
         c->stage_cap = need;
     }
     double *d = c->d_stage;
+    // One point, streaming variant, one launch group, and enough samples for 2-4 efficient slices: pipeline the call (PAPER.md L97:
+    // blocks "generated on the CPU and transferred to the board" -- the transfer of the next part hides behind the kernels of this one).
+    const bool streaming = c->copy_stream && (c->variant == 4 || (c->variant == 0 && c->stream_ok));
+    // slices: 2-4 while the batch is one launch group, else one per launch group (at most ILE_PIPE_MAX_SLICES: 1.6e7 samples)
+    int64_t S = n / ILE_PIPE_MIN_SLICE < 4 ? n / ILE_PIPE_MIN_SLICE : 4;
+    const int64_t groups = (n + c->chunk_samples - 1) / (c->chunk_samples > 0 ? c->chunk_samples : 1);
+    if (S < groups) S = groups;
+    const int64_t per = S > 0 ? (((n + S - 1) / S) + 1023) & ~(int64_t)1023 : 0;  // slice starts stay 8 KiB aligned
+    if (np == 1 && streaming && S >= 2 && S <= ILE_PIPE_MAX_SLICES && per <= c->chunk_samples) {
+        double *d_out = d + (size_t)8 * tot;
+        CK(cudaEventRecord(c->ev_copy_go, st));  // the staging buffer is free once the caller's stream gets here
+        CK(cudaStreamWaitEvent(c->copy_stream, c->ev_copy_go, 0));
+        int n_sl = 0;
+        for (int64_t lo = 0; lo < n; lo += per, ++n_sl) {  // every upload is queued up front, in the order the kernels want them
+            const size_t cnt = (size_t)(n - lo < per ? n - lo : per);
+            for (int i = 0; i < 8; ++i) {
+                if (src[i]) CK(cudaMemcpyAsync(d + (size_t)i * tot + lo, src[i] + lo, cnt * sizeof(double), cudaMemcpyHostToDevice, c->copy_stream));
+                if (i == 2) CK(cudaEventRecord(c->ev_pipe[3 * n_sl], c->copy_stream));  // ra, dec, t_ref: what the sort reads
+            }
+            CK(cudaEventRecord(c->ev_pipe[3 * n_sl + 1], c->copy_stream));
+        }
+        int nl = 0;
+        cudaError_t e = ile_launch_evidence_reset(1, c->d_pipe_state, st, &nl);
+        c->launches += nl;
+        if (e != cudaSuccess) return cuda_fail(e);
+        int sl = 0;
+        for (int64_t lo = 0; lo < n; lo += per, ++sl) {
+            const int64_t cnt = n - lo < per ? n - lo : per;
+            CK(cudaStreamWaitEvent(st, c->ev_pipe[3 * sl], 0));
+            c->ss.ev_late = c->ev_pipe[3 * sl + 1];  // the coefficient kernel (side stream) waits for the other five arrays
+            int r = eval_dispatch(c, point0, 1, cnt, d + lo, d + tot + lo, d + 2 * tot + lo, d + 3 * tot + lo, d + 4 * tot + lo,
+                                  d + 5 * tot + lo, d + 6 * tot + lo, d_out + lo, nullptr, st);
+            c->ss.ev_late = nullptr;
+            if (r != ILE_OK) return r;
+            CK(cudaStreamWaitEvent(st, c->ev_pipe[3 * sl + 1], 0));  // log_w; a non-streaming slice (tiny tail) has not waited yet
+            r = ile_evidence(c, 1, cnt, d_out + lo, src[7] ? d + 7 * tot + lo : nullptr, c->d_pipe_state, c->d_small, c->d_small + 1, st);
+            if (r != ILE_OK) return r;
+            if (lnL_margT) {
+                CK(cudaEventRecord(c->ev_pipe[3 * sl + 2], st));
+                CK(cudaStreamWaitEvent(c->d2h_stream, c->ev_pipe[3 * sl + 2], 0));
+                CK(cudaMemcpyAsync(lnL_margT + lo, d_out + lo, (size_t)cnt * sizeof(double), cudaMemcpyDeviceToHost, c->d2h_stream));
+            }
+        }
+        CK(cudaMemcpyAsync(c->h_small, c->d_small, 2 * sizeof(double), cudaMemcpyDeviceToHost, st));
+        if (lnL_margT) {  // the downloads belong to the caller's stream order too
+            CK(cudaEventRecord(c->ev_d2h_done, c->d2h_stream));
+            CK(cudaStreamWaitEvent(st, c->ev_d2h_done, 0));
+        }
+        CK(cudaStreamSynchronize(st));
+        lnZ[0] = c->h_small[0];
+        if (n_eff) n_eff[0] = c->h_small[1];
+        return ILE_OK;
+    }
     // The sort needs ra, dec, t_ref only.  When the streaming variant will run as ONE launch group, the other arrays are
     // copied on a second queue and only the coefficient kernel (side stream) waits for them: their transfer overlaps the
     // index kernel, the scan and the scatter.

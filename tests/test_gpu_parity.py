@@ -423,6 +423,36 @@ def test_run_host_matches_device_path(gpu_lib):
     ctx.close()
 
 
+@pytest.mark.parametrize("n", [200_000, 237_777, 430_001])
+def test_run_host_sliced_pipeline_every_sample(gpu_lib, n):
+    """From 200,000 samples on (one point, one launch group) ile_run_host cuts the batch into 2-4 slices and uploads slice
+    i + 1 / downloads slice i - 1 while slice i computes, with the evidence state carried over the slices on the device.
+    EVERY lnL_margT, lnZ and n_eff against the oracle, with and without weights and the lnL download; repeated on one
+    context so that a second call finds the staging buffers and events of the first."""
+    import torch
+
+    cfg = gi.make_config(1, n=n)
+    s = gi.make_samples(cfg["sample_seeds"][0] + 1, n)
+    lw = gi.make_log_weights(6, n)
+    ref, _, _ = oracle.eval_batch(cfg, s, n_threads=ORACLE_THREADS)
+    rZ, rN = oracle.evidence(ref, lw)
+    ctx = gpu_lib.Context(cfg)
+    host = {k: torch.from_numpy(v).pin_memory() for k, v in s.items()}
+    for rep in range(2):
+        out, lnZ, neff = ctx.run_host(host, torch.from_numpy(lw).pin_memory())
+        assert rel_err(ref, out.numpy()) <= TOL
+        assert rel_err([rZ], [lnZ]) <= TOL and rel_err([rN], [neff]) <= TOL
+    out2, lnZ2, neff2 = ctx.run_host(host, None, want_lnL=False)
+    r0 = oracle.evidence(ref)
+    assert out2 is None and rel_err([r0[0]], [lnZ2]) <= TOL and rel_err([r0[1]], [neff2]) <= TOL
+    pageable = {k: torch.from_numpy(v.copy()) for k, v in s.items()}          # not pinned: the copies are staged by the driver
+    out3, lnZ3, _ = ctx.run_host(pageable, None)
+    assert rel_err(ref, out3.numpy()) <= TOL and rel_err([r0[0]], [lnZ3]) <= TOL
+    n_bad, _ = ctx.status()
+    assert n_bad == 0
+    ctx.close()
+
+
 def test_run_host_all_matches_the_oracle_per_point(gpu_lib):
     """ile_run_host_all: host [P][n] arrays through ONE C-ABI call (H2D, ile_eval_all, ile_evidence per point, D2H);
     n large enough that the streaming path runs, weighted."""
